@@ -1,0 +1,137 @@
+/* sp2_b200.h -- C ABI of libsp2b200.so: the SP2 density-matrix hot path of arxiv 2101.06385
+ * ("Mixed Precision Fermi-Operator Expansion on Tensor Cores From a Machine Learning Perspective")
+ * as hand-written sm_100a CUDA.  Citations: P:n = line n of the paper text.
+ *
+ * What the library computes (Alg. 1, with Alg. 2, as the activation):
+ *   S_0 = (eps_max I - H) / (eps_max - eps_min)                      (W_0, B_0 of Alg. 1)
+ *   X_n = f(S_{n-1}) = S_{n-1}^2 ~ FP32[ X0 X0 + X0 X1 + (X0 X1)^T ]   (Eq. 15) with
+ *         X0 = FP16[c S], X1 = FP16[c S - X0]                         (Eqs. 12-13; c = 2^k, see opts)
+ *   standard:    S_n = sigma_n X_n + (1 - sigma_n) S_{n-1},  sigma_n from the trace rule of Alg. 1
+ *   generalized: S_n = th1 X_n + th2 S_{n-1} + th3 I                  (Eq. 17 in matrix form)
+ * with the branch / convergence control evaluated on the device.
+ *
+ * Conventions for every entry point
+ *   - Matrices are dense, row-major, FP32, assumed symmetric; only the LOWER triangle of H is read.
+ *   - Pointers named *_dev are CUDA device pointers, *_host are host pointers; the caller owns all of
+ *     them; inputs are never modified.  `stream` is a cudaStream_t passed as void* (NULL = default stream).
+ *   - All work is enqueued on `stream`; each solve call ends with ONE cudaStreamSynchronize after copying
+ *     the per-layer statistics back (no host round trip per layer).
+ *   - Return value: SP2_OK (0); > 0 = result written but flagged; < 0 = error, outputs undefined.
+ *     No exceptions, no stdout.  There is no CPU fallback: without a CUDA device calls return SP2_ERR_CUDA.
+ */
+#ifndef SP2_B200_H
+#define SP2_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sp2_handle_s* sp2_handle_t;   /* owns workspace, TMA tensor maps, CUDA graphs */
+
+typedef enum {
+    SP2_OK = 0,
+    SP2_NOT_CONVERGED = 1,          /* max_layers reached before any convergence test fired; D = S_{max_layers} */
+    SP2_ERR_INVALID_ARG = -1,
+    SP2_ERR_BOUNDS_DEGENERATE = -2, /* eps_max <= eps_min (given, or Gershgorin of a multiple of I) */
+    SP2_ERR_NONFINITE = -3,         /* a trace became NaN/Inf */
+    SP2_ERR_WORKSPACE = -4,         /* problem larger than the handle was created for */
+    SP2_ERR_CUDA = -5,              /* a CUDA call failed; sp2_last_cuda_error() has the text */
+    SP2_ERR_UNSUPPORTED_N = -6
+} sp2_status_t;
+
+/* stop_reason values (Alg. 1's two tests; tol / max_layers are the caller's extra tests) */
+enum { SP2_STOP_NONE = 0, SP2_STOP_IDERR_NONPOS = 1, SP2_STOP_PARAM_FREE = 2, SP2_STOP_TOL = 3,
+       SP2_STOP_MAX_LAYERS = 4, SP2_STOP_NONFINITE = 5 };
+
+/* Per-layer statistics, entry n-1 describes layer n (n = 1..n_layers), Alg. 1's notation. */
+typedef struct {
+    double trace_S;       /* N_S = Tr[S_n] after the layer: FP64 sum of the FP32 diagonal of S_n            */
+    double trace_X;       /* N_X = Tr[X_n] used by the control, evaluated as ||S_{n-1}||_F^2 (= Tr[S^2] for
+                             symmetric S) in FP64 while S_{n-1} was written                           */
+    double trace_X_diag;  /* cross-check: FP64 sum of the diagonal of the tensor-core X_n                    */
+    double iderr;         /* IdErr_n = N_S(before) - N_X = Tr[S_{n-1} - S_{n-1}^2]           */
+    int    sigma;         /* +1: S_n = X_n ; -1: S_n = 2 S_{n-1} - X_n ; 0 in generalized runs               */
+    int    stop_reason;   /* SP2_STOP_* : nonzero only on the last layer                                     */
+} sp2_layer_stat_t;
+
+typedef struct {
+    int    auto_bounds;     /* 1: Gershgorin bounds computed on the device; 0: use eps_min/eps_max verbatim  */
+    double eps_min, eps_max;
+    double tol;             /* > 0: also stop when IdErr_n <= tol (absolute); <= 0: paper's rule only        */
+    int    max_layers;      /* 1..handle's max_layers                                                        */
+    double eps_alt;         /* Alg. 1's small epsilon, default 0                                     */
+    int    fp16_scale_log2; /* k: the split is applied to 2^k S (exact rescale; 0 = Eq. 13 literally).
+                               -1 = library default (13): keeps X1 out of FP16's subnormal range            */
+    int    control;         /* 0: device-side loop in a CUDA graph (WHILE node); 1: host-stepped (debug:
+                               one sync per layer); 2: graph of max_layers guarded launches, no WHILE node   */
+    int    tile_config;     /* 0: choose by N; 1: 128x128 1-CTA; 2: 128x256 1-CTA; 3: 256x256 2-CTA          */
+} sp2_opts_t;
+
+/* Fill *o with defaults: auto_bounds=1, tol=0, max_layers=120, eps_alt=0, fp16_scale_log2=-1, control=0. */
+void sp2_default_opts(sp2_opts_t* o);
+
+/* Create a handle able to solve one matrix up to N_max, or a batch of batch_max matrices of N <= 256,
+ * with at most max_layers layers.  Allocates device workspace (sp2_workspace_bytes). */
+sp2_status_t sp2_create(sp2_handle_t* h, int N_max, int batch_max, int max_layers);
+sp2_status_t sp2_destroy(sp2_handle_t h);
+size_t       sp2_workspace_bytes(int N_max, int batch_max, int max_layers);
+
+/* Alg. 1: H (N x N, leading dimension ldh >= N) -> D (leading dimension ldd >= N).
+ * stats_host: [opts->max_layers] entries (may be NULL); n_layers: layers executed (may be NULL);
+ * bounds_out[2]: the spectral bounds used (may be NULL).  0 <= N_occ <= N. */
+sp2_status_t sp2_density_matrix(sp2_handle_t h, const float* H_dev, int N, int ldh, double N_occ,
+                                const sp2_opts_t* opts, float* D_dev, int ldd,
+                                sp2_layer_stat_t* stats_host, int* n_layers, double bounds_out[2],
+                                void* stream);
+
+/* Same call with HOST buffers: copies H to the device, solves, copies D back (end-to-end path). */
+sp2_status_t sp2_density_matrix_host(sp2_handle_t h, const float* H_host, int N, int ldh, double N_occ,
+                                     const sp2_opts_t* opts, float* D_host, int ldd,
+                                     sp2_layer_stat_t* stats_host, int* n_layers, double bounds_out[2],
+                                     void* stream);
+
+/* Generalized network (Eq. 17): L fixed layers S_n = th1 S_{n-1}^2 + th2 S_{n-1} + th3 I,
+ * theta_host = [L][3] doubles; no convergence test.  eps_min >= eps_max -> Gershgorin bounds.
+ * opts may be NULL (defaults); only fp16_scale_log2, control, tile_config are read. */
+sp2_status_t sp2_generalized(sp2_handle_t h, const float* H_dev, int N, int ldh,
+                             const double* theta_host, int L, double eps_min, double eps_max,
+                             const sp2_opts_t* opts, float* X_L_dev, int ldx,
+                             sp2_layer_stat_t* stats_host, void* stream);
+
+/* Convenience form of the same network with per-layer branch, weight and bias scalars (BASELINE north_star):
+ * S_n = w_n (sigma_n X_n + (1 - sigma_n) S_{n-1}) + b_n I, i.e. theta_n = (w sigma, w (1 - sigma), b).
+ * sigma == NULL means all +1. */
+sp2_status_t sp2_generalized_wb(sp2_handle_t h, const float* H_dev, int N, int ldh, const int* sigma,
+                                const double* weights, const double* biases, int L,
+                                double eps_min, double eps_max, const sp2_opts_t* opts,
+                                float* X_L_dev, int ldx, sp2_layer_stat_t* stats_host, void* stream);
+
+/* Batched small-N: B independent matrices H[B][N][N] (contiguous, N <= 256), one launch, one CTA
+ * cluster per matrix, per-matrix branch sequence and stop layer.  N_occ: [B] values, or one value if
+ * nocc_is_scalar.  stats_host: [B][opts->max_layers] (may be NULL); n_layers: [B]; status_out: [B] per-matrix
+ * sp2_status_t (may be NULL).  Returns the worst per-matrix status. */
+sp2_status_t sp2_density_matrix_batched(sp2_handle_t h, const float* H_dev, int N, int B,
+                                        const double* N_occ, int nocc_is_scalar, const sp2_opts_t* opts,
+                                        float* D_dev, sp2_layer_stat_t* stats_host, int* n_layers,
+                                        int* status_out, void* stream);
+
+/* Stand-alone pieces of the path (rows a1, a3 of DESIGN.md), asynchronous on `stream` except where noted. */
+/* Eqs. 12-13: hi = FP16[2^k X], lo = FP16[2^k X - hi]; X N x N (ldx), hi/lo N x N (ldo), as uint16 bits */
+sp2_status_t sp2_split_fp16(const float* X_dev, int N, int ldx, unsigned short* hi_dev, unsigned short* lo_dev,
+                            int ldo, int fp16_scale_log2, void* stream);
+/* Gershgorin bounds of the lower-triangle-symmetrised H; synchronises; bounds_host[2] = {eps_min, eps_max}. */
+sp2_status_t sp2_gershgorin(sp2_handle_t h, const float* H_dev, int N, int ldh, double bounds_host[2], void* stream);
+
+const char* sp2_status_string(sp2_status_t s);
+const char* sp2_last_cuda_error(void);
+/* Number of kernels the last solve call on this handle launched (graph nodes executed are counted by the
+ * device-side layer counter: setup kernels + layers + copy-out). */
+int         sp2_last_launch_count(sp2_handle_t h);
+const char* sp2_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SP2_B200_H */

@@ -1,0 +1,568 @@
+// C ABI of libsp2b200.so (include/sp2_b200.h): handle / workspace lifecycle, TMA tensor maps, the CUDA graph
+// that holds the device-side layer loop, and the solve entry points.
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <map>
+#include <mutex>
+#include <tuple>
+#include <vector>
+
+#include "sp2_kernels.h"
+
+using namespace sp2;
+
+static thread_local char g_cuda_err[512] = "";
+
+static sp2_status_t cuda_fail(cudaError_t e, const char* what) {
+    snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", what, cudaGetErrorString(e));
+    return SP2_ERR_CUDA;
+}
+#define CK(call)                                              \
+    do {                                                      \
+        cudaError_t e__ = (call);                             \
+        if (e__ != cudaSuccess) return cuda_fail(e__, #call); \
+    } while (0)
+
+typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                    const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+struct LoopGraph {
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t exec = nullptr;
+};
+
+struct sp2_handle_s {
+    int N_max = 0, batch_max = 0, max_layers = 0;
+    int Np_max = 0;
+    int num_sms = 0, device = 0;
+    // single-matrix workspace
+    float* S = nullptr;
+    __half* hl[2][2] = {{nullptr, nullptr}, {nullptr, nullptr}};   // [ping-pong][hi, lo]
+    double* R = nullptr;
+    double* diag = nullptr;
+    Ctrl* ctrl = nullptr;
+    sp2_layer_stat_t* stats_dev = nullptr;
+    double* thetas_dev = nullptr;
+    int2* tiles_dev = nullptr;
+    int tiles_cap = 0;
+    // batched workspace
+    sp2_layer_stat_t* bstats_dev = nullptr;
+    int* bnl_dev = nullptr;
+    int* bstatus_dev = nullptr;
+    double* bbounds_dev = nullptr;
+    double* bnocc_dev = nullptr;
+    // pinned host mirrors
+    Ctrl* ctrl_host = nullptr;
+    sp2_layer_stat_t* stats_host = nullptr;
+    double* thetas_host = nullptr;
+    double* bounds_host = nullptr;
+    // host staging for the *_host entry point
+    float* stage_H = nullptr;
+    float* stage_D = nullptr;
+    size_t stage_elems = 0;
+    PFN_encodeTiled encode = nullptr;
+    std::map<std::tuple<int, int, int, int>, LoopGraph> graphs;   // (N, Np, cfg, scale_log2)
+    int tiles_key_nt = -1, tiles_key_band = -1;
+    int n_super = 0;
+    int last_launches = 0;
+    cudaStream_t cap_stream = nullptr;
+};
+
+static int round_up(int x, int m) { return (x + m - 1) / m * m; }
+
+static size_t ctrl_header_bytes() { return offsetof(Ctrl, partial); }
+
+extern "C" const char* sp2_status_string(sp2_status_t s) {
+    switch (s) {
+        case SP2_OK: return "SP2_OK";
+        case SP2_NOT_CONVERGED: return "SP2_NOT_CONVERGED";
+        case SP2_ERR_INVALID_ARG: return "SP2_ERR_INVALID_ARG";
+        case SP2_ERR_BOUNDS_DEGENERATE: return "SP2_ERR_BOUNDS_DEGENERATE";
+        case SP2_ERR_NONFINITE: return "SP2_ERR_NONFINITE";
+        case SP2_ERR_WORKSPACE: return "SP2_ERR_WORKSPACE";
+        case SP2_ERR_CUDA: return "SP2_ERR_CUDA";
+        case SP2_ERR_UNSUPPORTED_N: return "SP2_ERR_UNSUPPORTED_N";
+    }
+    return "SP2_UNKNOWN";
+}
+extern "C" const char* sp2_last_cuda_error(void) { return g_cuda_err; }
+extern "C" const char* sp2_version(void) { return "sp2b200 0.1 (sm_100a)"; }
+
+extern "C" void sp2_default_opts(sp2_opts_t* o) {
+    if (!o) return;
+    o->auto_bounds = 1;
+    o->eps_min = 0.0;
+    o->eps_max = 0.0;
+    o->tol = 0.0;
+    o->max_layers = 120;
+    o->eps_alt = 0.0;
+    o->fp16_scale_log2 = -1;
+    o->control = 0;
+    o->tile_config = 0;
+}
+
+extern "C" size_t sp2_workspace_bytes(int N_max, int batch_max, int max_layers) {
+    if (N_max < 1 || max_layers < 1) return 0;
+    const size_t Np = (size_t)round_up(N_max, 256);
+    size_t b = Np * Np * 4 + 4 * Np * Np * 2;                 // S + two hi/lo pairs
+    b += 2 * Np * sizeof(double);                             // Gershgorin radii, diagonal
+    b += sizeof(Ctrl) + (size_t)max_layers * (sizeof(sp2_layer_stat_t) + 3 * sizeof(double));
+    b += (Np / 128) * (Np / 128 + 1) / 2 * sizeof(int2);
+    if (batch_max > 0)
+        b += (size_t)batch_max * ((size_t)max_layers * sizeof(sp2_layer_stat_t) + 2 * sizeof(int) + 3 * sizeof(double));
+    return b;
+}
+
+extern "C" sp2_status_t sp2_destroy(sp2_handle_t h) {
+    if (!h) return SP2_ERR_INVALID_ARG;
+    for (auto& kv : h->graphs) {
+        if (kv.second.exec) cudaGraphExecDestroy(kv.second.exec);
+        if (kv.second.graph) cudaGraphDestroy(kv.second.graph);
+    }
+    if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
+    cudaFree(h->S);
+    for (int a = 0; a < 2; ++a)
+        for (int b = 0; b < 2; ++b) cudaFree(h->hl[a][b]);
+    cudaFree(h->R); cudaFree(h->diag); cudaFree(h->ctrl); cudaFree(h->stats_dev); cudaFree(h->thetas_dev);
+    cudaFree(h->tiles_dev); cudaFree(h->bstats_dev); cudaFree(h->bnl_dev); cudaFree(h->bstatus_dev);
+    cudaFree(h->bbounds_dev); cudaFree(h->bnocc_dev);
+    cudaFreeHost(h->ctrl_host); cudaFreeHost(h->stats_host); cudaFreeHost(h->thetas_host);
+    cudaFreeHost(h->bounds_host); cudaFree(h->stage_H); cudaFree(h->stage_D);
+    delete h;
+    return SP2_OK;
+}
+
+extern "C" sp2_status_t sp2_create(sp2_handle_t* out, int N_max, int batch_max, int max_layers) {
+    if (!out || N_max < 1 || batch_max < 0 || max_layers < 1 || max_layers > 4096) return SP2_ERR_INVALID_ARG;
+    if (batch_max > 0 && N_max > 256 && batch_max > 1) { /* batched problems are limited to N <= 256, checked per call */ }
+    int dev = 0;
+    CK(cudaGetDevice(&dev));
+    cudaDeviceProp prop;
+    CK(cudaGetDeviceProperties(&prop, dev));
+    if (prop.major != 10) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "device is sm_%d%d; this library is built for sm_100a only", prop.major,
+                 prop.minor);
+        return SP2_ERR_CUDA;
+    }
+    sp2_handle_s* h = new sp2_handle_s();
+    h->N_max = N_max; h->batch_max = batch_max; h->max_layers = max_layers;
+    h->Np_max = round_up(N_max, 256);
+    h->num_sms = prop.multiProcessorCount; h->device = dev;
+    const size_t Np = (size_t)h->Np_max;
+    sp2_status_t st = SP2_OK;
+    auto A = [&](void** p, size_t bytes) {
+        if (st != SP2_OK) return;
+        cudaError_t e = cudaMalloc(p, bytes);
+        if (e != cudaSuccess) st = cuda_fail(e, "cudaMalloc(workspace)");
+    };
+    A((void**)&h->S, Np * Np * 4);
+    for (int a = 0; a < 2; ++a)
+        for (int b = 0; b < 2; ++b) A((void**)&h->hl[a][b], Np * Np * 2);
+    A((void**)&h->R, Np * sizeof(double));
+    A((void**)&h->diag, Np * sizeof(double));
+    A((void**)&h->ctrl, sizeof(Ctrl));
+    A((void**)&h->stats_dev, (size_t)max_layers * sizeof(sp2_layer_stat_t));
+    A((void**)&h->thetas_dev, (size_t)max_layers * 3 * sizeof(double));
+    h->tiles_cap = (int)((Np / 128) * (Np / 128 + 1) / 2);
+    A((void**)&h->tiles_dev, (size_t)h->tiles_cap * sizeof(int2));
+    if (batch_max > 0) {
+        A((void**)&h->bstats_dev, (size_t)batch_max * max_layers * sizeof(sp2_layer_stat_t));
+        A((void**)&h->bnl_dev, (size_t)batch_max * sizeof(int));
+        A((void**)&h->bstatus_dev, (size_t)batch_max * sizeof(int));
+        A((void**)&h->bbounds_dev, (size_t)batch_max * 2 * sizeof(double));
+        A((void**)&h->bnocc_dev, (size_t)batch_max * sizeof(double));
+    }
+    auto AH = [&](void** p, size_t bytes) {
+        if (st != SP2_OK) return;
+        cudaError_t e = cudaMallocHost(p, bytes);
+        if (e != cudaSuccess) st = cuda_fail(e, "cudaMallocHost");
+    };
+    AH((void**)&h->ctrl_host, sizeof(Ctrl));
+    AH((void**)&h->stats_host, (size_t)max_layers * sizeof(sp2_layer_stat_t));
+    AH((void**)&h->thetas_host, (size_t)max_layers * 3 * sizeof(double));
+    AH((void**)&h->bounds_host, 2 * sizeof(double));
+    if (st == SP2_OK) {
+        cudaError_t e = cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking);
+        if (e != cudaSuccess) st = cuda_fail(e, "cudaStreamCreate");
+    }
+    if (st == SP2_OK) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+        if (e != cudaSuccess || qres != cudaDriverEntryPointSuccess || !fn)
+            st = cuda_fail(e == cudaSuccess ? cudaErrorUnknown : e, "cudaGetDriverEntryPoint(cuTensorMapEncodeTiled)");
+        h->encode = (PFN_encodeTiled)fn;
+    }
+    for (int cfg = TILE_128x128; cfg <= TILE_256x256_PAIR && st == SP2_OK; ++cfg) {
+        cudaError_t e = layer_kernel_setup(cfg);
+        if (e != cudaSuccess) st = cuda_fail(e, "cudaFuncSetAttribute(layer kernel)");
+    }
+    if (st == SP2_OK) {
+        cudaError_t e = resident_kernel_setup();
+        if (e != cudaSuccess) st = cuda_fail(e, "cudaFuncSetAttribute(resident kernel)");
+    }
+    if (st != SP2_OK) { sp2_destroy(h); return st; }
+    *out = h;
+    return SP2_OK;
+}
+
+// K-major FP16 operand map: Np x Np row-major, box = 64 (K) x 128 (rows), 128-byte swizzle.
+static sp2_status_t make_tmap(sp2_handle_s* h, CUtensorMap* tm, void* base, int Np) {
+    cuuint64_t gdim[2] = {(cuuint64_t)Np, (cuuint64_t)Np};
+    cuuint64_t gstr[1] = {(cuuint64_t)Np * 2};
+    cuuint32_t box[2] = {64, 128};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = h->encode(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, base, gdim, gstr, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "cuTensorMapEncodeTiled failed: %d", (int)r);
+        return SP2_ERR_CUDA;
+    }
+    return SP2_OK;
+}
+
+// Supertile launch order over the lower triangle: bands of `band` supertile rows, column-major inside a band, so
+// that the CTAs resident at the same time share few row panels (L2 reuse of the operands).
+static void build_tile_order(int nt, int band, std::vector<int2>& out) {
+    out.clear();
+    for (int i0 = 0; i0 < nt; i0 += band) {
+        const int i1 = (i0 + band < nt) ? i0 + band : nt;
+        for (int j = 0; j < i1; ++j)
+            for (int i = (j > i0 ? j : i0); i < i1; ++i) out.push_back(make_int2(i, j));
+    }
+}
+
+static int choose_tile_config(int N, int requested, int num_sms) {
+    if (requested >= TILE_128x128 && requested <= TILE_256x256_PAIR) return requested;
+    const int n128 = round_up(N, 128) / 128;
+    const long long t128 = (long long)n128 * (n128 + 1) / 2;
+    // enough 256x256 supertiles to keep every CTA pair busy for several waves -> paired 256x256 tiles
+    const int n256 = round_up(N, 256) / 256;
+    const long long t256 = (long long)n256 * (n256 + 1) / 2;
+    if (t256 >= 4LL * (num_sms / 2)) return TILE_256x256_PAIR;
+    (void)t128;
+    return TILE_128x128;
+}
+
+struct Problem {
+    int N, Np, cfg, scale_log2, n_super;
+    float scale, inv_scale2;
+};
+
+static sp2_status_t prepare_problem(sp2_handle_s* h, int N, const sp2_opts_t* o, Problem* pb, cudaStream_t st) {
+    pb->N = N;
+    pb->cfg = choose_tile_config(N, o ? o->tile_config : 0, h->num_sms);
+    const int edge = tile_super_edge(pb->cfg);
+    pb->Np = round_up(N, edge);
+    if (pb->Np > h->Np_max) return SP2_ERR_WORKSPACE;
+    int k = o ? o->fp16_scale_log2 : -1;
+    if (k < 0) k = 13;
+    if (k > 14) return SP2_ERR_INVALID_ARG;
+    pb->scale_log2 = k;
+    pb->scale = ldexpf(1.0f, k);
+    pb->inv_scale2 = ldexpf(1.0f, -2 * k);
+    const int nt = pb->Np / edge;
+    const int band = (pb->cfg == TILE_256x256_PAIR) ? 8 : 12;
+    if (h->tiles_key_nt != nt || h->tiles_key_band != band) {
+        std::vector<int2> order;
+        build_tile_order(nt, band, order);
+        if ((int)order.size() > h->tiles_cap) return SP2_ERR_WORKSPACE;
+        // synchronous small copy: happens only when the problem shape changes
+        CK(cudaMemcpyAsync(h->tiles_dev, order.data(), order.size() * sizeof(int2), cudaMemcpyHostToDevice, st));
+        CK(cudaStreamSynchronize(st));
+        h->tiles_key_nt = nt; h->tiles_key_band = band;
+        h->n_super = (int)order.size();
+    }
+    pb->n_super = h->n_super;
+    return SP2_OK;
+}
+
+static LayerParams layer_params(sp2_handle_s* h, const Problem& pb, int parity, unsigned long long cond) {
+    LayerParams p;
+    p.ctrl = h->ctrl; p.stats = h->stats_dev; p.thetas = h->thetas_dev; p.S = h->S;
+    p.hi_out = h->hl[parity ^ 1][0]; p.lo_out = h->hl[parity ^ 1][1];
+    p.tiles = h->tiles_dev; p.ld = pb.Np; p.N = pb.N; p.Np = pb.Np; p.n_super = pb.n_super;
+    p.scale = pb.scale; p.inv_scale2 = pb.inv_scale2; p.cond_handle = cond;
+    return p;
+}
+
+static sp2_status_t launch_one_layer(sp2_handle_s* h, const Problem& pb, int parity, unsigned long long cond,
+                                     cudaStream_t st) {
+    CUtensorMap tm_hi, tm_lo;
+    sp2_status_t s = make_tmap(h, &tm_hi, h->hl[parity][0], pb.Np);
+    if (s != SP2_OK) return s;
+    s = make_tmap(h, &tm_lo, h->hl[parity][1], pb.Np);
+    if (s != SP2_OK) return s;
+    LayerParams p = layer_params(h, pb, parity, cond);
+    CK(launch_layer(pb.cfg, tm_hi, tm_lo, p, h->num_sms, st));
+    return SP2_OK;
+}
+
+// WHILE(ctrl->running) { layer(ping -> pong); layer(pong -> ping); } as a CUDA graph with a conditional node; the
+// condition is set on the device by the last CTA of each layer kernel (cudaGraphSetConditional).
+static sp2_status_t get_loop_graph(sp2_handle_s* h, const Problem& pb, LoopGraph** out) {
+    auto key = std::make_tuple(pb.N, pb.Np, pb.cfg, pb.scale_log2);
+    auto it = h->graphs.find(key);
+    if (it != h->graphs.end()) { *out = &it->second; return SP2_OK; }
+    LoopGraph lg;
+    CK(cudaGraphCreate(&lg.graph, 0));
+    cudaGraphConditionalHandle handle;
+    CK(cudaGraphConditionalHandleCreate(&handle, lg.graph, 1, cudaGraphCondAssignDefault));
+    cudaGraphNodeParams np = {cudaGraphNodeTypeConditional};
+    np.type = cudaGraphNodeTypeConditional;
+    np.conditional.handle = handle;
+    np.conditional.type = cudaGraphCondTypeWhile;
+    np.conditional.size = 1;
+    cudaGraphNode_t node;
+    CK(cudaGraphAddNode(&node, lg.graph, nullptr, 0, &np));
+    cudaGraph_t body = np.conditional.phGraph_out[0];
+    CK(cudaStreamBeginCaptureToGraph(h->cap_stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed));
+    sp2_status_t s = launch_one_layer(h, pb, 0, (unsigned long long)handle, h->cap_stream);
+    if (s == SP2_OK) s = launch_one_layer(h, pb, 1, (unsigned long long)handle, h->cap_stream);
+    cudaGraph_t captured = nullptr;
+    cudaError_t e = cudaStreamEndCapture(h->cap_stream, &captured);
+    if (s != SP2_OK) { cudaGraphDestroy(lg.graph); return s; }
+    if (e != cudaSuccess) { cudaGraphDestroy(lg.graph); return cuda_fail(e, "cudaStreamEndCapture"); }
+    e = cudaGraphInstantiate(&lg.exec, lg.graph, 0);
+    if (e != cudaSuccess) { cudaGraphDestroy(lg.graph); return cuda_fail(e, "cudaGraphInstantiate"); }
+    auto ins = h->graphs.emplace(key, lg);
+    *out = &ins.first->second;
+    return SP2_OK;
+}
+
+static sp2_status_t check_common(sp2_handle_s* h, const void* in, int N, int ldin, const void* outp, int ldout) {
+    if (!h || !in || !outp || N < 1 || ldin < N || ldout < N) return SP2_ERR_INVALID_ARG;
+    if (N > h->N_max) return SP2_ERR_WORKSPACE;
+    return SP2_OK;
+}
+
+// Shared body of the single-matrix solves.  mode = MODE_STANDARD or MODE_GENERALIZED (thetas already in
+// h->thetas_host[0..3L)).
+static sp2_status_t solve_single(sp2_handle_s* h, const float* H_dev, int N, int ldh, double N_occ, int mode,
+                                 const sp2_opts_t* o, float* D_dev, int ldd, sp2_layer_stat_t* stats_out,
+                                 int* n_layers_out, double bounds_out[2], cudaStream_t st) {
+    Problem pb;
+    sp2_status_t s = prepare_problem(h, N, o, &pb, st);
+    if (s != SP2_OK) return s;
+    const int max_layers = o->max_layers;
+    // ---- control block
+    Ctrl* c = h->ctrl_host;
+    memset(c, 0, ctrl_header_bytes());
+    c->N_occ = N_occ; c->eps_alt = o->eps_alt; c->tol = o->tol;
+    c->eps_min = o->eps_min; c->eps_max = o->eps_max;
+    c->N = N; c->mode = mode; c->max_layers = max_layers; c->auto_bounds = o->auto_bounds;
+    CK(cudaMemcpyAsync(h->ctrl, c, ctrl_header_bytes(), cudaMemcpyHostToDevice, st));
+    if (mode == MODE_GENERALIZED)
+        CK(cudaMemcpyAsync(h->thetas_dev, h->thetas_host, (size_t)max_layers * 3 * sizeof(double),
+                           cudaMemcpyHostToDevice, st));
+    CK(cudaMemsetAsync(h->stats_dev, 0, (size_t)max_layers * sizeof(sp2_layer_stat_t), st));
+    // ---- padding rows/columns of S_0 are zero (inert: eigenvalue 0 is a fixed point of both branches)
+    const size_t NpNp = (size_t)pb.Np * pb.Np;
+    if (pb.Np != N) {
+        CK(cudaMemsetAsync(h->S, 0, NpNp * 4, st));
+        CK(cudaMemsetAsync(h->hl[0][0], 0, NpNp * 2, st));
+        CK(cudaMemsetAsync(h->hl[0][1], 0, NpNp * 2, st));
+    }
+    // ---- a1: bounds, a2: initial affine layer + first split + first control step
+    if (o->auto_bounds) CK(launch_gershgorin(H_dev, N, ldh, h->R, h->diag, h->ctrl, nullptr, h->num_sms, st));
+    CK(launch_affine_split(H_dev, N, ldh, h->S, h->hl[0][0], h->hl[0][1], pb.Np, pb.scale, h->ctrl, h->stats_dev,
+                           h->thetas_dev, h->num_sms, st));
+    // ---- a4-a8: the layer loop
+    if (o->control == 0) {
+        LoopGraph* lg = nullptr;
+        s = get_loop_graph(h, pb, &lg);
+        if (s != SP2_OK) return s;
+        CK(cudaGraphLaunch(lg->exec, st));
+    } else if (o->control == 1) {
+        for (int n = 0; n < max_layers; ++n) {
+            CK(cudaMemcpyAsync(&h->ctrl_host->running, &h->ctrl->running, sizeof(int), cudaMemcpyDeviceToHost, st));
+            CK(cudaStreamSynchronize(st));
+            if (!h->ctrl_host->running) break;
+            s = launch_one_layer(h, pb, n & 1, 0, st);
+            if (s != SP2_OK) return s;
+        }
+    } else {
+        for (int n = 0; n < max_layers; ++n) {
+            s = launch_one_layer(h, pb, n & 1, 0, st);
+            if (s != SP2_OK) return s;
+        }
+    }
+    // ---- results
+    CK(cudaMemcpy2DAsync(D_dev, (size_t)ldd * 4, h->S, (size_t)pb.Np * 4, (size_t)N * 4, (size_t)N,
+                         cudaMemcpyDeviceToDevice, st));
+    CK(cudaMemcpyAsync(h->ctrl_host, h->ctrl, ctrl_header_bytes(), cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(h->stats_host, h->stats_dev, (size_t)max_layers * sizeof(sp2_layer_stat_t),
+                       cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    CK(cudaGetLastError());
+    c = h->ctrl_host;
+    h->last_launches = c->launches;
+    if (bounds_out) { bounds_out[0] = c->eps_min; bounds_out[1] = c->eps_max; }
+    if (n_layers_out) *n_layers_out = c->n;
+    if (stats_out) memcpy(stats_out, h->stats_host, (size_t)(c->n < max_layers ? c->n : max_layers) * sizeof(sp2_layer_stat_t));
+    if (c->error < 0) return (sp2_status_t)c->error;
+    if (c->running) return SP2_ERR_CUDA;     // loop ended while the device still wanted layers: should not happen
+    if (mode == MODE_STANDARD && c->stop_reason == SP2_STOP_MAX_LAYERS) return SP2_NOT_CONVERGED;
+    return SP2_OK;
+}
+
+extern "C" sp2_status_t sp2_density_matrix(sp2_handle_t h, const float* H_dev, int N, int ldh, double N_occ,
+                                           const sp2_opts_t* opts, float* D_dev, int ldd,
+                                           sp2_layer_stat_t* stats_host, int* n_layers, double bounds_out[2],
+                                           void* stream) {
+    sp2_status_t s = check_common(h, H_dev, N, ldh, D_dev, ldd);
+    if (s != SP2_OK) return s;
+    sp2_opts_t o;
+    if (opts) o = *opts; else sp2_default_opts(&o);
+    if (!(N_occ >= 0.0 && N_occ <= (double)N)) return SP2_ERR_INVALID_ARG;
+    if (o.max_layers < 1 || o.max_layers > h->max_layers) return SP2_ERR_INVALID_ARG;
+    if (!o.auto_bounds) {
+        if (!isfinite(o.eps_min) || !isfinite(o.eps_max)) return SP2_ERR_INVALID_ARG;
+        if (!(o.eps_max > o.eps_min)) return SP2_ERR_BOUNDS_DEGENERATE;
+    }
+    return solve_single(h, H_dev, N, ldh, N_occ, MODE_STANDARD, &o, D_dev, ldd, stats_host, n_layers, bounds_out,
+                        (cudaStream_t)stream);
+}
+
+extern "C" sp2_status_t sp2_density_matrix_host(sp2_handle_t h, const float* H_host, int N, int ldh, double N_occ,
+                                                const sp2_opts_t* opts, float* D_host, int ldd,
+                                                sp2_layer_stat_t* stats_host, int* n_layers, double bounds_out[2],
+                                                void* stream) {
+    sp2_status_t s = check_common(h, H_host, N, ldh, D_host, ldd);
+    if (s != SP2_OK) return s;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t elems = (size_t)N * N;
+    if (h->stage_elems < elems) {
+        cudaFree(h->stage_H); cudaFree(h->stage_D);
+        h->stage_H = h->stage_D = nullptr; h->stage_elems = 0;
+        CK(cudaMalloc((void**)&h->stage_H, elems * 4));
+        CK(cudaMalloc((void**)&h->stage_D, elems * 4));
+        h->stage_elems = elems;
+    }
+    CK(cudaMemcpy2DAsync(h->stage_H, (size_t)N * 4, H_host, (size_t)ldh * 4, (size_t)N * 4, (size_t)N,
+                         cudaMemcpyHostToDevice, st));
+    s = sp2_density_matrix(h, h->stage_H, N, N, N_occ, opts, h->stage_D, N, stats_host, n_layers, bounds_out, stream);
+    if (s < 0) return s;
+    CK(cudaMemcpy2DAsync(D_host, (size_t)ldd * 4, h->stage_D, (size_t)N * 4, (size_t)N * 4, (size_t)N,
+                         cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return s;
+}
+
+extern "C" sp2_status_t sp2_generalized(sp2_handle_t h, const float* H_dev, int N, int ldh, const double* theta_host,
+                                        int L, double eps_min, double eps_max, const sp2_opts_t* opts, float* X_L_dev,
+                                        int ldx, sp2_layer_stat_t* stats_host, void* stream) {
+    sp2_status_t s = check_common(h, H_dev, N, ldh, X_L_dev, ldx);
+    if (s != SP2_OK) return s;
+    if (!theta_host || L < 1 || L > h->max_layers) return SP2_ERR_INVALID_ARG;
+    sp2_opts_t o;
+    if (opts) o = *opts; else sp2_default_opts(&o);
+    o.max_layers = L;
+    o.tol = 0.0;
+    o.eps_alt = 0.0;
+    o.auto_bounds = !(eps_max > eps_min);
+    o.eps_min = eps_min; o.eps_max = eps_max;
+    if (!o.auto_bounds && (!isfinite(eps_min) || !isfinite(eps_max))) return SP2_ERR_INVALID_ARG;
+    for (int i = 0; i < 3 * L; ++i) {
+        if (!isfinite(theta_host[i])) return SP2_ERR_INVALID_ARG;
+        h->thetas_host[i] = theta_host[i];
+    }
+    int nl = 0;
+    return solve_single(h, H_dev, N, ldh, 0.0, MODE_GENERALIZED, &o, X_L_dev, ldx, stats_host, &nl, nullptr,
+                        (cudaStream_t)stream);
+}
+
+extern "C" sp2_status_t sp2_generalized_wb(sp2_handle_t h, const float* H_dev, int N, int ldh, const int* sigma,
+                                           const double* weights, const double* biases, int L, double eps_min,
+                                           double eps_max, const sp2_opts_t* opts, float* X_L_dev, int ldx,
+                                           sp2_layer_stat_t* stats_host, void* stream) {
+    if (!h || !weights || !biases || L < 1 || L > h->max_layers) return SP2_ERR_INVALID_ARG;
+    std::vector<double> th((size_t)3 * L);
+    for (int n = 0; n < L; ++n) {
+        const int sg = sigma ? sigma[n] : 1;
+        if (sg != 1 && sg != -1) return SP2_ERR_INVALID_ARG;
+        th[3 * n + 0] = weights[n] * sg;           // theta_1 = w sigma
+        th[3 * n + 1] = weights[n] * (1 - sg);     // theta_2 = w (1 - sigma)
+        th[3 * n + 2] = biases[n];                 // theta_3 = b
+    }
+    return sp2_generalized(h, H_dev, N, ldh, th.data(), L, eps_min, eps_max, opts, X_L_dev, ldx, stats_host, stream);
+}
+
+extern "C" sp2_status_t sp2_density_matrix_batched(sp2_handle_t h, const float* H_dev, int N, int B,
+                                                   const double* N_occ, int nocc_is_scalar, const sp2_opts_t* opts,
+                                                   float* D_dev, sp2_layer_stat_t* stats_host, int* n_layers,
+                                                   int* status_out, void* stream) {
+    if (!h || !H_dev || !D_dev || !N_occ || N < 1 || B < 1) return SP2_ERR_INVALID_ARG;
+    if (N > 256) return SP2_ERR_UNSUPPORTED_N;
+    if (B > h->batch_max) return SP2_ERR_WORKSPACE;
+    sp2_opts_t o;
+    if (opts) o = *opts; else sp2_default_opts(&o);
+    if (o.max_layers < 1 || o.max_layers > h->max_layers) return SP2_ERR_INVALID_ARG;
+    if (!o.auto_bounds && !(o.eps_max > o.eps_min)) return SP2_ERR_BOUNDS_DEGENERATE;
+    for (int i = 0; i < (nocc_is_scalar ? 1 : B); ++i)
+        if (!(N_occ[i] >= 0.0 && N_occ[i] <= (double)N)) return SP2_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    int k = o.fp16_scale_log2;
+    if (k < 0) k = 13;
+    if (k > 14) return SP2_ERR_INVALID_ARG;
+    CK(cudaMemcpyAsync(h->bnocc_dev, N_occ, (size_t)(nocc_is_scalar ? 1 : B) * sizeof(double), cudaMemcpyHostToDevice, st));
+    CK(cudaMemsetAsync(h->bstats_dev, 0, (size_t)B * o.max_layers * sizeof(sp2_layer_stat_t), st));
+    ResidentParams p;
+    memset(&p, 0, sizeof(p));
+    p.H = H_dev; p.D = D_dev; p.N_occ = h->bnocc_dev; p.nocc_is_scalar = nocc_is_scalar; p.N = N; p.B = B;
+    p.auto_bounds = o.auto_bounds; p.eps_min = o.eps_min; p.eps_max = o.eps_max; p.tol = o.tol; p.eps_alt = o.eps_alt;
+    p.max_layers = o.max_layers; p.mode = MODE_STANDARD; p.thetas = nullptr;
+    p.scale = ldexpf(1.0f, k); p.inv_scale2 = ldexpf(1.0f, -2 * k);
+    p.stats = h->bstats_dev; p.n_layers = h->bnl_dev; p.status = h->bstatus_dev; p.bounds = h->bbounds_dev;
+    CK(launch_resident(p, h->num_sms, st));
+    std::vector<int> nl((size_t)B), stt((size_t)B);
+    CK(cudaMemcpyAsync(nl.data(), h->bnl_dev, (size_t)B * sizeof(int), cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(stt.data(), h->bstatus_dev, (size_t)B * sizeof(int), cudaMemcpyDeviceToHost, st));
+    if (stats_host)
+        CK(cudaMemcpyAsync(stats_host, h->bstats_dev, (size_t)B * o.max_layers * sizeof(sp2_layer_stat_t),
+                           cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    CK(cudaGetLastError());
+    h->last_launches = 1;
+    int worst = SP2_OK;
+    for (int i = 0; i < B; ++i) {
+        if (n_layers) n_layers[i] = nl[i];
+        if (status_out) status_out[i] = stt[i];
+        if (stt[i] < 0) { if (worst >= 0 || stt[i] < worst) worst = stt[i]; }
+        else if (stt[i] > worst && worst >= 0) worst = stt[i];
+    }
+    return (sp2_status_t)worst;
+}
+
+extern "C" sp2_status_t sp2_split_fp16(const float* X_dev, int N, int ldx, unsigned short* hi_dev,
+                                       unsigned short* lo_dev, int ldo, int fp16_scale_log2, void* stream) {
+    if (!X_dev || !hi_dev || !lo_dev || N < 1 || ldx < N || ldo < N) return SP2_ERR_INVALID_ARG;
+    if (fp16_scale_log2 < 0 || fp16_scale_log2 > 14) return SP2_ERR_INVALID_ARG;
+    int dev = 0, sms = 0;
+    CK(cudaGetDevice(&dev));
+    CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    CK(launch_split(X_dev, N, ldx, (__half*)hi_dev, (__half*)lo_dev, ldo, ldexpf(1.0f, fp16_scale_log2), sms,
+                    (cudaStream_t)stream));
+    return SP2_OK;
+}
+
+extern "C" sp2_status_t sp2_gershgorin(sp2_handle_t h, const float* H_dev, int N, int ldh, double bounds_host[2],
+                                       void* stream) {
+    if (!h || !H_dev || !bounds_host || N < 1 || ldh < N) return SP2_ERR_INVALID_ARG;
+    if (N > h->N_max) return SP2_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    CK(launch_gershgorin(H_dev, N, ldh, h->R, h->diag, h->ctrl, nullptr, h->num_sms, st));
+    CK(cudaMemcpyAsync(h->bounds_host, &h->ctrl->eps_min, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    bounds_host[0] = h->bounds_host[0];
+    bounds_host[1] = h->bounds_host[1];
+    return SP2_OK;
+}
+
+extern "C" int sp2_last_launch_count(sp2_handle_t h) { return h ? h->last_launches : 0; }

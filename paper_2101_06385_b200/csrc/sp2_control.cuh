@@ -1,0 +1,109 @@
+// Device-side branch and convergence control of Alg. 1 (stop rule P:186-190, Thm 1).
+// One Ctrl block per problem lives in device memory; the last CTA of each layer kernel calls
+// control_after_layer(), so no scalar crosses to the host between layers.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "../../include/sp2_b200.h"
+
+namespace sp2 {
+
+constexpr int kMaxPartials = 1024;   // per-CTA FP64 partial slots (>= largest grid of a layer kernel)
+
+enum { MODE_STANDARD = 0, MODE_GENERALIZED = 1 };
+
+struct Ctrl {
+    // ---- problem constants (written by the host before launch)
+    double N_occ, eps_alt, tol;
+    double eps_min, eps_max;         // spectral bounds (given, or written by the Gershgorin kernel)
+    int    N, mode, max_layers, auto_bounds;
+    // ---- state
+    int    n;                        // layers applied so far
+    int    running;                  // 1 while another layer has to run
+    int    stop_reason;              // SP2_STOP_* once finished
+    int    pending_stop;             // stop test of the layer in flight already fired (applied after it)
+    int    sigma_prev, sigma_prev2;  // sigma_{n}, sigma_{n-1} of applied layers
+    int    error;                    // sp2_status_t < 0 raised on the device
+    int    launches;                 // kernels that did work (for sp2_last_launch_count)
+    double N_S;                      // Tr S_n (measured)
+    double fro2;                     // ||S_n||_F^2 = N_X of layer n+1
+    double iderr_prev, iderr_prev2;  // IdErr_n, IdErr_{n-1}
+    float  theta[4];                 // th1, th2, th3 of the NEXT layer (FP32: the epilogue's arithmetic type)
+    unsigned int done_counter;       // CTAs finished in the current kernel
+    unsigned int pad_;
+    double partial[kMaxPartials][4]; // per-CTA {Tr S, ||S||_F^2, Tr X (diag), unused}
+};
+
+// Decide layer n+1 from N_S = Tr S_n and N_X = ||S_n||_F^2, exactly in Alg. 1's order:
+// IdErr, sigma, (W_n, B_n) -> theta, stop tests.  The stop tests belong to layer n+1 and take effect after
+// that layer has been applied (reading C1 of DESIGN.md).  thetas = per-layer [L][3] list in generalized mode.
+__device__ inline void control_plan_next(Ctrl* c, sp2_layer_stat_t* stats, const double* thetas) {
+    const int m = c->n + 1;                      // layer about to run
+    if (c->mode == MODE_GENERALIZED) {
+        if (c->n >= c->max_layers) { c->running = 0; c->stop_reason = SP2_STOP_MAX_LAYERS; return; }
+        c->theta[0] = (float)thetas[3 * c->n + 0];
+        c->theta[1] = (float)thetas[3 * c->n + 1];
+        c->theta[2] = (float)thetas[3 * c->n + 2];
+        stats[m - 1].trace_X = c->fro2;
+        stats[m - 1].iderr = c->N_S - c->fro2;
+        stats[m - 1].sigma = 0;
+        stats[m - 1].stop_reason = (m == c->max_layers) ? SP2_STOP_MAX_LAYERS : SP2_STOP_NONE;
+        c->running = 1;
+        return;
+    }
+    const double N_S = c->N_S, N_X = c->fro2, N_occ = c->N_occ;
+    const double iderr = N_S - N_X;                                            // IdErr_m
+    const double d = fabs(2.0 * N_S - N_X - N_occ) - fabs(N_X - N_occ) - (double)c->sigma_prev * c->eps_alt;
+    int sigma;
+    if (d > 0.0) sigma = 1;
+    else if (d < 0.0) sigma = -1;
+    else sigma = (c->sigma_prev != 0) ? -c->sigma_prev : 1;                   // Sign(0): alternate (C4)
+    if (!(isfinite(N_S) && isfinite(N_X))) {
+        c->running = 0; c->stop_reason = SP2_STOP_NONFINITE; c->error = SP2_ERR_NONFINITE;
+        return;
+    }
+    c->theta[0] = (float)sigma;            // W_m = sigma I
+    c->theta[1] = (float)(1 - sigma);      // B_m = (I - W_m) S_{m-1}
+    c->theta[2] = 0.0f;
+    int pend = SP2_STOP_NONE;
+    if (iderr <= 0.0) pend = SP2_STOP_IDERR_NONPOS;
+    else if (m > 2 && c->sigma_prev != c->sigma_prev2 && iderr > 4.5 * c->iderr_prev2 * c->iderr_prev2)
+        pend = SP2_STOP_PARAM_FREE;        // sigma_{m-1} != sigma_{m-2} and IdErr_m > 4.5 IdErr_{m-2}^2
+    else if (c->tol > 0.0 && iderr <= c->tol) pend = SP2_STOP_TOL;
+    else if (m >= c->max_layers) pend = SP2_STOP_MAX_LAYERS;
+    c->pending_stop = pend;
+    stats[m - 1].trace_X = N_X;
+    stats[m - 1].iderr = iderr;
+    stats[m - 1].sigma = sigma;
+    stats[m - 1].stop_reason = pend;
+    c->sigma_prev2 = c->sigma_prev;
+    c->sigma_prev = sigma;
+    c->iderr_prev2 = c->iderr_prev;
+    c->iderr_prev = iderr;
+    c->running = 1;
+}
+
+// Called by ONE thread once every CTA of the layer kernel has published its partial sums.
+__device__ inline void control_after_layer(Ctrl* c, sp2_layer_stat_t* stats, const double* thetas, int n_partials) {
+    double trS = 0.0, fro2 = 0.0, trX = 0.0;
+    for (int i = 0; i < n_partials; ++i) {       // fixed order: deterministic for a static tile schedule
+        trS += c->partial[i][0];
+        fro2 += c->partial[i][1];
+        trX += c->partial[i][2];
+    }
+    c->n += 1;
+    c->launches += 1;
+    c->N_S = trS;
+    c->fro2 = fro2;
+    stats[c->n - 1].trace_S = trS;
+    stats[c->n - 1].trace_X_diag = trX;
+    c->done_counter = 0;
+    if (c->mode == MODE_STANDARD && c->pending_stop != SP2_STOP_NONE) {
+        c->running = 0;
+        c->stop_reason = c->pending_stop;
+        return;
+    }
+    control_plan_next(c, stats, thetas);
+}
+
+}  // namespace sp2

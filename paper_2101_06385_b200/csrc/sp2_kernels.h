@@ -1,0 +1,70 @@
+// Internal declarations shared by the .cu files of libsp2b200.so (not part of the C ABI).
+#pragma once
+#include <cuda.h>
+#include <cuda_fp16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "../../include/sp2_b200.h"
+#include "sp2_control.cuh"
+
+namespace sp2 {
+
+// ---- HBM-bound kernels (sp2_elementwise.cu)
+cudaError_t launch_gershgorin(const float* H, int N, long long ldh, double* R, double* diag, Ctrl* ctrl,
+                              double* bounds_out, int num_sms, cudaStream_t st);
+cudaError_t launch_affine_split(const float* H, int N, long long ldh, float* S, __half* hi, __half* lo, long long ld,
+                                float scale, Ctrl* ctrl, sp2_layer_stat_t* stats, const double* thetas, int num_sms,
+                                cudaStream_t st);
+cudaError_t launch_split(const float* X, int N, long long ldx, __half* hi, __half* lo, long long ldo, float scale,
+                         int num_sms, cudaStream_t st);
+
+// ---- fused symmetric square layer (sp2_square_tiled.cu)
+enum TileConfig { TILE_AUTO = 0, TILE_128x128 = 1, TILE_128x256 = 2, TILE_256x256_PAIR = 3 };
+
+struct LayerParams {
+    Ctrl* ctrl;
+    sp2_layer_stat_t* stats;
+    const double* thetas;          // generalized mode: [L][3] on the device
+    float* S;                      // FP32 master, Np x Np, updated in place
+    __half* hi_out;                // next layer's operands (the other ping-pong pair)
+    __half* lo_out;
+    const int2* tiles;             // supertile list (I, J), I >= J, in launch order
+    long long ld;                  // = Np
+    int N, Np;
+    int n_super;                   // number of supertiles
+    float scale;                   // c = 2^k of the split
+    float inv_scale2;              // 1 / c^2
+    unsigned long long cond_handle;  // cudaGraphConditionalHandle (0 = none)
+};
+
+// Supertile edge for a tile configuration (128 or 256) and CTAs launched per supertile-slot.
+int tile_super_edge(int cfg);
+size_t tile_smem_bytes(int cfg);
+// Launch one layer: reads hi/lo through the tensor maps (K-major, 128B swizzle, box 64 x 128), writes S, hi_out, lo_out.
+cudaError_t launch_layer(int cfg, const CUtensorMap& tm_hi, const CUtensorMap& tm_lo, const LayerParams& p,
+                         int num_sms, cudaStream_t st);
+cudaError_t layer_kernel_setup(int cfg);   // cudaFuncSetAttribute(max dynamic smem), once per process
+
+// ---- resident small-N kernel (sp2_resident.cu): whole solve in one launch, one CTA (pair) per matrix
+struct ResidentParams {
+    const float* H;                // [B][N][N]
+    float* D;                      // [B][N][N]
+    const double* N_occ;           // [B] or [1]
+    int nocc_is_scalar;
+    int N, B;
+    int auto_bounds;
+    double eps_min, eps_max, tol, eps_alt;
+    int max_layers;
+    int mode;                      // MODE_STANDARD / MODE_GENERALIZED
+    const double* thetas;          // generalized: [L][3]
+    float scale, inv_scale2;
+    sp2_layer_stat_t* stats;       // [B][max_layers] (device)
+    int* n_layers;                 // [B]
+    int* status;                   // [B]
+    double* bounds;                // [B][2]
+};
+cudaError_t resident_kernel_setup();
+cudaError_t launch_resident(const ResidentParams& p, int num_sms, cudaStream_t st);
+size_t resident_smem_bytes(int N);
+
+}  // namespace sp2

@@ -1,0 +1,364 @@
+// Fused symmetric-square layer of the SP2 network (rows a4-a8 of DESIGN.md) for sm_100a.
+//
+// One launch = one layer of Alg. 1 with Alg. 2 as the activation:
+//   acc(I,J) = sum_k  hi[I,k] hi[J,k] + hi[I,k] lo[J,k] + lo[I,k] hi[J,k]       (Eq. 15; X symmetric so the
+//                                                                              transpose term is lo[I,:] . hi[J,:])
+//   S_n      = th1 acc / c^2 + th2 S_{n-1} + th3 I                              (Alg. 1's W_n, B_n; Eq. 17)
+//   epilogue: Tr S_n, ||S_n||_F^2 (= next layer's N_X), Tr X_n in FP64; next layer's hi/lo (Eqs. 12-13);
+//   last CTA: sigma_{n+1}, IdErr_{n+1}, stop tests (control_after_layer).
+// Only lower-triangle tiles (I >= J) are computed; every value is also stored at its mirrored position, so
+// S, hi, lo stay exactly symmetric and the next layer can read full row panels as K-major operands.
+//
+// Structure: persistent CTAs (or CTA pairs), static round-robin over a host-ordered supertile list;
+// warp 0 = TMA producer, warp 1 = tcgen05.mma issuer (+ TMEM alloc), warps 2-5 = epilogue
+// (TMEM -> registers -> global).  Two TMEM accumulator buffers overlap the epilogue with the next tile's MMAs.
+#include "sp2_kernels.h"
+#include "sp2_ptx.cuh"
+
+namespace sp2 {
+
+template <int BN_, int CG_>
+struct TileCfg {
+    static constexpr int BN = BN_;                 // accumulator columns = supertile edge
+    static constexpr int CG = CG_;                 // CTAs cooperating on one MMA (cta_group)
+    static constexpr int BM = 128;                 // accumulator rows per CTA (TMEM lanes)
+    static constexpr int BK = 64;                  // K per pipeline stage (one 128-byte swizzle row of FP16)
+    static constexpr int BNL = BN / CG;            // B-operand rows this CTA loads
+    static constexpr int A_BYTES = BM * BK * 2;
+    static constexpr int B_BYTES = BNL * BK * 2;
+    static constexpr int STAGE_BYTES = 2 * A_BYTES + 2 * B_BYTES;   // hi and lo of both panels
+    static constexpr int STAGES = (STAGE_BYTES > 65536) ? 2 : 3;
+    static constexpr int SUB = (BN / BM) / CG;     // 128-row work items per supertile per CTA slot
+    static constexpr int TMEM_COLS = 2 * BN;       // two accumulator buffers
+    static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*align*/ + 256 /*barriers*/;
+    static constexpr int THREADS = 192;
+};
+
+template <class C>
+__global__ void __launch_bounds__(C::THREADS, 1)
+k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ CUtensorMap tm_lo,
+            const LayerParams p) {
+    constexpr int BN = C::BN, CG = C::CG, BM = C::BM, BK = C::BK, STAGES = C::STAGES;
+    Ctrl* ctrl = p.ctrl;
+    // Device-side loop control: a layer launched after convergence does nothing (all CTAs agree: the flag only
+    // changes at the very end of a layer kernel).
+    if (*((volatile int*)&ctrl->running) == 0) {
+        if (p.cond_handle != 0 && blockIdx.x == 0 && threadIdx.x == 0) cudaGraphSetConditional(p.cond_handle, 0);
+        return;
+    }
+
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + STAGES * C::STAGE_BYTES);
+    uint64_t* full_bar = bars;                       // [STAGES]
+    uint64_t* empty_bar = bars + STAGES;             // [STAGES]
+    uint64_t* tfull_bar = bars + 2 * STAGES;         // [2]
+    uint64_t* tempty_bar = bars + 2 * STAGES + 2;    // [2]
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * STAGES + 4);
+    __shared__ double red[4][3];
+
+    const int warp = threadIdx.x >> 5;
+    const int lane = threadIdx.x & 31;
+    const uint32_t rank = (CG == 2) ? cluster_ctarank() : 0u;
+    const int slot = blockIdx.x / CG;
+    const int nslots = gridDim.x / CG;
+    const int n_work = p.n_super * C::SUB;
+    const int KB = p.Np / BK;
+
+    if (warp == 0 && lane == 0) {
+        tma_prefetch_desc(&tm_hi);
+        tma_prefetch_desc(&tm_lo);
+    }
+    if (warp == 1) {
+        if (lane == 0) {
+            for (int s = 0; s < STAGES; ++s) {
+                mbar_init(&full_bar[s], CG);
+                mbar_init(&empty_bar[s], 1);
+            }
+            for (int b = 0; b < 2; ++b) {
+                mbar_init(&tfull_bar[b], 1);
+                mbar_init(&tempty_bar[b], 4 * CG);
+            }
+            fence_barrier_init();
+        }
+        __syncwarp();
+        tmem_alloc<CG>(tmem_slot, C::TMEM_COLS);
+        tmem_relinquish<CG>();
+    }
+    tc_fence_before();
+    if (CG == 2) cluster_sync_all(); else __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *((volatile uint32_t*)tmem_slot);
+
+    if (warp == 0) {
+        // =============================== TMA producer (one elected lane)
+        if (lane == 0) {
+            int s = 0;
+            uint32_t ph = 0;
+            for (int w = slot; w < n_work; w += nslots) {
+                const int2 sj = p.tiles[w / C::SUB];
+                const int sub = w % C::SUB;
+                const int m0 = sj.x * BN + (sub * CG + (int)rank) * BM;      // A rows of this CTA
+                const int n0 = sj.y * BN + (int)rank * C::BNL;               // B rows this CTA loads
+                for (int kb = 0; kb < KB; ++kb) {
+                    mbar_wait(&empty_bar[s], ph ^ 1u);
+                    uint8_t* st = smem + s * C::STAGE_BYTES;
+                    const int k0 = kb * BK;
+                    if (CG == 1) {
+                        mbar_arrive_expect_tx(&full_bar[s], C::STAGE_BYTES);
+                        tma_load_2d(st, &tm_hi, &full_bar[s], k0, m0);
+                        tma_load_2d(st + C::A_BYTES, &tm_lo, &full_bar[s], k0, m0);
+#pragma unroll
+                        for (int h = 0; h < C::BNL / 128; ++h) {
+                            tma_load_2d(st + 2 * C::A_BYTES + h * 16384, &tm_hi, &full_bar[s], k0, n0 + h * 128);
+                            tma_load_2d(st + 2 * C::A_BYTES + C::B_BYTES + h * 16384, &tm_lo, &full_bar[s], k0,
+                                        n0 + h * 128);
+                        }
+                    } else {
+                        if (rank == 0) mbar_arrive_expect_tx(&full_bar[s], 2 * C::STAGE_BYTES);
+                        else mbar_arrive_cluster(&full_bar[s], 0);
+                        tma_load_2d_pair(st, &tm_hi, &full_bar[s], k0, m0);
+                        tma_load_2d_pair(st + C::A_BYTES, &tm_lo, &full_bar[s], k0, m0);
+#pragma unroll
+                        for (int h = 0; h < C::BNL / 128; ++h) {
+                            tma_load_2d_pair(st + 2 * C::A_BYTES + h * 16384, &tm_hi, &full_bar[s], k0, n0 + h * 128);
+                            tma_load_2d_pair(st + 2 * C::A_BYTES + C::B_BYTES + h * 16384, &tm_lo, &full_bar[s], k0,
+                                             n0 + h * 128);
+                        }
+                    }
+                    if (++s == STAGES) { s = 0; ph ^= 1u; }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // =============================== MMA issuer (leader CTA only, one elected lane)
+        if (rank == 0) {
+            constexpr uint32_t idesc = umma_idesc_f16(BM * CG, BN);
+            int s = 0;
+            uint32_t ph = 0;
+            int it = 0;
+            for (int w = slot; w < n_work; w += nslots, ++it) {
+                const int buf = it & 1;
+                const uint32_t use = (uint32_t)(it >> 1);
+                mbar_wait(&tempty_bar[buf], (use & 1u) ^ 1u);       // epilogue has drained this accumulator
+                tc_fence_after();
+                const uint32_t d_tmem = tmem_base + (uint32_t)(buf * BN);
+                for (int kb = 0; kb < KB; ++kb) {
+                    mbar_wait(&full_bar[s], ph);
+                    tc_fence_after();
+                    if (lane == 0) {
+                        const uint32_t a_hi = smem_u32(smem + s * C::STAGE_BYTES);
+                        const uint32_t a_lo = a_hi + C::A_BYTES;
+                        const uint32_t b_hi = a_hi + 2 * C::A_BYTES;
+                        const uint32_t b_lo = b_hi + C::B_BYTES;
+#pragma unroll
+                        for (int k = 0; k < BK / 16; ++k) {
+                            const uint64_t dah = umma_desc_sw128(a_hi + k * 32);
+                            const uint64_t dal = umma_desc_sw128(a_lo + k * 32);
+                            const uint64_t dbh = umma_desc_sw128(b_hi + k * 32);
+                            const uint64_t dbl = umma_desc_sw128(b_lo + k * 32);
+                            umma_f16<CG>(d_tmem, dah, dbh, idesc, (kb | k) != 0);   // X0 X0
+                            umma_f16<CG>(d_tmem, dah, dbl, idesc, 1u);              // X0 X1
+                            umma_f16<CG>(d_tmem, dal, dbh, idesc, 1u);              // (X0 X1)^T
+                        }
+                        if (CG == 1) umma_commit(&empty_bar[s]); else umma_commit_pair(&empty_bar[s], 0x3);
+                        if (kb == KB - 1) {
+                            if (CG == 1) umma_commit(&tfull_bar[buf]); else umma_commit_pair(&tfull_bar[buf], 0x3);
+                        }
+                    }
+                    __syncwarp();
+                    if (++s == STAGES) { s = 0; ph ^= 1u; }
+                }
+            }
+        }
+    } else {
+        // =============================== epilogue warps (TMEM lane quarter = warp % 4)
+        const int q = warp & 3;
+        const int rl = q * 32 + lane;                       // accumulator row (TMEM lane) of this thread
+        const float th1s = ((volatile float*)ctrl->theta)[0] * p.inv_scale2;
+        const float th2 = ((volatile float*)ctrl->theta)[1];
+        const float th3 = ((volatile float*)ctrl->theta)[2];
+        const float cs = p.scale;
+        const float inv2 = p.inv_scale2;
+        const long long ld = p.ld;
+        float* __restrict__ S = p.S;
+        __half* __restrict__ HO = p.hi_out;
+        __half* __restrict__ LO = p.lo_out;
+        double trS = 0.0, fro2 = 0.0, trX = 0.0;
+        int it = 0;
+        for (int w = slot; w < n_work; w += nslots, ++it) {
+            const int buf = it & 1;
+            const uint32_t use = (uint32_t)(it >> 1);
+            const int2 sj = p.tiles[w / C::SUB];
+            const int sub = w % C::SUB;
+            const int m0 = sj.x * BN + (sub * CG + (int)rank) * BM;
+            const int n0 = sj.y * BN;
+            const int gi = m0 + rl;
+            const int gi_wmin = m0 + q * 32, gi_wmax = gi_wmin + 31;
+            mbar_wait(&tfull_bar[buf], use & 1u);
+            tc_fence_after();
+            const uint32_t taddr = tmem_base + (uint32_t)(buf * BN) + ((uint32_t)(q * 32) << 16);
+#pragma unroll 1
+            for (int c0 = 0; c0 < BN; c0 += 32) {
+                const int gj0 = n0 + c0;
+                if (gj0 > gi_wmax) break;                   // rest of the row block lies above the diagonal
+                uint32_t v[32];
+                float so[32];
+                tmem_ld_32x32(taddr + (uint32_t)c0, v);
+                const bool below = (gj0 + 31 <= gi_wmin);   // whole 32x32 chunk strictly in the lower triangle
+                // S_{n-1}: read at the mirrored position (S is exactly symmetric) -> coalesced across the warp
+#pragma unroll
+                for (int c = 0; c < 32; ++c) so[c] = S[(long long)(gj0 + c) * ld + gi];
+                tmem_ld_wait();
+                float sn[32];
+                uint32_t hp[16], lp[16];                    // FP16 pairs (element 2c in the low half)
+#pragma unroll
+                for (int c = 0; c < 32; ++c) {
+                    const int gj = gj0 + c;
+                    const float x = __uint_as_float(v[c]);
+                    float val = fmaf(th1s, x, th2 * so[c]);
+                    const bool on_diag = (gj == gi);
+                    if (on_diag && gi < p.N) val += th3;
+                    sn[c] = val;
+                    __half h, l;
+                    split_hi_lo(val, cs, h, l);
+                    const uint32_t hb = __half_as_ushort(h), lb = __half_as_ushort(l);
+                    if (c & 1) { hp[c >> 1] |= hb << 16; lp[c >> 1] |= lb << 16; }
+                    else { hp[c >> 1] = hb; lp[c >> 1] = lb; }
+                    const bool own = below || (gj <= gi);
+                    const double vd = (double)val;
+                    if (own) fro2 += on_diag ? vd * vd : 2.0 * vd * vd;
+                    if (on_diag) { trS += vd; trX += (double)(x * inv2); }
+                }
+                unsigned short* HOu = reinterpret_cast<unsigned short*>(HO);
+                unsigned short* LOu = reinterpret_cast<unsigned short*>(LO);
+                if (below) {
+                    // mirrored position: one 128-byte (FP32) / 64-byte (FP16) warp store per column
+#pragma unroll
+                    for (int c = 0; c < 32; ++c) {
+                        const long long o = (long long)(gj0 + c) * ld + gi;
+                        S[o] = sn[c];
+                        HOu[o] = (unsigned short)(hp[c >> 1] >> (16 * (c & 1)));
+                        LOu[o] = (unsigned short)(lp[c >> 1] >> (16 * (c & 1)));
+                    }
+                    // own position: 128 contiguous bytes (FP32) / 64 (FP16) per thread
+                    float4* dS = reinterpret_cast<float4*>(S + (long long)gi * ld + gj0);
+                    uint4* dH = reinterpret_cast<uint4*>(HO + (long long)gi * ld + gj0);
+                    uint4* dL = reinterpret_cast<uint4*>(LO + (long long)gi * ld + gj0);
+#pragma unroll
+                    for (int c = 0; c < 8; ++c) dS[c] = make_float4(sn[4 * c], sn[4 * c + 1], sn[4 * c + 2], sn[4 * c + 3]);
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) {
+                        dH[c] = make_uint4(hp[4 * c], hp[4 * c + 1], hp[4 * c + 2], hp[4 * c + 3]);
+                        dL[c] = make_uint4(lp[4 * c], lp[4 * c + 1], lp[4 * c + 2], lp[4 * c + 3]);
+                    }
+                } else {
+                    // chunk crosses the diagonal: only gj <= gi is authoritative (exact symmetry inside the tile)
+#pragma unroll
+                    for (int c = 0; c < 32; ++c) {
+                        const int gj = gj0 + c;
+                        if (gj <= gi) {
+                            const long long o = (long long)gj * ld + gi, o2 = (long long)gi * ld + gj;
+                            const unsigned short hb = (unsigned short)(hp[c >> 1] >> (16 * (c & 1)));
+                            const unsigned short lb = (unsigned short)(lp[c >> 1] >> (16 * (c & 1)));
+                            S[o] = sn[c]; HOu[o] = hb; LOu[o] = lb;
+                            S[o2] = sn[c]; HOu[o2] = hb; LOu[o2] = lb;
+                        }
+                    }
+                }
+            }
+            // all tcgen05.ld of this accumulator have completed (tmem_ld_wait above): hand it back to the MMA warp
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) {
+                if (CG == 1) mbar_arrive(&tempty_bar[buf]); else mbar_arrive_cluster(&tempty_bar[buf], 0);
+            }
+        }
+        // ---- block partials -> ctrl -> last CTA runs the control step
+        for (int o = 16; o > 0; o >>= 1) {
+            trS += __shfl_xor_sync(0xffffffffu, trS, o);
+            fro2 += __shfl_xor_sync(0xffffffffu, fro2, o);
+            trX += __shfl_xor_sync(0xffffffffu, trX, o);
+        }
+        if (lane == 0) { red[q][0] = trS; red[q][1] = fro2; red[q][2] = trX; }
+        asm volatile("bar.sync 1, 128;\n" ::: "memory");     // the four epilogue warps only
+        if (warp == 2 && lane == 0) {
+            double a = 0.0, b = 0.0, c = 0.0;
+            for (int i = 0; i < 4; ++i) { a += red[i][0]; b += red[i][1]; c += red[i][2]; }
+            ctrl->partial[blockIdx.x][0] = a;
+            ctrl->partial[blockIdx.x][1] = b;
+            ctrl->partial[blockIdx.x][2] = c;
+            __threadfence();
+            const unsigned int done = atomicAdd(&ctrl->done_counter, 1u);
+            if (done == gridDim.x - 1) {
+                __threadfence();
+                control_after_layer(ctrl, p.stats, p.thetas, (int)gridDim.x);
+                __threadfence();
+                if (p.cond_handle != 0) cudaGraphSetConditional(p.cond_handle, ctrl->running ? 1u : 0u);
+            }
+        }
+    }
+
+    // ---- teardown
+    tc_fence_before();
+    if (CG == 2) cluster_sync_all(); else __syncthreads();
+    if (warp == 1) tmem_dealloc<CG>(tmem_base, C::TMEM_COLS);
+}
+
+using Cfg128 = TileCfg<128, 1>;
+using Cfg256 = TileCfg<256, 1>;
+using Cfg256P = TileCfg<256, 2>;
+
+int tile_super_edge(int cfg) { return cfg == TILE_128x128 ? 128 : 256; }
+size_t tile_smem_bytes(int cfg) {
+    return cfg == TILE_128x128 ? Cfg128::SMEM_BYTES : cfg == TILE_128x256 ? Cfg256::SMEM_BYTES : Cfg256P::SMEM_BYTES;
+}
+
+cudaError_t layer_kernel_setup(int cfg) {
+    switch (cfg) {
+        case TILE_128x128:
+            return cudaFuncSetAttribute(k_sp2_layer<Cfg128>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                        Cfg128::SMEM_BYTES);
+        case TILE_128x256:
+            return cudaFuncSetAttribute(k_sp2_layer<Cfg256>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                        Cfg256::SMEM_BYTES);
+        case TILE_256x256_PAIR:
+            return cudaFuncSetAttribute(k_sp2_layer<Cfg256P>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                        Cfg256P::SMEM_BYTES);
+    }
+    return cudaErrorInvalidValue;
+}
+
+template <class C>
+static cudaError_t launch_cfg(const CUtensorMap& tm_hi, const CUtensorMap& tm_lo, const LayerParams& p, int num_sms,
+                              cudaStream_t st) {
+    const int n_work = p.n_super * C::SUB;
+    int slots = num_sms / C::CG;
+    if (slots > n_work) slots = n_work;
+    if (slots * C::CG > kMaxPartials) slots = kMaxPartials / C::CG;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)(slots * C::CG));
+    cfg.blockDim = dim3(C::THREADS);
+    cfg.dynamicSmemBytes = C::SMEM_BYTES;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = C::CG;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, k_sp2_layer<C>, tm_hi, tm_lo, p);
+}
+
+cudaError_t launch_layer(int cfg, const CUtensorMap& tm_hi, const CUtensorMap& tm_lo, const LayerParams& p,
+                         int num_sms, cudaStream_t st) {
+    switch (cfg) {
+        case TILE_128x128: return launch_cfg<Cfg128>(tm_hi, tm_lo, p, num_sms, st);
+        case TILE_128x256: return launch_cfg<Cfg256>(tm_hi, tm_lo, p, num_sms, st);
+        case TILE_256x256_PAIR: return launch_cfg<Cfg256P>(tm_hi, tm_lo, p, num_sms, st);
+    }
+    return cudaErrorInvalidValue;
+}
+
+}  // namespace sp2
