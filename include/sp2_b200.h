@@ -54,6 +54,7 @@ typedef struct {
     double iderr;         /* IdErr_n = N_S(before) - N_X = Tr[S_{n-1} - S_{n-1}^2]           */
     int    sigma;         /* +1: S_n = X_n ; -1: S_n = 2 S_{n-1} - X_n ; 0 in generalized runs               */
     int    stop_reason;   /* SP2_STOP_* : nonzero only on the last layer                                     */
+    unsigned long long t_end_ns; /* device %globaltimer when the layer's last CTA finished (per-layer timeline) */
 } sp2_layer_stat_t;
 
 typedef struct {

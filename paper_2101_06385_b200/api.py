@@ -25,7 +25,7 @@ EXPORTS = ["sp2_default_opts", "sp2_create", "sp2_destroy", "sp2_workspace_bytes
 
 class LayerStat(C.Structure):
     _fields_ = [("trace_S", C.c_double), ("trace_X", C.c_double), ("trace_X_diag", C.c_double),
-                ("iderr", C.c_double), ("sigma", C.c_int), ("stop_reason", C.c_int)]
+                ("iderr", C.c_double), ("sigma", C.c_int), ("stop_reason", C.c_int), ("t_end_ns", C.c_ulonglong)]
 
 
 class Opts(C.Structure):
@@ -102,7 +102,7 @@ def _dev_f32(t, name):
 
 
 def _stats_to_dict(stats, n):
-    keys = ("trace_S", "trace_X", "trace_X_diag", "iderr", "sigma", "stop_reason")
+    keys = ("trace_S", "trace_X", "trace_X_diag", "iderr", "sigma", "stop_reason", "t_end_ns")
     return {k: [getattr(stats[i], k) for i in range(n)] for k in keys}
 
 
@@ -161,15 +161,21 @@ class Handle:
 
     def density_matrix_host(self, H_host: np.ndarray, N_occ, opts: Optional[Opts] = None, out=None, stream=None):
         """Host buffers in, host buffers out (H2D and D2H inside the call)."""
-        H_host = np.ascontiguousarray(H_host, dtype=np.float32)
+        def _ptr(a):
+            return a.ctypes.data if isinstance(a, np.ndarray) else a.data_ptr()
+
+        if isinstance(H_host, np.ndarray):
+            H_host = np.ascontiguousarray(H_host, dtype=np.float32)
+        elif H_host.is_cuda or not H_host.is_contiguous():
+            raise TypeError("H_host must be a contiguous host buffer (numpy array or CPU torch tensor)")
         N = H_host.shape[0]
         opts = opts or make_opts()
         D = np.empty((N, N), dtype=np.float32) if out is None else out
         stats = (LayerStat * opts.max_layers)()
         nl = C.c_int(0)
         bounds = (C.c_double * 2)()
-        st = self.lib.sp2_density_matrix_host(self._h, H_host.ctypes.data, N, N, float(N_occ), C.byref(opts),
-                                              D.ctypes.data, N, stats, C.byref(nl), bounds, _stream_ptr(stream))
+        st = self.lib.sp2_density_matrix_host(self._h, _ptr(H_host), N, N, float(N_occ), C.byref(opts),
+                                              _ptr(D), N, stats, C.byref(nl), bounds, _stream_ptr(stream))
         if st < 0:
             raise SP2Error(st, "sp2_density_matrix_host")
         info = _stats_to_dict(stats, nl.value)
@@ -259,7 +265,7 @@ def batched_stats(info, m: int):
     """Per-layer statistics of matrix m of a batched solve."""
     n = int(info["n_layers"][m])
     base = m * info["max_layers"]
-    keys = ("trace_S", "trace_X", "trace_X_diag", "iderr", "sigma", "stop_reason")
+    keys = ("trace_S", "trace_X", "trace_X_diag", "iderr", "sigma", "stop_reason", "t_end_ns")
     return {k: [getattr(info["stats"][base + i], k) for i in range(n)] for k in keys}
 
 

@@ -75,7 +75,7 @@ struct sp2_handle_s {
 
 static int round_up(int x, int m) { return (x + m - 1) / m * m; }
 
-static size_t ctrl_header_bytes() { return offsetof(Ctrl, partial); }
+static size_t ctrl_header_bytes() { return sizeof(CtrlCore); }
 
 extern "C" const char* sp2_status_string(sp2_status_t s) {
     switch (s) {

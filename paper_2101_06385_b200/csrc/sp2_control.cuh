@@ -12,7 +12,7 @@ constexpr int kMaxPartials = 1024;   // per-CTA FP64 partial slots (>= largest g
 
 enum { MODE_STANDARD = 0, MODE_GENERALIZED = 1 };
 
-struct Ctrl {
+struct CtrlCore {
     // ---- problem constants (written by the host before launch)
     double N_occ, eps_alt, tol;
     double eps_min, eps_max;         // spectral bounds (given, or written by the Gershgorin kernel)
@@ -31,23 +31,27 @@ struct Ctrl {
     float  theta[4];                 // th1, th2, th3 of the NEXT layer (FP32: the epilogue's arithmetic type)
     unsigned int done_counter;       // CTAs finished in the current kernel
     unsigned int pad_;
+};
+struct Ctrl : CtrlCore {
     double partial[kMaxPartials][4]; // per-CTA {Tr S, ||S||_F^2, Tr X (diag), unused}
 };
 
 // Decide layer n+1 from N_S = Tr S_n and N_X = ||S_n||_F^2, exactly in Alg. 1's order:
 // IdErr, sigma, (W_n, B_n) -> theta, stop tests.  The stop tests belong to layer n+1 and take effect after
 // that layer has been applied (reading C1 of DESIGN.md).  thetas = per-layer [L][3] list in generalized mode.
-__device__ inline void control_plan_next(Ctrl* c, sp2_layer_stat_t* stats, const double* thetas) {
+__device__ inline void control_plan_next(CtrlCore* c, sp2_layer_stat_t* stats, const double* thetas) {
     const int m = c->n + 1;                      // layer about to run
     if (c->mode == MODE_GENERALIZED) {
         if (c->n >= c->max_layers) { c->running = 0; c->stop_reason = SP2_STOP_MAX_LAYERS; return; }
         c->theta[0] = (float)thetas[3 * c->n + 0];
         c->theta[1] = (float)thetas[3 * c->n + 1];
         c->theta[2] = (float)thetas[3 * c->n + 2];
-        stats[m - 1].trace_X = c->fro2;
-        stats[m - 1].iderr = c->N_S - c->fro2;
-        stats[m - 1].sigma = 0;
-        stats[m - 1].stop_reason = (m == c->max_layers) ? SP2_STOP_MAX_LAYERS : SP2_STOP_NONE;
+        if (stats) {
+            stats[m - 1].trace_X = c->fro2;
+            stats[m - 1].iderr = c->N_S - c->fro2;
+            stats[m - 1].sigma = 0;
+            stats[m - 1].stop_reason = (m == c->max_layers) ? SP2_STOP_MAX_LAYERS : SP2_STOP_NONE;
+        }
         c->running = 1;
         return;
     }
@@ -72,15 +76,41 @@ __device__ inline void control_plan_next(Ctrl* c, sp2_layer_stat_t* stats, const
     else if (c->tol > 0.0 && iderr <= c->tol) pend = SP2_STOP_TOL;
     else if (m >= c->max_layers) pend = SP2_STOP_MAX_LAYERS;
     c->pending_stop = pend;
-    stats[m - 1].trace_X = N_X;
-    stats[m - 1].iderr = iderr;
-    stats[m - 1].sigma = sigma;
-    stats[m - 1].stop_reason = pend;
+    if (stats) {
+        stats[m - 1].trace_X = N_X;
+        stats[m - 1].iderr = iderr;
+        stats[m - 1].sigma = sigma;
+        stats[m - 1].stop_reason = pend;
+    }
     c->sigma_prev2 = c->sigma_prev;
     c->sigma_prev = sigma;
     c->iderr_prev2 = c->iderr_prev;
     c->iderr_prev = iderr;
     c->running = 1;
+}
+
+// Book-keeping after layer n has been applied: N_S = Tr S_n (measured), ||S_n||_F^2, then either stop (the
+// layer's own stop test had fired) or plan layer n+1.
+__device__ inline void control_finish_layer(CtrlCore* c, sp2_layer_stat_t* stats, const double* thetas, double trS,
+                                            double fro2, double trX) {
+    c->n += 1;
+    c->launches += 1;
+    c->N_S = trS;
+    c->fro2 = fro2;
+    if (stats) {
+        stats[c->n - 1].trace_S = trS;
+        stats[c->n - 1].trace_X_diag = trX;
+        unsigned long long t;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+        stats[c->n - 1].t_end_ns = t;
+    }
+    c->done_counter = 0;
+    if (c->mode == MODE_STANDARD && c->pending_stop != SP2_STOP_NONE) {
+        c->running = 0;
+        c->stop_reason = c->pending_stop;
+        return;
+    }
+    control_plan_next(c, stats, thetas);
 }
 
 // Called by ONE thread once every CTA of the layer kernel has published its partial sums.
@@ -91,19 +121,7 @@ __device__ inline void control_after_layer(Ctrl* c, sp2_layer_stat_t* stats, con
         fro2 += c->partial[i][1];
         trX += c->partial[i][2];
     }
-    c->n += 1;
-    c->launches += 1;
-    c->N_S = trS;
-    c->fro2 = fro2;
-    stats[c->n - 1].trace_S = trS;
-    stats[c->n - 1].trace_X_diag = trX;
-    c->done_counter = 0;
-    if (c->mode == MODE_STANDARD && c->pending_stop != SP2_STOP_NONE) {
-        c->running = 0;
-        c->stop_reason = c->pending_stop;
-        return;
-    }
-    control_plan_next(c, stats, thetas);
+    control_finish_layer(c, stats, thetas, trS, fro2, trX);
 }
 
 }  // namespace sp2
