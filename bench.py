@@ -205,7 +205,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--n", type=int, default=16384)
+    ap.add_argument("--n", "--size", dest="n", type=int, default=16384)
     ap.add_argument("--seed", type=int, default=0)
     ap.add_argument("--bounds", choices=["auto", "explicit"], default="auto")
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")

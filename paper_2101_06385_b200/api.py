@@ -261,6 +261,17 @@ class Handle:
         return out[0], out[1]
 
 
+def shard_range(n_items: int, rank: int, world: int):
+    """Contiguous [start, stop) slice of a batch of independent matrices owned by `rank` of `world` processes
+    (one process per GPU).  The batched path shards with no data-path collective:
+    the first n_items % world ranks get one extra item."""
+    if world < 1 or not (0 <= rank < world) or n_items < 0:
+        raise ValueError("bad shard arguments")
+    base, extra = divmod(n_items, world)
+    start = rank * base + min(rank, extra)
+    return start, start + base + (1 if rank < extra else 0)
+
+
 def batched_stats(info, m: int):
     """Per-layer statistics of matrix m of a batched solve."""
     n = int(info["n_layers"][m])

@@ -1,0 +1,71 @@
+"""Oracle against values the paper prints (tests/golden/*.txt, each with its citation) and against the frozen
+small-case fixture written by tests/golden/make_golden.py from the oracle alone."""
+import json
+import os
+
+import numpy as np
+
+from oracle import sp2_oracle as O
+from paper_2101_06385_b200 import workloads as W
+
+G = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
+def _kv(name):
+    out = {}
+    with open(os.path.join(G, name)) as f:
+        for line in f:
+            line = line.split("#")[0].strip()
+            if line:
+                k, v = line.split()
+                out[k] = float(v)
+    return out
+
+
+def test_theorem1_constant_as_printed():
+    """C = (71 + 17 sqrt 17)/32 ~ 4.41; and C is the maximum of Eqs. 22-23, by brute force."""
+    g = _kv("theorem1_constant.txt")
+    C = (g["closed_form_numerator_a"] + g["closed_form_numerator_b"] * np.sqrt(g["closed_form_radicand"])) / \
+        g["closed_form_denominator"]
+    assert abs(C - O.THEOREM1_C) < 1e-15
+    assert round(C, 2) == g["printed_value"]
+    lam = np.linspace(1e-6, 1 - 1e-6, 2_000_001)
+    den = (lam - lam ** 2) ** 2
+    p = 2 * lam - lam ** 2
+    q = 2 * lam ** 2 - lam ** 4
+    assert abs(((p ** 2 - p ** 4) / den).max() - C) < 1e-9          # Eq. 22
+    assert abs(((q - q ** 2) / den).max() - C) < 1e-9               # Eq. 23
+
+
+def test_paper_text_numbers():
+    g = _kv("paper_text_numbers.txt")
+    # each layer doubles the polynomial order -> 2^30 > 1e9 after 30 steps
+    assert 2 ** 30 > g["polynomial_order_after_30_steps_exceeds"]
+    # the oracle's stop rule uses 4.5 literally (reading C7): a sequence built to sit between 4.41 and 4.5
+    assert g["stop_rule_constant"] == 4.5
+    import inspect
+    assert "4.5 *" in inspect.getsource(O.sp2_ref) and "4.5 *" in inspect.getsource(O.scalar_recursion)
+    # "28 layers" for an unspecified 100x100, N_occ = 10 -> plausibility range on inputs of that shape
+    for seed in range(3):
+        H32 = W.uniform_symmetric(seed, 100)
+        D, st = O.sp2_ref(H32, 10.0, None, tol=0.0, max_layers=100)      # paper's parameter-free rule only
+        assert 0.6 * g["layers_plain_100x100_nocc10"] <= st["n_layers"] <= 1.6 * g["layers_plain_100x100_nocc10"]
+        De, _ = O.eig_density(H32, 10.0)
+        assert np.abs(D - De).max() < 1e-6
+
+
+def test_golden_small_cases():
+    with open(os.path.join(G, "oracle_small_cases.json")) as f:
+        gold = json.load(f)
+    import importlib.util
+    spec = importlib.util.spec_from_file_location("make_golden", os.path.join(G, "make_golden.py"))
+    mg = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mg)
+    now = mg.build()
+    assert set(now) == set(gold)
+    for k in gold:
+        assert now[k]["sigma"] == gold[k]["sigma"], k
+        assert now[k]["n_layers"] == gold[k]["n_layers"] and now[k]["stop_reason"] == gold[k]["stop_reason"]
+        assert np.allclose(now[k]["trace_S"], gold[k]["trace_S"], rtol=0, atol=1e-9)
+        assert abs(now[k]["D00"] - gold[k]["D00"]) < 1e-9
+        assert abs(gold[k]["trace_D"] - gold[k]["n_occ"]) < 1e-6        # Tr D = N_occ
