@@ -210,6 +210,10 @@ def main():
     ap.add_argument("--bounds", choices=["auto", "explicit"], default="auto")
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--tile", type=int, default=0)
+    ap.add_argument("--control", type=int, default=0,
+                    help="0: device-side WHILE graph (default, the product path); 2: max_layers guarded launches "
+                         "(same kernels, no graph: lets ncu see every layer launch)")
+    ap.add_argument("--exact-diag", type=int, default=1)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -233,7 +237,8 @@ def main():
     D = torch.empty_like(H)
     h = api.Handle(N, 0, 120)
     bounds = None if args.bounds == "auto" else w.bounds
-    opts = api.make_opts(bounds=bounds, tol=w.tol, max_layers=w.max_layers, tile_config=args.tile)
+    opts = api.make_opts(bounds=bounds, tol=w.tol, max_layers=w.max_layers, tile_config=args.tile,
+                         control=args.control, exact_diag=args.exact_diag)
     stream = torch.cuda.current_stream()
 
     def solve():
@@ -280,7 +285,8 @@ def main():
     info_timed = info
 
     # ---- dominant kernel (fused layer) duration: CUDA events, (T(all layers) - T(1 layer)) / (layers - 1)
-    opts1 = api.make_opts(bounds=bounds, tol=w.tol, max_layers=1, tile_config=args.tile)
+    opts1 = api.make_opts(bounds=bounds, tol=w.tol, max_layers=1, tile_config=args.tile, control=args.control,
+                          exact_diag=args.exact_diag)
     e1 = []
     for i in range(4):
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -342,7 +348,8 @@ def main():
             "config": {"workload": f"config3: gapped dense symmetric H = Q diag(eps) Q^T, N={N}, N_occ={int(w.N_occ)}, "
                                    f"seed {args.seed} (BASELINE.json configs[2])",
                        "bounds": "Gershgorin on device" if bounds is None else f"explicit {bounds}",
-                       "tol": w.tol, "max_layers": w.max_layers, "tile_config": args.tile,
+                       "tol": w.tol, "max_layers": w.max_layers, "tile_config": args.tile, "control": args.control,
+                       "exact_diag": args.exact_diag,
                        "parallelism": "replicas only (no sharding, no collective)" if world > 1 else "single GPU",
                        "l2": "inputs (1 GiB H, 3 GiB workspace) exceed the 126 MB L2; no flush needed"},
             "detail": {"layers_per_solve": n_layers, "ms_per_converged_D": ms_per_step,

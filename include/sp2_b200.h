@@ -43,7 +43,11 @@ typedef enum {
 
 /* stop_reason values (Alg. 1's two tests; tol / max_layers are the caller's extra tests) */
 enum { SP2_STOP_NONE = 0, SP2_STOP_IDERR_NONPOS = 1, SP2_STOP_PARAM_FREE = 2, SP2_STOP_TOL = 3,
-       SP2_STOP_MAX_LAYERS = 4, SP2_STOP_NONFINITE = 5 };
+       SP2_STOP_MAX_LAYERS = 4, SP2_STOP_NONFINITE = 5,
+       /* Alg. 1's first test "IdErr_n <= 0" taken at the resolution of the arithmetic (reading C25):
+          after layer n, IdErr_n <= |Tr X_n(tensor core) - N_X(exact, FP64)|, i.e. the idempotency estimate has
+          dropped below the measured error of the trace it is built from.  Reduces to test 1 in exact arithmetic. */
+       SP2_STOP_NOISE_FLOOR = 6 };
 
 /* Per-layer statistics, entry n-1 describes layer n (n = 1..n_layers), Alg. 1's notation. */
 typedef struct {
@@ -68,9 +72,15 @@ typedef struct {
     int    control;         /* 0: device-side loop in a CUDA graph (WHILE node); 1: host-stepped (debug:
                                one sync per layer); 2: graph of max_layers guarded launches, no WHILE node   */
     int    tile_config;     /* 0: choose by N; 1: 128x128 1-CTA; 2: 128x256 1-CTA; 3: 256x256 2-CTA          */
+    int    exact_diag;      /* 1 (default): diag(X_n)_i = sum_j S_ij^2 is taken from FP32/FP64 row sums of the
+                               FP32 S_{n-1} (the same identity that gives N_X = ||S||_F^2) instead of the
+                               tensor-core accumulator, whose truncating FP32 accumulation biases the large
+                               diagonal by ~ (3N/32) ulp, ramping along the diagonal (reading C24);
+                               0: Alg. 2 literally (tensor-core diagonal). Single-matrix path only.           */
 } sp2_opts_t;
 
-/* Fill *o with defaults: auto_bounds=1, tol=0, max_layers=120, eps_alt=0, fp16_scale_log2=-1, control=0. */
+/* Fill *o with defaults: auto_bounds=1, tol=0, max_layers=120, eps_alt=0, fp16_scale_log2=-1, control=0,
+ * tile_config=0, exact_diag=1. */
 void sp2_default_opts(sp2_opts_t* o);
 
 /* Create a handle able to solve one matrix up to N_max, or a batch of batch_max matrices of N <= 256,

@@ -14,7 +14,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libsp2b200.so")
 
 SP2_OK, SP2_NOT_CONVERGED = 0, 1
-STOP_NAMES = {0: "none", 1: "iderr<=0", 2: "param_free", 3: "tol", 4: "max_layers", 5: "nonfinite"}
+STOP_NAMES = {0: "none", 1: "iderr<=0", 2: "param_free", 3: "tol", 4: "max_layers", 5: "nonfinite", 6: "noise_floor"}
 TILE_AUTO, TILE_128x128, TILE_128x256, TILE_256x256_PAIR = 0, 1, 2, 3
 
 EXPORTS = ["sp2_default_opts", "sp2_create", "sp2_destroy", "sp2_workspace_bytes", "sp2_density_matrix",
@@ -31,7 +31,7 @@ class LayerStat(C.Structure):
 class Opts(C.Structure):
     _fields_ = [("auto_bounds", C.c_int), ("eps_min", C.c_double), ("eps_max", C.c_double), ("tol", C.c_double),
                 ("max_layers", C.c_int), ("eps_alt", C.c_double), ("fp16_scale_log2", C.c_int),
-                ("control", C.c_int), ("tile_config", C.c_int)]
+                ("control", C.c_int), ("tile_config", C.c_int), ("exact_diag", C.c_int)]
 
 
 class SP2Error(RuntimeError):
@@ -106,13 +106,15 @@ def _stats_to_dict(stats, n):
     return {k: [getattr(stats[i], k) for i in range(n)] for k in keys}
 
 
-def make_opts(bounds=None, tol=0.0, max_layers=120, eps_alt=0.0, fp16_scale_log2=-1, control=0, tile_config=0) -> Opts:
+def make_opts(bounds=None, tol=0.0, max_layers=120, eps_alt=0.0, fp16_scale_log2=-1, control=0, tile_config=0,
+              exact_diag=1) -> Opts:
     o = Opts()
     load().sp2_default_opts(C.byref(o))
     if bounds is not None:
         o.auto_bounds, o.eps_min, o.eps_max = 0, float(bounds[0]), float(bounds[1])
     o.tol, o.max_layers, o.eps_alt = float(tol), int(max_layers), float(eps_alt)
     o.fp16_scale_log2, o.control, o.tile_config = int(fp16_scale_log2), int(control), int(tile_config)
+    o.exact_diag = int(exact_diag)
     return o
 
 

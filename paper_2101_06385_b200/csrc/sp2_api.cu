@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <map>
@@ -45,6 +46,7 @@ struct sp2_handle_s {
     __half* hl[2][2] = {{nullptr, nullptr}, {nullptr, nullptr}};   // [ping-pong][hi, lo]
     double* R = nullptr;
     double* diag = nullptr;
+    unsigned long long* rowsq[2] = {nullptr, nullptr};   // fixed-point row sums of squares of S (ping-pong)
     Ctrl* ctrl = nullptr;
     sp2_layer_stat_t* stats_dev = nullptr;
     double* thetas_dev = nullptr;
@@ -66,10 +68,11 @@ struct sp2_handle_s {
     float* stage_D = nullptr;
     size_t stage_elems = 0;
     PFN_encodeTiled encode = nullptr;
-    std::map<std::tuple<int, int, int, int>, LoopGraph> graphs;   // (N, Np, cfg, scale_log2)
+    std::map<std::tuple<int, int, int, int, int>, LoopGraph> graphs;   // (N, Np, cfg, scale_log2, exact_diag)
     int tiles_key_nt = -1, tiles_key_band = -1;
     int n_super = 0;
     int last_launches = 0;
+    double noise_kappa = 0.125;
     cudaStream_t cap_stream = nullptr;
 };
 
@@ -104,13 +107,14 @@ extern "C" void sp2_default_opts(sp2_opts_t* o) {
     o->fp16_scale_log2 = -1;
     o->control = 0;
     o->tile_config = 0;
+    o->exact_diag = 1;
 }
 
 extern "C" size_t sp2_workspace_bytes(int N_max, int batch_max, int max_layers) {
     if (N_max < 1 || max_layers < 1) return 0;
     const size_t Np = (size_t)round_up(N_max, 256);
     size_t b = Np * Np * 4 + 4 * Np * Np * 2;                 // S + two hi/lo pairs
-    b += 2 * Np * sizeof(double);                             // Gershgorin radii, diagonal
+    b += 4 * Np * sizeof(double);                             // Gershgorin radii, diagonal, two row-sum vectors
     b += sizeof(Ctrl) + (size_t)max_layers * (sizeof(sp2_layer_stat_t) + 3 * sizeof(double));
     b += (Np / 128) * (Np / 128 + 1) / 2 * sizeof(int2);
     if (batch_max > 0)
@@ -128,6 +132,7 @@ extern "C" sp2_status_t sp2_destroy(sp2_handle_t h) {
     cudaFree(h->S);
     for (int a = 0; a < 2; ++a)
         for (int b = 0; b < 2; ++b) cudaFree(h->hl[a][b]);
+    cudaFree(h->rowsq[0]); cudaFree(h->rowsq[1]);
     cudaFree(h->R); cudaFree(h->diag); cudaFree(h->ctrl); cudaFree(h->stats_dev); cudaFree(h->thetas_dev);
     cudaFree(h->tiles_dev); cudaFree(h->bstats_dev); cudaFree(h->bnl_dev); cudaFree(h->bstatus_dev);
     cudaFree(h->bbounds_dev); cudaFree(h->bnocc_dev);
@@ -151,6 +156,7 @@ extern "C" sp2_status_t sp2_create(sp2_handle_t* out, int N_max, int batch_max, 
     }
     sp2_handle_s* h = new sp2_handle_s();
     h->N_max = N_max; h->batch_max = batch_max; h->max_layers = max_layers;
+    if (const char* e = getenv("SP2_NOISE_KAPPA")) h->noise_kappa = atof(e);   // tuning hook (C25)
     h->Np_max = round_up(N_max, 256);
     h->num_sms = prop.multiProcessorCount; h->device = dev;
     const size_t Np = (size_t)h->Np_max;
@@ -165,6 +171,8 @@ extern "C" sp2_status_t sp2_create(sp2_handle_t* out, int N_max, int batch_max, 
         for (int b = 0; b < 2; ++b) A((void**)&h->hl[a][b], Np * Np * 2);
     A((void**)&h->R, Np * sizeof(double));
     A((void**)&h->diag, Np * sizeof(double));
+    A((void**)&h->rowsq[0], Np * sizeof(unsigned long long));
+    A((void**)&h->rowsq[1], Np * sizeof(unsigned long long));
     A((void**)&h->ctrl, sizeof(Ctrl));
     A((void**)&h->stats_dev, (size_t)max_layers * sizeof(sp2_layer_stat_t));
     A((void**)&h->thetas_dev, (size_t)max_layers * 3 * sizeof(double));
@@ -251,7 +259,7 @@ static int choose_tile_config(int N, int requested, int num_sms) {
 }
 
 struct Problem {
-    int N, Np, cfg, scale_log2, n_super;
+    int N, Np, cfg, scale_log2, n_super, exact_diag;
     float scale, inv_scale2;
 };
 
@@ -265,6 +273,7 @@ static sp2_status_t prepare_problem(sp2_handle_s* h, int N, const sp2_opts_t* o,
     if (k < 0) k = 13;
     if (k > 14) return SP2_ERR_INVALID_ARG;
     pb->scale_log2 = k;
+    pb->exact_diag = (o && o->exact_diag == 0) ? 0 : 1;
     pb->scale = ldexpf(1.0f, k);
     pb->inv_scale2 = ldexpf(1.0f, -2 * k);
     const int nt = pb->Np / edge;
@@ -287,6 +296,8 @@ static LayerParams layer_params(sp2_handle_s* h, const Problem& pb, int parity, 
     LayerParams p;
     p.ctrl = h->ctrl; p.stats = h->stats_dev; p.thetas = h->thetas_dev; p.S = h->S;
     p.hi_out = h->hl[parity ^ 1][0]; p.lo_out = h->hl[parity ^ 1][1];
+    p.rowsq_cur = pb.exact_diag ? h->rowsq[parity] : nullptr;
+    p.rowsq_next = pb.exact_diag ? h->rowsq[parity ^ 1] : nullptr;
     p.tiles = h->tiles_dev; p.ld = pb.Np; p.N = pb.N; p.Np = pb.Np; p.n_super = pb.n_super;
     p.scale = pb.scale; p.inv_scale2 = pb.inv_scale2; p.cond_handle = cond;
     return p;
@@ -307,7 +318,7 @@ static sp2_status_t launch_one_layer(sp2_handle_s* h, const Problem& pb, int par
 // WHILE(ctrl->running) { layer(ping -> pong); layer(pong -> ping); } as a CUDA graph with a conditional node; the
 // condition is set on the device by the last CTA of each layer kernel (cudaGraphSetConditional).
 static sp2_status_t get_loop_graph(sp2_handle_s* h, const Problem& pb, LoopGraph** out) {
-    auto key = std::make_tuple(pb.N, pb.Np, pb.cfg, pb.scale_log2);
+    auto key = std::make_tuple(pb.N, pb.Np, pb.cfg, pb.scale_log2, pb.exact_diag);
     auto it = h->graphs.find(key);
     if (it != h->graphs.end()) { *out = &it->second; return SP2_OK; }
     LoopGraph lg;
@@ -357,6 +368,7 @@ static sp2_status_t solve_single(sp2_handle_s* h, const float* H_dev, int N, int
     c->N_occ = N_occ; c->eps_alt = o->eps_alt; c->tol = o->tol;
     c->eps_min = o->eps_min; c->eps_max = o->eps_max;
     c->N = N; c->mode = mode; c->max_layers = max_layers; c->auto_bounds = o->auto_bounds;
+    c->noise_kappa = h->noise_kappa;
     CK(cudaMemcpyAsync(h->ctrl, c, ctrl_header_bytes(), cudaMemcpyHostToDevice, st));
     if (mode == MODE_GENERALIZED)
         CK(cudaMemcpyAsync(h->thetas_dev, h->thetas_host, (size_t)max_layers * 3 * sizeof(double),
@@ -371,8 +383,12 @@ static sp2_status_t solve_single(sp2_handle_s* h, const float* H_dev, int N, int
     }
     // ---- a1: bounds, a2: initial affine layer + first split + first control step
     if (o->auto_bounds) CK(launch_gershgorin(H_dev, N, ldh, h->R, h->diag, h->ctrl, nullptr, h->num_sms, st));
+    if (pb.exact_diag) {
+        CK(cudaMemsetAsync(h->rowsq[0], 0, (size_t)pb.Np * sizeof(unsigned long long), st));
+        CK(cudaMemsetAsync(h->rowsq[1], 0, (size_t)pb.Np * sizeof(unsigned long long), st));
+    }
     CK(launch_affine_split(H_dev, N, ldh, h->S, h->hl[0][0], h->hl[0][1], pb.Np, pb.scale, h->ctrl, h->stats_dev,
-                           h->thetas_dev, h->num_sms, st));
+                           h->thetas_dev, pb.exact_diag ? h->rowsq[0] : nullptr, h->num_sms, st));
     // ---- a4-a8: the layer loop
     if (o->control == 0) {
         LoopGraph* lg = nullptr;
@@ -517,7 +533,7 @@ extern "C" sp2_status_t sp2_density_matrix_batched(sp2_handle_t h, const float* 
     memset(&p, 0, sizeof(p));
     p.H = H_dev; p.D = D_dev; p.N_occ = h->bnocc_dev; p.nocc_is_scalar = nocc_is_scalar; p.N = N; p.B = B;
     p.auto_bounds = o.auto_bounds; p.eps_min = o.eps_min; p.eps_max = o.eps_max; p.tol = o.tol; p.eps_alt = o.eps_alt;
-    p.max_layers = o.max_layers; p.mode = MODE_STANDARD; p.thetas = nullptr;
+    p.max_layers = o.max_layers; p.mode = MODE_STANDARD; p.thetas = nullptr; p.noise_kappa = h->noise_kappa;
     p.scale = ldexpf(1.0f, k); p.inv_scale2 = ldexpf(1.0f, -2 * k);
     p.stats = h->bstats_dev; p.n_layers = h->bnl_dev; p.status = h->bstatus_dev; p.bounds = h->bbounds_dev;
     CK(launch_resident(p, h->num_sms, st));

@@ -28,6 +28,8 @@ struct CtrlCore {
     double N_S;                      // Tr S_n (measured)
     double fro2;                     // ||S_n||_F^2 = N_X of layer n+1
     double iderr_prev, iderr_prev2;  // IdErr_n, IdErr_{n-1}
+    double nx_inflight;              // N_X of the layer in flight (exact, FP64 pre-trace)
+    double noise_kappa;              // reading C25: stop when IdErr_n <= kappa |Tr X_n(tc) - N_X|; 0 disables
     float  theta[4];                 // th1, th2, th3 of the NEXT layer (FP32: the epilogue's arithmetic type)
     unsigned int done_counter;       // CTAs finished in the current kernel
     unsigned int pad_;
@@ -76,6 +78,7 @@ __device__ inline void control_plan_next(CtrlCore* c, sp2_layer_stat_t* stats, c
     else if (c->tol > 0.0 && iderr <= c->tol) pend = SP2_STOP_TOL;
     else if (m >= c->max_layers) pend = SP2_STOP_MAX_LAYERS;
     c->pending_stop = pend;
+    c->nx_inflight = N_X;
     if (stats) {
         stats[m - 1].trace_X = N_X;
         stats[m - 1].iderr = iderr;
@@ -105,6 +108,13 @@ __device__ inline void control_finish_layer(CtrlCore* c, sp2_layer_stat_t* stats
         stats[c->n - 1].t_end_ns = t;
     }
     c->done_counter = 0;
+    // Reading C25: "IdErr_n <= 0" at the resolution of the arithmetic.  iderr_prev = IdErr_n of the layer just
+    // applied; |trX - nx_inflight| = measured error of the tensor-core trace of X_n.
+    if (c->mode == MODE_STANDARD && c->pending_stop == SP2_STOP_NONE && c->n > 2 &&
+        c->noise_kappa > 0.0 && c->iderr_prev <= c->noise_kappa * fabs(trX - c->nx_inflight)) {
+        c->pending_stop = SP2_STOP_NOISE_FLOOR;
+        if (stats) stats[c->n - 1].stop_reason = SP2_STOP_NOISE_FLOOR;
+    }
     if (c->mode == MODE_STANDARD && c->pending_stop != SP2_STOP_NONE) {
         c->running = 0;
         c->stop_reason = c->pending_stop;

@@ -98,8 +98,10 @@ constexpr int AT = 32;
 __global__ void __launch_bounds__(256) k_affine_split(const float* __restrict__ H, int N, long long ldh,
                                                       float* __restrict__ S, __half* __restrict__ hi,
                                                       __half* __restrict__ lo, long long ld, float scale, Ctrl* ctrl,
-                                                      sp2_layer_stat_t* stats, const double* thetas) {
+                                                      sp2_layer_stat_t* stats, const double* thetas,
+                                                      unsigned long long* __restrict__ rowsq) {
     __shared__ float ts[AT][AT + 1];
+    __shared__ double colsq[8][AT];
     __shared__ double red[8][2];
     __shared__ int is_last;
     const double e0 = ctrl->eps_min, e1 = ctrl->eps_max;
@@ -119,11 +121,13 @@ __global__ void __launch_bounds__(256) k_affine_split(const float* __restrict__ 
     for (long long t = blockIdx.x; t < ntiles; t += gridDim.x) {
         int I, J;
         tri_decode(t, I, J);
+        double csq = 0.0;                                    // this thread's column j, rows of this warp
 #pragma unroll
         for (int r = 0; r < 4; ++r) {
             const int li = ty + 8 * r;
             const int i = I * AT + li, j = J * AT + tx;
             float s = 0.f;
+            double rsq = 0.0;
             if (i < N && j <= i) {
                 s = w0 * __ldg(H + (long long)i * ldh + j);
                 if (i == j) s += b0;
@@ -133,12 +137,25 @@ __global__ void __launch_bounds__(256) k_affine_split(const float* __restrict__ 
                 hi[(long long)i * ld + j] = h;
                 lo[(long long)i * ld + j] = l;
                 const double sd = (double)s;
+                rsq = sd * sd;
                 if (i == j) { trS += sd; fro2 += sd * sd; }
-                else fro2 += 2.0 * sd * sd;
+                else { fro2 += 2.0 * sd * sd; csq += rsq; }
             }
             ts[li][tx] = s;
+            if (rowsq) {                                     // row i: sum over this warp's 32 columns (j <= i)
+                rsq = warp_sum(rsq);
+                if (tx == 0 && i < N) atomicAdd(rowsq + i, rowsq_fix(rsq));
+            }
         }
+        colsq[ty][tx] = csq;
         __syncthreads();
+        if (rowsq && ty == 0) {                              // column j (= row j of the mirrored part), j < i only
+            double c = 0.0;
+#pragma unroll
+            for (int w8 = 0; w8 < 8; ++w8) c += colsq[w8][tx];
+            const int j = J * AT + tx;
+            if (j < N && c != 0.0) atomicAdd(rowsq + j, rowsq_fix(c));
+        }
 #pragma unroll
         for (int r = 0; r < 4; ++r) {
             const int lj = ty + 8 * r;                      // row of the mirrored tile = column of the source
@@ -232,14 +249,14 @@ cudaError_t launch_gershgorin(const float* H, int N, long long ldh, double* R, d
 }
 
 cudaError_t launch_affine_split(const float* H, int N, long long ldh, float* S, __half* hi, __half* lo, long long ld,
-                                float scale, Ctrl* ctrl, sp2_layer_stat_t* stats, const double* thetas, int num_sms,
-                                cudaStream_t st) {
+                                float scale, Ctrl* ctrl, sp2_layer_stat_t* stats, const double* thetas,
+                                unsigned long long* rowsq, int num_sms, cudaStream_t st) {
     const int nt = (N + AT - 1) / AT;
     const long long ntiles = (long long)nt * (nt + 1) / 2;
     long long cap = (long long)num_sms * 6;
     if (cap > kMaxPartials) cap = kMaxPartials;
     const int grid = (int)(ntiles < cap ? ntiles : cap);
-    k_affine_split<<<grid, 256, 0, st>>>(H, N, ldh, S, hi, lo, ld, scale, ctrl, stats, thetas);
+    k_affine_split<<<grid, 256, 0, st>>>(H, N, ldh, S, hi, lo, ld, scale, ctrl, stats, thetas, rowsq);
     return cudaGetLastError();
 }
 

@@ -13,8 +13,16 @@ namespace sp2 {
 cudaError_t launch_gershgorin(const float* H, int N, long long ldh, double* R, double* diag, Ctrl* ctrl,
                               double* bounds_out, int num_sms, cudaStream_t st);
 cudaError_t launch_affine_split(const float* H, int N, long long ldh, float* S, __half* hi, __half* lo, long long ld,
-                                float scale, Ctrl* ctrl, sp2_layer_stat_t* stats, const double* thetas, int num_sms,
-                                cudaStream_t st);
+                                float scale, Ctrl* ctrl, sp2_layer_stat_t* stats, const double* thetas,
+                                unsigned long long* rowsq, int num_sms, cudaStream_t st);
+
+// Row sums of squares r_i = sum_j S_ij^2 (= diag(S^2)_i for symmetric S) are kept in 2^44 fixed point so that the
+// atomic accumulation is order-independent (bit-reproducible results).
+constexpr double kRowSqScale = 17592186044416.0;           // 2^44
+constexpr double kRowSqInv = 1.0 / 17592186044416.0;
+__device__ __forceinline__ unsigned long long rowsq_fix(double x) {
+    return (unsigned long long)__double2ll_rn(x * kRowSqScale);
+}
 cudaError_t launch_split(const float* X, int N, long long ldx, __half* hi, __half* lo, long long ldo, float scale,
                          int num_sms, cudaStream_t st);
 
@@ -28,6 +36,8 @@ struct LayerParams {
     float* S;                      // FP32 master, Np x Np, updated in place
     __half* hi_out;                // next layer's operands (the other ping-pong pair)
     __half* lo_out;
+    unsigned long long* rowsq_cur; // r_i of S_{n-1} (read at the diagonal, then zeroed); nullptr = tensor-core diagonal
+    unsigned long long* rowsq_next;// r_i of S_n (accumulated by this launch)
     const int2* tiles;             // supertile list (I, J), I >= J, in launch order
     long long ld;                  // = Np
     int N, Np;
@@ -53,7 +63,7 @@ struct ResidentParams {
     int nocc_is_scalar;
     int N, B;
     int auto_bounds;
-    double eps_min, eps_max, tol, eps_alt;
+    double eps_min, eps_max, tol, eps_alt, noise_kappa;
     int max_layers;
     int mode;                      // MODE_STANDARD / MODE_GENERALIZED
     const double* thetas;          // generalized: [L][3]

@@ -175,7 +175,8 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
         // =============================== epilogue warps (TMEM lane quarter = warp % 4)
         const int q = warp & 3;
         const int rl = q * 32 + lane;                       // accumulator row (TMEM lane) of this thread
-        const float th1s = ((volatile float*)ctrl->theta)[0] * p.inv_scale2;
+        const float th1 = ((volatile float*)ctrl->theta)[0];
+        const float th1s = th1 * p.inv_scale2;
         const float th2 = ((volatile float*)ctrl->theta)[1];
         const float th3 = ((volatile float*)ctrl->theta)[2];
         const float cs = p.scale;
@@ -184,6 +185,8 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
         float* __restrict__ S = p.S;
         __half* __restrict__ HO = p.hi_out;
         __half* __restrict__ LO = p.lo_out;
+        unsigned long long* __restrict__ Rcur = p.rowsq_cur;
+        unsigned long long* __restrict__ Rnext = p.rowsq_next;
         double trS = 0.0, fro2 = 0.0, trX = 0.0;
         int it = 0;
         for (int w = slot; w < n_work; w += nslots, ++it) {
@@ -195,6 +198,7 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
             const int n0 = sj.y * BN;
             const int gi = m0 + rl;
             const int gi_wmin = m0 + q * 32, gi_wmax = gi_wmin + 31;
+            double rowacc = 0.0;                            // sum_j S_n(gi, j)^2 over the own entries (j <= gi) of this tile
             mbar_wait(&tfull_bar[buf], use & 1u);
             tc_fence_after();
             const uint32_t taddr = tmem_base + (uint32_t)(buf * BN) + ((uint32_t)(q * 32) << 16);
@@ -209,16 +213,27 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                 // S_{n-1}: read at the mirrored position (S is exactly symmetric) -> coalesced across the warp
 #pragma unroll
                 for (int c = 0; c < 32; ++c) so[c] = S[(long long)(gj0 + c) * ld + gi];
+                // exact diagonal of X_n: diag(S_{n-1}^2)_i = sum_j S_{n-1}(i,j)^2, accumulated while S_{n-1} was written
+                float xdiag = 0.f;
+                const bool diag_chunk = (gj0 == gi_wmin);
+                if (Rcur != nullptr && diag_chunk) {
+                    xdiag = (float)((double)(long long)Rcur[gi] * kRowSqInv);
+                    Rcur[gi] = 0ull;                        // this buffer is the accumulator of the layer after next
+                }
                 tmem_ld_wait();
                 float sn[32];
                 uint32_t hp[16], lp[16];                    // FP16 pairs (element 2c in the low half)
+                double sq_own = 0.0;
 #pragma unroll
                 for (int c = 0; c < 32; ++c) {
                     const int gj = gj0 + c;
                     const float x = __uint_as_float(v[c]);
-                    float val = fmaf(th1s, x, th2 * so[c]);
                     const bool on_diag = (gj == gi);
-                    if (on_diag && gi < p.N) val += th3;
+                    float val = fmaf(th1s, x, th2 * so[c]);
+                    if (on_diag) {
+                        if (Rcur != nullptr) val = fmaf(th1, xdiag, th2 * so[c]);
+                        if (gi < p.N) val += th3;
+                    }
                     sn[c] = val;
                     __half h, l;
                     split_hi_lo(val, cs, h, l);
@@ -227,8 +242,29 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                     else { hp[c >> 1] = hb; lp[c >> 1] = lb; }
                     const bool own = below || (gj <= gi);
                     const double vd = (double)val;
-                    if (own) fro2 += on_diag ? vd * vd : 2.0 * vd * vd;
+                    if (own) {
+                        sq_own += vd * vd;
+                        if (on_diag) { fro2 += vd * vd; } else { fro2 += 2.0 * vd * vd; }
+                    }
                     if (on_diag) { trS += vd; trX += (double)(x * inv2); }
+                    // column sums below need the square of the strictly-lower own entries only
+                    so[c] = (own && !on_diag) ? val * val : 0.f;
+                }
+                rowacc += sq_own;
+                if (Rnext != nullptr) {
+                    // sum over the warp's 32 rows of so[c] for every column c: butterfly transpose-reduce, lane c
+                    // ends with column c's sum (31 shuffles), then one fixed-point atomic per column.
+#pragma unroll
+                    for (int sft = 16; sft >= 1; sft >>= 1) {
+                        const bool up = (lane & sft) != 0;
+#pragma unroll
+                        for (int i = 0; i < sft; ++i) {
+                            const float send = up ? so[i] : so[i + sft];
+                            const float keep = up ? so[i + sft] : so[i];
+                            so[i] = keep + __shfl_xor_sync(0xffffffffu, send, sft);
+                        }
+                    }
+                    if (so[0] != 0.f) atomicAdd(Rnext + gj0 + lane, rowsq_fix((double)so[0]));
                 }
                 unsigned short* HOu = reinterpret_cast<unsigned short*>(HO);
                 unsigned short* LOu = reinterpret_cast<unsigned short*>(LO);
@@ -267,6 +303,7 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                     }
                 }
             }
+            if (Rnext != nullptr && rowacc != 0.0) atomicAdd(Rnext + gi, rowsq_fix(rowacc));
             // all tcgen05.ld of this accumulator have completed (tmem_ld_wait above): hand it back to the MMA warp
             tc_fence_before();
             __syncwarp();

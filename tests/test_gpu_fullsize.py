@@ -1,0 +1,76 @@
+"""Parity at BASELINE.json's full size (config 3, N = 16384) in the launch configuration bench.py times (default
+options, device-side WHILE graph, automatic tile choice).  The FP64 oracle cannot finish this size in seconds, so
+the result is checked on sampled outputs the oracle computes one by one (closed form D*_ij = sum_{k<N_occ} Q_ik Q_jk,
+Eq. 6) and through properties that hold at any size: trace, idempotency (FP64 product, harness side),
+exact symmetry, commutation with H, per-layer traces against the scalar recursion replayed under the GPU's sigma."""
+import numpy as np
+import pytest
+
+from oracle import sp2_oracle as O
+from paper_2101_06385_b200 import workloads as W
+from tests import parity_util as P
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def big(cuda_device):
+    import torch
+
+    from paper_2101_06385_b200 import api
+
+    torch.cuda.set_device(0)
+    w = W.config3(0, 16384, device="cuda")
+    h = api.Handle(16384, 0, 120)
+    yield api, h, torch, w, torch.from_numpy(w.H32).cuda()
+    h.close()
+
+
+@pytest.mark.parametrize("auto", [False, True])
+def test_config3_full_size(big, auto):
+    api, h, torch, w, H = big
+    N = w.N
+    opts = api.make_opts(bounds=None if auto else w.bounds, tol=w.tol, max_layers=w.max_layers)
+    D, info = h.density_matrix(H, w.N_occ, opts)
+    assert info["status"] == 0 and info["stop_reason"] in (1, 2, 3, 6)
+    used = info["bounds"]
+    assert used[0] <= w.eps.min() and w.eps.max() <= used[1]
+    # sampled entries (half of them on the diagonal, where the tensor core's accumulator is largest)
+    rng = np.random.default_rng(7)
+    ri, ci = rng.integers(0, N, 4096), rng.integers(0, N, 4096)
+    ri[:2048] = ci[:2048]
+    ref = O.closed_form_density_entries(w.Q, w.N_occ, ri, ci)
+    Dc = D.double()
+    err = float(np.abs(Dc[ri, ci].cpu().numpy() - ref).max())
+    tr = float(torch.trace(Dc))
+    idem = float(torch.linalg.norm(Dc @ Dc - Dc) / np.sqrt(N))
+    Hd = H.double()
+    Hs = torch.tril(Hd) + torch.tril(Hd, -1).T
+    comm = float(torch.linalg.norm(Hs @ Dc - Dc @ Hs) / torch.linalg.norm(Hs))
+    print(f"config3 N={N} auto={auto}: layers={info['n_layers']} stop={info['stop_reason']} max sampled err={err:.2e} "
+          f"trace-N_occ={tr - w.N_occ:.3e} idem={idem:.2e} rel commutator={comm:.2e}")
+    assert err <= P.TOL_D
+    assert abs(tr - w.N_occ) <= P.TOL_TRACE_REL * w.N_occ
+    assert idem <= P.TOL_IDEM
+    assert comm <= 1e-3
+    assert torch.equal(D, D.T)
+    # branch sequence / traces per reading C6: scalar recursion on the known eigenvalues
+    st = O.scalar_recursion(w.eps, w.N_occ, used[0], used[1], tol=w.tol, max_layers=w.max_layers)
+    P.branch_prefix_check(info, st, w.N_occ)
+    P.replay_check(info, None, w.N_occ, used, eigs=w.eps)
+    assert info["n_layers"] <= st["n_layers"] + 2 and info["n_layers"] >= st["n_layers"] - 6
+
+
+def test_config3_literal_tensor_core_diagonal_explicit_bounds(big):
+    """exact_diag = 0 (Alg. 2 literally) still meets the bars with caller bounds at full size."""
+    api, h, torch, w, H = big
+    opts = api.make_opts(bounds=w.bounds, tol=w.tol, max_layers=w.max_layers, exact_diag=0)
+    D, info = h.density_matrix(H, w.N_occ, opts)
+    rng = np.random.default_rng(8)
+    ri, ci = rng.integers(0, w.N, 2048), rng.integers(0, w.N, 2048)
+    ri[:1024] = ci[:1024]
+    ref = O.closed_form_density_entries(w.Q, w.N_occ, ri, ci)
+    Dc = D.double()
+    assert float(np.abs(Dc[ri, ci].cpu().numpy() - ref).max()) <= P.TOL_D
+    assert abs(float(torch.trace(Dc)) - w.N_occ) <= P.TOL_TRACE_REL * w.N_occ
+    assert float(torch.linalg.norm(Dc @ Dc - Dc) / np.sqrt(w.N)) <= 2 * P.TOL_IDEM   # noisier stop (C24)

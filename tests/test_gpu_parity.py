@@ -41,7 +41,7 @@ def test_config1_all_tiles_and_control_modes(env, tile, control):
     P.branch_prefix_check(info, st, w.N_occ)
     P.replay_check(info, w.H32, w.N_occ, w.bounds, eigs=w.eps)
     assert abs(info["n_layers"] - st["n_layers"]) <= 2
-    assert info["stop_reason"] in (1, 2, 3)
+    assert info["stop_reason"] in (1, 2, 3, 6)
     assert info["status"] == 0
 
 
