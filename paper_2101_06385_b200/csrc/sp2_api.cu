@@ -113,7 +113,7 @@ extern "C" void sp2_default_opts(sp2_opts_t* o) {
 extern "C" size_t sp2_workspace_bytes(int N_max, int batch_max, int max_layers) {
     if (N_max < 1 || max_layers < 1) return 0;
     const size_t Np = (size_t)round_up(N_max, 256);
-    size_t b = Np * Np * 4 + 4 * Np * Np * 2;                 // S + two hi/lo pairs
+    size_t b = Np * (size_t)ws_ld_f32((int)Np) * 4 + 4 * Np * (size_t)ws_ld_f16((int)Np) * 2;   // S + two hi/lo pairs
     b += 4 * Np * sizeof(double);                             // Gershgorin radii, diagonal, two row-sum vectors
     b += sizeof(Ctrl) + (size_t)max_layers * (sizeof(sp2_layer_stat_t) + 3 * sizeof(double));
     b += (Np / 128) * (Np / 128 + 1) / 2 * sizeof(int2);
@@ -166,9 +166,9 @@ extern "C" sp2_status_t sp2_create(sp2_handle_t* out, int N_max, int batch_max, 
         cudaError_t e = cudaMalloc(p, bytes);
         if (e != cudaSuccess) st = cuda_fail(e, "cudaMalloc(workspace)");
     };
-    A((void**)&h->S, Np * Np * 4);
+    A((void**)&h->S, Np * (size_t)ws_ld_f32(h->Np_max) * 4);
     for (int a = 0; a < 2; ++a)
-        for (int b = 0; b < 2; ++b) A((void**)&h->hl[a][b], Np * Np * 2);
+        for (int b = 0; b < 2; ++b) A((void**)&h->hl[a][b], Np * (size_t)ws_ld_f16(h->Np_max) * 2);
     A((void**)&h->R, Np * sizeof(double));
     A((void**)&h->diag, Np * sizeof(double));
     A((void**)&h->rowsq[0], Np * sizeof(unsigned long long));
@@ -219,10 +219,11 @@ extern "C" sp2_status_t sp2_create(sp2_handle_t* out, int N_max, int batch_max, 
     return SP2_OK;
 }
 
-// K-major FP16 operand map: Np x Np row-major, box = 64 (K) x 128 (rows), 128-byte swizzle.
+// K-major FP16 operand map: Np x Np row-major (leading dimension ws_ld_f16), box = 64 (K) x 128 (rows),
+// 128-byte swizzle.
 static sp2_status_t make_tmap(sp2_handle_s* h, CUtensorMap* tm, void* base, int Np) {
     cuuint64_t gdim[2] = {(cuuint64_t)Np, (cuuint64_t)Np};
-    cuuint64_t gstr[1] = {(cuuint64_t)Np * 2};
+    cuuint64_t gstr[1] = {(cuuint64_t)ws_ld_f16(Np) * 2};
     cuuint32_t box[2] = {64, 128};
     cuuint32_t estr[2] = {1, 1};
     CUresult r = h->encode(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, base, gdim, gstr, box, estr,
@@ -298,7 +299,7 @@ static LayerParams layer_params(sp2_handle_s* h, const Problem& pb, int parity, 
     p.hi_out = h->hl[parity ^ 1][0]; p.lo_out = h->hl[parity ^ 1][1];
     p.rowsq_cur = pb.exact_diag ? h->rowsq[parity] : nullptr;
     p.rowsq_next = pb.exact_diag ? h->rowsq[parity ^ 1] : nullptr;
-    p.tiles = h->tiles_dev; p.ld = pb.Np; p.N = pb.N; p.Np = pb.Np; p.n_super = pb.n_super;
+    p.tiles = h->tiles_dev; p.ld = ws_ld_f32(pb.Np); p.ldf = ws_ld_f16(pb.Np); p.N = pb.N; p.Np = pb.Np; p.n_super = pb.n_super;
     p.scale = pb.scale; p.inv_scale2 = pb.inv_scale2; p.cond_handle = cond;
     return p;
 }
@@ -375,11 +376,11 @@ static sp2_status_t solve_single(sp2_handle_s* h, const float* H_dev, int N, int
                            cudaMemcpyHostToDevice, st));
     CK(cudaMemsetAsync(h->stats_dev, 0, (size_t)max_layers * sizeof(sp2_layer_stat_t), st));
     // ---- padding rows/columns of S_0 are zero (inert: eigenvalue 0 is a fixed point of both branches)
-    const size_t NpNp = (size_t)pb.Np * pb.Np;
+    const size_t ldS = (size_t)ws_ld_f32(pb.Np), ldF = (size_t)ws_ld_f16(pb.Np);
     if (pb.Np != N) {
-        CK(cudaMemsetAsync(h->S, 0, NpNp * 4, st));
-        CK(cudaMemsetAsync(h->hl[0][0], 0, NpNp * 2, st));
-        CK(cudaMemsetAsync(h->hl[0][1], 0, NpNp * 2, st));
+        CK(cudaMemsetAsync(h->S, 0, (size_t)pb.Np * ldS * 4, st));
+        CK(cudaMemsetAsync(h->hl[0][0], 0, (size_t)pb.Np * ldF * 2, st));
+        CK(cudaMemsetAsync(h->hl[0][1], 0, (size_t)pb.Np * ldF * 2, st));
     }
     // ---- a1: bounds, a2: initial affine layer + first split + first control step
     if (o->auto_bounds) CK(launch_gershgorin(H_dev, N, ldh, h->R, h->diag, h->ctrl, nullptr, h->num_sms, st));
@@ -387,7 +388,7 @@ static sp2_status_t solve_single(sp2_handle_s* h, const float* H_dev, int N, int
         CK(cudaMemsetAsync(h->rowsq[0], 0, (size_t)pb.Np * sizeof(unsigned long long), st));
         CK(cudaMemsetAsync(h->rowsq[1], 0, (size_t)pb.Np * sizeof(unsigned long long), st));
     }
-    CK(launch_affine_split(H_dev, N, ldh, h->S, h->hl[0][0], h->hl[0][1], pb.Np, pb.scale, h->ctrl, h->stats_dev,
+    CK(launch_affine_split(H_dev, N, ldh, h->S, h->hl[0][0], h->hl[0][1], (long long)ldS, (long long)ldF, pb.scale, h->ctrl, h->stats_dev,
                            h->thetas_dev, pb.exact_diag ? h->rowsq[0] : nullptr, h->num_sms, st));
     // ---- a4-a8: the layer loop
     if (o->control == 0) {
@@ -410,7 +411,7 @@ static sp2_status_t solve_single(sp2_handle_s* h, const float* H_dev, int N, int
         }
     }
     // ---- results
-    CK(cudaMemcpy2DAsync(D_dev, (size_t)ldd * 4, h->S, (size_t)pb.Np * 4, (size_t)N * 4, (size_t)N,
+    CK(cudaMemcpy2DAsync(D_dev, (size_t)ldd * 4, h->S, ldS * 4, (size_t)N * 4, (size_t)N,
                          cudaMemcpyDeviceToDevice, st));
     CK(cudaMemcpyAsync(h->ctrl_host, h->ctrl, ctrl_header_bytes(), cudaMemcpyDeviceToHost, st));
     CK(cudaMemcpyAsync(h->stats_host, h->stats_dev, (size_t)max_layers * sizeof(sp2_layer_stat_t),

@@ -97,7 +97,8 @@ __global__ void __launch_bounds__(1024) k_gershgorin_finalize(const double* __re
 constexpr int AT = 32;
 __global__ void __launch_bounds__(256) k_affine_split(const float* __restrict__ H, int N, long long ldh,
                                                       float* __restrict__ S, __half* __restrict__ hi,
-                                                      __half* __restrict__ lo, long long ld, float scale, Ctrl* ctrl,
+                                                      __half* __restrict__ lo, long long ld, long long ldf,
+                                                      float scale, Ctrl* ctrl,
                                                       sp2_layer_stat_t* stats, const double* thetas,
                                                       unsigned long long* __restrict__ rowsq) {
     __shared__ float ts[AT][AT + 1];
@@ -134,8 +135,8 @@ __global__ void __launch_bounds__(256) k_affine_split(const float* __restrict__ 
                 S[(long long)i * ld + j] = s;
                 __half h, l;
                 split_hi_lo(s, scale, h, l);
-                hi[(long long)i * ld + j] = h;
-                lo[(long long)i * ld + j] = l;
+                hi[(long long)i * ldf + j] = h;
+                lo[(long long)i * ldf + j] = l;
                 const double sd = (double)s;
                 rsq = sd * sd;
                 if (i == j) { trS += sd; fro2 += sd * sd; }
@@ -165,8 +166,8 @@ __global__ void __launch_bounds__(256) k_affine_split(const float* __restrict__ 
                 S[(long long)jj * ld + ii] = s;
                 __half h, l;
                 split_hi_lo(s, scale, h, l);
-                hi[(long long)jj * ld + ii] = h;
-                lo[(long long)jj * ld + ii] = l;
+                hi[(long long)jj * ldf + ii] = h;
+                lo[(long long)jj * ldf + ii] = l;
             }
         }
         __syncthreads();
@@ -249,14 +250,14 @@ cudaError_t launch_gershgorin(const float* H, int N, long long ldh, double* R, d
 }
 
 cudaError_t launch_affine_split(const float* H, int N, long long ldh, float* S, __half* hi, __half* lo, long long ld,
-                                float scale, Ctrl* ctrl, sp2_layer_stat_t* stats, const double* thetas,
+                                long long ldf, float scale, Ctrl* ctrl, sp2_layer_stat_t* stats, const double* thetas,
                                 unsigned long long* rowsq, int num_sms, cudaStream_t st) {
     const int nt = (N + AT - 1) / AT;
     const long long ntiles = (long long)nt * (nt + 1) / 2;
     long long cap = (long long)num_sms * 6;
     if (cap > kMaxPartials) cap = kMaxPartials;
     const int grid = (int)(ntiles < cap ? ntiles : cap);
-    k_affine_split<<<grid, 256, 0, st>>>(H, N, ldh, S, hi, lo, ld, scale, ctrl, stats, thetas, rowsq);
+    k_affine_split<<<grid, 256, 0, st>>>(H, N, ldh, S, hi, lo, ld, ldf, scale, ctrl, stats, thetas, rowsq);
     return cudaGetLastError();
 }
 

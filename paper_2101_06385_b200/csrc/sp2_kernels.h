@@ -13,7 +13,7 @@ namespace sp2 {
 cudaError_t launch_gershgorin(const float* H, int N, long long ldh, double* R, double* diag, Ctrl* ctrl,
                               double* bounds_out, int num_sms, cudaStream_t st);
 cudaError_t launch_affine_split(const float* H, int N, long long ldh, float* S, __half* hi, __half* lo, long long ld,
-                                float scale, Ctrl* ctrl, sp2_layer_stat_t* stats, const double* thetas,
+                                long long ldf, float scale, Ctrl* ctrl, sp2_layer_stat_t* stats, const double* thetas,
                                 unsigned long long* rowsq, int num_sms, cudaStream_t st);
 
 // Row sums of squares r_i = sum_j S_ij^2 (= diag(S^2)_i for symmetric S) are kept in 2^44 fixed point so that the
@@ -25,6 +25,12 @@ __device__ __forceinline__ unsigned long long rowsq_fix(double x) {
 }
 cudaError_t launch_split(const float* X, int N, long long ldx, __half* hi, __half* lo, long long ldo, float scale,
                          int num_sms, cudaStream_t st);
+
+// Leading dimensions of the workspace matrices: rows are padded by 128 bytes so that walking down a column (the
+// mirrored accesses of the epilogue, the 128-byte rows of a TMA box) does not stride by a power of two, which
+// would map a whole panel slice onto a few L2 sets.
+inline long long ws_ld_f32(int Np) { return (long long)Np + 32; }
+inline long long ws_ld_f16(int Np) { return (long long)Np + 64; }
 
 // ---- fused symmetric square layer (sp2_square_tiled.cu)
 enum TileConfig { TILE_AUTO = 0, TILE_128x128 = 1, TILE_128x256 = 2, TILE_256x256_PAIR = 3 };
@@ -39,7 +45,8 @@ struct LayerParams {
     unsigned long long* rowsq_cur; // r_i of S_{n-1} (read at the diagonal, then zeroed); nullptr = tensor-core diagonal
     unsigned long long* rowsq_next;// r_i of S_n (accumulated by this launch)
     const int2* tiles;             // supertile list (I, J), I >= J, in launch order
-    long long ld;                  // = Np
+    long long ld;                  // leading dimension of S (floats)
+    long long ldf;                 // leading dimension of hi/lo (halves)
     int N, Np;
     int n_super;                   // number of supertiles
     float scale;                   // c = 2^k of the split

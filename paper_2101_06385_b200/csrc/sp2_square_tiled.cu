@@ -181,13 +181,17 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
         const float th3 = ((volatile float*)ctrl->theta)[2];
         const float cs = p.scale;
         const float inv2 = p.inv_scale2;
-        const long long ld = p.ld;
+        const long long ld = p.ld, ldf = p.ldf;
         float* __restrict__ S = p.S;
         __half* __restrict__ HO = p.hi_out;
         __half* __restrict__ LO = p.lo_out;
         unsigned long long* __restrict__ Rcur = p.rowsq_cur;
         unsigned long long* __restrict__ Rnext = p.rowsq_next;
-        double trS = 0.0, fro2 = 0.0, trX = 0.0;
+        // FP64 is kept off the per-element path (the FP64 pipe of sm_100 is narrow: per-element DMUL/DFMA made the
+        // epilogue as long as the mainloop).  Off-diagonal squares are summed in FP32 over one 32-element chunk
+        // (4 independent partial sums, |error| <= ~2^-22 of a sum of ~1e-3) and promoted to FP64 once per chunk;
+        // the diagonal chunk (one per 128 rows of a diagonal supertile) keeps per-element FP64.
+        double trS = 0.0, off2 = 0.0, dg2 = 0.0, trX = 0.0;   // ||S_n||_F^2 = 2 off2 + dg2
         int it = 0;
         for (int w = slot; w < n_work; w += nslots, ++it) {
             const int buf = it & 1;
@@ -202,6 +206,8 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
             mbar_wait(&tfull_bar[buf], use & 1u);
             tc_fence_after();
             const uint32_t taddr = tmem_base + (uint32_t)(buf * BN) + ((uint32_t)(q * 32) << 16);
+            unsigned short* HOu = reinterpret_cast<unsigned short*>(HO);
+            unsigned short* LOu = reinterpret_cast<unsigned short*>(LO);
 #pragma unroll 1
             for (int c0 = 0; c0 < BN; c0 += 32) {
                 const int gj0 = n0 + c0;
@@ -213,44 +219,80 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                 // S_{n-1}: read at the mirrored position (S is exactly symmetric) -> coalesced across the warp
 #pragma unroll
                 for (int c = 0; c < 32; ++c) so[c] = S[(long long)(gj0 + c) * ld + gi];
-                // exact diagonal of X_n: diag(S_{n-1}^2)_i = sum_j S_{n-1}(i,j)^2, accumulated while S_{n-1} was written
-                float xdiag = 0.f;
-                const bool diag_chunk = (gj0 == gi_wmin);
-                if (Rcur != nullptr && diag_chunk) {
-                    xdiag = (float)((double)(long long)Rcur[gi] * kRowSqInv);
-                    Rcur[gi] = 0ull;                        // this buffer is the accumulator of the layer after next
-                }
-                tmem_ld_wait();
-                float sn[32];
-                uint32_t hp[16], lp[16];                    // FP16 pairs (element 2c in the low half)
-                double sq_own = 0.0;
+                if (below) {
+                    tmem_ld_wait();
+                    float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
+                    float* __restrict__ rowS = S + (long long)gi * ld + gj0;          // own position
+                    __half* __restrict__ rowH = HO + (long long)gi * ldf + gj0;
+                    __half* __restrict__ rowL = LO + (long long)gi * ldf + gj0;
 #pragma unroll
-                for (int c = 0; c < 32; ++c) {
-                    const int gj = gj0 + c;
-                    const float x = __uint_as_float(v[c]);
-                    const bool on_diag = (gj == gi);
-                    float val = fmaf(th1s, x, th2 * so[c]);
-                    if (on_diag) {
-                        if (Rcur != nullptr) val = fmaf(th1, xdiag, th2 * so[c]);
-                        if (gi < p.N) val += th3;
+                    for (int g = 0; g < 4; ++g) {           // 8 columns at a time: values leave registers early
+                        float sn[8];
+                        uint32_t hp[4], lp[4];              // FP16 pairs (even column in the low half)
+#pragma unroll
+                        for (int e = 0; e < 8; ++e) {
+                            const int c = 8 * g + e;
+                            const float val = fmaf(th1s, __uint_as_float(v[c]), th2 * so[c]);
+                            sn[e] = val;
+                            __half h, l;
+                            split_hi_lo(val, cs, h, l);
+                            const uint32_t hb = __half_as_ushort(h), lb = __half_as_ushort(l);
+                            if (e & 1) { hp[e >> 1] |= hb << 16; lp[e >> 1] |= lb << 16; }
+                            else { hp[e >> 1] = hb; lp[e >> 1] = lb; }
+                            const float sq = val * val;
+                            so[c] = sq;                     // column sums below: square of the mirrored entry
+                            if ((e & 3) == 0) a0 += sq; else if ((e & 3) == 1) a1 += sq;
+                            else if ((e & 3) == 2) a2 += sq; else a3 += sq;
+                            // mirrored position: one 128-byte (FP32) / 64-byte (FP16) warp store per column
+                            S[(long long)(gj0 + c) * ld + gi] = val;
+                            const long long o = (long long)(gj0 + c) * ldf + gi;
+                            HOu[o] = (unsigned short)hb;
+                            LOu[o] = (unsigned short)lb;
+                        }
+                        // own position: 32 contiguous bytes (FP32) / 16 (FP16) per thread per group
+                        reinterpret_cast<float4*>(rowS)[2 * g] = make_float4(sn[0], sn[1], sn[2], sn[3]);
+                        reinterpret_cast<float4*>(rowS)[2 * g + 1] = make_float4(sn[4], sn[5], sn[6], sn[7]);
+                        reinterpret_cast<uint4*>(rowH)[g] = make_uint4(hp[0], hp[1], hp[2], hp[3]);
+                        reinterpret_cast<uint4*>(rowL)[g] = make_uint4(lp[0], lp[1], lp[2], lp[3]);
                     }
-                    sn[c] = val;
-                    __half h, l;
-                    split_hi_lo(val, cs, h, l);
-                    const uint32_t hb = __half_as_ushort(h), lb = __half_as_ushort(l);
-                    if (c & 1) { hp[c >> 1] |= hb << 16; lp[c >> 1] |= lb << 16; }
-                    else { hp[c >> 1] = hb; lp[c >> 1] = lb; }
-                    const bool own = below || (gj <= gi);
-                    const double vd = (double)val;
-                    if (own) {
-                        sq_own += vd * vd;
-                        if (on_diag) { fro2 += vd * vd; } else { fro2 += 2.0 * vd * vd; }
+                    const double sd = (double)((a0 + a1) + (a2 + a3));
+                    off2 += sd;
+                    rowacc += sd;
+                } else {
+                    // diagonal chunk: only gj <= gi is authoritative (exact symmetry inside the tile).  Exact diagonal
+                    // of X_n: diag(S_{n-1}^2)_i = sum_j S_{n-1}(i,j)^2, accumulated while S_{n-1} was written
+                    float xdiag = 0.f;
+                    if (Rcur != nullptr) {
+                        xdiag = (float)((double)(long long)Rcur[gi] * kRowSqInv);
+                        Rcur[gi] = 0ull;                    // this buffer is the accumulator of the layer after next
                     }
-                    if (on_diag) { trS += vd; trX += (double)(x * inv2); }
-                    // column sums below need the square of the strictly-lower own entries only
-                    so[c] = (own && !on_diag) ? val * val : 0.f;
+                    tmem_ld_wait();
+                    double sq_own = 0.0;
+#pragma unroll
+                    for (int c = 0; c < 32; ++c) {
+                        const int gj = gj0 + c;
+                        const float x = __uint_as_float(v[c]);
+                        const bool on_diag = (gj == gi);
+                        float val = fmaf(th1s, x, th2 * so[c]);
+                        if (on_diag) {
+                            if (Rcur != nullptr) val = fmaf(th1, xdiag, th2 * so[c]);
+                            if (gi < p.N) val += th3;
+                        }
+                        __half h, l;
+                        split_hi_lo(val, cs, h, l);
+                        const unsigned short hb = __half_as_ushort(h), lb = __half_as_ushort(l);
+                        const double vd = (double)val;
+                        if (gj < gi) { sq_own += vd * vd; off2 += vd * vd; }
+                        if (on_diag) { sq_own += vd * vd; dg2 += vd * vd; trS += vd; trX += (double)(x * inv2); }
+                        so[c] = (gj < gi) ? val * val : 0.f;
+                        if (gj <= gi) {
+                            const long long o = (long long)gj * ldf + gi, o2 = (long long)gi * ldf + gj;
+                            S[(long long)gj * ld + gi] = val; HOu[o] = hb; LOu[o] = lb;
+                            S[(long long)gi * ld + gj] = val; HOu[o2] = hb; LOu[o2] = lb;
+                        }
+                    }
+                    rowacc += sq_own;
                 }
-                rowacc += sq_own;
                 if (Rnext != nullptr) {
                     // sum over the warp's 32 rows of so[c] for every column c: butterfly transpose-reduce, lane c
                     // ends with column c's sum (31 shuffles), then one fixed-point atomic per column.
@@ -266,42 +308,6 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                     }
                     if (so[0] != 0.f) atomicAdd(Rnext + gj0 + lane, rowsq_fix((double)so[0]));
                 }
-                unsigned short* HOu = reinterpret_cast<unsigned short*>(HO);
-                unsigned short* LOu = reinterpret_cast<unsigned short*>(LO);
-                if (below) {
-                    // mirrored position: one 128-byte (FP32) / 64-byte (FP16) warp store per column
-#pragma unroll
-                    for (int c = 0; c < 32; ++c) {
-                        const long long o = (long long)(gj0 + c) * ld + gi;
-                        S[o] = sn[c];
-                        HOu[o] = (unsigned short)(hp[c >> 1] >> (16 * (c & 1)));
-                        LOu[o] = (unsigned short)(lp[c >> 1] >> (16 * (c & 1)));
-                    }
-                    // own position: 128 contiguous bytes (FP32) / 64 (FP16) per thread
-                    float4* dS = reinterpret_cast<float4*>(S + (long long)gi * ld + gj0);
-                    uint4* dH = reinterpret_cast<uint4*>(HO + (long long)gi * ld + gj0);
-                    uint4* dL = reinterpret_cast<uint4*>(LO + (long long)gi * ld + gj0);
-#pragma unroll
-                    for (int c = 0; c < 8; ++c) dS[c] = make_float4(sn[4 * c], sn[4 * c + 1], sn[4 * c + 2], sn[4 * c + 3]);
-#pragma unroll
-                    for (int c = 0; c < 4; ++c) {
-                        dH[c] = make_uint4(hp[4 * c], hp[4 * c + 1], hp[4 * c + 2], hp[4 * c + 3]);
-                        dL[c] = make_uint4(lp[4 * c], lp[4 * c + 1], lp[4 * c + 2], lp[4 * c + 3]);
-                    }
-                } else {
-                    // chunk crosses the diagonal: only gj <= gi is authoritative (exact symmetry inside the tile)
-#pragma unroll
-                    for (int c = 0; c < 32; ++c) {
-                        const int gj = gj0 + c;
-                        if (gj <= gi) {
-                            const long long o = (long long)gj * ld + gi, o2 = (long long)gi * ld + gj;
-                            const unsigned short hb = (unsigned short)(hp[c >> 1] >> (16 * (c & 1)));
-                            const unsigned short lb = (unsigned short)(lp[c >> 1] >> (16 * (c & 1)));
-                            S[o] = sn[c]; HOu[o] = hb; LOu[o] = lb;
-                            S[o2] = sn[c]; HOu[o2] = hb; LOu[o2] = lb;
-                        }
-                    }
-                }
             }
             if (Rnext != nullptr && rowacc != 0.0) atomicAdd(Rnext + gi, rowsq_fix(rowacc));
             // all tcgen05.ld of this accumulator have completed (tmem_ld_wait above): hand it back to the MMA warp
@@ -312,6 +318,7 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
             }
         }
         // ---- block partials -> ctrl -> last CTA runs the control step
+        double fro2 = 2.0 * off2 + dg2;
         for (int o = 16; o > 0; o >>= 1) {
             trS += __shfl_xor_sync(0xffffffffu, trS, o);
             fro2 += __shfl_xor_sync(0xffffffffu, fro2, o);
