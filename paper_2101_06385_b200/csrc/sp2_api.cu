@@ -73,6 +73,8 @@ struct sp2_handle_s {
     int n_super = 0;
     int last_launches = 0;
     double noise_kappa = 0.125;
+    int l2_prefetch = 0;
+    int round_sync = 1;
     cudaStream_t cap_stream = nullptr;
 };
 
@@ -157,6 +159,8 @@ extern "C" sp2_status_t sp2_create(sp2_handle_t* out, int N_max, int batch_max, 
     sp2_handle_s* h = new sp2_handle_s();
     h->N_max = N_max; h->batch_max = batch_max; h->max_layers = max_layers;
     if (const char* e = getenv("SP2_NOISE_KAPPA")) h->noise_kappa = atof(e);   // tuning hook (C25)
+    if (const char* e = getenv("SP2_L2_PREFETCH")) h->l2_prefetch = atoi(e);   // tuning hook
+    if (const char* e = getenv("SP2_ROUND_SYNC")) h->round_sync = atoi(e);     // tuning hook
     h->Np_max = round_up(N_max, 256);
     h->num_sms = prop.multiProcessorCount; h->device = dev;
     const size_t Np = (size_t)h->Np_max;
@@ -238,12 +242,24 @@ static sp2_status_t make_tmap(sp2_handle_s* h, CUtensorMap* tm, void* base, int 
 
 // Supertile launch order over the lower triangle: bands of `band` supertile rows, column-major inside a band, so
 // that the CTAs resident at the same time share few row panels (L2 reuse of the operands).
-static void build_tile_order(int nt, int band, std::vector<int2>& out) {
+static void build_tile_order(int nt, int band, int round, std::vector<int2>& out) {
     out.clear();
     for (int i0 = 0; i0 < nt; i0 += band) {
         const int i1 = (i0 + band < nt) ? i0 + band : nt;
         for (int j = 0; j < i1; ++j)
             for (int i = (j > i0 ? j : i0); i < i1; ++i) out.push_back(make_int2(i, j));
+    }
+    // L2 prefetch ownership: within each round (`round` consecutive entries run concurrently, one per CTA slot) the
+    // first tile that touches a row panel prefetches it (as its A panel if it is the tile's I, as its B panel if J).
+    if (round < 1) return;
+    std::vector<int> seen((size_t)nt, -1);
+    for (size_t t = 0; t < out.size(); ++t) {
+        const int r = (int)(t / (size_t)round);
+        const int I = out[t].x, J = out[t].y;
+        int flags = 0;
+        if (seen[I] != r) { seen[I] = r; flags |= kTilePrefetchA; }
+        if (seen[J] != r) { seen[J] = r; flags |= kTilePrefetchB; }
+        out[t].y = J | flags;
     }
 }
 
@@ -281,7 +297,7 @@ static sp2_status_t prepare_problem(sp2_handle_s* h, int N, const sp2_opts_t* o,
     const int band = (pb->cfg == TILE_256x256_PAIR) ? 8 : 12;
     if (h->tiles_key_nt != nt || h->tiles_key_band != band) {
         std::vector<int2> order;
-        build_tile_order(nt, band, order);
+        build_tile_order(nt, band, pb->cfg == TILE_256x256_PAIR ? h->num_sms / 2 : 0, order);
         if ((int)order.size() > h->tiles_cap) return SP2_ERR_WORKSPACE;
         // synchronous small copy: happens only when the problem shape changes
         CK(cudaMemcpyAsync(h->tiles_dev, order.data(), order.size() * sizeof(int2), cudaMemcpyHostToDevice, st));
@@ -300,7 +316,7 @@ static LayerParams layer_params(sp2_handle_s* h, const Problem& pb, int parity, 
     p.rowsq_cur = pb.exact_diag ? h->rowsq[parity] : nullptr;
     p.rowsq_next = pb.exact_diag ? h->rowsq[parity ^ 1] : nullptr;
     p.tiles = h->tiles_dev; p.ld = ws_ld_f32(pb.Np); p.ldf = ws_ld_f16(pb.Np); p.N = pb.N; p.Np = pb.Np; p.n_super = pb.n_super;
-    p.scale = pb.scale; p.inv_scale2 = pb.inv_scale2; p.cond_handle = cond;
+    p.scale = pb.scale; p.inv_scale2 = pb.inv_scale2; p.cond_handle = cond; p.l2_prefetch = h->l2_prefetch; p.round_sync = h->round_sync;
     return p;
 }
 

@@ -32,7 +32,7 @@ struct CtrlCore {
     double noise_kappa;              // reading C25: stop when IdErr_n <= kappa |Tr X_n(tc) - N_X|; 0 disables
     float  theta[4];                 // th1, th2, th3 of the NEXT layer (FP32: the epilogue's arithmetic type)
     unsigned int done_counter;       // CTAs finished in the current kernel
-    unsigned int pad_;
+    unsigned int round_counter;      // CTAs that reached a round boundary of the current layer kernel (round sync)
 };
 struct Ctrl : CtrlCore {
     double partial[kMaxPartials][4]; // per-CTA {Tr S, ||S||_F^2, Tr X (diag), unused}
@@ -108,6 +108,7 @@ __device__ inline void control_finish_layer(CtrlCore* c, sp2_layer_stat_t* stats
         stats[c->n - 1].t_end_ns = t;
     }
     c->done_counter = 0;
+    c->round_counter = 0;
     // Reading C25: "IdErr_n <= 0" at the resolution of the arithmetic.  iderr_prev = IdErr_n of the layer just
     // applied; |trX - nx_inflight| = measured error of the tensor-core trace of X_n.
     if (c->mode == MODE_STANDARD && c->pending_stop == SP2_STOP_NONE && c->n > 2 &&

@@ -35,6 +35,10 @@ inline long long ws_ld_f16(int Np) { return (long long)Np + 64; }
 // ---- fused symmetric square layer (sp2_square_tiled.cu)
 enum TileConfig { TILE_AUTO = 0, TILE_128x128 = 1, TILE_128x256 = 2, TILE_256x256_PAIR = 3 };
 
+// flag bits in tiles[].y (J is the low 16 bits): this tile issues the L2 prefetches of its A / B panel
+constexpr int kTilePrefetchA = 1 << 16;
+constexpr int kTilePrefetchB = 1 << 17;
+
 struct LayerParams {
     Ctrl* ctrl;
     sp2_layer_stat_t* stats;
@@ -44,13 +48,15 @@ struct LayerParams {
     __half* lo_out;
     unsigned long long* rowsq_cur; // r_i of S_{n-1} (read at the diagonal, then zeroed); nullptr = tensor-core diagonal
     unsigned long long* rowsq_next;// r_i of S_n (accumulated by this launch)
-    const int2* tiles;             // supertile list (I, J), I >= J, in launch order
+    const int2* tiles;             // supertile list (I, J | flags), I >= J, in launch order
     long long ld;                  // leading dimension of S (floats)
     long long ldf;                 // leading dimension of hi/lo (halves)
     int N, Np;
     int n_super;                   // number of supertiles
     float scale;                   // c = 2^k of the split
     float inv_scale2;              // 1 / c^2
+    int l2_prefetch;               // L2 prefetch lead of the TMA producer in k-blocks (0 = off)
+    int round_sync;                // 1: producers of all CTAs meet at every round boundary (keeps the wave in lockstep)
     unsigned long long cond_handle;  // cudaGraphConditionalHandle (0 = none)
 };
 

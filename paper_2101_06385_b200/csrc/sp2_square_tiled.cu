@@ -72,7 +72,7 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
     if (warp == 1) {
         if (lane == 0) {
             for (int s = 0; s < STAGES; ++s) {
-                mbar_init(&full_bar[s], CG);
+                mbar_init(&full_bar[s], 1);           // leader's arrive.expect_tx only; the peer's bytes are counted too
                 mbar_init(&empty_bar[s], 1);
             }
             for (int b = 0; b < 2; ++b) {
@@ -95,35 +95,90 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
         if (lane == 0) {
             int s = 0;
             uint32_t ph = 0;
-            for (int w = slot; w < n_work; w += nslots) {
+            const uint64_t pol = l2_policy_evict_last();     // operand panels: reused by the other CTAs of the wave
+            // L2 prefetch cursor, PF k-blocks ahead of the loads (across tile boundaries): the loads then hit L2 and
+            // the three smem stages only have to cover L2 latency, not HBM latency.
+            // Only the first tile of a round (= nslots consecutive list entries, which run concurrently) that uses
+            // a panel prefetches it (flag bits set by the host in tiles[].y): every panel slice is requested from
+            // HBM once per round instead of once per CTA.
+            const int PF = p.l2_prefetch;                   // k-blocks of lead; 0 = off
+            int w_pf = slot, kb_pf = 0, m0_pf = 0, n0_pf = 0;
+            bool pfA = false, pfB = false;
+            auto pf_tile = [&]() {
+                if (w_pf < n_work) {
+                    const int2 t = p.tiles[w_pf / C::SUB];
+                    m0_pf = t.x * BN + ((w_pf % C::SUB) * CG + (int)rank) * BM;
+                    n0_pf = (t.y & 0xffff) * BN + (int)rank * C::BNL;
+                    pfA = (t.y & kTilePrefetchA) != 0;
+                    pfB = (t.y & kTilePrefetchB) != 0;
+                }
+            };
+            auto pf_step = [&]() {
+                if (w_pf >= n_work) return;
+                const int k0 = kb_pf * BK;
+                if (pfA) {
+                    tma_prefetch_l2_2d(&tm_hi, k0, m0_pf, pol);
+                    tma_prefetch_l2_2d(&tm_lo, k0, m0_pf, pol);
+                }
+                if (pfB) {
+#pragma unroll
+                    for (int h = 0; h < C::BNL / 128; ++h) {
+                        tma_prefetch_l2_2d(&tm_hi, k0, n0_pf + h * 128, pol);
+                        tma_prefetch_l2_2d(&tm_lo, k0, n0_pf + h * 128, pol);
+                    }
+                }
+                if (++kb_pf == KB) { kb_pf = 0; w_pf += nslots; pf_tile(); }
+            };
+            pf_tile();
+            for (int i = 0; i < PF; ++i) pf_step();
+            // Round sync: the CTAs of a round share row panels through L2 only while they walk K together.  Nothing
+            // else keeps them together (each runs its tiles back to back), so every producer checks in at each round
+            // boundary and starts the next tile's loads when all have (bounded spin: never a hang, at worst no sync).
+            const int n_rounds = (n_work + nslots - 1) / nslots;
+            int round = 0;
+            for (int w = slot; ; w += nslots, ++round) {
+                if (p.round_sync && round > 0 && round < n_rounds) {
+                    __threadfence();
+                    atomicAdd(&ctrl->round_counter, 1u);
+                    if (w < n_work) {
+                        const unsigned int target = (unsigned int)round * gridDim.x;
+                        unsigned int spins = 0;
+                        while (*((volatile unsigned int*)&ctrl->round_counter) < target && ++spins < (1u << 16))
+                            __nanosleep(64);
+                    }
+                }
+                if (w >= n_work) break;
                 const int2 sj = p.tiles[w / C::SUB];
                 const int sub = w % C::SUB;
                 const int m0 = sj.x * BN + (sub * CG + (int)rank) * BM;      // A rows of this CTA
-                const int n0 = sj.y * BN + (int)rank * C::BNL;               // B rows this CTA loads
+                const int n0 = (sj.y & 0xffff) * BN + (int)rank * C::BNL;    // B rows this CTA loads
                 for (int kb = 0; kb < KB; ++kb) {
+                    if (PF > 0) pf_step();
                     mbar_wait(&empty_bar[s], ph ^ 1u);
                     uint8_t* st = smem + s * C::STAGE_BYTES;
                     const int k0 = kb * BK;
                     if (CG == 1) {
                         mbar_arrive_expect_tx(&full_bar[s], C::STAGE_BYTES);
-                        tma_load_2d(st, &tm_hi, &full_bar[s], k0, m0);
-                        tma_load_2d(st + C::A_BYTES, &tm_lo, &full_bar[s], k0, m0);
+                        tma_load_2d_hint(st, &tm_hi, &full_bar[s], k0, m0, pol);
+                        tma_load_2d_hint(st + C::A_BYTES, &tm_lo, &full_bar[s], k0, m0, pol);
 #pragma unroll
                         for (int h = 0; h < C::BNL / 128; ++h) {
-                            tma_load_2d(st + 2 * C::A_BYTES + h * 16384, &tm_hi, &full_bar[s], k0, n0 + h * 128);
-                            tma_load_2d(st + 2 * C::A_BYTES + C::B_BYTES + h * 16384, &tm_lo, &full_bar[s], k0,
-                                        n0 + h * 128);
+                            tma_load_2d_hint(st + 2 * C::A_BYTES + h * 16384, &tm_hi, &full_bar[s], k0, n0 + h * 128, pol);
+                            tma_load_2d_hint(st + 2 * C::A_BYTES + C::B_BYTES + h * 16384, &tm_lo, &full_bar[s], k0,
+                                             n0 + h * 128, pol);
                         }
                     } else {
+                        // both CTAs' loads complete_tx on the leader's barrier; only the leader arrives (a peer
+                        // load landing first just leaves the transaction count negative until the expect_tx)
                         if (rank == 0) mbar_arrive_expect_tx(&full_bar[s], 2 * C::STAGE_BYTES);
-                        else mbar_arrive_cluster(&full_bar[s], 0);
-                        tma_load_2d_pair(st, &tm_hi, &full_bar[s], k0, m0);
-                        tma_load_2d_pair(st + C::A_BYTES, &tm_lo, &full_bar[s], k0, m0);
+                        tma_load_2d_pair_hint(st, &tm_hi, &full_bar[s], k0, m0, pol);
+                        tma_load_2d_pair_hint(st + C::A_BYTES, &tm_lo, &full_bar[s], k0, m0, pol);
 #pragma unroll
                         for (int h = 0; h < C::BNL / 128; ++h) {
-                            tma_load_2d_pair(st + 2 * C::A_BYTES + h * 16384, &tm_hi, &full_bar[s], k0, n0 + h * 128);
-                            tma_load_2d_pair(st + 2 * C::A_BYTES + C::B_BYTES + h * 16384, &tm_lo, &full_bar[s], k0,
-                                             n0 + h * 128);
+                            tma_load_2d_pair_hint(st + 2 * C::A_BYTES + h * 16384, &tm_hi, &full_bar[s], k0, n0 + h * 128,
+                                                  pol);
+                            tma_load_2d_pair_hint(st + 2 * C::A_BYTES + C::B_BYTES + h * 16384, &tm_lo, &full_bar[s], k0,
+                                                  n0 + h * 128, pol);
                         }
                     }
                     if (++s == STAGES) { s = 0; ph ^= 1u; }
@@ -199,7 +254,7 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
             const int2 sj = p.tiles[w / C::SUB];
             const int sub = w % C::SUB;
             const int m0 = sj.x * BN + (sub * CG + (int)rank) * BM;
-            const int n0 = sj.y * BN;
+            const int n0 = (sj.y & 0xffff) * BN;
             const int gi = m0 + rl;
             const int gi_wmin = m0 + q * 32, gi_wmax = gi_wmin + 31;
             double rowacc = 0.0;                            // sum_j S_n(gi, j)^2 over the own entries (j <= gi) of this tile
@@ -218,7 +273,7 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                 const bool below = (gj0 + 31 <= gi_wmin);   // whole 32x32 chunk strictly in the lower triangle
                 // S_{n-1}: read at the mirrored position (S is exactly symmetric) -> coalesced across the warp
 #pragma unroll
-                for (int c = 0; c < 32; ++c) so[c] = S[(long long)(gj0 + c) * ld + gi];
+                for (int c = 0; c < 32; ++c) so[c] = __ldcs(S + (long long)(gj0 + c) * ld + gi);
                 if (below) {
                     tmem_ld_wait();
                     float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
@@ -244,16 +299,16 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                             if ((e & 3) == 0) a0 += sq; else if ((e & 3) == 1) a1 += sq;
                             else if ((e & 3) == 2) a2 += sq; else a3 += sq;
                             // mirrored position: one 128-byte (FP32) / 64-byte (FP16) warp store per column
-                            S[(long long)(gj0 + c) * ld + gi] = val;
+                            __stcs(S + (long long)(gj0 + c) * ld + gi, val);
                             const long long o = (long long)(gj0 + c) * ldf + gi;
-                            HOu[o] = (unsigned short)hb;
-                            LOu[o] = (unsigned short)lb;
+                            __stcs(HOu + o, (unsigned short)hb);
+                            __stcs(LOu + o, (unsigned short)lb);
                         }
                         // own position: 32 contiguous bytes (FP32) / 16 (FP16) per thread per group
-                        reinterpret_cast<float4*>(rowS)[2 * g] = make_float4(sn[0], sn[1], sn[2], sn[3]);
-                        reinterpret_cast<float4*>(rowS)[2 * g + 1] = make_float4(sn[4], sn[5], sn[6], sn[7]);
-                        reinterpret_cast<uint4*>(rowH)[g] = make_uint4(hp[0], hp[1], hp[2], hp[3]);
-                        reinterpret_cast<uint4*>(rowL)[g] = make_uint4(lp[0], lp[1], lp[2], lp[3]);
+                        __stcs(reinterpret_cast<float4*>(rowS) + 2 * g, make_float4(sn[0], sn[1], sn[2], sn[3]));
+                        __stcs(reinterpret_cast<float4*>(rowS) + 2 * g + 1, make_float4(sn[4], sn[5], sn[6], sn[7]));
+                        __stcs(reinterpret_cast<uint4*>(rowH) + g, make_uint4(hp[0], hp[1], hp[2], hp[3]));
+                        __stcs(reinterpret_cast<uint4*>(rowL) + g, make_uint4(lp[0], lp[1], lp[2], lp[3]));
                     }
                     const double sd = (double)((a0 + a1) + (a2 + a3));
                     off2 += sd;
