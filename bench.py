@@ -314,6 +314,44 @@ def main():
         except Exception:
             pass
 
+    # ---- HBM-bound kernels of the path (a1 Gershgorin, a3 split) timed alone, and a same-run cuBLAS FP16 yardstick
+    def _time(fn, reps=5):
+        ts = []
+        for i in range(reps + 1):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream); fn(); b.record(stream)
+            torch.cuda.synchronize()
+            if i:
+                ts.append(a.elapsed_time(b))
+        return float(np.median(ts))
+
+    hbm_peak = float(peaks["hbm_gbs"])
+    t_g = _time(lambda: h.gershgorin(H, stream=stream))
+    t_s = _time(lambda: api.split_fp16(H, 13, stream=stream))
+    hbm_kernels = {
+        "gershgorin": {"ms": t_g, "algorithmic_GBps": 4.0 * N * N / (t_g * 1e-3) / 1e9,
+                       "read_GBps_lower_triangle_only": 2.0 * N * N / (t_g * 1e-3) / 1e9,
+                       "frac_of_measured_hbm": 4.0 * N * N / (t_g * 1e-3) / 1e9 / hbm_peak,
+                       "note": "SURVEY 8(d): 4 B/element; the kernel reads only H's lower triangle (2 B/element), "
+                               "time includes the call's final sync + 16-byte D2H"},
+        "split_fp16": {"ms": t_s, "algorithmic_GBps": 8.0 * N * N / (t_s * 1e-3) / 1e9,
+                       "frac_of_measured_hbm": 8.0 * N * N / (t_s * 1e-3) / 1e9 / hbm_peak,
+                       "note": "4 B read + 4 B written per element; time includes two torch.empty allocations"},
+        "setup_ms_bounds_affine_split_copyout": t_one - t_layer_ms,
+    }
+    yard = None
+    if rank == 0:
+        a16 = torch.randn(8192, 8192, device=dev).half()
+        b16 = torch.randn(8192, 8192, device=dev).half()
+        c16 = torch.empty_like(a16)
+        for _ in range(3):
+            torch.matmul(a16, b16, out=c16)
+        reps = 150
+        t_y = _time(lambda: [torch.matmul(a16, b16, out=c16) for _ in range(reps)], reps=2)
+        yard = {"tflops": 2.0 * 8192 ** 3 * reps / (t_y * 1e-3) / 1e12,
+                "what": "torch.matmul FP16 8192^3 (cuBLAS), 150 back-to-back calls (~0.13 s), same process and box"}
+        del a16, b16, c16
+
     # ---- end to end through the C ABI with HOST buffers (pinned): H2D + solve + D2H inside the timed region
     e2e = None
     if not args.no_e2e:
@@ -361,6 +399,8 @@ def main():
                        "stop_reason": api.STOP_NAMES.get(info_timed["stop_reason"]), "bounds_used": info_timed["bounds"],
                        "trace_minus_nocc": tr - w.N_occ, "max_err_256_sampled_entries_vs_closed_form": samp_err,
                        "D_exactly_symmetric": symmetric,
+                       "frac_of_same_run_cublas_fp16": (exec_tflops / yard["tflops"]) if yard else None,
+                       "cublas_fp16_yardstick": yard, "hbm_kernels": hbm_kernels,
                        "paper_context": "paper: ~120 TFLOP/s on A100 (P:204), other hardware, count unstated",
                        "wall_s_timed_region": t_wall},
             "clocks": clocks, "roofline": roofline, "e2e": e2e, "cpu_baseline": cpu,
