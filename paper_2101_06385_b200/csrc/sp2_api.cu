@@ -50,8 +50,8 @@ struct sp2_handle_s {
     Ctrl* ctrl = nullptr;
     sp2_layer_stat_t* stats_dev = nullptr;
     double* thetas_dev = nullptr;
-    int2* tiles_dev = nullptr;
-    int tiles_cap = 0;
+    WorkItem* items_dev = nullptr;
+    int items_cap = 0;
     // batched workspace
     sp2_layer_stat_t* bstats_dev = nullptr;
     int* bnl_dev = nullptr;
@@ -69,11 +69,11 @@ struct sp2_handle_s {
     size_t stage_elems = 0;
     PFN_encodeTiled encode = nullptr;
     std::map<std::tuple<int, int, int, int, int>, LoopGraph> graphs;   // (N, Np, cfg, scale_log2, exact_diag)
-    int tiles_key_nt = -1, tiles_key_band = -1;
-    int n_super = 0;
+    int items_key_np = -1, items_key_cfg = -1, items_key_split = -1;
+    int n_items = 0, n_slots = 0;
+    int tail_split = 1;
     int last_launches = 0;
     double noise_kappa = 0.125;
-    int l2_prefetch = 0;
     int round_sync = 1;
     cudaStream_t cap_stream = nullptr;
 };
@@ -118,7 +118,7 @@ extern "C" size_t sp2_workspace_bytes(int N_max, int batch_max, int max_layers) 
     size_t b = Np * (size_t)ws_ld_f32((int)Np) * 4 + 4 * Np * (size_t)ws_ld_f16((int)Np) * 2;   // S + two hi/lo pairs
     b += 4 * Np * sizeof(double);                             // Gershgorin radii, diagonal, two row-sum vectors
     b += sizeof(Ctrl) + (size_t)max_layers * (sizeof(sp2_layer_stat_t) + 3 * sizeof(double));
-    b += (Np / 128) * (Np / 128 + 1) / 2 * sizeof(int2);
+    b += ((Np / 128) * (Np / 128 + 1) / 2 + 1024) * sizeof(WorkItem);
     if (batch_max > 0)
         b += (size_t)batch_max * ((size_t)max_layers * sizeof(sp2_layer_stat_t) + 2 * sizeof(int) + 3 * sizeof(double));
     return b;
@@ -136,7 +136,7 @@ extern "C" sp2_status_t sp2_destroy(sp2_handle_t h) {
         for (int b = 0; b < 2; ++b) cudaFree(h->hl[a][b]);
     cudaFree(h->rowsq[0]); cudaFree(h->rowsq[1]);
     cudaFree(h->R); cudaFree(h->diag); cudaFree(h->ctrl); cudaFree(h->stats_dev); cudaFree(h->thetas_dev);
-    cudaFree(h->tiles_dev); cudaFree(h->bstats_dev); cudaFree(h->bnl_dev); cudaFree(h->bstatus_dev);
+    cudaFree(h->items_dev); cudaFree(h->bstats_dev); cudaFree(h->bnl_dev); cudaFree(h->bstatus_dev);
     cudaFree(h->bbounds_dev); cudaFree(h->bnocc_dev);
     cudaFreeHost(h->ctrl_host); cudaFreeHost(h->stats_host); cudaFreeHost(h->thetas_host);
     cudaFreeHost(h->bounds_host); cudaFree(h->stage_H); cudaFree(h->stage_D);
@@ -159,7 +159,7 @@ extern "C" sp2_status_t sp2_create(sp2_handle_t* out, int N_max, int batch_max, 
     sp2_handle_s* h = new sp2_handle_s();
     h->N_max = N_max; h->batch_max = batch_max; h->max_layers = max_layers;
     if (const char* e = getenv("SP2_NOISE_KAPPA")) h->noise_kappa = atof(e);   // tuning hook (C25)
-    if (const char* e = getenv("SP2_L2_PREFETCH")) h->l2_prefetch = atoi(e);   // tuning hook
+    if (const char* e = getenv("SP2_TAIL_SPLIT")) h->tail_split = atoi(e);     // tuning hook
     if (const char* e = getenv("SP2_ROUND_SYNC")) h->round_sync = atoi(e);     // tuning hook
     h->Np_max = round_up(N_max, 256);
     h->num_sms = prop.multiProcessorCount; h->device = dev;
@@ -180,8 +180,8 @@ extern "C" sp2_status_t sp2_create(sp2_handle_t* out, int N_max, int batch_max, 
     A((void**)&h->ctrl, sizeof(Ctrl));
     A((void**)&h->stats_dev, (size_t)max_layers * sizeof(sp2_layer_stat_t));
     A((void**)&h->thetas_dev, (size_t)max_layers * 3 * sizeof(double));
-    h->tiles_cap = (int)((Np / 128) * (Np / 128 + 1) / 2);
-    A((void**)&h->tiles_dev, (size_t)h->tiles_cap * sizeof(int2));
+    h->items_cap = (int)((Np / 128) * (Np / 128 + 1) / 2) + 1024;
+    A((void**)&h->items_dev, (size_t)h->items_cap * sizeof(WorkItem));
     if (batch_max > 0) {
         A((void**)&h->bstats_dev, (size_t)batch_max * max_layers * sizeof(sp2_layer_stat_t));
         A((void**)&h->bnl_dev, (size_t)batch_max * sizeof(int));
@@ -240,27 +240,42 @@ static sp2_status_t make_tmap(sp2_handle_s* h, CUtensorMap* tm, void* base, int 
     return SP2_OK;
 }
 
-// Supertile launch order over the lower triangle: bands of `band` supertile rows, column-major inside a band, so
-// that the CTAs resident at the same time share few row panels (L2 reuse of the operands).
-static void build_tile_order(int nt, int band, int round, std::vector<int2>& out) {
+// Work list of a layer (launch order).  Supertiles of the lower triangle in bands of `band` supertile rows,
+// column-major inside a band, so that the CTAs of one round (n_slots consecutive items run concurrently) share few
+// row panels (L2 reuse of the operands).  If the last round is partial and short enough, its items are cut into
+// 2 or 4 column strips each (ncols = E/2, E/4 >= 64): more CTAs share the tail and it ends sooner.
+static void build_work_list(int nt, int band, int edge, int subs, int cta_group, int num_sms, int tail_split,
+                            std::vector<WorkItem>& out, int* n_slots) {
     out.clear();
     for (int i0 = 0; i0 < nt; i0 += band) {
         const int i1 = (i0 + band < nt) ? i0 + band : nt;
         for (int j = 0; j < i1; ++j)
-            for (int i = (j > i0 ? j : i0); i < i1; ++i) out.push_back(make_int2(i, j));
+            for (int i = (j > i0 ? j : i0); i < i1; ++i)
+                for (int sub = 0; sub < subs; ++sub) {
+                    WorkItem w = {};
+                    w.I = (short)i; w.J = (short)j; w.sub = (short)sub; w.col0 = 0; w.ncols = (short)edge;
+                    out.push_back(w);
+                }
     }
-    // L2 prefetch ownership: within each round (`round` consecutive entries run concurrently, one per CTA slot) the
-    // first tile that touches a row panel prefetches it (as its A panel if it is the tile's I, as its B panel if J).
-    if (round < 1) return;
-    std::vector<int> seen((size_t)nt, -1);
-    for (size_t t = 0; t < out.size(); ++t) {
-        const int r = (int)(t / (size_t)round);
-        const int I = out[t].x, J = out[t].y;
-        int flags = 0;
-        if (seen[I] != r) { seen[I] = r; flags |= kTilePrefetchA; }
-        if (seen[J] != r) { seen[J] = r; flags |= kTilePrefetchB; }
-        out[t].y = J | flags;
-    }
+    int slots = num_sms / cta_group;
+    if (slots > (int)out.size()) slots = (int)out.size();
+    if (slots * cta_group > kMaxPartials) slots = kMaxPartials / cta_group;
+    *n_slots = slots;
+    const int n = (int)out.size();
+    const int r = n % slots;
+    if (!tail_split || n <= slots || r == 0) return;
+    int f = 1;
+    while (f < 4 && r * (2 * f) <= slots && edge / (2 * f) >= 64) f *= 2;
+    if (f == 1) return;
+    std::vector<WorkItem> tail(out.end() - r, out.end());
+    out.resize((size_t)(n - r));
+    for (int q = 0; q < f; ++q)
+        for (const WorkItem& t : tail) {
+            WorkItem w = t;
+            w.ncols = (short)(edge / f);
+            w.col0 = (short)(q * (edge / f));
+            out.push_back(w);
+        }
 }
 
 static int choose_tile_config(int N, int requested, int num_sms) {
@@ -276,7 +291,7 @@ static int choose_tile_config(int N, int requested, int num_sms) {
 }
 
 struct Problem {
-    int N, Np, cfg, scale_log2, n_super, exact_diag;
+    int N, Np, cfg, scale_log2, n_items, n_slots, exact_diag;
     float scale, inv_scale2;
 };
 
@@ -295,17 +310,21 @@ static sp2_status_t prepare_problem(sp2_handle_s* h, int N, const sp2_opts_t* o,
     pb->inv_scale2 = ldexpf(1.0f, -2 * k);
     const int nt = pb->Np / edge;
     const int band = (pb->cfg == TILE_256x256_PAIR) ? 8 : 12;
-    if (h->tiles_key_nt != nt || h->tiles_key_band != band) {
-        std::vector<int2> order;
-        build_tile_order(nt, band, pb->cfg == TILE_256x256_PAIR ? h->num_sms / 2 : 0, order);
-        if ((int)order.size() > h->tiles_cap) return SP2_ERR_WORKSPACE;
+    if (h->items_key_np != pb->Np || h->items_key_cfg != pb->cfg || h->items_key_split != h->tail_split) {
+        std::vector<WorkItem> list;
+        int slots = 0;
+        build_work_list(nt, band, edge, tile_subs(pb->cfg), tile_cta_group(pb->cfg), h->num_sms, h->tail_split, list,
+                        &slots);
+        if ((int)list.size() > h->items_cap) return SP2_ERR_WORKSPACE;
         // synchronous small copy: happens only when the problem shape changes
-        CK(cudaMemcpyAsync(h->tiles_dev, order.data(), order.size() * sizeof(int2), cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(h->items_dev, list.data(), list.size() * sizeof(WorkItem), cudaMemcpyHostToDevice, st));
         CK(cudaStreamSynchronize(st));
-        h->tiles_key_nt = nt; h->tiles_key_band = band;
-        h->n_super = (int)order.size();
+        h->items_key_np = pb->Np; h->items_key_cfg = pb->cfg; h->items_key_split = h->tail_split;
+        h->n_items = (int)list.size();
+        h->n_slots = slots;
     }
-    pb->n_super = h->n_super;
+    pb->n_items = h->n_items;
+    pb->n_slots = h->n_slots;
     return SP2_OK;
 }
 
@@ -315,8 +334,9 @@ static LayerParams layer_params(sp2_handle_s* h, const Problem& pb, int parity, 
     p.hi_out = h->hl[parity ^ 1][0]; p.lo_out = h->hl[parity ^ 1][1];
     p.rowsq_cur = pb.exact_diag ? h->rowsq[parity] : nullptr;
     p.rowsq_next = pb.exact_diag ? h->rowsq[parity ^ 1] : nullptr;
-    p.tiles = h->tiles_dev; p.ld = ws_ld_f32(pb.Np); p.ldf = ws_ld_f16(pb.Np); p.N = pb.N; p.Np = pb.Np; p.n_super = pb.n_super;
-    p.scale = pb.scale; p.inv_scale2 = pb.inv_scale2; p.cond_handle = cond; p.l2_prefetch = h->l2_prefetch; p.round_sync = h->round_sync;
+    p.items = h->items_dev; p.ld = ws_ld_f32(pb.Np); p.ldf = ws_ld_f16(pb.Np); p.N = pb.N; p.Np = pb.Np;
+    p.n_items = pb.n_items; p.n_slots = pb.n_slots;
+    p.scale = pb.scale; p.inv_scale2 = pb.inv_scale2; p.cond_handle = cond; p.round_sync = h->round_sync;
     return p;
 }
 

@@ -35,9 +35,15 @@ inline long long ws_ld_f16(int Np) { return (long long)Np + 64; }
 // ---- fused symmetric square layer (sp2_square_tiled.cu)
 enum TileConfig { TILE_AUTO = 0, TILE_128x128 = 1, TILE_128x256 = 2, TILE_256x256_PAIR = 3 };
 
-// flag bits in tiles[].y (J is the low 16 bits): this tile issues the L2 prefetches of its A / B panel
-constexpr int kTilePrefetchA = 1 << 16;
-constexpr int kTilePrefetchB = 1 << 17;
+// One unit of work of a layer kernel: rows [(I * E + (sub * CG + rank) * 128), +128) per CTA of supertile (I, J),
+// I >= J, E = supertile edge; columns [J * E + col0, + ncols).  ncols = E except for the items of the last, partial
+// round, which the host cuts into narrower ones (ncols = E/2 or E/4) so that more CTAs share that round.
+struct WorkItem {
+    short I, J;
+    short sub, col0;
+    short ncols, pad0;
+    int pad1;
+};
 
 struct LayerParams {
     Ctrl* ctrl;
@@ -48,20 +54,23 @@ struct LayerParams {
     __half* lo_out;
     unsigned long long* rowsq_cur; // r_i of S_{n-1} (read at the diagonal, then zeroed); nullptr = tensor-core diagonal
     unsigned long long* rowsq_next;// r_i of S_n (accumulated by this launch)
-    const int2* tiles;             // supertile list (I, J | flags), I >= J, in launch order
+    const WorkItem* items;         // work list in launch order: item w runs on CTA slot w % n_slots in round w / n_slots
     long long ld;                  // leading dimension of S (floats)
     long long ldf;                 // leading dimension of hi/lo (halves)
     int N, Np;
-    int n_super;                   // number of supertiles
+    int n_items;                   // length of the work list
+    int n_slots;                   // CTA slots (CTAs / CG) of the launch
     float scale;                   // c = 2^k of the split
     float inv_scale2;              // 1 / c^2
-    int l2_prefetch;               // L2 prefetch lead of the TMA producer in k-blocks (0 = off)
     int round_sync;                // 1: producers of all CTAs meet at every round boundary (keeps the wave in lockstep)
     unsigned long long cond_handle;  // cudaGraphConditionalHandle (0 = none)
 };
 
 // Supertile edge for a tile configuration (128 or 256) and CTAs launched per supertile-slot.
 int tile_super_edge(int cfg);
+int tile_subs(int cfg);        // 128-row work items per supertile
+int tile_cta_group(int cfg);
+int layer_slots(int cfg, int n_items, int num_sms);   // CTA slots a launch of n_items uses
 size_t tile_smem_bytes(int cfg);
 // Launch one layer: reads hi/lo through the tensor maps (K-major, 128B swizzle, box 64 x 128), writes S, hi_out, lo_out.
 cudaError_t launch_layer(int cfg, const CUtensorMap& tm_hi, const CUtensorMap& tm_lo, const LayerParams& p,

@@ -62,7 +62,7 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
     const uint32_t rank = (CG == 2) ? cluster_ctarank() : 0u;
     const int slot = blockIdx.x / CG;
     const int nslots = gridDim.x / CG;
-    const int n_work = p.n_super * C::SUB;
+    const int n_work = p.n_items;
     const int KB = p.Np / BK;
 
     if (warp == 0 && lane == 0) {
@@ -96,41 +96,6 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
             int s = 0;
             uint32_t ph = 0;
             const uint64_t pol = l2_policy_evict_last();     // operand panels: reused by the other CTAs of the wave
-            // L2 prefetch cursor, PF k-blocks ahead of the loads (across tile boundaries): the loads then hit L2 and
-            // the three smem stages only have to cover L2 latency, not HBM latency.
-            // Only the first tile of a round (= nslots consecutive list entries, which run concurrently) that uses
-            // a panel prefetches it (flag bits set by the host in tiles[].y): every panel slice is requested from
-            // HBM once per round instead of once per CTA.
-            const int PF = p.l2_prefetch;                   // k-blocks of lead; 0 = off
-            int w_pf = slot, kb_pf = 0, m0_pf = 0, n0_pf = 0;
-            bool pfA = false, pfB = false;
-            auto pf_tile = [&]() {
-                if (w_pf < n_work) {
-                    const int2 t = p.tiles[w_pf / C::SUB];
-                    m0_pf = t.x * BN + ((w_pf % C::SUB) * CG + (int)rank) * BM;
-                    n0_pf = (t.y & 0xffff) * BN + (int)rank * C::BNL;
-                    pfA = (t.y & kTilePrefetchA) != 0;
-                    pfB = (t.y & kTilePrefetchB) != 0;
-                }
-            };
-            auto pf_step = [&]() {
-                if (w_pf >= n_work) return;
-                const int k0 = kb_pf * BK;
-                if (pfA) {
-                    tma_prefetch_l2_2d(&tm_hi, k0, m0_pf, pol);
-                    tma_prefetch_l2_2d(&tm_lo, k0, m0_pf, pol);
-                }
-                if (pfB) {
-#pragma unroll
-                    for (int h = 0; h < C::BNL / 128; ++h) {
-                        tma_prefetch_l2_2d(&tm_hi, k0, n0_pf + h * 128, pol);
-                        tma_prefetch_l2_2d(&tm_lo, k0, n0_pf + h * 128, pol);
-                    }
-                }
-                if (++kb_pf == KB) { kb_pf = 0; w_pf += nslots; pf_tile(); }
-            };
-            pf_tile();
-            for (int i = 0; i < PF; ++i) pf_step();
             // Round sync: the CTAs of a round share row panels through L2 only while they walk K together.  Nothing
             // else keeps them together (each runs its tiles back to back), so every producer checks in at each round
             // boundary and starts the next tile's loads when all have (bounded spin: never a hang, at worst no sync).
@@ -148,12 +113,12 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                     }
                 }
                 if (w >= n_work) break;
-                const int2 sj = p.tiles[w / C::SUB];
-                const int sub = w % C::SUB;
-                const int m0 = sj.x * BN + (sub * CG + (int)rank) * BM;      // A rows of this CTA
-                const int n0 = (sj.y & 0xffff) * BN + (int)rank * C::BNL;    // B rows this CTA loads
+                const WorkItem wi = p.items[w];
+                const int m0 = wi.I * BN + (wi.sub * CG + (int)rank) * BM;                 // A rows of this CTA
+                // B rows this CTA loads: its share of the item's ncols columns (always a full 128-row box per load:
+                // for a narrow tail item the rows beyond ncols / CG are loaded but not used by the MMA)
+                const int n0 = wi.J * BN + wi.col0 + (int)rank * (wi.ncols / CG);
                 for (int kb = 0; kb < KB; ++kb) {
-                    if (PF > 0) pf_step();
                     mbar_wait(&empty_bar[s], ph ^ 1u);
                     uint8_t* st = smem + s * C::STAGE_BYTES;
                     const int k0 = kb * BK;
@@ -188,13 +153,13 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
     } else if (warp == 1) {
         // =============================== MMA issuer (leader CTA only, one elected lane)
         if (rank == 0) {
-            constexpr uint32_t idesc = umma_idesc_f16(BM * CG, BN);
             int s = 0;
             uint32_t ph = 0;
             int it = 0;
             for (int w = slot; w < n_work; w += nslots, ++it) {
                 const int buf = it & 1;
                 const uint32_t use = (uint32_t)(it >> 1);
+                const uint32_t idesc = umma_idesc_f16(BM * CG, p.items[w].ncols);   // N = 256, or 128 / 64 in the tail
                 mbar_wait(&tempty_bar[buf], (use & 1u) ^ 1u);       // epilogue has drained this accumulator
                 tc_fence_after();
                 const uint32_t d_tmem = tmem_base + (uint32_t)(buf * BN);
@@ -251,10 +216,10 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
         for (int w = slot; w < n_work; w += nslots, ++it) {
             const int buf = it & 1;
             const uint32_t use = (uint32_t)(it >> 1);
-            const int2 sj = p.tiles[w / C::SUB];
-            const int sub = w % C::SUB;
-            const int m0 = sj.x * BN + (sub * CG + (int)rank) * BM;
-            const int n0 = (sj.y & 0xffff) * BN;
+            const WorkItem wi = p.items[w];
+            const int m0 = wi.I * BN + (wi.sub * CG + (int)rank) * BM;
+            const int n0 = wi.J * BN + wi.col0;
+            const int ncols = wi.ncols;
             const int gi = m0 + rl;
             const int gi_wmin = m0 + q * 32, gi_wmax = gi_wmin + 31;
             double rowacc = 0.0;                            // sum_j S_n(gi, j)^2 over the own entries (j <= gi) of this tile
@@ -264,7 +229,7 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
             unsigned short* HOu = reinterpret_cast<unsigned short*>(HO);
             unsigned short* LOu = reinterpret_cast<unsigned short*>(LO);
 #pragma unroll 1
-            for (int c0 = 0; c0 < BN; c0 += 32) {
+            for (int c0 = 0; c0 < ncols; c0 += 32) {
                 const int gj0 = n0 + c0;
                 if (gj0 > gi_wmax) break;                   // rest of the row block lies above the diagonal
                 uint32_t v[32];
@@ -409,6 +374,15 @@ using Cfg256 = TileCfg<256, 1>;
 using Cfg256P = TileCfg<256, 2>;
 
 int tile_super_edge(int cfg) { return cfg == TILE_128x128 ? 128 : 256; }
+int tile_subs(int cfg) { return cfg == TILE_128x256 ? Cfg256::SUB : 1; }
+int tile_cta_group(int cfg) { return cfg == TILE_256x256_PAIR ? 2 : 1; }
+int layer_slots(int cfg, int n_items, int num_sms) {
+    const int cg = tile_cta_group(cfg);
+    int slots = num_sms / cg;
+    if (slots > n_items) slots = n_items;
+    if (slots * cg > kMaxPartials) slots = kMaxPartials / cg;
+    return slots;
+}
 size_t tile_smem_bytes(int cfg) {
     return cfg == TILE_128x128 ? Cfg128::SMEM_BYTES : cfg == TILE_128x256 ? Cfg256::SMEM_BYTES : Cfg256P::SMEM_BYTES;
 }
@@ -431,10 +405,8 @@ cudaError_t layer_kernel_setup(int cfg) {
 template <class C>
 static cudaError_t launch_cfg(const CUtensorMap& tm_hi, const CUtensorMap& tm_lo, const LayerParams& p, int num_sms,
                               cudaStream_t st) {
-    const int n_work = p.n_super * C::SUB;
-    int slots = num_sms / C::CG;
-    if (slots > n_work) slots = n_work;
-    if (slots * C::CG > kMaxPartials) slots = kMaxPartials / C::CG;
+    (void)num_sms;
+    const int slots = p.n_slots;          // chosen by the host together with the item list (layer_slots)
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)(slots * C::CG));
     cfg.blockDim = dim3(C::THREADS);
