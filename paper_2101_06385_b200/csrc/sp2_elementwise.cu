@@ -16,51 +16,82 @@ __device__ __forceinline__ float warp_sum(float v) {
     return v;
 }
 
-// Map a linear index t over the lower triangle (I >= J) of an nt x nt tile grid to (I, J).
+// Map a linear index t over the lower triangle (I >= J) of an nt x nt tile grid to (I, J).  Float estimate plus
+// integer correction: exact, and no FP64 (the FP64 pipe of sm_100 is narrow).
 __device__ __forceinline__ void tri_decode(long long t, int& I, int& J) {
-    long long i = (long long)((sqrt(8.0 * (double)t + 1.0) - 1.0) * 0.5);
+    long long i = (long long)((sqrtf(8.0f * (float)t + 1.0f) - 1.0f) * 0.5f);
     while ((i + 1) * (i + 2) / 2 <= t) ++i;
     while (i * (i + 1) / 2 > t) --i;
     I = (int)i;
     J = (int)(t - i * (i + 1) / 2);
 }
 
+// Both kernels below walk 64 x 64 tiles of the lower triangle with 256 threads; thread t owns the float4 at
+// row (t / 16) + 16 k, k = 0..3, columns 4 (t % 16) .. +3: a row of the tile is one 256-byte segment read by 16 lanes.
+constexpr int ET = 64;
+__device__ __forceinline__ float4 ld_tile4(const float* __restrict__ H, int N, long long ldh, int i, int j, bool vec) {
+    float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (i >= N) return v;
+    const float* p = H + (long long)i * ldh + j;
+    if (vec && j + 3 < N) return __ldg(reinterpret_cast<const float4*>(p));
+    if (j < N) v.x = __ldg(p);
+    if (j + 1 < N) v.y = __ldg(p + 1);
+    if (j + 2 < N) v.z = __ldg(p + 2);
+    if (j + 3 < N) v.w = __ldg(p + 3);
+    return v;
+}
+// sum over the 16 lanes that share a tile row (lanes differ in bits 0-3)
+__device__ __forceinline__ float row16_sum(float v) {
+#pragma unroll
+    for (int o = 8; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
 // ------------------------------------------------------------------------------------------------ a1
-// Gershgorin radii of the lower-triangle-symmetrised H: R_i = sum_{j<i} |H_ij| + sum_{j>i} |H_ji|.
-// One 64x64 lower-triangle tile per block iteration: element (i,j), i>j, adds |H_ij| to R_i and to R_j.
-constexpr int GT = 64;
+// Gershgorin radii of the lower-triangle-symmetrised H: R_i = sum_{j<i} |H_ij| + sum_{j>i} |H_ji|: element (i,j),
+// i > j, adds |H_ij| to R_i (row sum) and to R_j (column sum).  FP32 sums inside a tile, FP64 atomics across tiles.
 __global__ void __launch_bounds__(256) k_gershgorin_rows(const float* __restrict__ H, int N, long long ldh,
                                                          double* __restrict__ R, double* __restrict__ diag) {
-    __shared__ float colacc[4][GT];
-    const int nt = (N + GT - 1) / GT;
+    __shared__ float colacc[16][ET];
+    const int nt = (N + ET - 1) / ET;
     const long long ntiles = (long long)nt * (nt + 1) / 2;
-    const int tx = threadIdx.x & 63, ty = threadIdx.x >> 6;   // ty 0..3 ; warps 2*ty, 2*ty+1
+    const int c4 = (threadIdx.x & 15) * 4, r0 = threadIdx.x >> 4;
+    const bool vec = ((ldh & 3) == 0) && ((reinterpret_cast<uintptr_t>(H) & 15) == 0);
     for (long long t = blockIdx.x; t < ntiles; t += gridDim.x) {
         int I, J;
         tri_decode(t, I, J);
-        const int j = J * GT + tx;
-        float v[16];
+        const int j = J * ET + c4;
+        float4 v[4];
 #pragma unroll
-        for (int r = 0; r < 16; ++r) {
-            const int i = I * GT + ty + 4 * r;
-            float x = 0.f;
-            if (i < N && j < i) x = fabsf(__ldg(H + (long long)i * ldh + j));
-            if (i < N && j == i) diag[i] = (double)__ldg(H + (long long)i * ldh + j);
-            v[r] = x;
-        }
-        float csum = 0.f;
+        for (int k = 0; k < 4; ++k) v[k] = ld_tile4(H, N, ldh, I * ET + r0 + 16 * k, j, vec);
+        float cs0 = 0.f, cs1 = 0.f, cs2 = 0.f, cs3 = 0.f;
 #pragma unroll
-        for (int r = 0; r < 16; ++r) {
-            csum += v[r];
-            const float rs = warp_sum(v[r]);                  // 32 of the 64 columns of row i
-            const int i = I * GT + ty + 4 * r;
-            if ((threadIdx.x & 31) == 0 && i < N && rs != 0.f) atomicAdd(R + i, (double)rs);
+        for (int k = 0; k < 4; ++k) {
+            const int i = I * ET + r0 + 16 * k;
+            float4 a = v[k];
+            if (I == J) {                                   // diagonal tile: strictly-lower entries only; pick up H_ii
+                if (i < N) {
+                    if (j == i) diag[i] = (double)a.x; else if (j + 1 == i) diag[i] = (double)a.y;
+                    else if (j + 2 == i) diag[i] = (double)a.z; else if (j + 3 == i) diag[i] = (double)a.w;
+                }
+                if (j >= i) a.x = 0.f;
+                if (j + 1 >= i) a.y = 0.f;
+                if (j + 2 >= i) a.z = 0.f;
+                if (j + 3 >= i) a.w = 0.f;
+            }
+            a.x = fabsf(a.x); a.y = fabsf(a.y); a.z = fabsf(a.z); a.w = fabsf(a.w);
+            cs0 += a.x; cs1 += a.y; cs2 += a.z; cs3 += a.w;
+            const float rs = row16_sum((a.x + a.y) + (a.z + a.w));
+            if ((threadIdx.x & 15) == 0 && i < N && rs != 0.f) atomicAdd(R + i, (double)rs);
         }
-        colacc[ty][tx] = csum;
+        *reinterpret_cast<float4*>(&colacc[r0][c4]) = make_float4(cs0, cs1, cs2, cs3);
         __syncthreads();
-        if (ty == 0 && j < N) {
-            const float c = colacc[0][tx] + colacc[1][tx] + colacc[2][tx] + colacc[3][tx];
-            if (c != 0.f) atomicAdd(R + j, (double)c);
+        if (threadIdx.x < ET) {
+            float c = 0.f;
+#pragma unroll
+            for (int g = 0; g < 16; ++g) c += colacc[g][threadIdx.x];
+            const int jj = J * ET + threadIdx.x;
+            if (jj < N && c != 0.f) atomicAdd(R + jj, (double)c);
         }
         __syncthreads();
     }
@@ -92,19 +123,38 @@ __global__ void __launch_bounds__(1024) k_gershgorin_finalize(const double* __re
 
 // ------------------------------------------------------------------------------------------------ a2
 // S_0 = (eps_max I - H) / (eps_max - eps_min)  (W_0, B_0 of Alg. 1), written as FP32 master + FP16 hi/lo
-// (Eqs. 12-13), both triangles from H's lower triangle; Tr S_0 and ||S_0||_F^2 in FP64.  32x32 tiles, the
-// mirrored tile goes through shared memory so that both global writes are coalesced.
-constexpr int AT = 32;
-__global__ void __launch_bounds__(256) k_affine_split(const float* __restrict__ H, int N, long long ldh,
-                                                      float* __restrict__ S, __half* __restrict__ hi,
-                                                      __half* __restrict__ lo, long long ld, long long ldf,
-                                                      float scale, Ctrl* ctrl,
-                                                      sp2_layer_stat_t* stats, const double* thetas,
-                                                      unsigned long long* __restrict__ rowsq) {
-    __shared__ float ts[AT][AT + 1];
-    __shared__ double colsq[8][AT];
+// (Eqs. 12-13) at (i,j) and (j,i) from H's lower triangle (the mirror goes through shared memory so that both global
+// writes are row segments); Tr S_0, ||S_0||_F^2 and the row sums of squares.  FP32 sums inside a tile (FP64 only for
+// the diagonal entries), FP64 / fixed point across tiles.
+__device__ __forceinline__ void store_s4(float* __restrict__ S, __half* __restrict__ hi, __half* __restrict__ lo,
+                                         long long ld, long long ldf, int i, int j, const float (&s)[4], float scale,
+                                         bool all4, const bool (&ok)[4]) {
+    __half h[4], l[4];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) split_hi_lo(s[e], scale, h[e], l[e]);
+    if (all4) {
+        *reinterpret_cast<float4*>(S + (long long)i * ld + j) = make_float4(s[0], s[1], s[2], s[3]);
+        *reinterpret_cast<uint2*>(hi + (long long)i * ldf + j) = *reinterpret_cast<uint2*>(h);
+        *reinterpret_cast<uint2*>(lo + (long long)i * ldf + j) = *reinterpret_cast<uint2*>(l);
+    } else {
+#pragma unroll
+        for (int e = 0; e < 4; ++e)
+            if (ok[e]) {
+                S[(long long)i * ld + j + e] = s[e];
+                hi[(long long)i * ldf + j + e] = h[e];
+                lo[(long long)i * ldf + j + e] = l[e];
+            }
+    }
+}
+
+__global__ void __launch_bounds__(256, 4) k_affine_split(const float* __restrict__ H, int N, long long ldh,
+                                                         float* __restrict__ S, __half* __restrict__ hi,
+                                                         __half* __restrict__ lo, long long ld, long long ldf,
+                                                         float scale, Ctrl* ctrl, sp2_layer_stat_t* stats,
+                                                         const double* thetas, unsigned long long* __restrict__ rowsq) {
+    __shared__ float ts[ET][ET + 1];
+    __shared__ float colacc[16][ET];
     __shared__ double red[8][2];
-    __shared__ int is_last;
     const double e0 = ctrl->eps_min, e1 = ctrl->eps_max;
     if (!(e1 > e0) || !isfinite(e0) || !isfinite(e1)) {
         if (blockIdx.x == 0 && threadIdx.x == 0) {
@@ -115,66 +165,81 @@ __global__ void __launch_bounds__(256) k_affine_split(const float* __restrict__ 
     }
     const float w0 = (float)(-1.0 / (e1 - e0));    // W_0
     const float b0 = (float)(e1 / (e1 - e0));      // B_0
-    const int nt = (N + AT - 1) / AT;
+    const int nt = (N + ET - 1) / ET;
     const long long ntiles = (long long)nt * (nt + 1) / 2;
-    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;    // 8 rows per pass
-    double trS = 0.0, fro2 = 0.0;
+    const int c4 = (threadIdx.x & 15) * 4, r0 = threadIdx.x >> 4;
+    const bool vec_in = ((ldh & 3) == 0) && ((reinterpret_cast<uintptr_t>(H) & 15) == 0);
+    double trS = 0.0, off2 = 0.0, dg2 = 0.0;       // ||S_0||_F^2 = 2 off2 + dg2
     for (long long t = blockIdx.x; t < ntiles; t += gridDim.x) {
         int I, J;
         tri_decode(t, I, J);
-        double csq = 0.0;                                    // this thread's column j, rows of this warp
+        const bool dtile = (I == J);
+        const int j = J * ET + c4;
+        float4 v[4];
 #pragma unroll
-        for (int r = 0; r < 4; ++r) {
-            const int li = ty + 8 * r;
-            const int i = I * AT + li, j = J * AT + tx;
-            float s = 0.f;
-            double rsq = 0.0;
-            if (i < N && j <= i) {
-                s = w0 * __ldg(H + (long long)i * ldh + j);
-                if (i == j) s += b0;
-                S[(long long)i * ld + j] = s;
-                __half h, l;
-                split_hi_lo(s, scale, h, l);
-                hi[(long long)i * ldf + j] = h;
-                lo[(long long)i * ldf + j] = l;
-                const double sd = (double)s;
-                rsq = sd * sd;
-                if (i == j) { trS += sd; fro2 += sd * sd; }
-                else { fro2 += 2.0 * sd * sd; csq += rsq; }
+        for (int k = 0; k < 4; ++k) v[k] = ld_tile4(H, N, ldh, I * ET + r0 + 16 * k, j, vec_in);
+        float offsq = 0.f;                          // squares of this thread's strictly-lower entries
+        float cs[4] = {0.f, 0.f, 0.f, 0.f};         // the same per column (rows of the mirrored part)
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const int lr = r0 + 16 * k, i = I * ET + lr;
+            const float hv[4] = {v[k].x, v[k].y, v[k].z, v[k].w};
+            float sv[4];
+            bool ok[4];
+            float rsq = 0.f;                        // row i: squares of its entries j <= i held by this thread
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                const int jj = j + e;
+                ok[e] = (i < N) && (jj <= i);       // jj <= i < N
+                float sx = ok[e] ? w0 * hv[e] : 0.f;
+                if (ok[e] && jj == i) {
+                    sx += b0;
+                    const double sd = (double)sx;
+                    trS += sd; dg2 += sd * sd;
+                    rsq += sx * sx;
+                } else {
+                    const float q = sx * sx;
+                    rsq += q; offsq += q; cs[e] += q;
+                }
+                sv[e] = sx;
+                ts[lr][c4 + e] = sx;
             }
-            ts[li][tx] = s;
-            if (rowsq) {                                     // row i: sum over this warp's 32 columns (j <= i)
-                rsq = warp_sum(rsq);
-                if (tx == 0 && i < N) atomicAdd(rowsq + i, rowsq_fix(rsq));
+            const bool all4 = !dtile && (i < N);    // off-diagonal tile: j + 3 < J*64 + 64 <= i
+            store_s4(S, hi, lo, ld, ldf, i, j, sv, scale, all4, ok);
+            if (rowsq) {
+                rsq = row16_sum(rsq);
+                if ((threadIdx.x & 15) == 0 && i < N) atomicAdd(rowsq + i, rowsq_fix((double)rsq));
             }
         }
-        colsq[ty][tx] = csq;
+        off2 += (double)offsq;
+        *reinterpret_cast<float4*>(&colacc[r0][c4]) = make_float4(cs[0], cs[1], cs[2], cs[3]);
         __syncthreads();
-        if (rowsq && ty == 0) {                              // column j (= row j of the mirrored part), j < i only
-            double c = 0.0;
+        if (rowsq && threadIdx.x < ET) {            // column j of the tile = row j of the mirrored part (j < i only)
+            float c = 0.f;
 #pragma unroll
-            for (int w8 = 0; w8 < 8; ++w8) c += colsq[w8][tx];
-            const int j = J * AT + tx;
-            if (j < N && c != 0.0) atomicAdd(rowsq + j, rowsq_fix(c));
+            for (int g = 0; g < 16; ++g) c += colacc[g][threadIdx.x];
+            const int jj = J * ET + threadIdx.x;
+            if (jj < N && c != 0.f) atomicAdd(rowsq + jj, rowsq_fix((double)c));
         }
+        // mirrored part: row jj = J*64 + lr, columns ii = I*64 + c4 .. +3, value s(ii, jj) for ii > jj
 #pragma unroll
-        for (int r = 0; r < 4; ++r) {
-            const int lj = ty + 8 * r;                      // row of the mirrored tile = column of the source
-            const int jj = J * AT + lj, ii = I * AT + tx;   // write S[jj][ii] = s(ii, jj) for ii > jj
-            if (ii < N && jj < ii) {
-                const float s = ts[tx][lj];
-                S[(long long)jj * ld + ii] = s;
-                __half h, l;
-                split_hi_lo(s, scale, h, l);
-                hi[(long long)jj * ldf + ii] = h;
-                lo[(long long)jj * ldf + ii] = l;
+        for (int k = 0; k < 4; ++k) {
+            const int lr = r0 + 16 * k, jj = J * ET + lr, ii = I * ET + c4;
+            float sv[4];
+            bool ok[4];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                sv[e] = ts[c4 + e][lr];
+                ok[e] = (ii + e < N) && (jj < ii + e);
             }
+            const bool all4 = !dtile && (ii + 3 < N);
+            if (jj < N) store_s4(S, hi, lo, ld, ldf, jj, ii, sv, scale, all4, ok);
         }
         __syncthreads();
     }
     trS = warp_sum(trS);
-    fro2 = warp_sum(fro2);
-    if (tx == 0) { red[ty][0] = trS; red[ty][1] = fro2; }
+    double fro2 = warp_sum(2.0 * off2 + dg2);
+    if ((threadIdx.x & 31) == 0) { red[threadIdx.x >> 5][0] = trS; red[threadIdx.x >> 5][1] = fro2; }
     __syncthreads();
     if (threadIdx.x == 0) {
         double a = 0.0, b = 0.0;
@@ -184,8 +249,7 @@ __global__ void __launch_bounds__(256) k_affine_split(const float* __restrict__ 
         ctrl->partial[blockIdx.x][2] = 0.0;
         __threadfence();
         const unsigned int done = atomicAdd(&ctrl->done_counter, 1u);
-        is_last = (done == gridDim.x - 1);
-        if (is_last) {
+        if (done == gridDim.x - 1) {
             __threadfence();
             double s0 = 0.0, s1 = 0.0;
             for (unsigned int i = 0; i < gridDim.x; ++i) {
@@ -196,6 +260,7 @@ __global__ void __launch_bounds__(256) k_affine_split(const float* __restrict__ 
             ctrl->fro2 = s1;
             ctrl->n = 0;
             ctrl->done_counter = 0;
+            ctrl->round_counter = 0;
             ctrl->launches += 1;
             control_plan_next(ctrl, stats, thetas);
         }
@@ -241,7 +306,7 @@ cudaError_t launch_gershgorin(const float* H, int N, long long ldh, double* R, d
                               double* bounds_out, int num_sms, cudaStream_t st) {
     cudaError_t e = cudaMemsetAsync(R, 0, sizeof(double) * (size_t)N, st);
     if (e != cudaSuccess) return e;
-    const int nt = (N + GT - 1) / GT;
+    const int nt = (N + ET - 1) / ET;
     const long long ntiles = (long long)nt * (nt + 1) / 2;
     const int grid = (int)(ntiles < (long long)num_sms * 16 ? ntiles : (long long)num_sms * 16);
     k_gershgorin_rows<<<grid, 256, 0, st>>>(H, N, ldh, R, diag);
@@ -252,9 +317,9 @@ cudaError_t launch_gershgorin(const float* H, int N, long long ldh, double* R, d
 cudaError_t launch_affine_split(const float* H, int N, long long ldh, float* S, __half* hi, __half* lo, long long ld,
                                 long long ldf, float scale, Ctrl* ctrl, sp2_layer_stat_t* stats, const double* thetas,
                                 unsigned long long* rowsq, int num_sms, cudaStream_t st) {
-    const int nt = (N + AT - 1) / AT;
+    const int nt = (N + ET - 1) / ET;
     const long long ntiles = (long long)nt * (nt + 1) / 2;
-    long long cap = (long long)num_sms * 6;
+    long long cap = (long long)num_sms * 4;
     if (cap > kMaxPartials) cap = kMaxPartials;
     const int grid = (int)(ntiles < cap ? ntiles : cap);
     k_affine_split<<<grid, 256, 0, st>>>(H, N, ldh, S, hi, lo, ld, ldf, scale, ctrl, stats, thetas, rowsq);
