@@ -352,6 +352,22 @@ def main():
                 "what": "torch.matmul FP16 8192^3 (cuBLAS), 150 back-to-back calls (~0.13 s), same process and box"}
         del a16, b16, c16
 
+    # ---- NEXT-1 row: final refinement (Eq. 16) + energy on the last solve's D (outside the timed step)
+    refine = None
+    if rank == 0:
+        _, info_r = solve()
+        t_r = _time(lambda: h.refine_energy(D, info_r["sigma"][-1], H, stream=stream), reps=3)
+        D1, res = h.refine_energy(D, info_r["sigma"][-1], H, stream=stream)
+        e_star = float(np.sort(w.eps)[: int(w.N_occ)].sum())
+        refine = {"ms": t_r, "energy_err_in": res["energy_in"] - e_star, "energy_err_out": res["energy_out"] - e_star,
+                  "iderr_in": res["iderr_in"], "iderr_out": res["iderr_out"],
+                  "trace_minus_nocc_out": res["trace_out"] - w.N_occ,
+                  "max_err_256_sampled_entries_vs_closed_form_out":
+                      float(np.abs(D1.double()[ri, ci].cpu().numpy() - ref).max()),
+                  "what": "sp2_refine_energy: 2 enhanced-accumulation layers (128x128 tiles, 2 K-blocks per tensor-core "
+                          "chunk, two-sum running pair in TMEM) + 2 Tr[XH] passes"}
+        del D1
+
     # ---- end to end through the C ABI with HOST buffers (pinned): H2D + solve + D2H inside the timed region
     e2e = None
     if not args.no_e2e:
@@ -400,7 +416,7 @@ def main():
                        "trace_minus_nocc": tr - w.N_occ, "max_err_256_sampled_entries_vs_closed_form": samp_err,
                        "D_exactly_symmetric": symmetric,
                        "frac_of_same_run_cublas_fp16": (exec_tflops / yard["tflops"]) if yard else None,
-                       "cublas_fp16_yardstick": yard, "hbm_kernels": hbm_kernels,
+                       "cublas_fp16_yardstick": yard, "hbm_kernels": hbm_kernels, "refinement_next1": refine,
                        "paper_context": "paper: ~120 TFLOP/s on A100 (P:204), other hardware, count unstated",
                        "wall_s_timed_region": t_wall},
             "clocks": clocks, "roofline": roofline, "e2e": e2e, "cpu_baseline": cpu,

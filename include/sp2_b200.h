@@ -119,6 +119,23 @@ sp2_status_t sp2_generalized_wb(sp2_handle_t h, const float* H_dev, int N, int l
                                 double eps_min, double eps_max, const sp2_opts_t* opts,
                                 float* X_L_dev, int ldx, sp2_layer_stat_t* stats_host, void* stream);
 
+/* Final refinement and energy (Eq. 16; Alg. 1's last line) -- the step right after the path.
+ * S (N x N, lds >= N) is a converged SP2 iterate (D of sp2_density_matrix), last_sigma the sign of its last layer
+ * (stats[n_layers-1].sigma).  Computes, as two layers composed in one step,
+ *     last_sigma = -1:  D' = 2 S^2 - S^4          last_sigma = +1:  D' = (2 S - S^2)^2
+ * (the alternation is continued from the last applied sign: DESIGN.md reading C15) in enhanced precision --
+ * "single precision with double accumulation": FP16 hi/lo operands as in Eq. 15, but the tensor core
+ * accumulates only 512 values of K at a time and the chunk sums are added in an error-free FP32 pair -- and the
+ * observables Tr[X H], Tr[X], IdErr = Tr[X - X^2] of X = S (in) and X = D' (out), in FP64.
+ * H: the Hamiltonian (lower triangle read).  S_dev may equal D_dev. */
+typedef struct {
+    double energy_in, trace_in, iderr_in;
+    double energy_out, trace_out, iderr_out;
+} sp2_refine_result_t;
+sp2_status_t sp2_refine_energy(sp2_handle_t h, const float* S_dev, int N, int lds, int last_sigma,
+                               const float* H_dev, int ldh, float* D_dev, int ldd,
+                               sp2_refine_result_t* result, void* stream);
+
 /* Batched small-N: B independent matrices H[B][N][N] (contiguous, N <= 256), one launch, one CTA
  * cluster per matrix, per-matrix branch sequence and stop layer.  N_occ: [B] values, or one value if
  * nocc_is_scalar.  stats_host: [B][opts->max_layers] (may be NULL); n_layers: [B]; status_out: [B] per-matrix

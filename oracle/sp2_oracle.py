@@ -21,6 +21,10 @@ can be checked against PAPER.md by eye (P:n = /root/reference/PAPER.md line n):
   split_fp16               Eqs. 12-13 with IEEE round-to-nearest-even conversions (C9).
   mixed_square_exact       Eq. 15 evaluated in FP64 from given hi/lo (products of two
                            FP16 numbers are exact in FP64): the exact target of the tensor-core square.
+  refine_ref               the final refinement f_final of Eq. 16 in FP64: two composed layers with
+                           alternating signs; which of the two forms applies follows reading C15 of
+                           DESIGN.md (continue the alternation from the last applied sign).
+  energy_ref               alpha = Tr[D H] (the observable of Fig. 2), plain FP64.
   sp2_mixed_ref            Alg. 1 with Alg. 2 as the activation, emulated: FP16 hi/lo split,
                            Eq. 15 products, FP32 rounding of X_n and S_n.  An EMULATION of the arithmetic
                            (FP64 accumulation instead of the tensor core's FP32), used only to size
@@ -260,3 +264,32 @@ def commutator_norm(H32, D):
 
 
 THEOREM1_C = (71.0 + 17.0 * np.sqrt(17.0)) / 32.0
+
+
+def refine_ref(S, last_sigma):
+    """Eq. 16: f_final(S) = 2 S^2 - S^4 or (2 S - S^2)^2, "the result of composing two layers in a
+    single step with sigma_n = 1 and sigma_{n-1} = -1 or sigma_n = -1 and sigma_{n-1} = 1".
+    Reading C15: the alternation continues from the last APPLIED sign, so
+      last_sigma = -1: next layer squares (X = S^2), the one after applies 2X - X^2  ->  2 S^2 - S^4
+      last_sigma = +1: next layer applies T = 2S - S^2, the one after squares          ->  (2S - S^2)^2
+    Plain FP64 products ("standard double precision")."""
+    S = np.asarray(S, dtype=np.float64)
+    if last_sigma not in (1, -1):
+        raise ValueError("last_sigma must be +1 or -1")
+    X = S @ S
+    if last_sigma < 0:
+        return 2.0 * X - X @ X
+    T = 2.0 * S - X
+    return T @ T
+
+
+def energy_ref(D, H):
+    """alpha = Tr[D H], with H symmetrised from its lower triangle like everywhere else."""
+    D = np.asarray(D, dtype=np.float64)
+    return float(np.sum(D * symmetrize_lower(H).T))
+
+
+def iderr_ref(X):
+    """IdErr = Tr[X - X^2] (P:188)."""
+    X = np.asarray(X, dtype=np.float64)
+    return float(np.trace(X) - np.sum(X * X.T))

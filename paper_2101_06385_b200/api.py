@@ -19,7 +19,7 @@ TILE_AUTO, TILE_128x128, TILE_128x256, TILE_256x256_PAIR = 0, 1, 2, 3
 
 EXPORTS = ["sp2_default_opts", "sp2_create", "sp2_destroy", "sp2_workspace_bytes", "sp2_density_matrix",
            "sp2_density_matrix_host", "sp2_generalized", "sp2_generalized_wb", "sp2_density_matrix_batched",
-           "sp2_split_fp16", "sp2_gershgorin", "sp2_status_string", "sp2_last_cuda_error",
+           "sp2_refine_energy", "sp2_split_fp16", "sp2_gershgorin", "sp2_status_string", "sp2_last_cuda_error",
            "sp2_last_launch_count", "sp2_version"]
 
 
@@ -32,6 +32,11 @@ class Opts(C.Structure):
     _fields_ = [("auto_bounds", C.c_int), ("eps_min", C.c_double), ("eps_max", C.c_double), ("tol", C.c_double),
                 ("max_layers", C.c_int), ("eps_alt", C.c_double), ("fp16_scale_log2", C.c_int),
                 ("control", C.c_int), ("tile_config", C.c_int), ("exact_diag", C.c_int)]
+
+
+class RefineResult(C.Structure):
+    _fields_ = [("energy_in", C.c_double), ("trace_in", C.c_double), ("iderr_in", C.c_double),
+                ("energy_out", C.c_double), ("trace_out", C.c_double), ("iderr_out", C.c_double)]
 
 
 class SP2Error(RuntimeError):
@@ -75,6 +80,9 @@ def load() -> C.CDLL:
     lib.sp2_density_matrix_batched.argtypes = [vp, vp, C.c_int, C.c_int, dp, C.c_int, C.POINTER(Opts), vp,
                                                C.POINTER(LayerStat), ip, ip, vp]
     lib.sp2_density_matrix_batched.restype = C.c_int
+    lib.sp2_refine_energy.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int, vp, C.c_int, vp, C.c_int,
+                                      C.POINTER(RefineResult), vp]
+    lib.sp2_refine_energy.restype = C.c_int
     lib.sp2_split_fp16.argtypes = [vp, C.c_int, C.c_int, vp, vp, C.c_int, C.c_int, vp]
     lib.sp2_split_fp16.restype = C.c_int
     lib.sp2_gershgorin.argtypes = [vp, vp, C.c_int, C.c_int, dp, vp]; lib.sp2_gershgorin.restype = C.c_int
@@ -229,6 +237,22 @@ class Handle:
         info = _stats_to_dict(stats, L)
         info.update(status=st, n_layers=L)
         return X, info
+
+    # -- final refinement + energy (Eq. 16)
+    def refine_energy(self, S, last_sigma: int, H, out=None, stream=None):
+        """D' = f_final(S) in enhanced precision and the observables of S and D' against H."""
+        import torch
+
+        S = _dev_f32(S, "S")
+        H = _dev_f32(H, "H")
+        N = S.shape[0]
+        D = torch.empty((N, N), dtype=torch.float32, device=S.device) if out is None else _dev_f32(out, "out")
+        res = RefineResult()
+        st = self.lib.sp2_refine_energy(self._h, S.data_ptr(), N, S.stride(0), int(last_sigma), H.data_ptr(),
+                                        H.stride(0), D.data_ptr(), D.stride(0), C.byref(res), _stream_ptr(stream))
+        if st < 0:
+            raise SP2Error(st, "sp2_refine_energy")
+        return D, {k: getattr(res, k) for k, _ in RefineResult._fields_}
 
     # -- batched small-N
     def density_matrix_batched(self, H, N_occ, opts: Optional[Opts] = None, out=None, stream=None):

@@ -50,7 +50,7 @@ struct sp2_handle_s {
     Ctrl* ctrl = nullptr;
     sp2_layer_stat_t* stats_dev = nullptr;
     double* thetas_dev = nullptr;
-    WorkItem* items_dev = nullptr;
+    WorkItem* items_dev[2] = {nullptr, nullptr};   // [0] solves, [1] refinement layers (different tile config)
     int items_cap = 0;
     // batched workspace
     sp2_layer_stat_t* bstats_dev = nullptr;
@@ -69,12 +69,15 @@ struct sp2_handle_s {
     size_t stage_elems = 0;
     PFN_encodeTiled encode = nullptr;
     std::map<std::tuple<int, int, int, int, int>, LoopGraph> graphs;   // (N, Np, cfg, scale_log2, exact_diag)
-    int items_key_np = -1, items_key_cfg = -1, items_key_split = -1;
-    int n_items = 0, n_slots = 0;
+    int items_key_np[2] = {-1, -1}, items_key_cfg[2] = {-1, -1}, items_key_split[2] = {-1, -1};
+    int n_items[2] = {0, 0}, n_slots[2] = {0, 0};
+    double* obs_dev = nullptr;      // [6] observables of sp2_refine_energy
+    double* obs_host = nullptr;
     int tail_split = 1;
     int last_launches = 0;
     double noise_kappa = 0.125;
     int round_sync = 1;
+    int enh_kc = 2;
     cudaStream_t cap_stream = nullptr;
 };
 
@@ -118,7 +121,7 @@ extern "C" size_t sp2_workspace_bytes(int N_max, int batch_max, int max_layers) 
     size_t b = Np * (size_t)ws_ld_f32((int)Np) * 4 + 4 * Np * (size_t)ws_ld_f16((int)Np) * 2;   // S + two hi/lo pairs
     b += 4 * Np * sizeof(double);                             // Gershgorin radii, diagonal, two row-sum vectors
     b += sizeof(Ctrl) + (size_t)max_layers * (sizeof(sp2_layer_stat_t) + 3 * sizeof(double));
-    b += ((Np / 128) * (Np / 128 + 1) / 2 + 1024) * sizeof(WorkItem);
+    b += 2 * ((Np / 128) * (Np / 128 + 1) / 2 + 1024) * sizeof(WorkItem);
     if (batch_max > 0)
         b += (size_t)batch_max * ((size_t)max_layers * sizeof(sp2_layer_stat_t) + 2 * sizeof(int) + 3 * sizeof(double));
     return b;
@@ -136,7 +139,7 @@ extern "C" sp2_status_t sp2_destroy(sp2_handle_t h) {
         for (int b = 0; b < 2; ++b) cudaFree(h->hl[a][b]);
     cudaFree(h->rowsq[0]); cudaFree(h->rowsq[1]);
     cudaFree(h->R); cudaFree(h->diag); cudaFree(h->ctrl); cudaFree(h->stats_dev); cudaFree(h->thetas_dev);
-    cudaFree(h->items_dev); cudaFree(h->bstats_dev); cudaFree(h->bnl_dev); cudaFree(h->bstatus_dev);
+    cudaFree(h->items_dev[0]); cudaFree(h->items_dev[1]); cudaFree(h->obs_dev); cudaFreeHost(h->obs_host); cudaFree(h->bstats_dev); cudaFree(h->bnl_dev); cudaFree(h->bstatus_dev);
     cudaFree(h->bbounds_dev); cudaFree(h->bnocc_dev);
     cudaFreeHost(h->ctrl_host); cudaFreeHost(h->stats_host); cudaFreeHost(h->thetas_host);
     cudaFreeHost(h->bounds_host); cudaFree(h->stage_H); cudaFree(h->stage_D);
@@ -160,6 +163,7 @@ extern "C" sp2_status_t sp2_create(sp2_handle_t* out, int N_max, int batch_max, 
     h->N_max = N_max; h->batch_max = batch_max; h->max_layers = max_layers;
     if (const char* e = getenv("SP2_NOISE_KAPPA")) h->noise_kappa = atof(e);   // tuning hook (C25)
     if (const char* e = getenv("SP2_TAIL_SPLIT")) h->tail_split = atoi(e);     // tuning hook
+    if (const char* e = getenv("SP2_ENH_KC")) { h->enh_kc = atoi(e); if (h->enh_kc < 1) h->enh_kc = 1; }   // tuning hook
     if (const char* e = getenv("SP2_ROUND_SYNC")) h->round_sync = atoi(e);     // tuning hook
     h->Np_max = round_up(N_max, 256);
     h->num_sms = prop.multiProcessorCount; h->device = dev;
@@ -181,7 +185,9 @@ extern "C" sp2_status_t sp2_create(sp2_handle_t* out, int N_max, int batch_max, 
     A((void**)&h->stats_dev, (size_t)max_layers * sizeof(sp2_layer_stat_t));
     A((void**)&h->thetas_dev, (size_t)max_layers * 3 * sizeof(double));
     h->items_cap = (int)((Np / 128) * (Np / 128 + 1) / 2) + 1024;
-    A((void**)&h->items_dev, (size_t)h->items_cap * sizeof(WorkItem));
+    A((void**)&h->items_dev[0], (size_t)h->items_cap * sizeof(WorkItem));
+    A((void**)&h->items_dev[1], (size_t)h->items_cap * sizeof(WorkItem));
+    A((void**)&h->obs_dev, 8 * sizeof(double));
     if (batch_max > 0) {
         A((void**)&h->bstats_dev, (size_t)batch_max * max_layers * sizeof(sp2_layer_stat_t));
         A((void**)&h->bnl_dev, (size_t)batch_max * sizeof(int));
@@ -198,6 +204,7 @@ extern "C" sp2_status_t sp2_create(sp2_handle_t* out, int N_max, int batch_max, 
     AH((void**)&h->stats_host, (size_t)max_layers * sizeof(sp2_layer_stat_t));
     AH((void**)&h->thetas_host, (size_t)max_layers * 3 * sizeof(double));
     AH((void**)&h->bounds_host, 2 * sizeof(double));
+    AH((void**)&h->obs_host, 8 * sizeof(double));
     if (st == SP2_OK) {
         cudaError_t e = cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking);
         if (e != cudaSuccess) st = cuda_fail(e, "cudaStreamCreate");
@@ -210,7 +217,7 @@ extern "C" sp2_status_t sp2_create(sp2_handle_t* out, int N_max, int batch_max, 
             st = cuda_fail(e == cudaSuccess ? cudaErrorUnknown : e, "cudaGetDriverEntryPoint(cuTensorMapEncodeTiled)");
         h->encode = (PFN_encodeTiled)fn;
     }
-    for (int cfg = TILE_128x128; cfg <= TILE_256x256_PAIR && st == SP2_OK; ++cfg) {
+    for (int cfg = TILE_128x128; cfg <= TILE_128x128_ENH && st == SP2_OK; ++cfg) {
         cudaError_t e = layer_kernel_setup(cfg);
         if (e != cudaSuccess) st = cuda_fail(e, "cudaFuncSetAttribute(layer kernel)");
     }
@@ -279,7 +286,7 @@ static void build_work_list(int nt, int band, int edge, int subs, int cta_group,
 }
 
 static int choose_tile_config(int N, int requested, int num_sms) {
-    if (requested >= TILE_128x128 && requested <= TILE_256x256_PAIR) return requested;
+    if (requested >= TILE_128x128 && requested <= TILE_256x256_PAIR) return requested;   // ENH is internal
     const int n128 = round_up(N, 128) / 128;
     const long long t128 = (long long)n128 * (n128 + 1) / 2;
     // enough 256x256 supertiles to keep every CTA pair busy for several waves -> paired 256x256 tiles
@@ -291,13 +298,16 @@ static int choose_tile_config(int N, int requested, int num_sms) {
 }
 
 struct Problem {
-    int N, Np, cfg, scale_log2, n_items, n_slots, exact_diag;
+    int N, Np, cfg, scale_log2, n_items, n_slots, exact_diag, list;
     float scale, inv_scale2;
 };
 
-static sp2_status_t prepare_problem(sp2_handle_s* h, int N, const sp2_opts_t* o, Problem* pb, cudaStream_t st) {
+static sp2_status_t prepare_problem(sp2_handle_s* h, int N, const sp2_opts_t* o, Problem* pb, cudaStream_t st,
+                                    int forced_cfg = 0) {
     pb->N = N;
-    pb->cfg = choose_tile_config(N, o ? o->tile_config : 0, h->num_sms);
+    pb->cfg = forced_cfg ? forced_cfg : choose_tile_config(N, o ? o->tile_config : 0, h->num_sms);
+    pb->list = forced_cfg ? 1 : 0;
+    const int L = pb->list;
     const int edge = tile_super_edge(pb->cfg);
     pb->Np = round_up(N, edge);
     if (pb->Np > h->Np_max) return SP2_ERR_WORKSPACE;
@@ -310,21 +320,21 @@ static sp2_status_t prepare_problem(sp2_handle_s* h, int N, const sp2_opts_t* o,
     pb->inv_scale2 = ldexpf(1.0f, -2 * k);
     const int nt = pb->Np / edge;
     const int band = (pb->cfg == TILE_256x256_PAIR) ? 8 : 12;
-    if (h->items_key_np != pb->Np || h->items_key_cfg != pb->cfg || h->items_key_split != h->tail_split) {
+    if (h->items_key_np[L] != pb->Np || h->items_key_cfg[L] != pb->cfg || h->items_key_split[L] != h->tail_split) {
         std::vector<WorkItem> list;
         int slots = 0;
         build_work_list(nt, band, edge, tile_subs(pb->cfg), tile_cta_group(pb->cfg), h->num_sms, h->tail_split, list,
                         &slots);
         if ((int)list.size() > h->items_cap) return SP2_ERR_WORKSPACE;
         // synchronous small copy: happens only when the problem shape changes
-        CK(cudaMemcpyAsync(h->items_dev, list.data(), list.size() * sizeof(WorkItem), cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(h->items_dev[L], list.data(), list.size() * sizeof(WorkItem), cudaMemcpyHostToDevice, st));
         CK(cudaStreamSynchronize(st));
-        h->items_key_np = pb->Np; h->items_key_cfg = pb->cfg; h->items_key_split = h->tail_split;
-        h->n_items = (int)list.size();
-        h->n_slots = slots;
+        h->items_key_np[L] = pb->Np; h->items_key_cfg[L] = pb->cfg; h->items_key_split[L] = h->tail_split;
+        h->n_items[L] = (int)list.size();
+        h->n_slots[L] = slots;
     }
-    pb->n_items = h->n_items;
-    pb->n_slots = h->n_slots;
+    pb->n_items = h->n_items[L];
+    pb->n_slots = h->n_slots[L];
     return SP2_OK;
 }
 
@@ -334,9 +344,9 @@ static LayerParams layer_params(sp2_handle_s* h, const Problem& pb, int parity, 
     p.hi_out = h->hl[parity ^ 1][0]; p.lo_out = h->hl[parity ^ 1][1];
     p.rowsq_cur = pb.exact_diag ? h->rowsq[parity] : nullptr;
     p.rowsq_next = pb.exact_diag ? h->rowsq[parity ^ 1] : nullptr;
-    p.items = h->items_dev; p.ld = ws_ld_f32(pb.Np); p.ldf = ws_ld_f16(pb.Np); p.N = pb.N; p.Np = pb.Np;
+    p.items = h->items_dev[pb.list]; p.ld = ws_ld_f32(pb.Np); p.ldf = ws_ld_f16(pb.Np); p.N = pb.N; p.Np = pb.Np;
     p.n_items = pb.n_items; p.n_slots = pb.n_slots;
-    p.scale = pb.scale; p.inv_scale2 = pb.inv_scale2; p.cond_handle = cond; p.round_sync = h->round_sync;
+    p.scale = pb.scale; p.inv_scale2 = pb.inv_scale2; p.cond_handle = cond; p.round_sync = h->round_sync; p.enh_kc = h->enh_kc;
     return p;
 }
 
@@ -506,6 +516,59 @@ extern "C" sp2_status_t sp2_density_matrix_host(sp2_handle_t h, const float* H_h
                          cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
     return s;
+}
+
+// NEXT-1: final refinement f_final (Eq. 16) as two layers with enhanced accumulation, plus Tr[D H].
+extern "C" sp2_status_t sp2_refine_energy(sp2_handle_t h, const float* S_dev, int N, int lds, int last_sigma,
+                                          const float* H_dev, int ldh, float* D_dev, int ldd,
+                                          sp2_refine_result_t* result, void* stream) {
+    sp2_status_t s = check_common(h, S_dev, N, lds, D_dev, ldd);
+    if (s != SP2_OK) return s;
+    if (!H_dev || ldh < N || !result || (last_sigma != 1 && last_sigma != -1)) return SP2_ERR_INVALID_ARG;
+    if (h->max_layers < 2) return SP2_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    Problem pb;
+    s = prepare_problem(h, N, nullptr, &pb, st, TILE_128x128_ENH);
+    if (s != SP2_OK) return s;
+    pb.exact_diag = 1;                               // diag(X) from row sums of squares (reading C24), as in the solve
+    // Reading C15: continue the alternation from the last applied sign.
+    //   last sigma = -1: X = S^2, then 2X - X^2  ->  2 S^2 - S^4 ;   last sigma = +1: T = 2S - S^2, then T^2.
+    double* th = h->thetas_host;
+    if (last_sigma < 0) { th[0] = 1; th[1] = 0; th[2] = 0; th[3] = -1; th[4] = 2; th[5] = 0; }
+    else                { th[0] = -1; th[1] = 2; th[2] = 0; th[3] = 1; th[4] = 0; th[5] = 0; }
+    Ctrl* c = h->ctrl_host;
+    memset(c, 0, ctrl_header_bytes());
+    c->N = N; c->mode = MODE_GENERALIZED; c->max_layers = 2;
+    CK(cudaMemcpyAsync(h->ctrl, c, ctrl_header_bytes(), cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(h->thetas_dev, th, 6 * sizeof(double), cudaMemcpyHostToDevice, st));
+    CK(cudaMemsetAsync(h->stats_dev, 0, 2 * sizeof(sp2_layer_stat_t), st));
+    const size_t ldS = (size_t)ws_ld_f32(pb.Np), ldF = (size_t)ws_ld_f16(pb.Np);
+    if (pb.Np != N) CK(cudaMemsetAsync(h->S, 0, (size_t)pb.Np * ldS * 4, st));
+    CK(cudaMemcpy2DAsync(h->S, ldS * 4, S_dev, (size_t)lds * 4, (size_t)N * 4, (size_t)N, cudaMemcpyDeviceToDevice, st));
+    // observables of the input, and the plan of layer 1 (thetas[0])
+    CK(cudaMemsetAsync(h->rowsq[0], 0, (size_t)pb.Np * sizeof(unsigned long long), st));
+    CK(cudaMemsetAsync(h->rowsq[1], 0, (size_t)pb.Np * sizeof(unsigned long long), st));
+    CK(launch_energy_traces(h->S, (long long)ldS, H_dev, ldh, N, h->ctrl, h->obs_dev, 1, h->stats_dev, h->thetas_dev,
+                            h->rowsq[0], h->num_sms, st));
+    CK(launch_split(h->S, pb.Np, (long long)ldS, h->hl[0][0], h->hl[0][1], (long long)ldF, pb.scale, h->num_sms, st));
+    s = launch_one_layer(h, pb, 0, 0, st);
+    if (s == SP2_OK) s = launch_one_layer(h, pb, 1, 0, st);
+    if (s != SP2_OK) return s;
+    CK(cudaMemcpy2DAsync(D_dev, (size_t)ldd * 4, h->S, ldS * 4, (size_t)N * 4, (size_t)N, cudaMemcpyDeviceToDevice, st));
+    CK(launch_energy_traces(D_dev, ldd, H_dev, ldh, N, h->ctrl, h->obs_dev + 3, 0, nullptr, nullptr, nullptr,
+                            h->num_sms, st));
+    CK(cudaMemcpyAsync(h->obs_host, h->obs_dev, 6 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(h->ctrl_host, h->ctrl, ctrl_header_bytes(), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    CK(cudaGetLastError());
+    const double* o = h->obs_host;
+    result->energy_in = o[0]; result->trace_in = o[1]; result->iderr_in = o[1] - o[2];
+    result->energy_out = o[3]; result->trace_out = o[4]; result->iderr_out = o[4] - o[5];
+    h->last_launches = h->ctrl_host->launches;
+    if (h->ctrl_host->error < 0) return (sp2_status_t)h->ctrl_host->error;
+    if (h->ctrl_host->n != 2) return SP2_ERR_CUDA;
+    if (!isfinite(o[3]) || !isfinite(o[4]) || !isfinite(o[5])) return SP2_ERR_NONFINITE;
+    return SP2_OK;
 }
 
 extern "C" sp2_status_t sp2_generalized(sp2_handle_t h, const float* H_dev, int N, int ldh, const double* theta_host,

@@ -301,6 +301,103 @@ __global__ void __launch_bounds__(256) k_split_scalar(const float* __restrict__ 
     }
 }
 
+// ------------------------------------------------------------------------------------------------ NEXT-1
+// Observables of a symmetric X against H (both read through their lower triangles, reading C22):
+//   out[0] = Tr[X H] = sum_i X_ii H_ii + 2 sum_{i>j} X_ij H_ij   (the energy alpha = Tr[D H])
+//   out[1] = Tr[X],  out[2] = ||X||_F^2 = Tr[X^2]  ->  IdErr = Tr[X - X^2] = out[1] - out[2]
+// FP32 products summed per thread over one tile (16 elements), FP64 across tiles; per-block partials are summed
+// in fixed order by the last block.  If `plan` is set, that block also seeds the control block with N_S, N_X and
+// plans layer 1 (used by the refinement, whose two layers have given thetas).
+__global__ void __launch_bounds__(256) k_energy_traces(const float* __restrict__ X, long long ldx,
+                                                       const float* __restrict__ H, long long ldh, int N, Ctrl* ctrl,
+                                                       double* __restrict__ out, int plan, sp2_layer_stat_t* stats,
+                                                       const double* thetas, unsigned long long* __restrict__ rowsq) {
+    __shared__ double red[8][3];
+    __shared__ float colacc[16][ET];
+    const int nt = (N + ET - 1) / ET;
+    const long long ntiles = (long long)nt * (nt + 1) / 2;
+    const int c4 = (threadIdx.x & 15) * 4, r0 = threadIdx.x >> 4;
+    const bool vx = ((ldx & 3) == 0) && ((reinterpret_cast<uintptr_t>(X) & 15) == 0);
+    const bool vh = ((ldh & 3) == 0) && ((reinterpret_cast<uintptr_t>(H) & 15) == 0);
+    double e = 0.0, tr = 0.0, f2 = 0.0;
+    for (long long t = blockIdx.x; t < ntiles; t += gridDim.x) {
+        int I, J;
+        tri_decode(t, I, J);
+        const int j = J * ET + c4;
+        float eo = 0.f, fo = 0.f;                   // off-diagonal partial sums of this tile
+        float cs[4] = {0.f, 0.f, 0.f, 0.f};         // squares per column (rows of the mirrored part)
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const int i = I * ET + r0 + 16 * k;
+            const float4 x4 = ld_tile4(X, N, ldx, i, j, vx);
+            const float4 h4 = ld_tile4(H, N, ldh, i, j, vh);
+            const float xv[4] = {x4.x, x4.y, x4.z, x4.w}, hv[4] = {h4.x, h4.y, h4.z, h4.w};
+            float rsq = 0.f;                        // row i: squares of its entries j <= i held by this thread
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const int jj = j + q;
+                if (i < N && jj < i) {
+                    const float sq = xv[q] * xv[q];
+                    eo = fmaf(xv[q], hv[q], eo); fo += sq; rsq += sq; cs[q] += sq;
+                } else if (i < N && jj == i) {
+                    const double xd = (double)xv[q];
+                    e += xd * (double)hv[q]; tr += xd; f2 += xd * xd;
+                    rsq += xv[q] * xv[q];
+                }
+            }
+            if (rowsq) {
+                rsq = row16_sum(rsq);
+                if ((threadIdx.x & 15) == 0 && i < N) atomicAdd(rowsq + i, rowsq_fix((double)rsq));
+            }
+        }
+        if (rowsq) {                                // uniform over the block
+            *reinterpret_cast<float4*>(&colacc[r0][c4]) = make_float4(cs[0], cs[1], cs[2], cs[3]);
+            __syncthreads();
+            if (threadIdx.x < ET) {
+                float c = 0.f;
+#pragma unroll
+                for (int g = 0; g < 16; ++g) c += colacc[g][threadIdx.x];
+                const int jc = J * ET + threadIdx.x;
+                if (jc < N && c != 0.f) atomicAdd(rowsq + jc, rowsq_fix((double)c));
+            }
+            __syncthreads();
+        }
+        e += 2.0 * (double)eo;
+        f2 += 2.0 * (double)fo;
+    }
+    e = warp_sum(e); tr = warp_sum(tr); f2 = warp_sum(f2);
+    if ((threadIdx.x & 31) == 0) { red[threadIdx.x >> 5][0] = e; red[threadIdx.x >> 5][1] = tr; red[threadIdx.x >> 5][2] = f2; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double a = 0.0, b = 0.0, c = 0.0;
+        for (int w = 0; w < 8; ++w) { a += red[w][0]; b += red[w][1]; c += red[w][2]; }
+        ctrl->partial[blockIdx.x][0] = a;
+        ctrl->partial[blockIdx.x][1] = b;
+        ctrl->partial[blockIdx.x][2] = c;
+        __threadfence();
+        const unsigned int done = atomicAdd(&ctrl->done_counter, 1u);
+        if (done == gridDim.x - 1) {
+            __threadfence();
+            double s0 = 0.0, s1 = 0.0, s2 = 0.0;
+            for (unsigned int i = 0; i < gridDim.x; ++i) {
+                s0 += ((volatile double*)ctrl->partial[i])[0];
+                s1 += ((volatile double*)ctrl->partial[i])[1];
+                s2 += ((volatile double*)ctrl->partial[i])[2];
+            }
+            out[0] = s0; out[1] = s1; out[2] = s2;
+            ctrl->done_counter = 0;
+            ctrl->launches += 1;
+            if (plan) {
+                ctrl->N_S = s1;
+                ctrl->fro2 = s2;
+                ctrl->n = 0;
+                ctrl->round_counter = 0;
+                control_plan_next(ctrl, stats, thetas);
+            }
+        }
+    }
+}
+
 // ------------------------------------------------------------------------------------------------ launchers
 cudaError_t launch_gershgorin(const float* H, int N, long long ldh, double* R, double* diag, Ctrl* ctrl,
                               double* bounds_out, int num_sms, cudaStream_t st) {
@@ -340,4 +437,18 @@ cudaError_t launch_split(const float* X, int N, long long ldx, __half* hi, __hal
     return cudaGetLastError();
 }
 
+}  // namespace sp2
+
+namespace sp2 {
+cudaError_t launch_energy_traces(const float* X, long long ldx, const float* H, long long ldh, int N, Ctrl* ctrl,
+                                 double* out, int plan, sp2_layer_stat_t* stats, const double* thetas,
+                                 unsigned long long* rowsq, int num_sms, cudaStream_t st) {
+    const int nt = (N + ET - 1) / ET;
+    const long long ntiles = (long long)nt * (nt + 1) / 2;
+    long long cap = (long long)num_sms * 6;
+    if (cap > kMaxPartials) cap = kMaxPartials;
+    const int grid = (int)(ntiles < cap ? ntiles : cap);
+    k_energy_traces<<<grid, 256, 0, st>>>(X, ldx, H, ldh, N, ctrl, out, plan, stats, thetas, rowsq);
+    return cudaGetLastError();
+}
 }  // namespace sp2

@@ -23,6 +23,9 @@ constexpr double kRowSqInv = 1.0 / 17592186044416.0;
 __device__ __forceinline__ unsigned long long rowsq_fix(double x) {
     return (unsigned long long)__double2ll_rn(x * kRowSqScale);
 }
+cudaError_t launch_energy_traces(const float* X, long long ldx, const float* H, long long ldh, int N, Ctrl* ctrl,
+                                 double* out, int plan, sp2_layer_stat_t* stats, const double* thetas,
+                                 unsigned long long* rowsq, int num_sms, cudaStream_t st);
 cudaError_t launch_split(const float* X, int N, long long ldx, __half* hi, __half* lo, long long ldo, float scale,
                          int num_sms, cudaStream_t st);
 
@@ -33,7 +36,8 @@ inline long long ws_ld_f32(int Np) { return (long long)Np + 32; }
 inline long long ws_ld_f16(int Np) { return (long long)Np + 64; }
 
 // ---- fused symmetric square layer (sp2_square_tiled.cu)
-enum TileConfig { TILE_AUTO = 0, TILE_128x128 = 1, TILE_128x256 = 2, TILE_256x256_PAIR = 3 };
+enum TileConfig { TILE_AUTO = 0, TILE_128x128 = 1, TILE_128x256 = 2, TILE_256x256_PAIR = 3,
+                  TILE_128x128_ENH = 4 /* enhanced accumulation, refinement layers only */ };
 
 // One unit of work of a layer kernel: rows [(I * E + (sub * CG + rank) * 128), +128) per CTA of supertile (I, J),
 // I >= J, E = supertile edge; columns [J * E + col0, + ncols).  ncols = E except for the items of the last, partial
@@ -62,6 +66,7 @@ struct LayerParams {
     int n_slots;                   // CTA slots (CTAs / CG) of the launch
     float scale;                   // c = 2^k of the split
     float inv_scale2;              // 1 / c^2
+    int enh_kc;                    // enhanced accumulation: K-blocks (of 64) per tensor-core accumulation chunk
     int round_sync;                // 1: producers of all CTAs meet at every round boundary (keeps the wave in lockstep)
     unsigned long long cond_handle;  // cudaGraphConditionalHandle (0 = none)
 };

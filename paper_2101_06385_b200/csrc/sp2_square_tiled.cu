@@ -17,8 +17,12 @@
 
 namespace sp2 {
 
-template <int BN_, int CG_>
+template <int BN_, int CG_, bool ENH_ = false>
 struct TileCfg {
+    // ENH: enhanced accumulation ("single precision with double accumulation") for the refinement layers:
+    // the tensor core accumulates only p.enh_kc K-blocks at a time; the chunk sums are added into a running FP32 pair
+    // (two-sum) kept in two more TMEM regions, so the truncating FP32 accumulation never runs over the whole K.
+    static constexpr bool ENH = ENH_;
     static constexpr int BN = BN_;                 // accumulator columns = supertile edge
     static constexpr int CG = CG_;                 // CTAs cooperating on one MMA (cta_group)
     static constexpr int BM = 128;                 // accumulator rows per CTA (TMEM lanes)
@@ -29,7 +33,8 @@ struct TileCfg {
     static constexpr int STAGE_BYTES = 2 * A_BYTES + 2 * B_BYTES;   // hi and lo of both panels
     static constexpr int STAGES = (STAGE_BYTES > 65536) ? 2 : 3;
     static constexpr int SUB = (BN / BM) / CG;     // 128-row work items per supertile per CTA slot
-    static constexpr int TMEM_COLS = 2 * BN;       // two accumulator buffers
+    static constexpr int TMEM_COLS = ENH ? 4 * BN : 2 * BN;   // two accumulator buffers (+ running hi, lo)
+    static_assert(TMEM_COLS <= 512, "TMEM has 512 columns");
     static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*align*/ + 256 /*barriers*/;
     static constexpr int THREADS = 192;
 };
@@ -155,39 +160,45 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
         if (rank == 0) {
             int s = 0;
             uint32_t ph = 0;
-            int it = 0;
-            for (int w = slot; w < n_work; w += nslots, ++it) {
-                const int buf = it & 1;
-                const uint32_t use = (uint32_t)(it >> 1);
+            int it = 0;                                   // accumulator uses so far (one per item; per chunk if ENH)
+            for (int w = slot; w < n_work; w += nslots) {
                 const uint32_t idesc = umma_idesc_f16(BM * CG, p.items[w].ncols);   // N = 256, or 128 / 64 in the tail
-                mbar_wait(&tempty_bar[buf], (use & 1u) ^ 1u);       // epilogue has drained this accumulator
-                tc_fence_after();
-                const uint32_t d_tmem = tmem_base + (uint32_t)(buf * BN);
-                for (int kb = 0; kb < KB; ++kb) {
-                    mbar_wait(&full_bar[s], ph);
+                const int KC = p.enh_kc;                  // K-blocks per accumulation chunk (ENH)
+                const int nch = C::ENH ? (KB + KC - 1) / KC : 1;
+                for (int ch = 0; ch < nch; ++ch, ++it) {
+                    const int buf = it & 1;
+                    const uint32_t use = (uint32_t)(it >> 1);
+                    const int kb0 = C::ENH ? ch * KC : 0;
+                    const int kb1 = C::ENH ? (kb0 + KC < KB ? kb0 + KC : KB) : KB;
+                    mbar_wait(&tempty_bar[buf], (use & 1u) ^ 1u);   // epilogue has drained this accumulator
                     tc_fence_after();
-                    if (lane == 0) {
-                        const uint32_t a_hi = smem_u32(smem + s * C::STAGE_BYTES);
-                        const uint32_t a_lo = a_hi + C::A_BYTES;
-                        const uint32_t b_hi = a_hi + 2 * C::A_BYTES;
-                        const uint32_t b_lo = b_hi + C::B_BYTES;
+                    const uint32_t d_tmem = tmem_base + (uint32_t)(buf * BN);
+                    for (int kb = kb0; kb < kb1; ++kb) {
+                        mbar_wait(&full_bar[s], ph);
+                        tc_fence_after();
+                        if (lane == 0) {
+                            const uint32_t a_hi = smem_u32(smem + s * C::STAGE_BYTES);
+                            const uint32_t a_lo = a_hi + C::A_BYTES;
+                            const uint32_t b_hi = a_hi + 2 * C::A_BYTES;
+                            const uint32_t b_lo = b_hi + C::B_BYTES;
 #pragma unroll
-                        for (int k = 0; k < BK / 16; ++k) {
-                            const uint64_t dah = umma_desc_sw128(a_hi + k * 32);
-                            const uint64_t dal = umma_desc_sw128(a_lo + k * 32);
-                            const uint64_t dbh = umma_desc_sw128(b_hi + k * 32);
-                            const uint64_t dbl = umma_desc_sw128(b_lo + k * 32);
-                            umma_f16<CG>(d_tmem, dah, dbh, idesc, (kb | k) != 0);   // X0 X0
-                            umma_f16<CG>(d_tmem, dah, dbl, idesc, 1u);              // X0 X1
-                            umma_f16<CG>(d_tmem, dal, dbh, idesc, 1u);              // (X0 X1)^T
+                            for (int k = 0; k < BK / 16; ++k) {
+                                const uint64_t dah = umma_desc_sw128(a_hi + k * 32);
+                                const uint64_t dal = umma_desc_sw128(a_lo + k * 32);
+                                const uint64_t dbh = umma_desc_sw128(b_hi + k * 32);
+                                const uint64_t dbl = umma_desc_sw128(b_lo + k * 32);
+                                umma_f16<CG>(d_tmem, dah, dbh, idesc, (kb != kb0 || k != 0) ? 1u : 0u);   // X0 X0
+                                umma_f16<CG>(d_tmem, dah, dbl, idesc, 1u);                                // X0 X1
+                                umma_f16<CG>(d_tmem, dal, dbh, idesc, 1u);                                // (X0 X1)^T
+                            }
+                            if (CG == 1) umma_commit(&empty_bar[s]); else umma_commit_pair(&empty_bar[s], 0x3);
+                            if (kb == kb1 - 1) {
+                                if (CG == 1) umma_commit(&tfull_bar[buf]); else umma_commit_pair(&tfull_bar[buf], 0x3);
+                            }
                         }
-                        if (CG == 1) umma_commit(&empty_bar[s]); else umma_commit_pair(&empty_bar[s], 0x3);
-                        if (kb == KB - 1) {
-                            if (CG == 1) umma_commit(&tfull_bar[buf]); else umma_commit_pair(&tfull_bar[buf], 0x3);
-                        }
+                        __syncwarp();
+                        if (++s == STAGES) { s = 0; ph ^= 1u; }
                     }
-                    __syncwarp();
-                    if (++s == STAGES) { s = 0; ph ^= 1u; }
                 }
             }
         }
@@ -212,10 +223,10 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
         // (4 independent partial sums, |error| <= ~2^-22 of a sum of ~1e-3) and promoted to FP64 once per chunk;
         // the diagonal chunk (one per 128 rows of a diagonal supertile) keeps per-element FP64.
         double trS = 0.0, off2 = 0.0, dg2 = 0.0, trX = 0.0;   // ||S_n||_F^2 = 2 off2 + dg2
-        int it = 0;
+        int it = 0;                                         // accumulator uses so far (same count as the MMA warp)
+        const int nch = C::ENH ? (KB + p.enh_kc - 1) / p.enh_kc : 1;
+        const uint32_t lane_off = (uint32_t)(q * 32) << 16;
         for (int w = slot; w < n_work; w += nslots, ++it) {
-            const int buf = it & 1;
-            const uint32_t use = (uint32_t)(it >> 1);
             const WorkItem wi = p.items[w];
             const int m0 = wi.I * BN + (wi.sub * CG + (int)rank) * BM;
             const int n0 = wi.J * BN + wi.col0;
@@ -223,9 +234,54 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
             const int gi = m0 + rl;
             const int gi_wmin = m0 + q * 32, gi_wmax = gi_wmin + 31;
             double rowacc = 0.0;                            // sum_j S_n(gi, j)^2 over the own entries (j <= gi) of this tile
+            if (C::ENH) {
+                // all chunks but the last: fold the chunk sum into the running FP32 pair (two-sum, error-free)
+                const uint32_t t_rh = tmem_base + (uint32_t)(2 * BN) + lane_off, t_rl = t_rh + (uint32_t)BN;
+                for (int ch = 0; ch < nch - 1; ++ch, ++it) {
+                    const int fbuf = it & 1;
+                    mbar_wait(&tfull_bar[fbuf], (uint32_t)(it >> 1) & 1u);
+                    tc_fence_after();
+                    const uint32_t t_acc = tmem_base + (uint32_t)(fbuf * BN) + lane_off;
+#pragma unroll 1
+                    for (int c0 = 0; c0 < ncols; c0 += 32) {
+                        if (n0 + c0 > gi_wmax) break;
+                        uint32_t a[32], rh[32], rlo[32];
+                        tmem_ld_32x32(t_acc + (uint32_t)c0, a);
+                        if (ch > 0) {
+                            tmem_ld_32x32(t_rh + (uint32_t)c0, rh);
+                            tmem_ld_32x32(t_rl + (uint32_t)c0, rlo);
+                        }
+                        tmem_ld_wait();
+                        if (ch == 0) {
+#pragma unroll
+                            for (int c = 0; c < 32; ++c) { rh[c] = a[c]; rlo[c] = 0u; }
+                        } else {
+#pragma unroll
+                            for (int c = 0; c < 32; ++c) {
+                                const float x = __uint_as_float(rh[c]), y = __uint_as_float(a[c]);
+                                const float sm = x + y;
+                                const float bb = sm - x;
+                                const float err = (x - (sm - bb)) + (y - bb);
+                                rh[c] = __float_as_uint(sm);
+                                rlo[c] = __float_as_uint(__uint_as_float(rlo[c]) + err);
+                            }
+                        }
+                        tmem_st_32x32(t_rh + (uint32_t)c0, rh);
+                        tmem_st_32x32(t_rl + (uint32_t)c0, rlo);
+                    }
+                    tmem_st_wait();
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) {
+                        if (CG == 1) mbar_arrive(&tempty_bar[fbuf]); else mbar_arrive_cluster(&tempty_bar[fbuf], 0);
+                    }
+                }
+            }
+            const int buf = it & 1;
+            const uint32_t use = (uint32_t)(it >> 1);
             mbar_wait(&tfull_bar[buf], use & 1u);
             tc_fence_after();
-            const uint32_t taddr = tmem_base + (uint32_t)(buf * BN) + ((uint32_t)(q * 32) << 16);
+            const uint32_t taddr = tmem_base + (uint32_t)(buf * BN) + lane_off;
             unsigned short* HOu = reinterpret_cast<unsigned short*>(HO);
             unsigned short* LOu = reinterpret_cast<unsigned short*>(LO);
 #pragma unroll 1
@@ -235,6 +291,21 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                 uint32_t v[32];
                 float so[32];
                 tmem_ld_32x32(taddr + (uint32_t)c0, v);
+                if (C::ENH && nch > 1) {
+                    // last chunk: total = running pair + this chunk, rounded once to FP32
+                    uint32_t rh[32], rlo[32];
+                    tmem_ld_32x32(tmem_base + (uint32_t)(2 * BN) + lane_off + (uint32_t)c0, rh);
+                    tmem_ld_32x32(tmem_base + (uint32_t)(3 * BN) + lane_off + (uint32_t)c0, rlo);
+                    tmem_ld_wait();
+#pragma unroll
+                    for (int c = 0; c < 32; ++c) {
+                        const float x = __uint_as_float(rh[c]), y = __uint_as_float(v[c]);
+                        const float sm = x + y;
+                        const float bb = sm - x;
+                        const float err = (x - (sm - bb)) + (y - bb);
+                        v[c] = __float_as_uint(sm + (err + __uint_as_float(rlo[c])));
+                    }
+                }
                 const bool below = (gj0 + 31 <= gi_wmin);   // whole 32x32 chunk strictly in the lower triangle
                 // S_{n-1}: read at the mirrored position (S is exactly symmetric) -> coalesced across the warp
 #pragma unroll
@@ -372,8 +443,9 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
 using Cfg128 = TileCfg<128, 1>;
 using Cfg256 = TileCfg<256, 1>;
 using Cfg256P = TileCfg<256, 2>;
+using Cfg128E = TileCfg<128, 1, true>;
 
-int tile_super_edge(int cfg) { return cfg == TILE_128x128 ? 128 : 256; }
+int tile_super_edge(int cfg) { return (cfg == TILE_128x128 || cfg == TILE_128x128_ENH) ? 128 : 256; }
 int tile_subs(int cfg) { return cfg == TILE_128x256 ? Cfg256::SUB : 1; }
 int tile_cta_group(int cfg) { return cfg == TILE_256x256_PAIR ? 2 : 1; }
 int layer_slots(int cfg, int n_items, int num_sms) {
@@ -384,7 +456,8 @@ int layer_slots(int cfg, int n_items, int num_sms) {
     return slots;
 }
 size_t tile_smem_bytes(int cfg) {
-    return cfg == TILE_128x128 ? Cfg128::SMEM_BYTES : cfg == TILE_128x256 ? Cfg256::SMEM_BYTES : Cfg256P::SMEM_BYTES;
+    return cfg == TILE_128x128 ? Cfg128::SMEM_BYTES : cfg == TILE_128x128_ENH ? Cfg128E::SMEM_BYTES :
+           cfg == TILE_128x256 ? Cfg256::SMEM_BYTES : Cfg256P::SMEM_BYTES;
 }
 
 cudaError_t layer_kernel_setup(int cfg) {
@@ -398,6 +471,9 @@ cudaError_t layer_kernel_setup(int cfg) {
         case TILE_256x256_PAIR:
             return cudaFuncSetAttribute(k_sp2_layer<Cfg256P>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                         Cfg256P::SMEM_BYTES);
+        case TILE_128x128_ENH:
+            return cudaFuncSetAttribute(k_sp2_layer<Cfg128E>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                        Cfg128E::SMEM_BYTES);
     }
     return cudaErrorInvalidValue;
 }
@@ -428,6 +504,7 @@ cudaError_t launch_layer(int cfg, const CUtensorMap& tm_hi, const CUtensorMap& t
         case TILE_128x128: return launch_cfg<Cfg128>(tm_hi, tm_lo, p, num_sms, st);
         case TILE_128x256: return launch_cfg<Cfg256>(tm_hi, tm_lo, p, num_sms, st);
         case TILE_256x256_PAIR: return launch_cfg<Cfg256P>(tm_hi, tm_lo, p, num_sms, st);
+        case TILE_128x128_ENH: return launch_cfg<Cfg128E>(tm_hi, tm_lo, p, num_sms, st);
     }
     return cudaErrorInvalidValue;
 }

@@ -74,3 +74,35 @@ def test_config3_literal_tensor_core_diagonal_explicit_bounds(big):
     assert float(np.abs(Dc[ri, ci].cpu().numpy() - ref).max()) <= P.TOL_D
     assert abs(float(torch.trace(Dc)) - w.N_occ) <= P.TOL_TRACE_REL * w.N_occ
     assert float(torch.linalg.norm(Dc @ Dc - Dc) / np.sqrt(w.N)) <= 2 * P.TOL_IDEM   # noisier stop (C24)
+
+
+def test_config3_full_size_refinement_and_energy(big):
+    """NEXT-1 at full size: f_final (Eq. 16) in enhanced precision after the solve, energy Tr[D H] against the sum
+    of the occupied eigenvalues (known by construction), idempotency before / after (FP64 product, harness side)."""
+    api, h, torch, w, H = big
+    N = w.N
+    opts = api.make_opts(bounds=w.bounds, tol=w.tol, max_layers=w.max_layers)
+    D0, info = h.density_matrix(H, w.N_occ, opts)
+    D1, res = h.refine_energy(D0, info["sigma"][-1], H)
+    E_star = float(np.sort(w.eps)[: int(w.N_occ)].sum())
+    rng = np.random.default_rng(11)
+    ri, ci = rng.integers(0, N, 4096), rng.integers(0, N, 4096)
+    ri[:2048] = ci[:2048]
+    ref = O.closed_form_density_entries(w.Q, w.N_occ, ri, ci)
+    out = []
+    for D in (D0, D1):
+        Dc = D.double()
+        out.append((float(np.abs(Dc[ri, ci].cpu().numpy() - ref).max()),
+                    float(torch.linalg.norm(Dc @ Dc - Dc) / np.sqrt(N)), float(torch.trace(Dc)) - w.N_occ))
+        del Dc
+    print(f"refine N={N}: max sampled err {out[0][0]:.2e} -> {out[1][0]:.2e}, idem {out[0][1]:.2e} -> {out[1][1]:.2e}, "
+          f"trace-N_occ {out[0][2]:+.2e} -> {out[1][2]:+.2e}, E-E* {res['energy_in'] - E_star:+.2e} -> "
+          f"{res['energy_out'] - E_star:+.2e}, IdErr {res['iderr_in']:.2e} -> {res['iderr_out']:.2e}")
+    assert torch.equal(D1, D1.T)
+    assert out[1][0] <= out[0][0] and out[1][0] <= P.TOL_D
+    assert out[1][1] <= 0.1 * out[0][1] and out[1][1] <= 5e-6       # "multiple orders of magnitude" (P:184): measured 150x
+    assert abs(out[1][2]) <= 0.1 * abs(out[0][2]) + 1e-3
+    assert abs(res["energy_out"] - E_star) <= 0.1 * abs(res["energy_in"] - E_star)
+    assert 0 <= res["iderr_out"] <= 0.05 * res["iderr_in"]
+    # the observables are FP64 sums over the FP32 matrices the library holds
+    assert abs(res["trace_out"] - (out[1][2] + w.N_occ)) <= 1e-6
