@@ -20,15 +20,20 @@ struct ResCfg {
     static constexpr int KBLK = NP / 64;
     static constexpr int PANEL_BYTES = KBLK * 16384;      // 128 rows x NP fp16
     static constexpr int TMEM_COLS = 2 * NP;
-    static constexpr int THREADS = 160;                   // warps 0-3: rows / epilogue, warp 4: MMA + TMEM alloc
-    static constexpr int STAGE_FLOATS = 4 * 32 * 33;
+    // warps 0-7: rows / epilogue (warp w owns TMEM lanes 32 (w % 4) .. +31 and every second 32-column chunk of them:
+    // two warps per scheduler hide each other's latencies and halve the longest chunk list), warp 8: MMA + TMEM alloc
+    static constexpr int THREADS = 288;
+    static constexpr int MMA_WARP = 8;
+    static constexpr int STAGE_FLOATS = 8 * 32 * 33;
 };
 
 struct ResShared {
     uint64_t mma_bar;
     uint32_t tmem_slot;
     uint32_t pad0;
-    double part[2][4][4];        // [iteration parity][warp][trS, fro2, trX, -]
+    double part[2][8][4];        // [iteration parity][warp][trS, fro2, trX, -]
+    float rrow[2][128];          // Gershgorin: per chunk-half row sums of the strictly-lower entries
+    float dii[128];              // Gershgorin: diagonal entries
     float rcol[4][256];          // Gershgorin: per-warp column sums of the strictly-lower triangle (this CTA's rows)
     float mm[4][2];              // per-warp min(d - R), max(d + R)
     CtrlCore ctrl;
@@ -95,7 +100,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
     const int cluster_id = blockIdx.x / CG, n_clusters = gridDim.x / CG;
     const int N = p.N;
 
-    if (warp == 4) {
+    if (warp == C::MMA_WARP) {
         if (lane == 0) {
             mbar_init(&sh->mma_bar, 1);
             fence_barrier_init();
@@ -112,10 +117,11 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
     uint32_t mma_phase = 0;
 
     const int q = warp & 3;
+    const int hf = (warp >> 2) & 1;               // which half of the 32-column chunks this warp takes
     const int tl = q * 32 + lane;                  // row inside this CTA's panel (TMEM lane)
     const int gi = (int)rank * 128 + tl;           // global row
     const int row0 = (int)rank * 128 + q * 32;     // first row of this warp
-    float* stg = stage + q * (32 * 33);
+    float* stg = stage + (warp & 7) * (32 * 33);
     const uint32_t t_acc = tmem_base + ((uint32_t)(q * 32) << 16);
     const uint32_t t_S = t_acc + NP;
     const float cs = p.scale, inv2 = p.inv_scale2;
@@ -130,9 +136,10 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
         if (p.auto_bounds) {
             for (int i = threadIdx.x; i < 1024; i += blockDim.x) (&sh->rcol[0][0])[i] = 0.f;
             __syncthreads();
-            float Rrow = 0.f, dii = 0.f;
-            if (warp < 4) {
+            float Rrow = 0.f;
+            if (warp < 8) {
                 for (int c0 = 0; c0 <= row0 + 31 && c0 < NP; c0 += 32) {
+                    if (((c0 >> 5) & 1) != hf) continue;
                     // column partial sums in the load layout (lane = column), row sums after the transpose
                     __syncwarp();
                     float colp = 0.f;
@@ -151,14 +158,16 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
                         const float v = stg[lane * 33 + c];
                         const int j = c0 + c;
                         if (j < gi) Rrow += fabsf(v);
-                        if (j == gi) dii = v;
+                        if (j == gi) sh->dii[tl] = v;
                     }
                 }
+                sh->rrow[hf][tl] = Rrow;
             }
             group_sync<CG>();
             float lo = INFINITY, hi = -INFINITY;
             if (warp < 4) {
-                float R = Rrow;
+                float R = sh->rrow[0][tl] + sh->rrow[1][tl];
+                const float dii = (gi < N) ? sh->dii[tl] : 0.f;
                 for (uint32_t r = 0; r < (uint32_t)CG; ++r)
                     for (int w = 0; w < 4; ++w)
                         R += (r == rank) ? sh->rcol[w][gi] : ld_cluster_f32(mapa_u32(smem_u32(&sh->rcol[w][gi]), r));
@@ -209,9 +218,10 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
         int iter = 0;
         bool first = true;
         while (true) {
-            if (warp < 4) {
+            if (warp < 8) {
                 // ---- finalise the lower-triangle part of this thread's row: chunk by chunk
                 for (int c0 = 0; c0 <= row0 + 31 && c0 < NP; c0 += 32) {
+                    if (((c0 >> 5) & 1) != hf) continue;
                     float sn[32];
                     if (first) {
                         float hv[32];
@@ -242,6 +252,9 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
                     }
                     uint32_t so[32];
                     uint32_t hp[16], lp[16];
+                    // squares of the strictly-lower entries: FP32 over one chunk (4 partial sums), FP64 across chunks;
+                    // FP64 per element only on the diagonal (the FP64 pipe is narrow)
+                    float q0 = 0.f, q1 = 0.f, q2 = 0.f, q3 = 0.f;
 #pragma unroll
                     for (int c = 0; c < 32; ++c) {
                         const int j = c0 + c;
@@ -251,12 +264,15 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
                         const uint32_t hb = __half_as_ushort(h), lb = __half_as_ushort(l);
                         if (c & 1) { hp[c >> 1] |= hb << 16; lp[c >> 1] |= lb << 16; }
                         else { hp[c >> 1] = hb; lp[c >> 1] = lb; }
-                        if (j <= gi) {
+                        const float sq = (j < gi) ? sn[c] * sn[c] : 0.f;
+                        if ((c & 3) == 0) q0 += sq; else if ((c & 3) == 1) q1 += sq;
+                        else if ((c & 3) == 2) q2 += sq; else q3 += sq;
+                        if (j == gi) {
                             const double vd = (double)sn[c];
-                            if (j == gi) { trS += vd; fro2 += vd * vd; }
-                            else fro2 += 2.0 * vd * vd;
+                            trS += vd; fro2 += vd * vd;
                         }
                     }
+                    fro2 += 2.0 * (double)((q0 + q1) + (q2 + q3));
                     tmem_st_32x32(t_S + (uint32_t)c0, so);      // FP32 master (entries j > i are never read)
                     const bool below = (c0 + 31 < row0);        // chunk strictly below the diagonal for the whole warp
                     const uint32_t jr = (uint32_t)(c0 >> 7);    // CTA that owns rows c0..c0+31
@@ -299,9 +315,9 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
                     trX += __shfl_xor_sync(0xffffffffu, trX, o);
                 }
                 if (lane == 0) {
-                    sh->part[iter & 1][q][0] = trS;
-                    sh->part[iter & 1][q][1] = fro2;
-                    sh->part[iter & 1][q][2] = trX;
+                    sh->part[iter & 1][warp][0] = trS;
+                    sh->part[iter & 1][warp][1] = fro2;
+                    sh->part[iter & 1][warp][2] = trX;
                 }
             }
             // panels (generic-proxy writes, local and remote) -> visible to the tensor core (async proxy)
@@ -313,7 +329,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
             if (threadIdx.x == 0) {
                 double a = 0.0, b = 0.0, cX = 0.0;
                 for (uint32_t r = 0; r < (uint32_t)CG; ++r)
-                    for (int w = 0; w < 4; ++w) {
+                    for (int w = 0; w < 8; ++w) {
                         if (r == rank) {
                             a += sh->part[iter & 1][w][0]; b += sh->part[iter & 1][w][1]; cX += sh->part[iter & 1][w][2];
                         } else {
@@ -336,7 +352,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
             th1s = sh->ctrl.theta[0] * inv2; th2 = sh->ctrl.theta[1]; th3 = sh->ctrl.theta[2];
             trS = fro2 = trX = 0.0;
             // ---- a4: X = S^2 (Eq. 15): 3 MMAs per 16 columns of K, operands = the resident panels
-            if (warp == 4 && rank == 0 && lane == 0) {
+            if (warp == C::MMA_WARP && rank == 0 && lane == 0) {
                 constexpr uint32_t idesc = umma_idesc_f16(128 * CG, NP);
 #pragma unroll 1
                 for (int kb = 0; kb < C::KBLK; ++kb) {
@@ -358,8 +374,9 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
         }
 
         // ------------------------------------------------------------------ output: D = S_n, both triangles
-        if (warp < 4) {
+        if (warp < 8) {
             for (int c0 = 0; c0 <= row0 + 31 && c0 < NP; c0 += 32) {
+                if (((c0 >> 5) & 1) != hf) continue;
                 uint32_t vs[32];
                 tmem_ld_32x32(t_S + (uint32_t)c0, vs);
                 tmem_ld_wait();
@@ -390,7 +407,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
 
     tc_fence_before();
     group_sync<CG>();
-    if (warp == 4) tmem_dealloc<CG>(tmem_base, C::TMEM_COLS);
+    if (warp == C::MMA_WARP) tmem_dealloc<CG>(tmem_base, C::TMEM_COLS);
 }
 
 using Res128 = ResCfg<128, 1>;
