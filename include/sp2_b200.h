@@ -111,6 +111,18 @@ sp2_status_t sp2_generalized(sp2_handle_t h, const float* H_dev, int N, int ldh,
                              const sp2_opts_t* opts, float* X_L_dev, int ldx,
                              sp2_layer_stat_t* stats_host, void* stream);
 
+/* The same network with the output mix of Eq. 18: the optimised finite-temperature Fermi-operator
+ * expansion  F~(H) = I - sum_{i=0..L} c_i E_i,  E_0 = (H - eps_min I) / (eps_max - eps_min) -- the rescaled H in
+ * NATURAL order, as Eq. 17's eps_0 (reading C26; Alg. 1's S_0 is the reversed one, S_0 = I - E_0) --
+ * E_n = th_{n,1} E_{n-1}^2 + th_{n,2} E_{n-1} + th_{n,3} I  (Eq. 17).  F~ then decreases with energy like the Fermi
+ * function of Eq. 20.  theta_host = [L][3], c_host = [L+1] (c_0 weights E_0).  The sum is accumulated in FP32 by the layer epilogues
+ * (one more N x N workspace matrix, allocated on the first call).  F_dev: N x N, leading dimension ldf.
+ * tile_config 2 is not available for this call. */
+sp2_status_t sp2_generalized_mix(sp2_handle_t h, const float* H_dev, int N, int ldh, const double* theta_host,
+                                 const double* c_host, int L, double eps_min, double eps_max,
+                                 const sp2_opts_t* opts, float* F_dev, int ldf, sp2_layer_stat_t* stats_host,
+                                 void* stream);
+
 /* Convenience form of the same network with per-layer branch, weight and bias scalars (BASELINE north_star):
  * S_n = w_n (sigma_n X_n + (1 - sigma_n) S_{n-1}) + b_n I, i.e. theta_n = (w sigma, w (1 - sigma), b).
  * sigma == NULL means all +1. */

@@ -21,6 +21,9 @@ can be checked against PAPER.md by eye (P:n = /root/reference/PAPER.md line n):
   split_fp16               Eqs. 12-13 with IEEE round-to-nearest-even conversions (C9).
   mixed_square_exact       Eq. 15 evaluated in FP64 from given hi/lo (products of two
                            FP16 numbers are exact in FP64): the exact target of the tensor-core square.
+  generalized_mix_ref      the optimised finite-temperature expansion of Eqs. 17-18 in matrix form:
+                           E_0 = rescaled H in natural order, E_n = th1 E^2 + th2 E + th3 I, F~ = I - sum c_i E_i.
+  fermi_function           Eq. 20.
   refine_ref               the final refinement f_final of Eq. 16 in FP64: two composed layers with
                            alternating signs; which of the two forms applies follows reading C15 of
                            DESIGN.md (continue the alternation from the last applied sign).
@@ -293,3 +296,28 @@ def iderr_ref(X):
     """IdErr = Tr[X - X^2] (P:188)."""
     X = np.asarray(X, dtype=np.float64)
     return float(np.trace(X) - np.sum(X * X.T))
+
+
+def generalized_mix_ref(H32, theta, c, bounds=None):
+    """Eqs. 17-18 in matrix form.  eps_0 of Eq. 17 is "the eigenvalues eps_i in [0,1] of the re-scaled
+    Hamiltonian" (P:230) in natural order (reading C26): E_0 = (H - eps_min I)/(eps_max - eps_min);
+    E_n = th_{n-1,1} E_{n-1}^2 + th_{n-1,2} E_{n-1} + th_{n-1,3} I (Eq. 17);  F~ = I - sum_{i=0}^{L} c_i E_i (Eq. 18)."""
+    H = symmetrize_lower(H32)
+    n = H.shape[0]
+    e0, e1 = gershgorin_bounds(H) if bounds is None else (float(bounds[0]), float(bounds[1]))
+    theta = np.asarray(theta, dtype=np.float64)
+    c = np.asarray(c, dtype=np.float64)
+    if c.shape != (theta.shape[0] + 1,):
+        raise ValueError("c must have L + 1 entries")
+    I = np.eye(n)
+    E = (H - e0 * I) / (e1 - e0)
+    acc = c[0] * E
+    for k in range(theta.shape[0]):
+        E = theta[k, 0] * (E @ E) + theta[k, 1] * E + theta[k, 2] * I
+        acc = acc + c[k + 1] * E
+    return I - acc
+
+
+def fermi_function(eps, beta):
+    """Eq. 20: F(eps) = (exp(beta (eps - 1/2)) + 1)^-1 on the rescaled energies eps in [0, 1]."""
+    return 1.0 / (np.exp(beta * (np.asarray(eps, dtype=np.float64) - 0.5)) + 1.0)

@@ -18,7 +18,7 @@ STOP_NAMES = {0: "none", 1: "iderr<=0", 2: "param_free", 3: "tol", 4: "max_layer
 TILE_AUTO, TILE_128x128, TILE_128x256, TILE_256x256_PAIR = 0, 1, 2, 3
 
 EXPORTS = ["sp2_default_opts", "sp2_create", "sp2_destroy", "sp2_workspace_bytes", "sp2_density_matrix",
-           "sp2_density_matrix_host", "sp2_generalized", "sp2_generalized_wb", "sp2_density_matrix_batched",
+           "sp2_density_matrix_host", "sp2_generalized", "sp2_generalized_mix", "sp2_generalized_wb", "sp2_density_matrix_batched",
            "sp2_refine_energy", "sp2_split_fp16", "sp2_gershgorin", "sp2_status_string", "sp2_last_cuda_error",
            "sp2_last_launch_count", "sp2_version"]
 
@@ -74,6 +74,9 @@ def load() -> C.CDLL:
     lib.sp2_generalized.argtypes = [vp, vp, C.c_int, C.c_int, dp, C.c_int, C.c_double, C.c_double,
                                     C.POINTER(Opts), vp, C.c_int, C.POINTER(LayerStat), vp]
     lib.sp2_generalized.restype = C.c_int
+    lib.sp2_generalized_mix.argtypes = [vp, vp, C.c_int, C.c_int, dp, dp, C.c_int, C.c_double, C.c_double,
+                                        C.POINTER(Opts), vp, C.c_int, C.POINTER(LayerStat), vp]
+    lib.sp2_generalized_mix.restype = C.c_int
     lib.sp2_generalized_wb.argtypes = [vp, vp, C.c_int, C.c_int, ip, dp, dp, C.c_int, C.c_double, C.c_double,
                                        C.POINTER(Opts), vp, C.c_int, C.POINTER(LayerStat), vp]
     lib.sp2_generalized_wb.restype = C.c_int
@@ -212,6 +215,32 @@ class Handle:
         info = _stats_to_dict(stats, L)
         info.update(status=st, n_layers=L)
         return X, info
+
+    def generalized_mix(self, H, theta: np.ndarray, c: np.ndarray, bounds=None, opts: Optional[Opts] = None,
+                        stream=None):
+        """F~(H) = I - sum_i c_i S_i (Eqs. 17-18): theta [L][3], c [L+1]."""
+        import torch
+
+        H = _dev_f32(H, "H")
+        N = H.shape[0]
+        theta = np.ascontiguousarray(theta, dtype=np.float64)
+        c = np.ascontiguousarray(c, dtype=np.float64)
+        L = theta.shape[0]
+        if c.shape != (L + 1,):
+            raise ValueError("c must have L + 1 entries (c_0 weights S_0)")
+        F = torch.empty((N, N), dtype=torch.float32, device=H.device)
+        stats = (LayerStat * L)()
+        e0, e1 = (0.0, 0.0) if bounds is None else (float(bounds[0]), float(bounds[1]))
+        st = self.lib.sp2_generalized_mix(self._h, H.data_ptr(), N, H.stride(0),
+                                          theta.ctypes.data_as(C.POINTER(C.c_double)),
+                                          c.ctypes.data_as(C.POINTER(C.c_double)), L, e0, e1,
+                                          C.byref(opts) if opts is not None else None, F.data_ptr(), F.stride(0),
+                                          stats, _stream_ptr(stream))
+        if st < 0:
+            raise SP2Error(st, "sp2_generalized_mix")
+        info = _stats_to_dict(stats, L)
+        info.update(status=st, n_layers=L)
+        return F, info
 
     def generalized_wb(self, H, sigma: Optional[Sequence[int]], weights, biases, bounds=None,
                        opts: Optional[Opts] = None, stream=None):

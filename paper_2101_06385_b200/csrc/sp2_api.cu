@@ -68,9 +68,10 @@ struct sp2_handle_s {
     float* stage_D = nullptr;
     size_t stage_elems = 0;
     PFN_encodeTiled encode = nullptr;
-    std::map<std::tuple<int, int, int, int, int>, LoopGraph> graphs;   // (N, Np, cfg, scale_log2, exact_diag)
+    std::map<std::tuple<int, int, int, int, int>, LoopGraph> graphs;   // (N, Np, cfg, scale_log2, exact_diag | mix << 1)
     int items_key_np[2] = {-1, -1}, items_key_cfg[2] = {-1, -1}, items_key_split[2] = {-1, -1};
     int n_items[2] = {0, 0}, n_slots[2] = {0, 0};
+    float* mix = nullptr;           // output mix M = sum_i c_i S_i (Eq. 18), allocated on first use
     double* obs_dev = nullptr;      // [6] observables of sp2_refine_energy
     double* obs_host = nullptr;
     int tail_split = 1;
@@ -120,7 +121,7 @@ extern "C" size_t sp2_workspace_bytes(int N_max, int batch_max, int max_layers) 
     const size_t Np = (size_t)round_up(N_max, 256);
     size_t b = Np * (size_t)ws_ld_f32((int)Np) * 4 + 4 * Np * (size_t)ws_ld_f16((int)Np) * 2;   // S + two hi/lo pairs
     b += 4 * Np * sizeof(double);                             // Gershgorin radii, diagonal, two row-sum vectors
-    b += sizeof(Ctrl) + (size_t)max_layers * (sizeof(sp2_layer_stat_t) + 3 * sizeof(double));
+    b += sizeof(Ctrl) + (size_t)max_layers * (sizeof(sp2_layer_stat_t) + kThetaStride * sizeof(double));
     b += 2 * ((Np / 128) * (Np / 128 + 1) / 2 + 1024) * sizeof(WorkItem);
     if (batch_max > 0)
         b += (size_t)batch_max * ((size_t)max_layers * sizeof(sp2_layer_stat_t) + 2 * sizeof(int) + 3 * sizeof(double));
@@ -139,7 +140,7 @@ extern "C" sp2_status_t sp2_destroy(sp2_handle_t h) {
         for (int b = 0; b < 2; ++b) cudaFree(h->hl[a][b]);
     cudaFree(h->rowsq[0]); cudaFree(h->rowsq[1]);
     cudaFree(h->R); cudaFree(h->diag); cudaFree(h->ctrl); cudaFree(h->stats_dev); cudaFree(h->thetas_dev);
-    cudaFree(h->items_dev[0]); cudaFree(h->items_dev[1]); cudaFree(h->obs_dev); cudaFreeHost(h->obs_host); cudaFree(h->bstats_dev); cudaFree(h->bnl_dev); cudaFree(h->bstatus_dev);
+    cudaFree(h->items_dev[0]); cudaFree(h->items_dev[1]); cudaFree(h->obs_dev); cudaFree(h->mix); cudaFreeHost(h->obs_host); cudaFree(h->bstats_dev); cudaFree(h->bnl_dev); cudaFree(h->bstatus_dev);
     cudaFree(h->bbounds_dev); cudaFree(h->bnocc_dev);
     cudaFreeHost(h->ctrl_host); cudaFreeHost(h->stats_host); cudaFreeHost(h->thetas_host);
     cudaFreeHost(h->bounds_host); cudaFree(h->stage_H); cudaFree(h->stage_D);
@@ -183,7 +184,7 @@ extern "C" sp2_status_t sp2_create(sp2_handle_t* out, int N_max, int batch_max, 
     A((void**)&h->rowsq[1], Np * sizeof(unsigned long long));
     A((void**)&h->ctrl, sizeof(Ctrl));
     A((void**)&h->stats_dev, (size_t)max_layers * sizeof(sp2_layer_stat_t));
-    A((void**)&h->thetas_dev, (size_t)max_layers * 3 * sizeof(double));
+    A((void**)&h->thetas_dev, (size_t)max_layers * kThetaStride * sizeof(double));
     h->items_cap = (int)((Np / 128) * (Np / 128 + 1) / 2) + 1024;
     A((void**)&h->items_dev[0], (size_t)h->items_cap * sizeof(WorkItem));
     A((void**)&h->items_dev[1], (size_t)h->items_cap * sizeof(WorkItem));
@@ -202,7 +203,7 @@ extern "C" sp2_status_t sp2_create(sp2_handle_t* out, int N_max, int batch_max, 
     };
     AH((void**)&h->ctrl_host, sizeof(Ctrl));
     AH((void**)&h->stats_host, (size_t)max_layers * sizeof(sp2_layer_stat_t));
-    AH((void**)&h->thetas_host, (size_t)max_layers * 3 * sizeof(double));
+    AH((void**)&h->thetas_host, (size_t)max_layers * kThetaStride * sizeof(double));
     AH((void**)&h->bounds_host, 2 * sizeof(double));
     AH((void**)&h->obs_host, 8 * sizeof(double));
     if (st == SP2_OK) {
@@ -299,7 +300,7 @@ static int choose_tile_config(int N, int requested, int num_sms) {
 }
 
 struct Problem {
-    int N, Np, cfg, scale_log2, n_items, n_slots, exact_diag, list;
+    int N, Np, cfg, scale_log2, n_items, n_slots, exact_diag, list, mix;
     float scale, inv_scale2;
 };
 
@@ -308,6 +309,7 @@ static sp2_status_t prepare_problem(sp2_handle_s* h, int N, const sp2_opts_t* o,
     pb->N = N;
     pb->cfg = forced_cfg ? forced_cfg : choose_tile_config(N, o ? o->tile_config : 0, h->num_sms);
     pb->list = forced_cfg ? 1 : 0;
+    pb->mix = 0;
     const int L = pb->list;
     const int edge = tile_super_edge(pb->cfg);
     pb->Np = round_up(N, edge);
@@ -342,6 +344,7 @@ static sp2_status_t prepare_problem(sp2_handle_s* h, int N, const sp2_opts_t* o,
 static LayerParams layer_params(sp2_handle_s* h, const Problem& pb, int parity, unsigned long long cond) {
     LayerParams p;
     p.ctrl = h->ctrl; p.stats = h->stats_dev; p.thetas = h->thetas_dev; p.S = h->S;
+    p.mix = pb.mix ? h->mix : nullptr;
     p.hi_out = h->hl[parity ^ 1][0]; p.lo_out = h->hl[parity ^ 1][1];
     p.rowsq_cur = pb.exact_diag ? h->rowsq[parity] : nullptr;
     p.rowsq_next = pb.exact_diag ? h->rowsq[parity ^ 1] : nullptr;
@@ -366,7 +369,7 @@ static sp2_status_t launch_one_layer(sp2_handle_s* h, const Problem& pb, int par
 // WHILE(ctrl->running) { layer(ping -> pong); layer(pong -> ping); } as a CUDA graph with a conditional node; the
 // condition is set on the device by the last CTA of each layer kernel (cudaGraphSetConditional).
 static sp2_status_t get_loop_graph(sp2_handle_s* h, const Problem& pb, LoopGraph** out) {
-    auto key = std::make_tuple(pb.N, pb.Np, pb.cfg, pb.scale_log2, pb.exact_diag);
+    auto key = std::make_tuple(pb.N, pb.Np, pb.cfg, pb.scale_log2, pb.exact_diag | (pb.mix << 1));
     auto it = h->graphs.find(key);
     if (it != h->graphs.end()) { *out = &it->second; return SP2_OK; }
     LoopGraph lg;
@@ -405,10 +408,16 @@ static sp2_status_t check_common(sp2_handle_s* h, const void* in, int N, int ldi
 // h->thetas_host[0..3L)).
 static sp2_status_t solve_single(sp2_handle_s* h, const float* H_dev, int N, int ldh, double N_occ, int mode,
                                  const sp2_opts_t* o, float* D_dev, int ldd, sp2_layer_stat_t* stats_out,
-                                 int* n_layers_out, double bounds_out[2], cudaStream_t st) {
+                                 int* n_layers_out, double bounds_out[2], cudaStream_t st, bool mix = false,
+                                 double c0 = 0.0, double mix_diag = 1.0) {
     Problem pb;
     sp2_status_t s = prepare_problem(h, N, o, &pb, st);
     if (s != SP2_OK) return s;
+    if (mix) {
+        if (pb.cfg == TILE_128x256) return SP2_ERR_INVALID_ARG;      // the mix epilogue exists for configs 1 and 3
+        if (!h->mix) CK(cudaMalloc((void**)&h->mix, (size_t)h->Np_max * (size_t)ws_ld_f32(h->Np_max) * 4));
+        pb.mix = 1;
+    }
     const int max_layers = o->max_layers;
     // ---- control block
     Ctrl* c = h->ctrl_host;
@@ -419,13 +428,14 @@ static sp2_status_t solve_single(sp2_handle_s* h, const float* H_dev, int N, int
     c->noise_kappa = h->noise_kappa;
     CK(cudaMemcpyAsync(h->ctrl, c, ctrl_header_bytes(), cudaMemcpyHostToDevice, st));
     if (mode == MODE_GENERALIZED)
-        CK(cudaMemcpyAsync(h->thetas_dev, h->thetas_host, (size_t)max_layers * 3 * sizeof(double),
+        CK(cudaMemcpyAsync(h->thetas_dev, h->thetas_host, (size_t)max_layers * kThetaStride * sizeof(double),
                            cudaMemcpyHostToDevice, st));
     CK(cudaMemsetAsync(h->stats_dev, 0, (size_t)max_layers * sizeof(sp2_layer_stat_t), st));
     // ---- padding rows/columns of S_0 are zero (inert: eigenvalue 0 is a fixed point of both branches)
     const size_t ldS = (size_t)ws_ld_f32(pb.Np), ldF = (size_t)ws_ld_f16(pb.Np);
     if (pb.Np != N) {
         CK(cudaMemsetAsync(h->S, 0, (size_t)pb.Np * ldS * 4, st));
+        if (pb.mix) CK(cudaMemsetAsync(h->mix, 0, (size_t)pb.Np * ldS * 4, st));
         CK(cudaMemsetAsync(h->hl[0][0], 0, (size_t)pb.Np * ldF * 2, st));
         CK(cudaMemsetAsync(h->hl[0][1], 0, (size_t)pb.Np * ldF * 2, st));
     }
@@ -436,7 +446,8 @@ static sp2_status_t solve_single(sp2_handle_s* h, const float* H_dev, int N, int
         CK(cudaMemsetAsync(h->rowsq[1], 0, (size_t)pb.Np * sizeof(unsigned long long), st));
     }
     CK(launch_affine_split(H_dev, N, ldh, h->S, h->hl[0][0], h->hl[0][1], (long long)ldS, (long long)ldF, pb.scale, h->ctrl, h->stats_dev,
-                           h->thetas_dev, pb.exact_diag ? h->rowsq[0] : nullptr, h->num_sms, st));
+                           h->thetas_dev, pb.exact_diag ? h->rowsq[0] : nullptr, pb.mix ? h->mix : nullptr, (float)c0,
+                           h->num_sms, st));
     // ---- a4-a8: the layer loop
     if (o->control == 0) {
         LoopGraph* lg = nullptr;
@@ -458,8 +469,11 @@ static sp2_status_t solve_single(sp2_handle_s* h, const float* H_dev, int N, int
         }
     }
     // ---- results
-    CK(cudaMemcpy2DAsync(D_dev, (size_t)ldd * 4, h->S, ldS * 4, (size_t)N * 4, (size_t)N,
-                         cudaMemcpyDeviceToDevice, st));
+    if (pb.mix)      // F = d I - M  (Eq. 18 in the library's variables, see generalized_impl)
+        CK(launch_one_minus(h->mix, (long long)ldS, D_dev, ldd, N, (float)mix_diag, h->num_sms, st));
+    else
+        CK(cudaMemcpy2DAsync(D_dev, (size_t)ldd * 4, h->S, ldS * 4, (size_t)N * 4, (size_t)N,
+                             cudaMemcpyDeviceToDevice, st));
     CK(cudaMemcpyAsync(h->ctrl_host, h->ctrl, ctrl_header_bytes(), cudaMemcpyDeviceToHost, st));
     CK(cudaMemcpyAsync(h->stats_host, h->stats_dev, (size_t)max_layers * sizeof(sp2_layer_stat_t),
                        cudaMemcpyDeviceToHost, st));
@@ -535,13 +549,14 @@ extern "C" sp2_status_t sp2_refine_energy(sp2_handle_t h, const float* S_dev, in
     // Reading C15: continue the alternation from the last applied sign.
     //   last sigma = -1: X = S^2, then 2X - X^2  ->  2 S^2 - S^4 ;   last sigma = +1: T = 2S - S^2, then T^2.
     double* th = h->thetas_host;
-    if (last_sigma < 0) { th[0] = 1; th[1] = 0; th[2] = 0; th[3] = -1; th[4] = 2; th[5] = 0; }
-    else                { th[0] = -1; th[1] = 2; th[2] = 0; th[3] = 1; th[4] = 0; th[5] = 0; }
+    memset(th, 0, 2 * kThetaStride * sizeof(double));
+    if (last_sigma < 0) { th[0] = 1; th[kThetaStride] = -1; th[kThetaStride + 1] = 2; }
+    else                { th[0] = -1; th[1] = 2; th[kThetaStride] = 1; }
     Ctrl* c = h->ctrl_host;
     memset(c, 0, ctrl_header_bytes());
     c->N = N; c->mode = MODE_GENERALIZED; c->max_layers = 2;
     CK(cudaMemcpyAsync(h->ctrl, c, ctrl_header_bytes(), cudaMemcpyHostToDevice, st));
-    CK(cudaMemcpyAsync(h->thetas_dev, th, 6 * sizeof(double), cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(h->thetas_dev, th, 2 * kThetaStride * sizeof(double), cudaMemcpyHostToDevice, st));
     CK(cudaMemsetAsync(h->stats_dev, 0, 2 * sizeof(sp2_layer_stat_t), st));
     const size_t ldS = (size_t)ws_ld_f32(pb.Np), ldF = (size_t)ws_ld_f16(pb.Np);
     if (pb.Np != N) CK(cudaMemsetAsync(h->S, 0, (size_t)pb.Np * ldS * 4, st));
@@ -572,10 +587,12 @@ extern "C" sp2_status_t sp2_refine_energy(sp2_handle_t h, const float* S_dev, in
     return SP2_OK;
 }
 
-extern "C" sp2_status_t sp2_generalized(sp2_handle_t h, const float* H_dev, int N, int ldh, const double* theta_host,
-                                        int L, double eps_min, double eps_max, const sp2_opts_t* opts, float* X_L_dev,
-                                        int ldx, sp2_layer_stat_t* stats_host, void* stream) {
-    sp2_status_t s = check_common(h, H_dev, N, ldh, X_L_dev, ldx);
+// Shared body of sp2_generalized / sp2_generalized_mix: c_host == nullptr -> output X_L = S_L, else F = I - sum c_i S_i.
+static sp2_status_t generalized_impl(sp2_handle_t h, const float* H_dev, int N, int ldh, const double* theta_host,
+                                     const double* c_host, int L, double eps_min, double eps_max,
+                                     const sp2_opts_t* opts, float* out_dev, int ldo, sp2_layer_stat_t* stats_host,
+                                     void* stream) {
+    sp2_status_t s = check_common(h, H_dev, N, ldh, out_dev, ldo);
     if (s != SP2_OK) return s;
     if (!theta_host || L < 1 || L > h->max_layers) return SP2_ERR_INVALID_ARG;
     sp2_opts_t o;
@@ -586,13 +603,49 @@ extern "C" sp2_status_t sp2_generalized(sp2_handle_t h, const float* H_dev, int 
     o.auto_bounds = !(eps_max > eps_min);
     o.eps_min = eps_min; o.eps_max = eps_max;
     if (!o.auto_bounds && (!isfinite(eps_min) || !isfinite(eps_max))) return SP2_ERR_INVALID_ARG;
-    for (int i = 0; i < 3 * L; ++i) {
-        if (!isfinite(theta_host[i])) return SP2_ERR_INVALID_ARG;
-        h->thetas_host[i] = theta_host[i];
+    for (int n = 0; n < L; ++n) {
+        for (int k = 0; k < 3; ++k) {
+            if (!isfinite(theta_host[3 * n + k])) return SP2_ERR_INVALID_ARG;
+            h->thetas_host[kThetaStride * n + k] = theta_host[3 * n + k];
+        }
+        const double cn = c_host ? c_host[n + 1] : 0.0;      // weight of the output of layer n+1
+        if (!isfinite(cn)) return SP2_ERR_INVALID_ARG;
+        h->thetas_host[kThetaStride * n + 3] = cn;
+    }
+    double c0 = 0.0, diag_const = 1.0;
+    if (c_host) {
+        if (!isfinite(c_host[0])) return SP2_ERR_INVALID_ARG;
+        // Eq. 17 starts from eps_0 = the rescaled H in NATURAL order (reading C26), the library's S_0 is the
+        // reversed one (Alg. 1): eps_0 = I - S_0.  Substituting into layer 1 and into the sum (exact algebra):
+        //   eps_1 = th1 S_0^2 - (2 th1 + th2) S_0 + (th1 + th2 + th3) I
+        //   F~ = I - sum c_i eps_i = (1 - c_0) I - [ (-c_0) S_0 + sum_{i>=1} c_i eps_i ]
+        const double t1 = theta_host[0], t2 = theta_host[1], t3 = theta_host[2];
+        h->thetas_host[0] = t1;
+        h->thetas_host[1] = -(2.0 * t1 + t2);
+        h->thetas_host[2] = t1 + t2 + t3;
+        c0 = -c_host[0];
+        diag_const = 1.0 - c_host[0];
     }
     int nl = 0;
-    return solve_single(h, H_dev, N, ldh, 0.0, MODE_GENERALIZED, &o, X_L_dev, ldx, stats_host, &nl, nullptr,
-                        (cudaStream_t)stream);
+    return solve_single(h, H_dev, N, ldh, 0.0, MODE_GENERALIZED, &o, out_dev, ldo, stats_host, &nl, nullptr,
+                        (cudaStream_t)stream, c_host != nullptr, c0, diag_const);
+}
+
+extern "C" sp2_status_t sp2_generalized(sp2_handle_t h, const float* H_dev, int N, int ldh, const double* theta_host,
+                                        int L, double eps_min, double eps_max, const sp2_opts_t* opts, float* X_L_dev,
+                                        int ldx, sp2_layer_stat_t* stats_host, void* stream) {
+    return generalized_impl(h, H_dev, N, ldh, theta_host, nullptr, L, eps_min, eps_max, opts, X_L_dev, ldx, stats_host,
+                            stream);
+}
+
+// NEXT-2: the optimised finite-temperature expansion F~(H) = I - sum_{i=0..L} c_i S_i (Eqs. 17-18).
+extern "C" sp2_status_t sp2_generalized_mix(sp2_handle_t h, const float* H_dev, int N, int ldh,
+                                            const double* theta_host, const double* c_host, int L, double eps_min,
+                                            double eps_max, const sp2_opts_t* opts, float* F_dev, int ldf,
+                                            sp2_layer_stat_t* stats_host, void* stream) {
+    if (!c_host) return SP2_ERR_INVALID_ARG;
+    return generalized_impl(h, H_dev, N, ldh, theta_host, c_host, L, eps_min, eps_max, opts, F_dev, ldf, stats_host,
+                            stream);
 }
 
 extern "C" sp2_status_t sp2_generalized_wb(sp2_handle_t h, const float* H_dev, int N, int ldh, const int* sigma,

@@ -12,6 +12,10 @@ constexpr int kMaxPartials = 1024;   // per-CTA FP64 partial slots (>= largest g
 
 enum { MODE_STANDARD = 0, MODE_GENERALIZED = 1 };
 
+// Device layout of the per-layer scalars of the generalized network: {th1, th2, th3, c} per layer, c = weight of the
+// layer's output S_n in the output mix sum_i c_i S_i (Eq. 18; 0 when no mix is formed).
+constexpr int kThetaStride = 4;
+
 struct CtrlCore {
     // ---- problem constants (written by the host before launch)
     double N_occ, eps_alt, tol;
@@ -30,7 +34,7 @@ struct CtrlCore {
     double iderr_prev, iderr_prev2;  // IdErr_n, IdErr_{n-1}
     double nx_inflight;              // N_X of the layer in flight (exact, FP64 pre-trace)
     double noise_kappa;              // reading C25: stop when IdErr_n <= kappa |Tr X_n(tc) - N_X|; 0 disables
-    float  theta[4];                 // th1, th2, th3 of the NEXT layer (FP32: the epilogue's arithmetic type)
+    float  theta[4];                 // th1, th2, th3, c of the NEXT layer (FP32: the epilogue's arithmetic type)
     unsigned int done_counter;       // CTAs finished in the current kernel
     unsigned int round_counter;      // CTAs that reached a round boundary of the current layer kernel (round sync)
 };
@@ -45,9 +49,10 @@ __device__ inline void control_plan_next(CtrlCore* c, sp2_layer_stat_t* stats, c
     const int m = c->n + 1;                      // layer about to run
     if (c->mode == MODE_GENERALIZED) {
         if (c->n >= c->max_layers) { c->running = 0; c->stop_reason = SP2_STOP_MAX_LAYERS; return; }
-        c->theta[0] = (float)thetas[3 * c->n + 0];
-        c->theta[1] = (float)thetas[3 * c->n + 1];
-        c->theta[2] = (float)thetas[3 * c->n + 2];
+        c->theta[0] = (float)thetas[kThetaStride * c->n + 0];
+        c->theta[1] = (float)thetas[kThetaStride * c->n + 1];
+        c->theta[2] = (float)thetas[kThetaStride * c->n + 2];
+        c->theta[3] = (float)thetas[kThetaStride * c->n + 3];
         if (stats) {
             stats[m - 1].trace_X = c->fro2;
             stats[m - 1].iderr = c->N_S - c->fro2;
@@ -71,6 +76,7 @@ __device__ inline void control_plan_next(CtrlCore* c, sp2_layer_stat_t* stats, c
     c->theta[0] = (float)sigma;            // W_m = sigma I
     c->theta[1] = (float)(1 - sigma);      // B_m = (I - W_m) S_{m-1}
     c->theta[2] = 0.0f;
+    c->theta[3] = 0.0f;
     int pend = SP2_STOP_NONE;
     if (iderr <= 0.0) pend = SP2_STOP_IDERR_NONPOS;
     else if (m > 2 && c->sigma_prev != c->sigma_prev2 && iderr > 4.5 * c->iderr_prev2 * c->iderr_prev2)

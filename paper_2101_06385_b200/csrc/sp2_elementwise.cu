@@ -128,7 +128,7 @@ __global__ void __launch_bounds__(1024) k_gershgorin_finalize(const double* __re
 // the diagonal entries), FP64 / fixed point across tiles.
 __device__ __forceinline__ void store_s4(float* __restrict__ S, __half* __restrict__ hi, __half* __restrict__ lo,
                                          long long ld, long long ldf, int i, int j, const float (&s)[4], float scale,
-                                         bool all4, const bool (&ok)[4]) {
+                                         bool all4, const bool (&ok)[4], float* __restrict__ mix, float c0) {
     __half h[4], l[4];
 #pragma unroll
     for (int e = 0; e < 4; ++e) split_hi_lo(s[e], scale, h[e], l[e]);
@@ -136,10 +136,13 @@ __device__ __forceinline__ void store_s4(float* __restrict__ S, __half* __restri
         *reinterpret_cast<float4*>(S + (long long)i * ld + j) = make_float4(s[0], s[1], s[2], s[3]);
         *reinterpret_cast<uint2*>(hi + (long long)i * ldf + j) = *reinterpret_cast<uint2*>(h);
         *reinterpret_cast<uint2*>(lo + (long long)i * ldf + j) = *reinterpret_cast<uint2*>(l);
+        if (mix)
+            *reinterpret_cast<float4*>(mix + (long long)i * ld + j) = make_float4(c0 * s[0], c0 * s[1], c0 * s[2], c0 * s[3]);
     } else {
 #pragma unroll
         for (int e = 0; e < 4; ++e)
             if (ok[e]) {
+                if (mix) mix[(long long)i * ld + j + e] = c0 * s[e];
                 S[(long long)i * ld + j + e] = s[e];
                 hi[(long long)i * ldf + j + e] = h[e];
                 lo[(long long)i * ldf + j + e] = l[e];
@@ -151,7 +154,8 @@ __global__ void __launch_bounds__(256, 4) k_affine_split(const float* __restrict
                                                          float* __restrict__ S, __half* __restrict__ hi,
                                                          __half* __restrict__ lo, long long ld, long long ldf,
                                                          float scale, Ctrl* ctrl, sp2_layer_stat_t* stats,
-                                                         const double* thetas, unsigned long long* __restrict__ rowsq) {
+                                                         const double* thetas, unsigned long long* __restrict__ rowsq,
+                                                         float* __restrict__ mix, float c0) {
     __shared__ float ts[ET][ET + 1];
     __shared__ float colacc[16][ET];
     __shared__ double red[8][2];
@@ -205,7 +209,7 @@ __global__ void __launch_bounds__(256, 4) k_affine_split(const float* __restrict
                 ts[lr][c4 + e] = sx;
             }
             const bool all4 = !dtile && (i < N);    // off-diagonal tile: j + 3 < J*64 + 64 <= i
-            store_s4(S, hi, lo, ld, ldf, i, j, sv, scale, all4, ok);
+            store_s4(S, hi, lo, ld, ldf, i, j, sv, scale, all4, ok, mix, c0);
             if (rowsq) {
                 rsq = row16_sum(rsq);
                 if ((threadIdx.x & 15) == 0 && i < N) atomicAdd(rowsq + i, rowsq_fix((double)rsq));
@@ -233,7 +237,7 @@ __global__ void __launch_bounds__(256, 4) k_affine_split(const float* __restrict
                 ok[e] = (ii + e < N) && (jj < ii + e);
             }
             const bool all4 = !dtile && (ii + 3 < N);
-            if (jj < N) store_s4(S, hi, lo, ld, ldf, jj, ii, sv, scale, all4, ok);
+            if (jj < N) store_s4(S, hi, lo, ld, ldf, jj, ii, sv, scale, all4, ok, mix, c0);
         }
         __syncthreads();
     }
@@ -398,6 +402,19 @@ __global__ void __launch_bounds__(256) k_energy_traces(const float* __restrict__
     }
 }
 
+// ------------------------------------------------------------------------------------------------ NEXT-2
+// F = d I - M  (Eq. 18: the Fermi-operator approximation is 1 - sum_i c_i eps_i; d = 1 - c_0 after the
+// change of variable of generalized_impl), N x N, M with leading dimension ldm, F with ldo.
+__global__ void __launch_bounds__(256) k_one_minus(const float* __restrict__ M, long long ldm, float* __restrict__ F,
+                                                   long long ldo, int N, float d) {
+    const long long total = (long long)N * N;
+    for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total;
+         idx += (long long)gridDim.x * blockDim.x) {
+        const int i = (int)(idx / N), j = (int)(idx % N);
+        F[(long long)i * ldo + j] = (i == j ? d : 0.0f) - M[(long long)i * ldm + j];
+    }
+}
+
 // ------------------------------------------------------------------------------------------------ launchers
 cudaError_t launch_gershgorin(const float* H, int N, long long ldh, double* R, double* diag, Ctrl* ctrl,
                               double* bounds_out, int num_sms, cudaStream_t st) {
@@ -413,13 +430,13 @@ cudaError_t launch_gershgorin(const float* H, int N, long long ldh, double* R, d
 
 cudaError_t launch_affine_split(const float* H, int N, long long ldh, float* S, __half* hi, __half* lo, long long ld,
                                 long long ldf, float scale, Ctrl* ctrl, sp2_layer_stat_t* stats, const double* thetas,
-                                unsigned long long* rowsq, int num_sms, cudaStream_t st) {
+                                unsigned long long* rowsq, float* mix, float c0, int num_sms, cudaStream_t st) {
     const int nt = (N + ET - 1) / ET;
     const long long ntiles = (long long)nt * (nt + 1) / 2;
     long long cap = (long long)num_sms * 4;
     if (cap > kMaxPartials) cap = kMaxPartials;
     const int grid = (int)(ntiles < cap ? ntiles : cap);
-    k_affine_split<<<grid, 256, 0, st>>>(H, N, ldh, S, hi, lo, ld, ldf, scale, ctrl, stats, thetas, rowsq);
+    k_affine_split<<<grid, 256, 0, st>>>(H, N, ldh, S, hi, lo, ld, ldf, scale, ctrl, stats, thetas, rowsq, mix, c0);
     return cudaGetLastError();
 }
 
@@ -440,6 +457,13 @@ cudaError_t launch_split(const float* X, int N, long long ldx, __half* hi, __hal
 }  // namespace sp2
 
 namespace sp2 {
+cudaError_t launch_one_minus(const float* M, long long ldm, float* F, long long ldo, int N, float d, int num_sms,
+                             cudaStream_t st) {
+    long long blocks = ((long long)N * N + 255) / 256;
+    if (blocks > (long long)num_sms * 32) blocks = (long long)num_sms * 32;
+    k_one_minus<<<(int)blocks, 256, 0, st>>>(M, ldm, F, ldo, N, d);
+    return cudaGetLastError();
+}
 cudaError_t launch_energy_traces(const float* X, long long ldx, const float* H, long long ldh, int N, Ctrl* ctrl,
                                  double* out, int plan, sp2_layer_stat_t* stats, const double* thetas,
                                  unsigned long long* rowsq, int num_sms, cudaStream_t st) {

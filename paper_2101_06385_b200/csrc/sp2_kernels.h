@@ -14,7 +14,9 @@ cudaError_t launch_gershgorin(const float* H, int N, long long ldh, double* R, d
                               double* bounds_out, int num_sms, cudaStream_t st);
 cudaError_t launch_affine_split(const float* H, int N, long long ldh, float* S, __half* hi, __half* lo, long long ld,
                                 long long ldf, float scale, Ctrl* ctrl, sp2_layer_stat_t* stats, const double* thetas,
-                                unsigned long long* rowsq, int num_sms, cudaStream_t st);
+                                unsigned long long* rowsq, float* mix, float c0, int num_sms, cudaStream_t st);
+cudaError_t launch_one_minus(const float* M, long long ldm, float* F, long long ldo, int N, float d, int num_sms,
+                             cudaStream_t st);
 
 // Row sums of squares r_i = sum_j S_ij^2 (= diag(S^2)_i for symmetric S) are kept in 2^44 fixed point so that the
 // atomic accumulation is order-independent (bit-reproducible results).
@@ -54,6 +56,7 @@ struct LayerParams {
     sp2_layer_stat_t* stats;
     const double* thetas;          // generalized mode: [L][3] on the device
     float* S;                      // FP32 master, Np x Np, updated in place
+    float* mix;                    // output mix M = sum_i c_i S_i (Eq. 18), same layout as S; nullptr = none
     __half* hi_out;                // next layer's operands (the other ping-pong pair)
     __half* lo_out;
     unsigned long long* rowsq_cur; // r_i of S_{n-1} (read at the diagonal, then zeroed); nullptr = tensor-core diagonal

@@ -17,8 +17,10 @@
 
 namespace sp2 {
 
-template <int BN_, int CG_, bool ENH_ = false>
+template <int BN_, int CG_, bool ENH_ = false, bool MIX_ = false>
 struct TileCfg {
+    // MIX: the epilogue also accumulates the output mix M += c_n S_n (Eq. 18) in one more FP32 matrix.
+    static constexpr bool MIX = MIX_;
     // ENH: enhanced accumulation ("single precision with double accumulation") for the refinement layers:
     // the tensor core accumulates only p.enh_kc K-blocks at a time; the chunk sums are added into a running FP32 pair
     // (two-sum) kept in two more TMEM regions, so the truncating FP32 accumulation never runs over the whole K.
@@ -210,6 +212,8 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
         const float th1s = th1 * p.inv_scale2;
         const float th2 = ((volatile float*)ctrl->theta)[1];
         const float th3 = ((volatile float*)ctrl->theta)[2];
+        const float cN = ((volatile float*)ctrl->theta)[3];   // weight of S_n in the output mix (MIX only)
+        float* __restrict__ M = p.mix;
         const float cs = p.scale;
         const float inv2 = p.inv_scale2;
         const long long ld = p.ld, ldf = p.ldf;
@@ -310,6 +314,11 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                 // S_{n-1}: read at the mirrored position (S is exactly symmetric) -> coalesced across the warp
 #pragma unroll
                 for (int c = 0; c < 32; ++c) so[c] = __ldcs(S + (long long)(gj0 + c) * ld + gi);
+                float mo[C::MIX ? 32 : 1];
+                if (C::MIX) {
+#pragma unroll
+                    for (int c = 0; c < 32; ++c) mo[C::MIX ? c : 0] = __ldcs(M + (long long)(gj0 + c) * ld + gi);
+                }
                 if (below) {
                     tmem_ld_wait();
                     float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
@@ -336,6 +345,11 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                             else if ((e & 3) == 2) a2 += sq; else a3 += sq;
                             // mirrored position: one 128-byte (FP32) / 64-byte (FP16) warp store per column
                             __stcs(S + (long long)(gj0 + c) * ld + gi, val);
+                            if (C::MIX) {
+                                const float mv = fmaf(cN, val, mo[C::MIX ? c : 0]);
+                                mo[C::MIX ? c : 0] = mv;
+                                __stcs(M + (long long)(gj0 + c) * ld + gi, mv);
+                            }
                             const long long o = (long long)(gj0 + c) * ldf + gi;
                             __stcs(HOu + o, (unsigned short)hb);
                             __stcs(LOu + o, (unsigned short)lb);
@@ -343,6 +357,14 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                         // own position: 32 contiguous bytes (FP32) / 16 (FP16) per thread per group
                         __stcs(reinterpret_cast<float4*>(rowS) + 2 * g, make_float4(sn[0], sn[1], sn[2], sn[3]));
                         __stcs(reinterpret_cast<float4*>(rowS) + 2 * g + 1, make_float4(sn[4], sn[5], sn[6], sn[7]));
+                        if (C::MIX) {
+                            float4* rowM = reinterpret_cast<float4*>(M + (long long)gi * ld + gj0);
+                            const int b8 = C::MIX ? 8 * g : 0;
+                            __stcs(rowM + 2 * g, make_float4(mo[b8], mo[b8 + (C::MIX ? 1 : 0)], mo[b8 + (C::MIX ? 2 : 0)],
+                                                             mo[b8 + (C::MIX ? 3 : 0)]));
+                            __stcs(rowM + 2 * g + 1, make_float4(mo[b8 + (C::MIX ? 4 : 0)], mo[b8 + (C::MIX ? 5 : 0)],
+                                                                 mo[b8 + (C::MIX ? 6 : 0)], mo[b8 + (C::MIX ? 7 : 0)]));
+                        }
                         __stcs(reinterpret_cast<uint4*>(rowH) + g, make_uint4(hp[0], hp[1], hp[2], hp[3]));
                         __stcs(reinterpret_cast<uint4*>(rowL) + g, make_uint4(lp[0], lp[1], lp[2], lp[3]));
                     }
@@ -380,6 +402,11 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                             const long long o = (long long)gj * ldf + gi, o2 = (long long)gi * ldf + gj;
                             S[(long long)gj * ld + gi] = val; HOu[o] = hb; LOu[o] = lb;
                             S[(long long)gi * ld + gj] = val; HOu[o2] = hb; LOu[o2] = lb;
+                            if (C::MIX) {
+                                const float mv = fmaf(cN, val, mo[C::MIX ? c : 0]);
+                                M[(long long)gj * ld + gi] = mv;
+                                M[(long long)gi * ld + gj] = mv;
+                            }
                         }
                     }
                     rowacc += sq_own;
@@ -444,6 +471,8 @@ using Cfg128 = TileCfg<128, 1>;
 using Cfg256 = TileCfg<256, 1>;
 using Cfg256P = TileCfg<256, 2>;
 using Cfg128E = TileCfg<128, 1, true>;
+using Cfg128M = TileCfg<128, 1, false, true>;
+using Cfg256PM = TileCfg<256, 2, false, true>;
 
 int tile_super_edge(int cfg) { return (cfg == TILE_128x128 || cfg == TILE_128x128_ENH) ? 128 : 256; }
 int tile_subs(int cfg) { return cfg == TILE_128x256 ? Cfg256::SUB : 1; }
@@ -471,9 +500,17 @@ cudaError_t layer_kernel_setup(int cfg) {
         case TILE_256x256_PAIR:
             return cudaFuncSetAttribute(k_sp2_layer<Cfg256P>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                         Cfg256P::SMEM_BYTES);
-        case TILE_128x128_ENH:
-            return cudaFuncSetAttribute(k_sp2_layer<Cfg128E>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                        Cfg128E::SMEM_BYTES);
+        case TILE_128x128_ENH: {
+            cudaError_t e = cudaFuncSetAttribute(k_sp2_layer<Cfg128E>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                 Cfg128E::SMEM_BYTES);
+            if (e != cudaSuccess) return e;
+            // the output-mix instantiations (generalized network with Eq. 18's sum) ride along
+            e = cudaFuncSetAttribute(k_sp2_layer<Cfg128M>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     Cfg128M::SMEM_BYTES);
+            if (e != cudaSuccess) return e;
+            return cudaFuncSetAttribute(k_sp2_layer<Cfg256PM>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                        Cfg256PM::SMEM_BYTES);
+        }
     }
     return cudaErrorInvalidValue;
 }
@@ -500,6 +537,11 @@ static cudaError_t launch_cfg(const CUtensorMap& tm_hi, const CUtensorMap& tm_lo
 
 cudaError_t launch_layer(int cfg, const CUtensorMap& tm_hi, const CUtensorMap& tm_lo, const LayerParams& p,
                          int num_sms, cudaStream_t st) {
+    if (p.mix != nullptr) {              // output mix: 128x128 or pair tiles only
+        if (cfg == TILE_128x128) return launch_cfg<Cfg128M>(tm_hi, tm_lo, p, num_sms, st);
+        if (cfg == TILE_256x256_PAIR) return launch_cfg<Cfg256PM>(tm_hi, tm_lo, p, num_sms, st);
+        return cudaErrorInvalidValue;
+    }
     switch (cfg) {
         case TILE_128x128: return launch_cfg<Cfg128>(tm_hi, tm_lo, p, num_sms, st);
         case TILE_128x256: return launch_cfg<Cfg256>(tm_hi, tm_lo, p, num_sms, st);
