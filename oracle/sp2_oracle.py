@@ -21,6 +21,11 @@ can be checked against PAPER.md by eye (P:n = /root/reference/PAPER.md line n):
   split_fp16               Eqs. 12-13 with IEEE round-to-nearest-even conversions (C9).
   mixed_square_exact       Eq. 15 evaluated in FP64 from given hi/lo (products of two
                            FP16 numbers are exact in FP64): the exact target of the tensor-core square.
+  sp2_accelerated_ref      the accelerated Deep-NN SP2 of section V.A: real-valued sigma_n chosen for the
+                           steepest projection at the HOMO / LUMO eigenvalues "without risking switching places", spectrum
+                           kept in [0, 1].  The paper's explicit W_n, B_n are in its supplementary material, which is not
+                           available: the formulas here are RE-DERIVED from that description (reading C27) and
+                           are "parity unpinned" against the paper's own; they are pinned by mathematics instead.
   generalized_mix_ref      the optimised finite-temperature expansion of Eqs. 17-18 in matrix form:
                            E_0 = rescaled H in natural order, E_n = th1 E^2 + th2 E + th3 I, F~ = I - sum c_i E_i.
   fermi_function           Eq. 20.
@@ -321,3 +326,78 @@ def generalized_mix_ref(H32, theta, c, bounds=None):
 def fermi_function(eps, beta):
     """Eq. 20: F(eps) = (exp(beta (eps - 1/2)) + 1)^-1 on the rescaled energies eps in [0, 1]."""
     return 1.0 / (np.exp(beta * (np.asarray(eps, dtype=np.float64) - 0.5)) + 1.0)
+
+
+def accelerated_layer(N_S, N_X, n_dim, N_occ, h, l, sigma_prev=0, eps_alt=0.0):
+    """One layer's weights of the accelerated scheme (section V.A; reading C27).
+
+    State: all eigenvalues of S in [0, 1]; unoccupied ones in [0, l], occupied ones in [h, 1], 0 <= l < h <= 1
+    (l, h = rescaled LUMO / HOMO estimates, "prior knowledge of the re-scaled HOMO and LUMO eigenvalues").
+    Two generalized projections, each the SP2 polynomial composed with an affine map (the "shift and re-scale"):
+      A(x) = (a x + 1 - a)^2,  a = 2 / (2 - l):  A(1) = 1, and A(0) = A(l): the largest a for which no unoccupied
+             eigenvalue is mapped above A(0) -- steepest at the HOMO side without switching places, range in [0, 1];
+      B(x) = 2 a x - (a x)^2,  a = 2 / (1 + h):  B(0) = 0, and B(h) = B(1).
+    a = 1 (l = 0 or h = 1) gives back x^2 and 2x - x^2.  The branch is chosen as in Alg. 1: the one whose
+    occupation Tr[.] is closer to N_occ, both traces following from N_S = Tr S, N_X = Tr S^2 and N.
+    Returns (sigma, theta (th1, th2, th3), h', l')."""
+    aA = 2.0 / (2.0 - l)
+    aB = 2.0 / (1.0 + h)
+    trA = aA * aA * N_X + 2.0 * aA * (1.0 - aA) * N_S + (1.0 - aA) ** 2 * n_dim
+    trB = 2.0 * aB * N_S - aB * aB * N_X
+    d = abs(trB - N_occ) - abs(trA - N_occ) - sigma_prev * eps_alt
+    if d > 0.0:
+        sigma = 1
+    elif d < 0.0:
+        sigma = -1
+    else:
+        sigma = -sigma_prev if sigma_prev != 0 else 1
+    if sigma > 0:
+        theta = (aA * aA, 2.0 * aA * (1.0 - aA), (1.0 - aA) ** 2)
+        h2 = (aA * h + 1.0 - aA) ** 2
+        l2 = max((1.0 - aA) ** 2, (aA * l + 1.0 - aA) ** 2)
+    else:
+        theta = (-aB * aB, 2.0 * aB, 0.0)
+        h2 = min(2.0 * aB * h - (aB * h) ** 2, 2.0 * aB - aB * aB)
+        l2 = 2.0 * aB * l - (aB * l) ** 2
+    return sigma, theta, h2, l2, d
+
+
+def sp2_accelerated_ref(H32, N_occ, bounds, homo, lumo, tol=0.0, max_layers=120, eps_alt=0.0, keep_history=False):
+    """Alg. 1 with the accelerated weights of section V.A.  homo / lumo: estimates of the highest occupied / lowest
+    unoccupied eigenvalue of H (energy units; lumo > homo), bounds: spectral bounds as in sp2_ref.
+    Stop tests: IdErr_n <= 0, IdErr_n <= tol, n = max_layers (the parameter-free test of Alg. 1 rests on Theorem 1,
+    which is proved for the alternating x^2 / 2x - x^2 pair only, so it is not applied here)."""
+    H = symmetrize_lower(H32)
+    n_dim = H.shape[0]
+    eps_min, eps_max = gershgorin_bounds(H) if bounds is None else (float(bounds[0]), float(bounds[1]))
+    S = initial_layer(H, eps_min, eps_max)
+    I = np.eye(n_dim)
+    h = (eps_max - homo) / (eps_max - eps_min)         # S_0 reverses the order: the HOMO is the smallest occupied value
+    l = (eps_max - lumo) / (eps_max - eps_min)
+    if not (0.0 <= l < h <= 1.0):
+        raise ValueError("need eps_min <= homo < lumo <= eps_max")
+    N_S = float(np.trace(S))
+    st = {"trace_S": [], "trace_X": [], "iderr": [], "sigma": [], "theta": [], "h": [], "l": [], "margin": [],
+          "S_hist": []}
+    n, stop, sigma_prev = 0, STOP_NONE, 0
+    while stop == STOP_NONE:
+        n += 1
+        X = S @ S
+        N_X = float(np.trace(X))
+        iderr = N_S - N_X
+        sigma, th, h, l, d = accelerated_layer(N_S, N_X, n_dim, N_occ, h, l, sigma_prev, eps_alt)
+        S = th[0] * X + th[1] * S + th[2] * I
+        N_S = float(np.trace(S))
+        sigma_prev = sigma
+        st["trace_S"].append(N_S); st["trace_X"].append(N_X); st["iderr"].append(iderr); st["sigma"].append(sigma)
+        st["theta"].append(th); st["h"].append(h); st["l"].append(l); st["margin"].append(d)
+        if keep_history:
+            st["S_hist"].append(S.copy())
+        if iderr <= 0.0:
+            stop = STOP_IDERR_NONPOS
+        elif tol > 0.0 and iderr <= tol:
+            stop = STOP_TOL
+        elif n >= max_layers:
+            stop = STOP_MAX_LAYERS
+    st["stop_reason"], st["n_layers"], st["bounds"] = stop, n, (eps_min, eps_max)
+    return S, st
