@@ -77,10 +77,19 @@ typedef struct {
                                tensor-core accumulator, whose truncating FP32 accumulation biases the large
                                diagonal by ~ (3N/32) ulp, ramping along the diagonal (reading C24);
                                0: Alg. 2 literally (tensor-core diagonal). Single-matrix path only.           */
+    int    accelerated;     /* 1: accelerated Deep-NN SP2 (section V.A): real-valued sigma_n from the
+                               HOMO / LUMO estimates below -- each layer is the SP2 polynomial composed with the
+                               steepest affine map that keeps the eigenvalue order and the range [0,1] (DESIGN.md
+                               reading C27; the paper's own W_n, B_n are in its unavailable supplement).  The
+                               parameter-free stop test is not applied (Theorem 1 covers the plain pair only).
+                               sp2_density_matrix only.  0 (default): Alg. 1.                                  */
+    double homo, lumo;      /* estimates of the highest occupied / lowest unoccupied eigenvalue of H (energy
+                               units), eps_min <= homo < lumo <= eps_max; they must bound the gap from inside:
+                               homo >= true HOMO, lumo <= true LUMO ("prior knowledge")                  */
 } sp2_opts_t;
 
 /* Fill *o with defaults: auto_bounds=1, tol=0, max_layers=120, eps_alt=0, fp16_scale_log2=-1, control=0,
- * tile_config=0, exact_diag=1. */
+ * tile_config=0, exact_diag=1, accelerated=0, homo=lumo=0. */
 void sp2_default_opts(sp2_opts_t* o);
 
 /* Create a handle able to solve one matrix up to N_max, or a batch of batch_max matrices of N <= 256,

@@ -31,7 +31,8 @@ class LayerStat(C.Structure):
 class Opts(C.Structure):
     _fields_ = [("auto_bounds", C.c_int), ("eps_min", C.c_double), ("eps_max", C.c_double), ("tol", C.c_double),
                 ("max_layers", C.c_int), ("eps_alt", C.c_double), ("fp16_scale_log2", C.c_int),
-                ("control", C.c_int), ("tile_config", C.c_int), ("exact_diag", C.c_int)]
+                ("control", C.c_int), ("tile_config", C.c_int), ("exact_diag", C.c_int), ("accelerated", C.c_int),
+                ("homo", C.c_double), ("lumo", C.c_double)]
 
 
 class RefineResult(C.Structure):
@@ -118,7 +119,7 @@ def _stats_to_dict(stats, n):
 
 
 def make_opts(bounds=None, tol=0.0, max_layers=120, eps_alt=0.0, fp16_scale_log2=-1, control=0, tile_config=0,
-              exact_diag=1) -> Opts:
+              exact_diag=1, homo_lumo=None) -> Opts:
     o = Opts()
     load().sp2_default_opts(C.byref(o))
     if bounds is not None:
@@ -126,6 +127,8 @@ def make_opts(bounds=None, tol=0.0, max_layers=120, eps_alt=0.0, fp16_scale_log2
     o.tol, o.max_layers, o.eps_alt = float(tol), int(max_layers), float(eps_alt)
     o.fp16_scale_log2, o.control, o.tile_config = int(fp16_scale_log2), int(control), int(tile_config)
     o.exact_diag = int(exact_diag)
+    if homo_lumo is not None:        # accelerated Deep-NN SP2 (section V.A)
+        o.accelerated, o.homo, o.lumo = 1, float(homo_lumo[0]), float(homo_lumo[1])
     return o
 
 

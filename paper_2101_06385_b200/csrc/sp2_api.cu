@@ -114,6 +114,9 @@ extern "C" void sp2_default_opts(sp2_opts_t* o) {
     o->control = 0;
     o->tile_config = 0;
     o->exact_diag = 1;
+    o->accelerated = 0;
+    o->homo = 0.0;
+    o->lumo = 0.0;
 }
 
 extern "C" size_t sp2_workspace_bytes(int N_max, int batch_max, int max_layers) {
@@ -426,6 +429,8 @@ static sp2_status_t solve_single(sp2_handle_s* h, const float* H_dev, int N, int
     c->eps_min = o->eps_min; c->eps_max = o->eps_max;
     c->N = N; c->mode = mode; c->max_layers = max_layers; c->auto_bounds = o->auto_bounds;
     c->noise_kappa = h->noise_kappa;
+    c->accelerated = (mode == MODE_STANDARD && o->accelerated) ? 1 : 0;
+    c->homo = o->homo; c->lumo = o->lumo;
     CK(cudaMemcpyAsync(h->ctrl, c, ctrl_header_bytes(), cudaMemcpyHostToDevice, st));
     if (mode == MODE_GENERALIZED)
         CK(cudaMemcpyAsync(h->thetas_dev, h->thetas_host, (size_t)max_layers * kThetaStride * sizeof(double),
@@ -503,6 +508,10 @@ extern "C" sp2_status_t sp2_density_matrix(sp2_handle_t h, const float* H_dev, i
     if (!o.auto_bounds) {
         if (!isfinite(o.eps_min) || !isfinite(o.eps_max)) return SP2_ERR_INVALID_ARG;
         if (!(o.eps_max > o.eps_min)) return SP2_ERR_BOUNDS_DEGENERATE;
+    }
+    if (o.accelerated) {
+        if (!isfinite(o.homo) || !isfinite(o.lumo) || !(o.lumo > o.homo)) return SP2_ERR_INVALID_ARG;
+        if (!o.auto_bounds && !(o.eps_min <= o.homo && o.lumo <= o.eps_max)) return SP2_ERR_INVALID_ARG;
     }
     return solve_single(h, H_dev, N, ldh, N_occ, MODE_STANDARD, &o, D_dev, ldd, stats_host, n_layers, bounds_out,
                         (cudaStream_t)stream);
@@ -675,6 +684,7 @@ extern "C" sp2_status_t sp2_density_matrix_batched(sp2_handle_t h, const float* 
     if (opts) o = *opts; else sp2_default_opts(&o);
     if (o.max_layers < 1 || o.max_layers > h->max_layers) return SP2_ERR_INVALID_ARG;
     if (!o.auto_bounds && !(o.eps_max > o.eps_min)) return SP2_ERR_BOUNDS_DEGENERATE;
+    if (o.accelerated) return SP2_ERR_INVALID_ARG;       // per-matrix HOMO/LUMO estimates: single-matrix call only
     for (int i = 0; i < (nocc_is_scalar ? 1 : B); ++i)
         if (!(N_occ[i] >= 0.0 && N_occ[i] <= (double)N)) return SP2_ERR_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)stream;

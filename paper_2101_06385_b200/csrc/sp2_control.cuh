@@ -33,6 +33,11 @@ struct CtrlCore {
     double fro2;                     // ||S_n||_F^2 = N_X of layer n+1
     double iderr_prev, iderr_prev2;  // IdErr_n, IdErr_{n-1}
     double nx_inflight;              // N_X of the layer in flight (exact, FP64 pre-trace)
+    double acc_h, acc_l;             // accelerated scheme (section V.A): lower bound of the occupied, upper bound of
+                                     // the unoccupied eigenvalues of S_n (rescaled HOMO / LUMO estimates)
+    double homo, lumo;               // the caller's estimates in energy units (rescaled once the bounds are known)
+    int    accelerated;              // 1: weights of reading C27 instead of sigma = +-1
+    int    pad_acc_;
     double noise_kappa;              // reading C25: stop when IdErr_n <= kappa |Tr X_n(tc) - N_X|; 0 disables
     float  theta[4];                 // th1, th2, th3, c of the NEXT layer (FP32: the epilogue's arithmetic type)
     unsigned int done_counter;       // CTAs finished in the current kernel
@@ -64,22 +69,59 @@ __device__ inline void control_plan_next(CtrlCore* c, sp2_layer_stat_t* stats, c
     }
     const double N_S = c->N_S, N_X = c->fro2, N_occ = c->N_occ;
     const double iderr = N_S - N_X;                                            // IdErr_m
-    const double d = fabs(2.0 * N_S - N_X - N_occ) - fabs(N_X - N_occ) - (double)c->sigma_prev * c->eps_alt;
-    int sigma;
-    if (d > 0.0) sigma = 1;
-    else if (d < 0.0) sigma = -1;
-    else sigma = (c->sigma_prev != 0) ? -c->sigma_prev : 1;                   // Sign(0): alternate (C4)
     if (!(isfinite(N_S) && isfinite(N_X))) {
         c->running = 0; c->stop_reason = SP2_STOP_NONFINITE; c->error = SP2_ERR_NONFINITE;
         return;
     }
-    c->theta[0] = (float)sigma;            // W_m = sigma I
-    c->theta[1] = (float)(1 - sigma);      // B_m = (I - W_m) S_{m-1}
-    c->theta[2] = 0.0f;
-    c->theta[3] = 0.0f;
+    int sigma;
+    if (c->accelerated) {
+        // Section V.A, reading C27: A(x) = (a x + 1 - a)^2 with a = 2 / (2 - l), B(x) = 2 a x - (a x)^2
+        // with a = 2 / (1 + h); the branch whose occupation is closer to N_occ (Alg. 1's rule on the new traces).
+        if (m == 1) {                                   // rescale the estimates once the spectral bounds are known
+            c->acc_h = (c->eps_max - c->homo) / (c->eps_max - c->eps_min);
+            c->acc_l = (c->eps_max - c->lumo) / (c->eps_max - c->eps_min);
+            if (!(c->acc_l >= 0.0 && c->acc_l < c->acc_h && c->acc_h <= 1.0)) {
+                c->running = 0; c->error = SP2_ERR_INVALID_ARG;
+                return;
+            }
+        }
+        const double h = c->acc_h, l = c->acc_l, n_dim = (double)c->N;
+        const double aA = 2.0 / (2.0 - l), aB = 2.0 / (1.0 + h);
+        const double trA = aA * aA * N_X + 2.0 * aA * (1.0 - aA) * N_S + (1.0 - aA) * (1.0 - aA) * n_dim;
+        const double trB = 2.0 * aB * N_S - aB * aB * N_X;
+        const double d = fabs(trB - N_occ) - fabs(trA - N_occ) - (double)c->sigma_prev * c->eps_alt;
+        if (d > 0.0) sigma = 1;
+        else if (d < 0.0) sigma = -1;
+        else sigma = (c->sigma_prev != 0) ? -c->sigma_prev : 1;
+        if (sigma > 0) {
+            c->theta[0] = (float)(aA * aA);
+            c->theta[1] = (float)(2.0 * aA * (1.0 - aA));
+            c->theta[2] = (float)((1.0 - aA) * (1.0 - aA));
+            const double hl = aA * l + 1.0 - aA;
+            c->acc_h = (aA * h + 1.0 - aA) * (aA * h + 1.0 - aA);
+            c->acc_l = fmax((1.0 - aA) * (1.0 - aA), hl * hl);
+        } else {
+            c->theta[0] = (float)(-aB * aB);
+            c->theta[1] = (float)(2.0 * aB);
+            c->theta[2] = 0.0f;
+            c->acc_h = fmin(2.0 * aB * h - aB * aB * h * h, 2.0 * aB - aB * aB);
+            c->acc_l = 2.0 * aB * l - aB * aB * l * l;
+        }
+        c->theta[3] = 0.0f;
+    } else {
+        const double d = fabs(2.0 * N_S - N_X - N_occ) - fabs(N_X - N_occ) - (double)c->sigma_prev * c->eps_alt;
+        if (d > 0.0) sigma = 1;
+        else if (d < 0.0) sigma = -1;
+        else sigma = (c->sigma_prev != 0) ? -c->sigma_prev : 1;                   // Sign(0): alternate (C4)
+        c->theta[0] = (float)sigma;            // W_m = sigma I
+        c->theta[1] = (float)(1 - sigma);      // B_m = (I - W_m) S_{m-1}
+        c->theta[2] = 0.0f;
+        c->theta[3] = 0.0f;
+    }
     int pend = SP2_STOP_NONE;
     if (iderr <= 0.0) pend = SP2_STOP_IDERR_NONPOS;
-    else if (m > 2 && c->sigma_prev != c->sigma_prev2 && iderr > 4.5 * c->iderr_prev2 * c->iderr_prev2)
+    else if (!c->accelerated && m > 2 && c->sigma_prev != c->sigma_prev2 &&
+             iderr > 4.5 * c->iderr_prev2 * c->iderr_prev2)   // Thm 1 holds for the plain alternating pair only
         pend = SP2_STOP_PARAM_FREE;        // sigma_{m-1} != sigma_{m-2} and IdErr_m > 4.5 IdErr_{m-2}^2
     else if (c->tol > 0.0 && iderr <= c->tol) pend = SP2_STOP_TOL;
     else if (m >= c->max_layers) pend = SP2_STOP_MAX_LAYERS;

@@ -201,6 +201,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
             c->n = 0; c->running = 0; c->stop_reason = 0; c->pending_stop = 0; c->sigma_prev = 0; c->sigma_prev2 = 0;
             c->error = bounds_ok ? 0 : SP2_ERR_BOUNDS_DEGENERATE; c->launches = 0;
             c->N_S = 0; c->fro2 = 0; c->iderr_prev = 0; c->iderr_prev2 = 0; c->nx_inflight = 0; c->noise_kappa = p.noise_kappa;
+            c->accelerated = 0; c->acc_h = 1.0; c->acc_l = 0.0; c->homo = 0.0; c->lumo = 0.0;
         }
         if (!bounds_ok) {           // uniform over the cluster (same e0, e1 everywhere)
             if (rank == 0 && threadIdx.x == 0) {

@@ -54,9 +54,10 @@ def test_struct_layouts_match_header():
 #include <stddef.h>
 #include "sp2_b200.h"
 int main(void) {
-  printf("%zu %zu %zu %zu %zu %zu %zu %zu\n", sizeof(sp2_layer_stat_t), offsetof(sp2_layer_stat_t, trace_X_diag),
+  printf("%zu %zu %zu %zu %zu %zu %zu %zu %zu %zu\n", sizeof(sp2_layer_stat_t), offsetof(sp2_layer_stat_t, trace_X_diag),
          offsetof(sp2_layer_stat_t, sigma), offsetof(sp2_layer_stat_t, t_end_ns), sizeof(sp2_opts_t),
-         offsetof(sp2_opts_t, tol), offsetof(sp2_opts_t, eps_alt), offsetof(sp2_opts_t, tile_config));
+         offsetof(sp2_opts_t, tol), offsetof(sp2_opts_t, eps_alt), offsetof(sp2_opts_t, tile_config),
+         offsetof(sp2_opts_t, accelerated), offsetof(sp2_opts_t, lumo));
   return 0; }'''
     import tempfile
 
@@ -68,7 +69,7 @@ int main(void) {
         got = [int(x) for x in subprocess.run([exe], capture_output=True, text=True, check=True).stdout.split()]
     L, Op = api.LayerStat, api.Opts
     want = [C.sizeof(L), L.trace_X_diag.offset, L.sigma.offset, L.t_end_ns.offset, C.sizeof(Op), Op.tol.offset,
-            Op.eps_alt.offset, Op.tile_config.offset]
+            Op.eps_alt.offset, Op.tile_config.offset, Op.accelerated.offset, Op.lumo.offset]
     assert got == want
 
 
