@@ -52,6 +52,30 @@ def test_paper_text_numbers():
         assert 0.6 * g["layers_plain_100x100_nocc10"] <= st["n_layers"] <= 1.6 * g["layers_plain_100x100_nocc10"]
         De, _ = O.eig_density(H32, 10.0)
         assert np.abs(D - De).max() < 1e-6
+        # "17 layers instead of 28" with acceleration: same shape, exact HOMO/LUMO, ratio within +-0.2 of 17/28
+        ev = np.linalg.eigvalsh(O.symmetrize_lower(H32))
+        b = O.gershgorin_bounds(O.symmetrize_lower(H32))
+        _, s0 = O.sp2_ref(H32, 10.0, b, tol=1e-9, max_layers=200)
+        _, s1 = O.sp2_accelerated_ref(H32, 10.0, b, ev[9], ev[10], tol=1e-9, max_layers=200)
+        want = g["layers_accelerated_100x100_nocc10"] / g["layers_plain_100x100_nocc10"]
+        assert abs(s1["n_layers"] / s0["n_layers"] - want) <= 0.2
+
+
+def test_golden_next_rows():
+    with open(os.path.join(G, "oracle_next_rows.json")) as f:
+        gold = json.load(f)
+    import importlib.util
+    spec = importlib.util.spec_from_file_location("make_golden", os.path.join(G, "make_golden.py"))
+    mg = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mg)
+    now = mg.build_next_rows()
+    assert set(now) == set(gold)
+    for k in gold:
+        for key, val in gold[k].items():
+            if isinstance(val, list) and val and isinstance(val[0], int):
+                assert now[k][key] == val, (k, key)
+            else:
+                assert np.allclose(now[k][key], val, rtol=0, atol=1e-9), (k, key)
 
 
 def test_golden_small_cases():
