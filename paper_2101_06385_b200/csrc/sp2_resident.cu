@@ -125,6 +125,11 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
     const uint32_t t_acc = tmem_base + ((uint32_t)(q * 32) << 16);
     const uint32_t t_S = t_acc + NP;
     const float cs = p.scale, inv2 = p.inv_scale2;
+    // mirror-store address pieces that depend on this thread's column gi only (panel_off(row, gi) split by row bits)
+    const uint32_t mir_base = (uint32_t)((gi >> 6) * 16384 + (gi & 7) * 2);
+    uint32_t mir_x[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) mir_x[k] = (uint32_t)(k * 128 + (((((gi & 63) >> 3) ^ k)) << 4));
 
     for (int m = cluster_id; m < p.B; m += n_clusters) {
         const float* __restrict__ Hm = p.H + (size_t)m * N * N;
@@ -285,22 +290,39 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
                             *reinterpret_cast<uint4*>(loP + off) = make_uint4(lp[4 * g], lp[4 * g + 1], lp[4 * g + 2], lp[4 * g + 3]);
                         }
                     }
+                    // mirror (j, i): row j = c0 + c of CTA jr, column gi.  Byte offset inside the 128-row panel
+                    // = mir_base + (c >> 3) * 1024 + mir_x[c & 7]  (see panel_off): one add per element
+                    const uint32_t mb = mir_base + (uint32_t)(((c0 & 127) >> 3) * 1024);
+                    if (below) {                                // every j < gi: straight-line stores
+                        if (CG == 2 && jr != rank) {
+                            const uint32_t rh = mapa_u32(hi_addr, jr) + mb, rl = mapa_u32(lo_addr, jr) + mb;
 #pragma unroll
-                    for (int c = 0; c < 32; ++c) {
-                        const int j = c0 + c;
-                        const unsigned short hb = (unsigned short)(hp[c >> 1] >> (16 * (c & 1)));
-                        const unsigned short lb = (unsigned short)(lp[c >> 1] >> (16 * (c & 1)));
-                        if (!below && j <= gi) {                // diagonal chunk: own entries one by one
-                            const uint32_t off = panel_off(tl, j);
-                            *reinterpret_cast<unsigned short*>(hiP + off) = hb;
-                            *reinterpret_cast<unsigned short*>(loP + off) = lb;
+                            for (int c = 0; c < 32; ++c) {
+                                const uint32_t off = (uint32_t)((c >> 3) * 1024) + mir_x[c & 7];
+                                st_cluster_u16(rh + off, (unsigned short)(hp[c >> 1] >> (16 * (c & 1))));
+                                st_cluster_u16(rl + off, (unsigned short)(lp[c >> 1] >> (16 * (c & 1))));
+                            }
+                        } else {
+#pragma unroll
+                            for (int c = 0; c < 32; ++c) {
+                                const uint32_t off = mb + (uint32_t)((c >> 3) * 1024) + mir_x[c & 7];
+                                *reinterpret_cast<unsigned short*>(hiP + off) = (unsigned short)(hp[c >> 1] >> (16 * (c & 1)));
+                                *reinterpret_cast<unsigned short*>(loP + off) = (unsigned short)(lp[c >> 1] >> (16 * (c & 1)));
+                            }
                         }
-                        if (j < gi) {                           // mirror (j, i): row j of CTA jr, column gi
-                            const uint32_t off = panel_off(j & 127, gi);
-                            if (CG == 2) {
-                                st_cluster_u16(mapa_u32(hi_addr + off, jr), hb);
-                                st_cluster_u16(mapa_u32(lo_addr + off, jr), lb);
-                            } else {
+                    } else {                                    // diagonal chunk (rows and columns of this CTA)
+#pragma unroll
+                        for (int c = 0; c < 32; ++c) {
+                            const int j = c0 + c;
+                            const unsigned short hb = (unsigned short)(hp[c >> 1] >> (16 * (c & 1)));
+                            const unsigned short lb = (unsigned short)(lp[c >> 1] >> (16 * (c & 1)));
+                            if (j <= gi) {                      // own entries one by one
+                                const uint32_t off = panel_off(tl, j);
+                                *reinterpret_cast<unsigned short*>(hiP + off) = hb;
+                                *reinterpret_cast<unsigned short*>(loP + off) = lb;
+                            }
+                            if (j < gi) {
+                                const uint32_t off = mb + (uint32_t)((c >> 3) * 1024) + mir_x[c & 7];
                                 *reinterpret_cast<unsigned short*>(hiP + off) = hb;
                                 *reinterpret_cast<unsigned short*>(loP + off) = lb;
                             }
