@@ -11,18 +11,6 @@ namespace sp2 {
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
     return static_cast<uint32_t>(__cvta_generic_to_shared(p));
 }
-__device__ __forceinline__ uint32_t lane_id() { return threadIdx.x & 31; }
-
-__device__ __forceinline__ bool elect_one() {
-    uint32_t pred = 0;
-    asm volatile(
-        "{\n\t.reg .pred p;\n\t"
-        "elect.sync _|p, 0xffffffff;\n\t"
-        "selp.u32 %0, 1, 0, p;\n\t}\n"
-        : "=r"(pred));
-    return pred != 0;
-}
-
 // ---------------------------------------------------------------- mbarrier
 __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count));
@@ -73,28 +61,9 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
 __device__ __forceinline__ void tma_prefetch_desc(const void* tmap) {
     asm volatile("prefetch.tensormap [%0];\n" ::"l"(tmap) : "memory");
 }
-// 2D tile load global -> shared (own CTA), completion on `bar` (own CTA).  c0 = innermost coordinate.
-__device__ __forceinline__ void tma_load_2d(void* dst, const void* tmap, uint64_t* bar, int c0, int c1) {
-    asm volatile(
-        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];\n" ::
-            "r"(smem_u32(dst)),
-        "l"(tmap), "r"(smem_u32(bar)), "r"(c0), "r"(c1)
-        : "memory");
-}
-// 2-CTA form: data lands in this CTA's smem, completion is signalled on the barrier at the same offset in
-// the LEADER CTA (rank 0) of the pair: the barrier address is this CTA's cluster-mapped address with the
-// peer bit cleared.
-__device__ __forceinline__ void tma_load_2d_pair(void* dst, const void* tmap, uint64_t* bar, int c0, int c1) {
-    uint32_t bar_addr = smem_u32(bar) & 0xFEFFFFFFu;
-    asm volatile(
-        "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, "
-        "%4}], [%2];\n" ::"r"(smem_u32(dst)),
-        "l"(tmap), "r"(bar_addr), "r"(c0), "r"(c1)
-        : "memory");
-}
-
-// Same loads with an L2 cache-policy operand (createpolicy): operand panels are re-read by the other CTAs of the
-// wave, the epilogue's traffic is not, so panels are kept (evict_last) and epilogue lines stream (evict_first).
+// 2D tile loads global -> shared with an L2 cache-policy operand (createpolicy): operand panels are re-read by the
+// other CTAs of the wave, the epilogue's traffic is not, so panels are kept (evict_last) and epilogue lines stream.
+// c0 = innermost coordinate; completion (complete_tx) on `bar`.
 __device__ __forceinline__ uint64_t l2_policy_evict_last() {
     uint64_t pol;
     asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;\n" : "=l"(pol));
@@ -108,6 +77,8 @@ __device__ __forceinline__ void tma_load_2d_hint(void* dst, const void* tmap, ui
         "l"(tmap), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "l"(pol)
         : "memory");
 }
+// 2-CTA form: data lands in this CTA's smem, completion is signalled on the barrier at the same offset in the LEADER
+// CTA (rank 0) of the pair: the barrier address is this CTA's cluster-mapped address with the peer bit cleared.
 __device__ __forceinline__ void tma_load_2d_pair_hint(void* dst, const void* tmap, uint64_t* bar, int c0, int c1,
                                                       uint64_t pol) {
     uint32_t bar_addr = smem_u32(bar) & 0xFEFFFFFFu;
@@ -116,13 +87,6 @@ __device__ __forceinline__ void tma_load_2d_pair_hint(void* dst, const void* tma
         "[%0], [%1, {%3, %4}], [%2], %5;\n" ::"r"(smem_u32(dst)),
         "l"(tmap), "r"(bar_addr), "r"(c0), "r"(c1), "l"(pol)
         : "memory");
-}
-
-// Prefetch a tile into L2 only (no shared-memory destination, no barrier).
-__device__ __forceinline__ void tma_prefetch_l2_2d(const void* tmap, int c0, int c1, uint64_t pol) {
-    asm volatile("cp.async.bulk.prefetch.tensor.2d.L2.global.L2::cache_hint [%0, {%1, %2}], %3;\n" ::"l"(tmap), "r"(c0),
-                 "r"(c1), "l"(pol)
-                 : "memory");
 }
 
 // ---------------------------------------------------------------- cluster
