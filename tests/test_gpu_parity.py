@@ -62,6 +62,28 @@ def test_config1_seeds_auto_and_explicit_bounds(env, seed, auto):
     P.replay_check(info, w.H32, w.N_occ, used, eigs=w.eps)
 
 
+@pytest.mark.parametrize("n,tile", [(3000, 3), (3500, 3), (3000, 1)])
+def test_ragged_sizes_with_several_rounds_and_tail_strips(env, n, tile):
+    """More work items than CTA slots, ragged N, and a last partial round that the host cuts into column strips
+    (256-pair tiles: N = 3000 -> 78 tiles on 74 slots, 4 left over -> 16 strips of 64 columns; N = 3500 -> 105 tiles,
+    31 left over -> 62 strips of 128; 128-tiles at N = 3000 -> 300 tiles on 148 slots, 4 left over -> 8 strips of 64).
+    The closed form D* = Q_occ Q_occ^T is the reference; the FP64 oracle is compared through the scalar recursion."""
+    api, h, torch = env
+    k = n // 2
+    w = W.gapped_dense(n, n, (-1.0, -0.15), (0.15, 1.0), k, "ragged-rounds", bounds=(-1.0, 1.0))
+    opts = api.make_opts(bounds=w.bounds, tol=1e-5, max_layers=80, tile_config=tile)
+    D, info = h.density_matrix(torch.from_numpy(w.H32).cuda(), float(k), opts)
+    D = D.cpu().numpy().astype(np.float64)
+    Dstar = O.closed_form_density(w.Q, w.N_occ)
+    st = O.scalar_recursion(w.eps, w.N_occ, -1.0, 1.0, tol=1e-5, max_layers=80)
+    print(f"N={n} tile={tile}: layers {info['n_layers']}/{st['n_layers']} max|D-D*|={np.abs(D - Dstar).max():.2e}")
+    P.assert_acceptance(D, Dstar, float(k), f"N={n} tile={tile}")
+    assert np.array_equal(D, D.T)
+    assert abs(info["n_layers"] - st["n_layers"]) <= 2
+    P.branch_prefix_check(info, st, w.N_occ)
+    P.replay_check(info, None, w.N_occ, (-1.0, 1.0), eigs=w.eps)
+
+
 @pytest.mark.parametrize("n", [1, 2, 10, 100, 127, 129, 300, 777])
 def test_ragged_and_tiny_sizes(env, n):
     """Sizes that are not a multiple of the tile (padding of S_0 must be inert), several tiles + ragged tail."""
