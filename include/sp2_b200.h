@@ -71,7 +71,9 @@ typedef struct {
                                -1 = library default (13): keeps X1 out of FP16's subnormal range            */
     int    control;         /* 0: device-side loop in a CUDA graph (WHILE node); 1: host-stepped (debug:
                                one sync per layer); 2: graph of max_layers guarded launches, no WHILE node   */
-    int    tile_config;     /* 0: choose by N; 1: 128x128 1-CTA; 2: 128x256 1-CTA; 3: 256x256 2-CTA          */
+    int    tile_config;     /* 0: choose by N; 1: 128x128 1-CTA; 2: 128x256 1-CTA; 3: 256x256 2-CTA;
+                               4: 128x128 1-CTA with the enhanced accumulation of sp2_refine_energy in EVERY
+                               layer (accuracy option, about 2x the time of 3 at large N)  */
     int    exact_diag;      /* 1 (default): diag(X_n)_i = sum_j S_ij^2 is taken from FP32/FP64 row sums of the
                                FP32 S_{n-1} (the same identity that gives N_X = ||S||_F^2) instead of the
                                tensor-core accumulator, whose truncating FP32 accumulation biases the large

@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libsp2b200.so")
 
 SP2_OK, SP2_NOT_CONVERGED = 0, 1
 STOP_NAMES = {0: "none", 1: "iderr<=0", 2: "param_free", 3: "tol", 4: "max_layers", 5: "nonfinite", 6: "noise_floor"}
-TILE_AUTO, TILE_128x128, TILE_128x256, TILE_256x256_PAIR = 0, 1, 2, 3
+TILE_AUTO, TILE_128x128, TILE_128x256, TILE_256x256_PAIR, TILE_128x128_ENH = 0, 1, 2, 3, 4
 
 EXPORTS = ["sp2_default_opts", "sp2_create", "sp2_destroy", "sp2_workspace_bytes", "sp2_density_matrix",
            "sp2_density_matrix_host", "sp2_generalized", "sp2_generalized_mix", "sp2_generalized_wb", "sp2_density_matrix_batched",

@@ -290,7 +290,7 @@ static void build_work_list(int nt, int band, int edge, int subs, int cta_group,
 }
 
 static int choose_tile_config(int N, int requested, int num_sms) {
-    if (requested >= TILE_128x128 && requested <= TILE_256x256_PAIR) return requested;   // ENH is internal
+    if (requested >= TILE_128x128 && requested <= TILE_128x128_ENH) return requested;
     const int n128 = round_up(N, 128) / 128;
     const long long t128 = (long long)n128 * (n128 + 1) / 2;
     // 256x256 pair tiles once there are at least 1.5 rounds of them (N >= ~3800 on 148 SMs; measured at N = 4096:
@@ -311,7 +311,7 @@ static sp2_status_t prepare_problem(sp2_handle_s* h, int N, const sp2_opts_t* o,
                                     int forced_cfg = 0) {
     pb->N = N;
     pb->cfg = forced_cfg ? forced_cfg : choose_tile_config(N, o ? o->tile_config : 0, h->num_sms);
-    pb->list = forced_cfg ? 1 : 0;
+    pb->list = (pb->cfg == TILE_128x128_ENH) ? 1 : 0;   // the enhanced-accumulation layers keep their own work list
     pb->mix = 0;
     const int L = pb->list;
     const int edge = tile_super_edge(pb->cfg);

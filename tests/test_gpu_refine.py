@@ -102,3 +102,21 @@ def test_refine_errors_and_tiny_sizes(env):
         h.refine_energy(big, 1, big)                           # larger than the handle's N_max
     with pytest.raises(TypeError):
         h.refine_energy(S.cpu(), 1, Hm)                        # no CPU fallback
+
+
+def test_enhanced_accumulation_in_every_layer_is_more_accurate(env):
+    """tile_config = 4: the whole solve with the chunked tensor-core accumulation (accuracy option, NEXT-4)."""
+    api, h, torch = env
+    w = W.config1(5, n=2048)
+    H = torch.from_numpy(w.H32).cuda()
+    Dstar = w.Q[:, : int(w.N_occ)] @ w.Q[:, : int(w.N_occ)].T
+    out = {}
+    for tile in (1, 4):
+        opts = api.make_opts(bounds=w.bounds, tol=w.tol, max_layers=w.max_layers, tile_config=tile)
+        D, info = h.density_matrix(H, w.N_occ, opts)
+        Dn = D.cpu().numpy().astype(np.float64)
+        out[tile] = (np.abs(Dn - Dstar).max(), O.idempotency_error(Dn), abs(np.trace(Dn) - w.N_occ), info["n_layers"])
+        assert np.array_equal(Dn, Dn.T) and info["status"] == 0
+    print(f"N=2048 plain (err, idem, trace err, layers) {out[1]}  enhanced {out[4]}")
+    assert out[4][0] <= 1e-3 and out[4][1] <= 1e-3
+    assert out[4][1] < 0.5 * out[1][1] and out[4][2] < 0.5 * out[1][2] + 1e-6
