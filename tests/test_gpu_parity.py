@@ -30,7 +30,7 @@ def _solve(env, w, bounds, **kw):
 
 
 @pytest.mark.parametrize("control", [0, 1, 2])
-@pytest.mark.parametrize("tile", [1, 2, 3])
+@pytest.mark.parametrize("tile", [1, 2, 3, 4])
 def test_config1_all_tiles_and_control_modes(env, tile, control):
     """BASELINE configs[0] (N=128, explicit bounds): every tile configuration and control mode gives the same
     result; D, trace, idempotency within tolerance; branch sequence per reading C6."""
