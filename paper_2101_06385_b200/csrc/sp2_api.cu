@@ -477,8 +477,7 @@ static sp2_status_t solve_single(sp2_handle_s* h, const float* H_dev, int N, int
     if (pb.mix)      // F = d I - M  (Eq. 18 in the library's variables, see generalized_impl)
         CK(launch_one_minus(h->mix, (long long)ldS, D_dev, ldd, N, (float)mix_diag, h->num_sms, st));
     else
-        CK(cudaMemcpy2DAsync(D_dev, (size_t)ldd * 4, h->S, ldS * 4, (size_t)N * 4, (size_t)N,
-                             cudaMemcpyDeviceToDevice, st));
+        CK(launch_copy_sym(h->S, (long long)ldS, D_dev, ldd, N, h->num_sms, st));
     CK(cudaMemcpyAsync(h->ctrl_host, h->ctrl, ctrl_header_bytes(), cudaMemcpyDeviceToHost, st));
     CK(cudaMemcpyAsync(h->stats_host, h->stats_dev, (size_t)max_layers * sizeof(sp2_layer_stat_t),
                        cudaMemcpyDeviceToHost, st));
@@ -579,7 +578,7 @@ extern "C" sp2_status_t sp2_refine_energy(sp2_handle_t h, const float* S_dev, in
     s = launch_one_layer(h, pb, 0, 0, st);
     if (s == SP2_OK) s = launch_one_layer(h, pb, 1, 0, st);
     if (s != SP2_OK) return s;
-    CK(cudaMemcpy2DAsync(D_dev, (size_t)ldd * 4, h->S, ldS * 4, (size_t)N * 4, (size_t)N, cudaMemcpyDeviceToDevice, st));
+    CK(launch_copy_sym(h->S, (long long)ldS, D_dev, ldd, N, h->num_sms, st));
     CK(launch_energy_traces(D_dev, ldd, H_dev, ldh, N, h->ctrl, h->obs_dev + 3, 0, nullptr, nullptr, nullptr,
                             h->num_sms, st));
     CK(cudaMemcpyAsync(h->obs_host, h->obs_dev, 6 * sizeof(double), cudaMemcpyDeviceToHost, st));

@@ -402,6 +402,57 @@ __global__ void __launch_bounds__(256) k_energy_traces(const float* __restrict__
     }
 }
 
+// ------------------------------------------------------------------------------------------------ copy-out
+// D = the symmetric matrix whose UPPER triangle (incl. diagonal) is stored in S.  The layer kernel keeps only the
+// upper triangle of the FP32 master current below the diagonal chunks (that is the part its epilogue reads back, at the
+// mirrored address), so the result is mirrored once here instead of once per layer.  64 x 64 tiles, transposed
+// through shared memory so that both global writes are row segments.
+__global__ void __launch_bounds__(256) k_copy_sym(const float* __restrict__ S, long long ld, float* __restrict__ D,
+                                                  long long ldd, int N) {
+    __shared__ float ts[ET][ET + 1];
+    const int nt = (N + ET - 1) / ET;
+    const long long ntiles = (long long)nt * (nt + 1) / 2;
+    const int c4 = (threadIdx.x & 15) * 4, r0 = threadIdx.x >> 4;
+    const bool vs = ((ld & 3) == 0) && ((reinterpret_cast<uintptr_t>(S) & 15) == 0);
+    const bool vd = ((ldd & 3) == 0) && ((reinterpret_cast<uintptr_t>(D) & 15) == 0);
+    for (long long t = blockIdx.x; t < ntiles; t += gridDim.x) {
+        int I, J;
+        tri_decode(t, I, J);                        // I >= J: source block rows J*64.., columns I*64..
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const int lr = r0 + 16 * k;
+            const float4 v = ld_tile4(S, N, ld, J * ET + lr, I * ET + c4, vs);
+            ts[lr][c4] = v.x; ts[lr][c4 + 1] = v.y; ts[lr][c4 + 2] = v.z; ts[lr][c4 + 3] = v.w;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const int lr = r0 + 16 * k;
+            float u[4], l[4];                       // upper block row lr, lower block row lr
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                const int lc = c4 + e;
+                // diagonal tile: (lr, lc) is authoritative only for lr <= lc
+                u[e] = (I != J || lr <= lc) ? ts[lr][lc] : ts[lc][lr];
+                l[e] = (I != J || lc <= lr) ? ts[lc][lr] : ts[lr][lc];
+            }
+            const int gu = J * ET + lr, gl = I * ET + lr;
+            const int cu = I * ET + c4, cl = J * ET + c4;
+            if (gu < N) {
+                if (vd && cu + 3 < N) *reinterpret_cast<float4*>(D + (long long)gu * ldd + cu) = make_float4(u[0], u[1], u[2], u[3]);
+                else
+                    for (int e = 0; e < 4; ++e) if (cu + e < N) D[(long long)gu * ldd + cu + e] = u[e];
+            }
+            if (I != J && gl < N) {
+                if (vd && cl + 3 < N) *reinterpret_cast<float4*>(D + (long long)gl * ldd + cl) = make_float4(l[0], l[1], l[2], l[3]);
+                else
+                    for (int e = 0; e < 4; ++e) if (cl + e < N) D[(long long)gl * ldd + cl + e] = l[e];
+            }
+        }
+        __syncthreads();
+    }
+}
+
 // ------------------------------------------------------------------------------------------------ NEXT-2
 // F = d I - M  (Eq. 18: the Fermi-operator approximation is 1 - sum_i c_i eps_i; d = 1 - c_0 after the
 // change of variable of generalized_impl), N x N, M with leading dimension ldm, F with ldo.
@@ -457,6 +508,13 @@ cudaError_t launch_split(const float* X, int N, long long ldx, __half* hi, __hal
 }  // namespace sp2
 
 namespace sp2 {
+cudaError_t launch_copy_sym(const float* S, long long ld, float* D, long long ldd, int N, int num_sms, cudaStream_t st) {
+    const int nt = (N + ET - 1) / ET;
+    const long long ntiles = (long long)nt * (nt + 1) / 2;
+    const long long cap = (long long)num_sms * 8;
+    k_copy_sym<<<(int)(ntiles < cap ? ntiles : cap), 256, 0, st>>>(S, ld, D, ldd, N);
+    return cudaGetLastError();
+}
 cudaError_t launch_one_minus(const float* M, long long ldm, float* F, long long ldo, int N, float d, int num_sms,
                              cudaStream_t st) {
     long long blocks = ((long long)N * N + 255) / 256;

@@ -15,6 +15,7 @@ cudaError_t launch_gershgorin(const float* H, int N, long long ldh, double* R, d
 cudaError_t launch_affine_split(const float* H, int N, long long ldh, float* S, __half* hi, __half* lo, long long ld,
                                 long long ldf, float scale, Ctrl* ctrl, sp2_layer_stat_t* stats, const double* thetas,
                                 unsigned long long* rowsq, float* mix, float c0, int num_sms, cudaStream_t st);
+cudaError_t launch_copy_sym(const float* S, long long ld, float* D, long long ldd, int N, int num_sms, cudaStream_t st);
 cudaError_t launch_one_minus(const float* M, long long ldm, float* F, long long ldo, int N, float d, int num_sms,
                              cudaStream_t st);
 
@@ -55,7 +56,8 @@ struct LayerParams {
     Ctrl* ctrl;
     sp2_layer_stat_t* stats;
     const double* thetas;          // generalized mode: [L][3] on the device
-    float* S;                      // FP32 master, Np x Np, updated in place
+    float* S;                      // FP32 master, Np x Np, updated in place; below the diagonal chunks only the UPPER
+                                   // triangle is kept current (it is what the epilogue reads back): see k_copy_sym
     float* mix;                    // output mix M = sum_i c_i S_i (Eq. 18), same layout as S; nullptr = none
     __half* hi_out;                // next layer's operands (the other ping-pong pair)
     __half* lo_out;

@@ -6,8 +6,10 @@
 //   S_n      = th1 acc / c^2 + th2 S_{n-1} + th3 I                              (Alg. 1's W_n, B_n; Eq. 17)
 //   epilogue: Tr S_n, ||S_n||_F^2 (= next layer's N_X), Tr X_n in FP64; next layer's hi/lo (Eqs. 12-13);
 //   last CTA: sigma_{n+1}, IdErr_{n+1}, stop tests (control_after_layer).
-// Only lower-triangle tiles (I >= J) are computed; every value is also stored at its mirrored position, so
-// S, hi, lo stay exactly symmetric and the next layer can read full row panels as K-major operands.
+// Only lower-triangle tiles (I >= J) are computed; every hi/lo value is also stored at its mirrored position, so the
+// operands stay exactly symmetric and the next layer can read full row panels as K-major operands.  Of the FP32
+// master only the mirrored (upper-triangle) copy is kept current outside the diagonal chunks: that is the copy the
+// epilogue reads back (coalesced), and k_copy_sym mirrors the final result once.
 //
 // Structure: persistent CTAs (or CTA pairs), static round-robin over a host-ordered supertile list;
 // warp 0 = TMA producer, warp 1 = tcgen05.mma issuer (+ TMEM alloc), warps 2-5 = epilogue
@@ -322,18 +324,15 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                 if (below) {
                     tmem_ld_wait();
                     float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
-                    float* __restrict__ rowS = S + (long long)gi * ld + gj0;          // own position
                     __half* __restrict__ rowH = HO + (long long)gi * ldf + gj0;
                     __half* __restrict__ rowL = LO + (long long)gi * ldf + gj0;
 #pragma unroll
                     for (int g = 0; g < 4; ++g) {           // 8 columns at a time: values leave registers early
-                        float sn[8];
                         uint32_t hp[4], lp[4];              // FP16 pairs (even column in the low half)
 #pragma unroll
                         for (int e = 0; e < 8; ++e) {
                             const int c = 8 * g + e;
                             const float val = fmaf(th1s, __uint_as_float(v[c]), th2 * so[c]);
-                            sn[e] = val;
                             __half h, l;
                             split_hi_lo(val, cs, h, l);
                             const uint32_t hb = __half_as_ushort(h), lb = __half_as_ushort(l);
@@ -354,9 +353,8 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                             __stcs(HOu + o, (unsigned short)hb);
                             __stcs(LOu + o, (unsigned short)lb);
                         }
-                        // own position: 32 contiguous bytes (FP32) / 16 (FP16) per thread per group
-                        __stcs(reinterpret_cast<float4*>(rowS) + 2 * g, make_float4(sn[0], sn[1], sn[2], sn[3]));
-                        __stcs(reinterpret_cast<float4*>(rowS) + 2 * g + 1, make_float4(sn[4], sn[5], sn[6], sn[7]));
+                        // own position: 16 contiguous bytes of each FP16 operand per thread per group (the FP32 master
+                        // is not written here: only its mirrored copy is ever read back; k_copy_sym mirrors the result)
                         if (C::MIX) {
                             float4* rowM = reinterpret_cast<float4*>(M + (long long)gi * ld + gj0);
                             const int b8 = C::MIX ? 8 * g : 0;
