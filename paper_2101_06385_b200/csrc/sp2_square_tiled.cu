@@ -130,7 +130,9 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                 for (int kb = 0; kb < KB; ++kb) {
                     mbar_wait(&empty_bar[s], ph ^ 1u);
                     uint8_t* st = smem + s * C::STAGE_BYTES;
-                    const int k0 = kb * BK;
+                    // odd rounds walk K backwards: the panels a CTA shares with the previous round (same band) are
+                    // still in L2 for the K-blocks that round finished with
+                    const int k0 = ((round & 1) ? (KB - 1 - kb) : kb) * BK;
                     if (CG == 1) {
                         mbar_arrive_expect_tx(&full_bar[s], C::STAGE_BYTES);
                         tma_load_2d_hint(st, &tm_hi, &full_bar[s], k0, m0, pol);
