@@ -484,7 +484,7 @@ static sp2_status_t solve_single(sp2_handle_s* h, const float* H_dev, int N, int
     CK(cudaStreamSynchronize(st));
     CK(cudaGetLastError());
     c = h->ctrl_host;
-    h->last_launches = c->launches;
+    h->last_launches = c->launches + 1;      // + the copy-out kernel (k_copy_sym / k_one_minus)
     if (bounds_out) { bounds_out[0] = c->eps_min; bounds_out[1] = c->eps_max; }
     if (n_layers_out) *n_layers_out = c->n;
     if (stats_out) memcpy(stats_out, h->stats_host, (size_t)(c->n < max_layers ? c->n : max_layers) * sizeof(sp2_layer_stat_t));
@@ -588,7 +588,7 @@ extern "C" sp2_status_t sp2_refine_energy(sp2_handle_t h, const float* S_dev, in
     const double* o = h->obs_host;
     result->energy_in = o[0]; result->trace_in = o[1]; result->iderr_in = o[1] - o[2];
     result->energy_out = o[3]; result->trace_out = o[4]; result->iderr_out = o[4] - o[5];
-    h->last_launches = h->ctrl_host->launches;
+    h->last_launches = h->ctrl_host->launches + 2;   // device-counted: 2 layers + 2 k_energy_traces; + split, copy-out
     if (h->ctrl_host->error < 0) return (sp2_status_t)h->ctrl_host->error;
     if (h->ctrl_host->n != 2) return SP2_ERR_CUDA;
     if (!isfinite(o[3]) || !isfinite(o[4]) || !isfinite(o[5])) return SP2_ERR_NONFINITE;
