@@ -96,3 +96,26 @@ def test_no_cpu_fallback_without_a_device(lib):
     with pytest.raises(api.SP2Error) as e:
         api.Handle(128, 0, 10)
     assert e.value.status == -5
+
+
+def test_oracle_and_product_are_independent():
+    """The oracle is test infrastructure: the package never imports it and it never imports the package; only the
+    seeded input generators (workloads.py, which hold none of the method's arithmetic) serve both."""
+    pkg = os.path.join(ROOT, "paper_2101_06385_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(from|import)\s+oracle\b", src, re.M), f"{f} imports the oracle"
+                assert "sp2_oracle" not in src, f"{f} mentions the oracle module"
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith(".py"):
+            src = open(os.path.join(ROOT, "oracle", f)).read()
+            assert not re.search(r"^\s*(from|import)\s+paper_2101_06385_b200\b", src, re.M), f"{f} imports the product"
+    # workloads.py: generators only -- no split, no square, no SP2 layer
+    wl = open(os.path.join(pkg, "workloads.py")).read()
+    for word in ("float16", "gershgorin", "@ S", "S @", "split_fp16"):
+        assert word not in wl, f"workloads.py contains method arithmetic: {word}"
+    # bench.py may execute the oracle only in its cpu_baseline / --impl reference legs
+    bench = open(os.path.join(ROOT, "bench.py")).read()
+    assert bench.count("from oracle import") == 1 and "def cpu_oracle_sample" in bench
