@@ -219,4 +219,15 @@ __device__ __forceinline__ void split_hi_lo(float x, float c, __half& hi, __half
     lo = __float2half_rn(xs - __half2float(hi));
 }
 
+// Two elements at once: the same roundings through the packed conversions (cvt.rn.f16x2.f32); returns the FP16
+// pairs as 32-bit words with x0 in the low half.
+__device__ __forceinline__ void split_hi_lo2(float x0, float x1, float c, uint32_t& hi2, uint32_t& lo2) {
+    const float a0 = x0 * c, a1 = x1 * c;
+    const __half2 h = __floats2half2_rn(a0, a1);
+    const float2 hf = __half22float2(h);
+    const __half2 l = __floats2half2_rn(a0 - hf.x, a1 - hf.y);
+    hi2 = *reinterpret_cast<const uint32_t*>(&h);
+    lo2 = *reinterpret_cast<const uint32_t*>(&l);
+}
+
 }  // namespace sp2

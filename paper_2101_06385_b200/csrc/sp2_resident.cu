@@ -265,11 +265,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
                     for (int c = 0; c < 32; ++c) {
                         const int j = c0 + c;
                         so[c] = __float_as_uint(sn[c]);
-                        __half h, l;
-                        split_hi_lo(sn[c], cs, h, l);
-                        const uint32_t hb = __half_as_ushort(h), lb = __half_as_ushort(l);
-                        if (c & 1) { hp[c >> 1] |= hb << 16; lp[c >> 1] |= lb << 16; }
-                        else { hp[c >> 1] = hb; lp[c >> 1] = lb; }
+                        if ((c & 1) == 0) split_hi_lo2(sn[c], sn[c + 1], cs, hp[c >> 1], lp[c >> 1]);
                         const float sq = (j < gi) ? sn[c] * sn[c] : 0.f;
                         if ((c & 3) == 0) q0 += sq; else if ((c & 3) == 1) q1 += sq;
                         else if ((c & 3) == 2) q2 += sq; else q3 += sq;

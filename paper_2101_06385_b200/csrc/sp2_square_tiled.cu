@@ -332,14 +332,17 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                     for (int g = 0; g < 4; ++g) {           // 8 columns at a time: values leave registers early
                         uint32_t hp[4], lp[4];              // FP16 pairs (even column in the low half)
 #pragma unroll
+                        float vals[8];
+#pragma unroll
+                        for (int e = 0; e < 8; ++e) vals[e] = fmaf(th1s, __uint_as_float(v[8 * g + e]), th2 * so[8 * g + e]);
+#pragma unroll
+                        for (int e = 0; e < 8; e += 2) split_hi_lo2(vals[e], vals[e + 1], cs, hp[e >> 1], lp[e >> 1]);
+#pragma unroll
                         for (int e = 0; e < 8; ++e) {
                             const int c = 8 * g + e;
-                            const float val = fmaf(th1s, __uint_as_float(v[c]), th2 * so[c]);
-                            __half h, l;
-                            split_hi_lo(val, cs, h, l);
-                            const uint32_t hb = __half_as_ushort(h), lb = __half_as_ushort(l);
-                            if (e & 1) { hp[e >> 1] |= hb << 16; lp[e >> 1] |= lb << 16; }
-                            else { hp[e >> 1] = hb; lp[e >> 1] = lb; }
+                            const float val = vals[e];
+                            const uint32_t hb = (hp[e >> 1] >> (16 * (e & 1))) & 0xffffu;
+                            const uint32_t lb = (lp[e >> 1] >> (16 * (e & 1))) & 0xffffu;
                             const float sq = val * val;
                             so[c] = sq;                     // column sums below: square of the mirrored entry
                             if ((e & 3) == 0) a0 += sq; else if ((e & 3) == 1) a1 += sq;
