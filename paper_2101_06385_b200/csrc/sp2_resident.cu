@@ -345,23 +345,35 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
             group_sync<CG>();
             tc_fence_after();
             // ---- a8: control (Alg. 1), evaluated redundantly by both CTAs from identical sums
-            if (threadIdx.x == 0) {
+            // Lane l < 8 CG of warp 0 fetches the partial sums of epilogue warp (l & 7) of CTA (l >> 3) (own shared
+            // memory or the peer's through DSMEM: all remote loads in flight at once), then a fixed xor-shuffle tree:
+            // the same order in both CTAs, so both take identical decisions.
+            if (warp == 0) {
                 double a = 0.0, b = 0.0, cX = 0.0;
-                for (uint32_t r = 0; r < (uint32_t)CG; ++r)
-                    for (int w = 0; w < 8; ++w) {
-                        if (r == rank) {
-                            a += sh->part[iter & 1][w][0]; b += sh->part[iter & 1][w][1]; cX += sh->part[iter & 1][w][2];
-                        } else {
-                            const uint32_t base = mapa_u32(smem_u32(&sh->part[iter & 1][w][0]), r);
-                            a += ld_cluster_f64(base); b += ld_cluster_f64(base + 8); cX += ld_cluster_f64(base + 16);
-                        }
+                if (lane < 8 * CG) {
+                    const uint32_t r = (uint32_t)lane >> 3;
+                    const int w = lane & 7;
+                    if (r == rank) {
+                        a = sh->part[iter & 1][w][0]; b = sh->part[iter & 1][w][1]; cX = sh->part[iter & 1][w][2];
+                    } else {
+                        const uint32_t base = mapa_u32(smem_u32(&sh->part[iter & 1][w][0]), r);
+                        a = ld_cluster_f64(base); b = ld_cluster_f64(base + 8); cX = ld_cluster_f64(base + 16);
                     }
-                CtrlCore* c = &sh->ctrl;
-                if (first) {
-                    c->N_S = a; c->fro2 = b;             // N_S = Tr[S_0]
-                    control_plan_next(c, stats_m, p.thetas);
-                } else {
-                    control_finish_layer(c, stats_m, p.thetas, a, b, cX);
+                }
+#pragma unroll
+                for (int o = 8; o > 0; o >>= 1) {
+                    a += __shfl_xor_sync(0xffffffffu, a, o);
+                    b += __shfl_xor_sync(0xffffffffu, b, o);
+                    cX += __shfl_xor_sync(0xffffffffu, cX, o);
+                }
+                if (lane == 0) {
+                    CtrlCore* c = &sh->ctrl;
+                    if (first) {
+                        c->N_S = a; c->fro2 = b;         // N_S = Tr[S_0]
+                        control_plan_next(c, stats_m, p.thetas);
+                    } else {
+                        control_finish_layer(c, stats_m, p.thetas, a, b, cX);
+                    }
                 }
             }
             __syncthreads();
