@@ -63,6 +63,21 @@ __device__ __forceinline__ uint32_t panel_off(int t, int j) {
                       (j & 7) * 2);
 }
 
+// Which 32-column chunks does the warp owning rows [row0, row0 + 31] finalise?  Every unordered pair {i, j} exactly
+// once.  Plain rule: the lower triangle (c0 <= row0).  With two CTAs that leaves CTA 1 (rows 128-255) 26 chunk tasks
+// and CTA 0 ten, so the block rows 192-255 x columns 0-127 is handed to CTA 0, which finalises it from its own
+// accumulator's transposed copy (rows 0-127, columns 192-255: the MMA computes the full square): 18 tasks each,
+// at most 3 per warp instead of 4.  Returns -1 not handled, 0 all 32 x 32 entries (off-diagonal), 1 diagonal chunk.
+template <int CG>
+__device__ __forceinline__ int chunk_kind(int row0, int c0) {
+    if (CG == 2) {
+        if (row0 < 128 && c0 >= 192) return 0;
+        if (row0 >= 192 && c0 < 128) return -1;
+    }
+    if (c0 > row0) return -1;
+    return c0 == row0 ? 1 : 0;
+}
+
 template <int CG>
 __device__ __forceinline__ void group_sync() {
     if (CG == 2) cluster_sync_all(); else __syncthreads();
@@ -143,11 +158,29 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
             __syncthreads();
             float Rrow = 0.f;
             if (warp < 8) {
-                for (int c0 = 0; c0 <= row0 + 31 && c0 < NP; c0 += 32) {
-                    if (((c0 >> 5) & 1) != hf) continue;
-                    // column partial sums in the load layout (lane = column), row sums after the transpose
+                for (int c0 = 0; c0 < NP; c0 += 32) {
+                    const int kind = chunk_kind<CG>(row0, c0);
+                    if (kind < 0 || ((c0 >> 5) & 1) != hf) continue;
                     __syncwarp();
                     float colp = 0.f;
+                    if (c0 > row0) {
+                        // transposed block: entry (gi, c0 + c) is read as H(c0 + c, gi) (lower triangle, reading C22);
+                        // lane = row already, the column sums go through the staging tile
+#pragma unroll 8
+                        for (int c = 0; c < 32; ++c) {
+                            const int j = c0 + c;
+                            float v = 0.f;
+                            if (gi < N && j < N) v = fabsf(__ldg(Hm + (size_t)j * N + gi));
+                            Rrow += v;
+                            stg[lane * 33 + c] = v;
+                        }
+                        __syncwarp();
+#pragma unroll 8
+                        for (int r = 0; r < 32; ++r) colp += stg[r * 33 + lane];
+                        sh->rcol[q][c0 + lane] = colp;
+                        continue;
+                    }
+                    // column partial sums in the load layout (lane = column), row sums after the transpose
 #pragma unroll 8
                     for (int r = 0; r < 32; ++r) {
                         const int i = row0 + r, j = c0 + lane;
@@ -226,17 +259,25 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
         while (true) {
             if (warp < 8) {
                 // ---- finalise the lower-triangle part of this thread's row: chunk by chunk
-                for (int c0 = 0; c0 <= row0 + 31 && c0 < NP; c0 += 32) {
-                    if (((c0 >> 5) & 1) != hf) continue;
+                for (int c0 = 0; c0 < NP; c0 += 32) {
+                    const int kind = chunk_kind<CG>(row0, c0);
+                    if (kind < 0 || ((c0 >> 5) & 1) != hf) continue;
+                    const bool upper = (c0 > row0);             // transposed block (columns beyond the rows)
                     float sn[32];
                     if (first) {
                         float hv[32];
-                        load_block_rows(Hm, N, row0, c0, stg, lane, hv);
+                        if (upper) {
+#pragma unroll 8
+                            for (int c = 0; c < 32; ++c)
+                                hv[c] = (gi < N && c0 + c < N) ? __ldg(Hm + (size_t)(c0 + c) * N + gi) : 0.f;
+                        } else {
+                            load_block_rows(Hm, N, row0, c0, stg, lane, hv);
+                        }
 #pragma unroll
                         for (int c = 0; c < 32; ++c) {
                             const int j = c0 + c;
                             float s = 0.f;
-                            if (gi < N && j <= gi) { s = w0 * hv[c]; if (j == gi) s += b0; }
+                            if (gi < N && (upper ? j < N : j <= gi)) { s = w0 * hv[c]; if (j == gi) s += b0; }
                             sn[c] = s;
                         }
                     } else {
@@ -266,7 +307,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
                         const int j = c0 + c;
                         so[c] = __float_as_uint(sn[c]);
                         if ((c & 1) == 0) split_hi_lo2(sn[c], sn[c + 1], cs, hp[c >> 1], lp[c >> 1]);
-                        const float sq = (j < gi) ? sn[c] * sn[c] : 0.f;
+                        const float sq = (upper || j < gi) ? sn[c] * sn[c] : 0.f;
                         if ((c & 3) == 0) q0 += sq; else if ((c & 3) == 1) q1 += sq;
                         else if ((c & 3) == 2) q2 += sq; else q3 += sq;
                         if (j == gi) {
@@ -276,7 +317,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
                     }
                     fro2 += 2.0 * (double)((q0 + q1) + (q2 + q3));
                     tmem_st_32x32(t_S + (uint32_t)c0, so);      // FP32 master (entries j > i are never read)
-                    const bool below = (c0 + 31 < row0);        // chunk strictly below the diagonal for the whole warp
+                    const bool below = (kind == 0);             // every entry of the chunk is off-diagonal and handled here
                     const uint32_t jr = (uint32_t)(c0 >> 7);    // CTA that owns rows c0..c0+31
                     if (below) {
 #pragma unroll
@@ -406,15 +447,16 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
 
         // ------------------------------------------------------------------ output: D = S_n, both triangles
         if (warp < 8) {
-            for (int c0 = 0; c0 <= row0 + 31 && c0 < NP; c0 += 32) {
-                if (((c0 >> 5) & 1) != hf) continue;
+            for (int c0 = 0; c0 < NP; c0 += 32) {
+                const int kind = chunk_kind<CG>(row0, c0);
+                if (kind < 0 || ((c0 >> 5) & 1) != hf) continue;
                 uint32_t vs[32];
                 tmem_ld_32x32(t_S + (uint32_t)c0, vs);
                 tmem_ld_wait();
 #pragma unroll
                 for (int c = 0; c < 32; ++c) {
                     const int j = c0 + c;
-                    if (gi < N && j <= gi) {
+                    if (gi < N && (c0 > row0 ? j < N : j <= gi)) {
                         const float v = __uint_as_float(vs[c]);
                         Dm[(size_t)j * N + gi] = v;      // mirrored position: coalesced across the warp
                         Dm[(size_t)gi * N + j] = v;
