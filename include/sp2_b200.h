@@ -102,7 +102,9 @@ size_t       sp2_workspace_bytes(int N_max, int batch_max, int max_layers);
 
 /* Alg. 1: H (N x N, leading dimension ldh >= N) -> D (leading dimension ldd >= N).
  * stats_host: [opts->max_layers] entries (may be NULL); n_layers: layers executed (may be NULL);
- * bounds_out[2]: the spectral bounds used (may be NULL).  0 <= N_occ <= N. */
+ * bounds_out[2]: the spectral bounds used (may be NULL).  0 <= N_occ <= N.
+ * N <= 256 with contiguous buffers (ldh == ldd == N) and default tile_config / control: solved by ONE launch of the
+ * batched path's resident kernel (the matrix stays on chip across all layers; exact_diag does not apply there). */
 sp2_status_t sp2_density_matrix(sp2_handle_t h, const float* H_dev, int N, int ldh, double N_occ,
                                 const sp2_opts_t* opts, float* D_dev, int ldd,
                                 sp2_layer_stat_t* stats_host, int* n_layers, double bounds_out[2],

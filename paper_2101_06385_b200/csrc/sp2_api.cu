@@ -126,8 +126,8 @@ extern "C" size_t sp2_workspace_bytes(int N_max, int batch_max, int max_layers) 
     b += 4 * Np * sizeof(double);                             // Gershgorin radii, diagonal, two row-sum vectors
     b += sizeof(Ctrl) + (size_t)max_layers * (sizeof(sp2_layer_stat_t) + kThetaStride * sizeof(double));
     b += 2 * ((Np / 128) * (Np / 128 + 1) / 2 + 1024) * sizeof(WorkItem);
-    if (batch_max > 0)
-        b += (size_t)batch_max * ((size_t)max_layers * sizeof(sp2_layer_stat_t) + 2 * sizeof(int) + 3 * sizeof(double));
+    b += (size_t)(batch_max > 0 ? batch_max : 1) *
+         ((size_t)max_layers * sizeof(sp2_layer_stat_t) + 2 * sizeof(int) + 3 * sizeof(double));
     return b;
 }
 
@@ -192,12 +192,13 @@ extern "C" sp2_status_t sp2_create(sp2_handle_t* out, int N_max, int batch_max, 
     A((void**)&h->items_dev[0], (size_t)h->items_cap * sizeof(WorkItem));
     A((void**)&h->items_dev[1], (size_t)h->items_cap * sizeof(WorkItem));
     A((void**)&h->obs_dev, 8 * sizeof(double));
-    if (batch_max > 0) {
-        A((void**)&h->bstats_dev, (size_t)batch_max * max_layers * sizeof(sp2_layer_stat_t));
-        A((void**)&h->bnl_dev, (size_t)batch_max * sizeof(int));
-        A((void**)&h->bstatus_dev, (size_t)batch_max * sizeof(int));
-        A((void**)&h->bbounds_dev, (size_t)batch_max * 2 * sizeof(double));
-        A((void**)&h->bnocc_dev, (size_t)batch_max * sizeof(double));
+    {   // at least one slot: single matrices of N <= 256 are solved by the resident kernel too
+        const size_t bm = (size_t)(batch_max > 0 ? batch_max : 1);
+        A((void**)&h->bstats_dev, bm * max_layers * sizeof(sp2_layer_stat_t));
+        A((void**)&h->bnl_dev, bm * sizeof(int));
+        A((void**)&h->bstatus_dev, bm * sizeof(int));
+        A((void**)&h->bbounds_dev, bm * 2 * sizeof(double));
+        A((void**)&h->bnocc_dev, bm * sizeof(double));
     }
     auto AH = [&](void** p, size_t bytes) {
         if (st != SP2_OK) return;
@@ -494,6 +495,10 @@ static sp2_status_t solve_single(sp2_handle_s* h, const float* H_dev, int N, int
     return SP2_OK;
 }
 
+static sp2_status_t resident_solve(sp2_handle_s* h, const float* H_dev, int N, int B, const double* N_occ,
+                                   int nocc_is_scalar, const sp2_opts_t& o, float* D_dev, sp2_layer_stat_t* stats_host,
+                                   int* n_layers, int* status_out, double* bounds_out, cudaStream_t st);
+
 extern "C" sp2_status_t sp2_density_matrix(sp2_handle_t h, const float* H_dev, int N, int ldh, double N_occ,
                                            const sp2_opts_t* opts, float* D_dev, int ldd,
                                            sp2_layer_stat_t* stats_host, int* n_layers, double bounds_out[2],
@@ -511,6 +516,15 @@ extern "C" sp2_status_t sp2_density_matrix(sp2_handle_t h, const float* H_dev, i
     if (o.accelerated) {
         if (!isfinite(o.homo) || !isfinite(o.lumo) || !(o.lumo > o.homo)) return SP2_ERR_INVALID_ARG;
         if (!o.auto_bounds && !(o.eps_min <= o.homo && o.lumo <= o.eps_max)) return SP2_ERR_INVALID_ARG;
+    }
+    if (N <= 256 && o.tile_config == TILE_AUTO && o.control == 0 && !o.accelerated && ldh == N && ldd == N) {
+        // small N: the whole solve in ONE launch of the resident kernel (matrix on chip across all layers) instead of
+        // one kernel per layer.  (exact_diag does not apply there: the diagonal comes from the tensor core.)
+        int nl = 0;
+        sp2_status_t s2 = resident_solve(h, H_dev, N, 1, &N_occ, 1, o, D_dev, stats_host, &nl, nullptr, bounds_out,
+                                         (cudaStream_t)stream);
+        if (n_layers) *n_layers = nl;
+        return s2;
     }
     return solve_single(h, H_dev, N, ldh, N_occ, MODE_STANDARD, &o, D_dev, ldd, stats_host, n_layers, bounds_out,
                         (cudaStream_t)stream);
@@ -672,21 +686,11 @@ extern "C" sp2_status_t sp2_generalized_wb(sp2_handle_t h, const float* H_dev, i
     return sp2_generalized(h, H_dev, N, ldh, th.data(), L, eps_min, eps_max, opts, X_L_dev, ldx, stats_host, stream);
 }
 
-extern "C" sp2_status_t sp2_density_matrix_batched(sp2_handle_t h, const float* H_dev, int N, int B,
-                                                   const double* N_occ, int nocc_is_scalar, const sp2_opts_t* opts,
-                                                   float* D_dev, sp2_layer_stat_t* stats_host, int* n_layers,
-                                                   int* status_out, void* stream) {
-    if (!h || !H_dev || !D_dev || !N_occ || N < 1 || B < 1) return SP2_ERR_INVALID_ARG;
-    if (N > 256) return SP2_ERR_UNSUPPORTED_N;
-    if (B > h->batch_max) return SP2_ERR_WORKSPACE;
-    sp2_opts_t o;
-    if (opts) o = *opts; else sp2_default_opts(&o);
-    if (o.max_layers < 1 || o.max_layers > h->max_layers) return SP2_ERR_INVALID_ARG;
-    if (!o.auto_bounds && !(o.eps_max > o.eps_min)) return SP2_ERR_BOUNDS_DEGENERATE;
-    if (o.accelerated) return SP2_ERR_INVALID_ARG;       // per-matrix HOMO/LUMO estimates: single-matrix call only
-    for (int i = 0; i < (nocc_is_scalar ? 1 : B); ++i)
-        if (!(N_occ[i] >= 0.0 && N_occ[i] <= (double)N)) return SP2_ERR_INVALID_ARG;
-    cudaStream_t st = (cudaStream_t)stream;
+// Shared body of the batched call and of small single matrices: B contiguous N x N problems, one resident-kernel launch.
+static sp2_status_t resident_solve(sp2_handle_s* h, const float* H_dev, int N, int B, const double* N_occ,
+                                   int nocc_is_scalar, const sp2_opts_t& o, float* D_dev, sp2_layer_stat_t* stats_host,
+                                   int* n_layers, int* status_out, double* bounds_out /*[B][2] or NULL*/,
+                                   cudaStream_t st) {
     int k = o.fp16_scale_log2;
     if (k < 0) k = 13;
     if (k > 14) return SP2_ERR_INVALID_ARG;
@@ -706,6 +710,8 @@ extern "C" sp2_status_t sp2_density_matrix_batched(sp2_handle_t h, const float* 
     if (stats_host)
         CK(cudaMemcpyAsync(stats_host, h->bstats_dev, (size_t)B * o.max_layers * sizeof(sp2_layer_stat_t),
                            cudaMemcpyDeviceToHost, st));
+    if (bounds_out)
+        CK(cudaMemcpyAsync(bounds_out, h->bbounds_dev, (size_t)B * 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
     CK(cudaGetLastError());
     h->last_launches = 1;
@@ -717,6 +723,24 @@ extern "C" sp2_status_t sp2_density_matrix_batched(sp2_handle_t h, const float* 
         else if (stt[i] > worst && worst >= 0) worst = stt[i];
     }
     return (sp2_status_t)worst;
+}
+
+extern "C" sp2_status_t sp2_density_matrix_batched(sp2_handle_t h, const float* H_dev, int N, int B,
+                                                   const double* N_occ, int nocc_is_scalar, const sp2_opts_t* opts,
+                                                   float* D_dev, sp2_layer_stat_t* stats_host, int* n_layers,
+                                                   int* status_out, void* stream) {
+    if (!h || !H_dev || !D_dev || !N_occ || N < 1 || B < 1) return SP2_ERR_INVALID_ARG;
+    if (N > 256) return SP2_ERR_UNSUPPORTED_N;
+    if (B > h->batch_max) return SP2_ERR_WORKSPACE;
+    sp2_opts_t o;
+    if (opts) o = *opts; else sp2_default_opts(&o);
+    if (o.max_layers < 1 || o.max_layers > h->max_layers) return SP2_ERR_INVALID_ARG;
+    if (!o.auto_bounds && !(o.eps_max > o.eps_min)) return SP2_ERR_BOUNDS_DEGENERATE;
+    if (o.accelerated) return SP2_ERR_INVALID_ARG;       // per-matrix HOMO/LUMO estimates: single-matrix call only
+    for (int i = 0; i < (nocc_is_scalar ? 1 : B); ++i)
+        if (!(N_occ[i] >= 0.0 && N_occ[i] <= (double)N)) return SP2_ERR_INVALID_ARG;
+    return resident_solve(h, H_dev, N, B, N_occ, nocc_is_scalar, o, D_dev, stats_host, n_layers, status_out, nullptr,
+                          (cudaStream_t)stream);
 }
 
 extern "C" sp2_status_t sp2_split_fp16(const float* X_dev, int N, int ldx, unsigned short* hi_dev,

@@ -251,9 +251,19 @@ def test_edge_cases_and_errors(env):
     # leading dimensions larger than N on both sides
     big = torch.zeros((128, 200), device="cuda"); big[:, :128] = Hd
     out = torch.full((128, 160), 7.0, device="cuda")
-    D2, _ = h.density_matrix(big[:, :128], 64.0, api.make_opts(bounds=(-1.0, 1.0), tol=1e-5, max_layers=60), out=out[:, :128])
-    D1, _ = h.density_matrix(Hd, 64.0, api.make_opts(bounds=(-1.0, 1.0), tol=1e-5, max_layers=60))
+    o1 = api.make_opts(bounds=(-1.0, 1.0), tol=1e-5, max_layers=60, tile_config=1)
+    D2, _ = h.density_matrix(big[:, :128], 64.0, o1, out=out[:, :128])
+    D1, i1 = h.density_matrix(Hd, 64.0, o1)
     assert torch.equal(D1, out[:, :128]) and float(out[:, 128:].min()) == 7.0
+    # small contiguous problems with default options take the one-launch resident kernel; strided ones the tiled
+    # kernels: same result within the arithmetic's noise, same branch sequence
+    o0 = api.make_opts(bounds=(-1.0, 1.0), tol=1e-5, max_layers=60)
+    D0, i0 = h.density_matrix(Hd, 64.0, o0)
+    D3, i3 = h.density_matrix(big[:, :128], 64.0, o0)
+    assert i0["launches"] == 1 and i3["launches"] > 1
+    k = min(i0["n_layers"], i3["n_layers"]) - 1
+    assert i0["sigma"][:k] == i3["sigma"][:k]
+    assert float((D0 - D3).abs().max()) <= 1e-5 and torch.equal(D0, D0.T)
 
 
 def test_host_buffer_entry_point_and_determinism(env):
