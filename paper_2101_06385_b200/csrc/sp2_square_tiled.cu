@@ -447,19 +447,38 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
         }
         if (lane == 0) { red[q][0] = trS; red[q][1] = fro2; red[q][2] = trX; }
         asm volatile("bar.sync 1, 128;\n" ::: "memory");     // the four epilogue warps only
-        if (warp == 2 && lane == 0) {
-            double a = 0.0, b = 0.0, c = 0.0;
-            for (int i = 0; i < 4; ++i) { a += red[i][0]; b += red[i][1]; c += red[i][2]; }
-            ctrl->partial[blockIdx.x][0] = a;
-            ctrl->partial[blockIdx.x][1] = b;
-            ctrl->partial[blockIdx.x][2] = c;
-            __threadfence();
-            const unsigned int done = atomicAdd(&ctrl->done_counter, 1u);
+        if (warp == 2) {
+            unsigned int done = 0;
+            if (lane == 0) {
+                double a = 0.0, b = 0.0, c = 0.0;
+                for (int i = 0; i < 4; ++i) { a += red[i][0]; b += red[i][1]; c += red[i][2]; }
+                ctrl->partial[blockIdx.x][0] = a;
+                ctrl->partial[blockIdx.x][1] = b;
+                ctrl->partial[blockIdx.x][2] = c;
+                __threadfence();
+                done = atomicAdd(&ctrl->done_counter, 1u);
+            }
+            done = __shfl_sync(0xffffffffu, done, 0);
             if (done == gridDim.x - 1) {
+                // last CTA: sum the per-CTA partials (each lane a strided subset in index order, then a fixed shuffle
+                // tree: deterministic for a given grid) and run the control step of Alg. 1
                 __threadfence();
-                control_after_layer(ctrl, p.stats, p.thetas, (int)gridDim.x);
-                __threadfence();
-                if (p.cond_handle != 0) cudaGraphSetConditional(p.cond_handle, ctrl->running ? 1u : 0u);
+                double a = 0.0, b = 0.0, c = 0.0;
+                for (unsigned int i = lane; i < gridDim.x; i += 32) {
+                    a += ((volatile double*)ctrl->partial[i])[0];
+                    b += ((volatile double*)ctrl->partial[i])[1];
+                    c += ((volatile double*)ctrl->partial[i])[2];
+                }
+                for (int o = 16; o > 0; o >>= 1) {
+                    a += __shfl_xor_sync(0xffffffffu, a, o);
+                    b += __shfl_xor_sync(0xffffffffu, b, o);
+                    c += __shfl_xor_sync(0xffffffffu, c, o);
+                }
+                if (lane == 0) {
+                    control_finish_layer(ctrl, p.stats, p.thetas, a, b, c);
+                    __threadfence();
+                    if (p.cond_handle != 0) cudaGraphSetConditional(p.cond_handle, ctrl->running ? 1u : 0u);
+                }
             }
         }
     }
