@@ -16,6 +16,9 @@
  *     them; inputs are never modified.  `stream` is a cudaStream_t passed as void* (NULL = default stream).
  *   - All work is enqueued on `stream`; each solve call ends with ONE cudaStreamSynchronize after copying
  *     the per-layer statistics back (no host round trip per layer).
+ *   - A handle serialises its own calls (one solve at a time per handle; use one handle per host thread / stream).
+ *     Tuning hooks read once at sp2_create from the environment (defaults in brackets): SP2_NOISE_KAPPA [0.125]
+ *     (reading C25), SP2_ROUND_SYNC [1], SP2_TAIL_SPLIT [1], SP2_ENH_KC [2] (DESIGN.md sections 6 and 9).
  *   - Return value: SP2_OK (0); > 0 = result written but flagged; < 0 = error, outputs undefined.
  *     No exceptions, no stdout.  There is no CPU fallback: without a CUDA device calls return SP2_ERR_CUDA.
  */

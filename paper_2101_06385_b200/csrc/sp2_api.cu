@@ -153,7 +153,6 @@ extern "C" sp2_status_t sp2_destroy(sp2_handle_t h) {
 
 extern "C" sp2_status_t sp2_create(sp2_handle_t* out, int N_max, int batch_max, int max_layers) {
     if (!out || N_max < 1 || batch_max < 0 || max_layers < 1 || max_layers > 4096) return SP2_ERR_INVALID_ARG;
-    if (batch_max > 0 && N_max > 256 && batch_max > 1) { /* batched problems are limited to N <= 256, checked per call */ }
     int dev = 0;
     CK(cudaGetDevice(&dev));
     cudaDeviceProp prop;
