@@ -42,6 +42,8 @@ struct CtrlCore {
     float  theta[4];                 // th1, th2, th3, c of the NEXT layer (FP32: the epilogue's arithmetic type)
     unsigned int done_counter;       // CTAs finished in the current kernel
     unsigned int round_counter;      // CTAs that reached a round boundary of the current layer kernel (round sync)
+    unsigned int round_sync_broken;  // a round wait timed out once (CTAs not co-resident): stop waiting in this solve
+    unsigned int pad_rs_;
 };
 struct Ctrl : CtrlCore {
     double partial[kMaxPartials][4]; // per-CTA {Tr S, ||S||_F^2, Tr X (diag), unused}

@@ -114,11 +114,14 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                 if (p.round_sync && round > 0 && round < n_rounds) {
                     __threadfence();
                     atomicAdd(&ctrl->round_counter, 1u);
-                    if (w < n_work) {
+                    if (w < n_work && *((volatile unsigned int*)&ctrl->round_sync_broken) == 0u) {
                         const unsigned int target = (unsigned int)round * gridDim.x;
                         unsigned int spins = 0;
                         while (*((volatile unsigned int*)&ctrl->round_counter) < target && ++spins < (1u << 16))
                             __nanosleep(64);
+                        // timed out: the grid is not co-resident (shared GPU); the sync is only an optimisation, so
+                        // give it up for the rest of this solve instead of paying the timeout at every boundary
+                        if (spins >= (1u << 16)) ctrl->round_sync_broken = 1u;
                     }
                 }
                 if (w >= n_work) break;
