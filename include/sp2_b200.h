@@ -16,11 +16,20 @@
  *     them; inputs are never modified.  `stream` is a cudaStream_t passed as void* (NULL = default stream).
  *   - All work is enqueued on `stream`; each solve call ends with ONE cudaStreamSynchronize after copying
  *     the per-layer statistics back (no host round trip per layer).
- *   - A handle serialises its own calls (one solve at a time per handle; use one handle per host thread / stream).
- *     Tuning hooks read once at sp2_create from the environment (defaults in brackets): SP2_NOISE_KAPPA [0.125]
- *     (reading C25), SP2_ROUND_SYNC [1], SP2_TAIL_SPLIT [1], SP2_ENH_KC [2] (DESIGN.md sections 6 and 9).
+ *   - A handle serialises its own calls (one solve at a time per handle; use one handle per host thread / stream)
+ *     and belongs to the device that was current at sp2_create; a call with another current device returns
+ *     SP2_ERR_INVALID_ARG.
+ *   - Every parameter that can change a RESULT is in sp2_opts_t.  The environment is read once, at sp2_create, for
+ *     three pure performance toggles only (results are bit-identical for any setting; defaults in brackets):
+ *     SP2_ROUND_SYNC [1] and SP2_ROUND_SYNC_SPINS [65536] (the round synchronisation of the layer kernel and the
+ *     bound of its wait), SP2_TAIL_SPLIT [1] (column strips for the last, partial round) -- DESIGN.md section 6.
  *   - Return value: SP2_OK (0); > 0 = result written but flagged; < 0 = error, outputs undefined.
  *     No exceptions, no stdout.  There is no CPU fallback: without a CUDA device calls return SP2_ERR_CUDA.
+ *   - Hang guard: every mbarrier wait inside the kernels is bounded (2^26 polls, seconds); a wait that runs out --
+ *     only a protocol bug or a faulted peer CTA can cause it -- executes `trap`.  The launch then fails with a
+ *     sticky CUDA error, the call returns SP2_ERR_CUDA and, as after any device-side fault, the CUDA context is
+ *     unusable for the caller.  (Built with -DSP2_DEBUG the kernel also prints the barrier to the device's stdout
+ *     first; release builds print nothing.)
  */
 #ifndef SP2_B200_H
 #define SP2_B200_H
@@ -73,7 +82,8 @@ typedef struct {
     int    fp16_scale_log2; /* k: the split is applied to 2^k S (exact rescale; 0 = Eq. 13 literally).
                                -1 = library default (13): keeps X1 out of FP16's subnormal range            */
     int    control;         /* 0: device-side loop in a CUDA graph (WHILE node); 1: host-stepped (debug:
-                               one sync per layer); 2: graph of max_layers guarded launches, no WHILE node   */
+                               one sync per layer); 2: max_layers plain stream launches of the layer kernel, each
+                               guarded on the device (a launch after convergence returns at once), no graph  */
     int    tile_config;     /* 0: choose by N; 1: 128x128 1-CTA; 2: 128x256 1-CTA; 3: 256x256 2-CTA;
                                4: 128x128 1-CTA with the enhanced accumulation of sp2_refine_energy in EVERY
                                layer (accuracy option, about 2x the time of 3 at large N)  */
@@ -90,18 +100,37 @@ typedef struct {
                                sp2_density_matrix only.  0 (default): Alg. 1.                                  */
     double homo, lumo;      /* estimates of the highest occupied / lowest unoccupied eigenvalue of H (energy
                                units), eps_min <= homo < lumo <= eps_max; they must bound the gap from inside:
-                               homo >= true HOMO, lumo <= true LUMO ("prior knowledge")                  */
+                               homo >= true HOMO, lumo <= true LUMO ("prior knowledge").  The batched
+                               call takes per-matrix estimates through its own arguments instead.             */
+    double noise_kappa;     /* kappa of the noise-floor stop (reading C25: Alg. 1's "IdErr_n <= 0", P:136,
+                               at the resolution of the arithmetic): stop after layer n > 2 when
+                               IdErr_n <= kappa |Tr X_n(tensor core) - N_X(FP64)|.  < 0: library default (0.125);
+                               0: test disabled (Alg. 1's printed tests, tol and max_layers only)              */
+    int    enh_kc;          /* enhanced accumulation (tile_config 4, sp2_refine_energy): K-blocks of 64 the tensor
+                               core accumulates before the chunk sum is folded into the error-free FP32 pair
+                               (DESIGN.md section 9).  <= 0: library default (2 = 128 values of K)       */
+    double trunc_tau;       /* blocked-sparse variant for decaying matrices (DESIGN.md section 9 NEXT-4):
+                               > 0: before every square, 128 x 128 blocks of S with Frobenius norm <= trunc_tau are
+                               set to zero and their tensor-core work is skipped.  0 (default): dense.
+                               sp2_density_matrix with tile_config 0 or 1 only.                               */
 } sp2_opts_t;
 
 /* Fill *o with defaults: auto_bounds=1, tol=0, max_layers=120, eps_alt=0, fp16_scale_log2=-1, control=0,
- * tile_config=0, exact_diag=1, accelerated=0, homo=lumo=0. */
+ * tile_config=0, exact_diag=1, accelerated=0, homo=lumo=0, noise_kappa=-1, enh_kc=0, trunc_tau=0. */
 void sp2_default_opts(sp2_opts_t* o);
 
 /* Create a handle able to solve one matrix up to N_max, or a batch of batch_max matrices of N <= 256,
- * with at most max_layers layers.  Allocates device workspace (sp2_workspace_bytes). */
+ * with at most max_layers layers.  Allocates the device workspace up front: sp2_workspace_bytes() bytes.
+ * Three more allocations happen lazily, on the first call that needs them, and stay with the handle:
+ * sp2_generalized_mix's running sum (Np (Np + 32) floats, Np = N_max rounded up to 256), the two device staging
+ * matrices of sp2_density_matrix_host (2 N^2 floats of the largest N seen), and the blocked-sparse variant's block
+ * norms (a few KB).  sp2_workspace_bytes_lazy() returns their total for a given N_max.  The handle also caches one
+ * instantiated CUDA graph per distinct (N, tile configuration, scale, flags); the cache is emptied when it reaches
+ * 16 entries. */
 sp2_status_t sp2_create(sp2_handle_t* h, int N_max, int batch_max, int max_layers);
 sp2_status_t sp2_destroy(sp2_handle_t h);
 size_t       sp2_workspace_bytes(int N_max, int batch_max, int max_layers);
+size_t       sp2_workspace_bytes_lazy(int N_max);
 
 /* Alg. 1: H (N x N, leading dimension ldh >= N) -> D (leading dimension ldd >= N).
  * stats_host: [opts->max_layers] entries (may be NULL); n_layers: layers executed (may be NULL);
@@ -133,7 +162,7 @@ sp2_status_t sp2_generalized(sp2_handle_t h, const float* H_dev, int N, int ldh,
  * E_n = th_{n,1} E_{n-1}^2 + th_{n,2} E_{n-1} + th_{n,3} I  (Eq. 17).  F~ then decreases with energy like the Fermi
  * function of Eq. 20.  theta_host = [L][3], c_host = [L+1] (c_0 weights E_0).  The sum is accumulated in FP32 by the layer epilogues
  * (one more N x N workspace matrix, allocated on the first call).  F_dev: N x N, leading dimension ldf.
- * tile_config 2 is not available for this call. */
+ * tile_config 2 and 4 are not available for this call (SP2_ERR_INVALID_ARG). */
 sp2_status_t sp2_generalized_mix(sp2_handle_t h, const float* H_dev, int N, int ldh, const double* theta_host,
                                  const double* c_host, int L, double eps_min, double eps_max,
                                  const sp2_opts_t* opts, float* F_dev, int ldf, sp2_layer_stat_t* stats_host,
@@ -153,25 +182,38 @@ sp2_status_t sp2_generalized_wb(sp2_handle_t h, const float* H_dev, int N, int l
  *     last_sigma = -1:  D' = 2 S^2 - S^4          last_sigma = +1:  D' = (2 S - S^2)^2
  * (the alternation is continued from the last applied sign: DESIGN.md reading C15) in enhanced precision --
  * "single precision with double accumulation": FP16 hi/lo operands as in Eq. 15, but the tensor core
- * accumulates only 512 values of K at a time and the chunk sums are added in an error-free FP32 pair -- and the
- * observables Tr[X H], Tr[X], IdErr = Tr[X - X^2] of X = S (in) and X = D' (out), in FP64.
- * H: the Hamiltonian (lower triangle read).  S_dev may equal D_dev. */
+ * accumulates only opts->enh_kc K-blocks (default 2 = 128 values of K) at a time and the chunk sums are added in an
+ * error-free FP32 pair -- and the observables Tr[X H], Tr[X], IdErr = Tr[X - X^2] of X = S (in) and X = D' (out), in
+ * FP64.  H: the Hamiltonian (lower triangle read).  S_dev may equal D_dev.  opts may be NULL (defaults); only
+ * fp16_scale_log2 and enh_kc are read. */
 typedef struct {
     double energy_in, trace_in, iderr_in;
     double energy_out, trace_out, iderr_out;
 } sp2_refine_result_t;
 sp2_status_t sp2_refine_energy(sp2_handle_t h, const float* S_dev, int N, int lds, int last_sigma,
-                               const float* H_dev, int ldh, float* D_dev, int ldd,
+                               const float* H_dev, int ldh, const sp2_opts_t* opts, float* D_dev, int ldd,
                                sp2_refine_result_t* result, void* stream);
 
 /* Batched small-N: B independent matrices H[B][N][N] (contiguous, N <= 256), one launch, one CTA
  * cluster per matrix, per-matrix branch sequence and stop layer.  N_occ: [B] values, or one value if
- * nocc_is_scalar.  stats_host: [B][opts->max_layers] (may be NULL); n_layers: [B]; status_out: [B] per-matrix
- * sp2_status_t (may be NULL).  Returns the worst per-matrix status. */
+ * nocc_is_scalar.  homo_lumo: NULL, or -- with opts->accelerated = 1 -- [B][2] per-matrix HOMO / LUMO estimates in
+ * energy units for the accelerated weights of section V.A (repeated small solves in molecular dynamics,
+ * P:226, are that scheme's use case); opts->homo / lumo are not read by this call.  stats_host:
+ * [B][opts->max_layers] (may be NULL); n_layers: [B]; status_out: [B] per-matrix sp2_status_t (may be NULL).
+ * Returns the worst per-matrix status. */
 sp2_status_t sp2_density_matrix_batched(sp2_handle_t h, const float* H_dev, int N, int B,
-                                        const double* N_occ, int nocc_is_scalar, const sp2_opts_t* opts,
-                                        float* D_dev, sp2_layer_stat_t* stats_host, int* n_layers,
-                                        int* status_out, void* stream);
+                                        const double* N_occ, int nocc_is_scalar, const double* homo_lumo,
+                                        const sp2_opts_t* opts, float* D_dev, sp2_layer_stat_t* stats_host,
+                                        int* n_layers, int* status_out, void* stream);
+
+/* The generalized network (Eq. 17) on a batch of small matrices: the same L layers
+ * S_n = th1 S_{n-1}^2 + th2 S_{n-1} + th3 I (theta_host = [L][3], shared by the batch) applied to each of the B
+ * inputs H[B][N][N] (N <= 256), one launch.  eps_min >= eps_max -> per-matrix Gershgorin bounds.  X_L_dev:
+ * [B][N][N]; stats_host: [B][L] (may be NULL); status_out: [B] (may be NULL).  opts may be NULL; only
+ * fp16_scale_log2 is read. */
+sp2_status_t sp2_generalized_batched(sp2_handle_t h, const float* H_dev, int N, int B, const double* theta_host,
+                                     int L, double eps_min, double eps_max, const sp2_opts_t* opts,
+                                     float* X_L_dev, sp2_layer_stat_t* stats_host, int* status_out, void* stream);
 
 /* Stand-alone pieces of the path (rows a1, a3 of DESIGN.md), asynchronous on `stream` except where noted. */
 /* Eqs. 12-13: hi = FP16[2^k X], lo = FP16[2^k X - hi]; X N x N (ldx), hi/lo N x N (ldo), as uint16 bits */
@@ -185,6 +227,9 @@ const char* sp2_last_cuda_error(void);
 /* Number of kernels the last solve call on this handle launched (graph nodes executed are counted by the
  * device-side layer counter: setup kernels + layers + copy-out). */
 int         sp2_last_launch_count(sp2_handle_t h);
+/* Diagnostic: 1 if, during the last single-matrix solve on this handle, a round-synchronisation wait of the layer
+ * kernel ran out and the kernel gave the synchronisation up (performance only: results are unaffected). */
+int         sp2_last_round_sync_broken(sp2_handle_t h);
 const char* sp2_version(void);
 
 #ifdef __cplusplus

@@ -166,9 +166,12 @@ def scalar_initial(eigs, eps_min, eps_max):
     return (eps_max - np.asarray(eigs, dtype=np.float64)) / (eps_max - eps_min)
 
 
-def scalar_recursion(eigs, N_occ, eps_min, eps_max, tol=0.0, max_layers=120, eps_alt=0.0, forced_sigma=None):
+def scalar_recursion(eigs, N_occ, eps_min, eps_max, tol=0.0, max_layers=120, eps_alt=0.0, forced_sigma=None,
+                     square=None):
     """Alg. 1 on the eigenvalues: lambda_j^(i) = lambda_j^(i-1) + sigma_i (lambda_j^(i-1) - (lambda_j^(i-1))^2)
-    (P:294), with N_S = sum lambda, N_X = sum lambda^2.  Same outputs as sp2_ref minus the matrix."""
+    (P:294), with N_S = sum lambda, N_X = sum lambda^2.  Same outputs as sp2_ref minus the matrix.
+    `square` replaces the elementwise activation like sp2_ref's hook (default: lam * lam); the stop-rule pins use
+    it to put a chosen error on one layer's X."""
     lam = scalar_initial(eigs, eps_min, eps_max)
     N_S = float(lam.sum())
     sig = [0]
@@ -177,7 +180,7 @@ def scalar_recursion(eigs, N_occ, eps_min, eps_max, tol=0.0, max_layers=120, eps
     n, stop = 0, STOP_NONE
     while stop == STOP_NONE:
         n += 1
-        x = lam * lam
+        x = (lam * lam) if square is None else square(lam)
         N_X = float(x.sum())
         iderr = N_S - N_X
         sigma, d = _sign_rule(N_S, N_X, N_occ, sig[n - 1], eps_alt)

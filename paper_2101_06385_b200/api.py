@@ -17,10 +17,11 @@ SP2_OK, SP2_NOT_CONVERGED = 0, 1
 STOP_NAMES = {0: "none", 1: "iderr<=0", 2: "param_free", 3: "tol", 4: "max_layers", 5: "nonfinite", 6: "noise_floor"}
 TILE_AUTO, TILE_128x128, TILE_128x256, TILE_256x256_PAIR, TILE_128x128_ENH = 0, 1, 2, 3, 4
 
-EXPORTS = ["sp2_default_opts", "sp2_create", "sp2_destroy", "sp2_workspace_bytes", "sp2_density_matrix",
-           "sp2_density_matrix_host", "sp2_generalized", "sp2_generalized_mix", "sp2_generalized_wb", "sp2_density_matrix_batched",
-           "sp2_refine_energy", "sp2_split_fp16", "sp2_gershgorin", "sp2_status_string", "sp2_last_cuda_error",
-           "sp2_last_launch_count", "sp2_version"]
+EXPORTS = ["sp2_default_opts", "sp2_create", "sp2_destroy", "sp2_workspace_bytes", "sp2_workspace_bytes_lazy",
+           "sp2_density_matrix", "sp2_density_matrix_host", "sp2_generalized", "sp2_generalized_mix", "sp2_generalized_wb",
+           "sp2_density_matrix_batched", "sp2_generalized_batched", "sp2_refine_energy", "sp2_split_fp16",
+           "sp2_gershgorin", "sp2_status_string", "sp2_last_cuda_error", "sp2_last_launch_count",
+           "sp2_last_round_sync_broken", "sp2_version"]
 
 
 class LayerStat(C.Structure):
@@ -32,7 +33,8 @@ class Opts(C.Structure):
     _fields_ = [("auto_bounds", C.c_int), ("eps_min", C.c_double), ("eps_max", C.c_double), ("tol", C.c_double),
                 ("max_layers", C.c_int), ("eps_alt", C.c_double), ("fp16_scale_log2", C.c_int),
                 ("control", C.c_int), ("tile_config", C.c_int), ("exact_diag", C.c_int), ("accelerated", C.c_int),
-                ("homo", C.c_double), ("lumo", C.c_double)]
+                ("homo", C.c_double), ("lumo", C.c_double), ("noise_kappa", C.c_double), ("enh_kc", C.c_int),
+                ("trunc_tau", C.c_double)]
 
 
 class RefineResult(C.Structure):
@@ -67,6 +69,7 @@ def load() -> C.CDLL:
     lib.sp2_create.argtypes = [C.POINTER(vp), C.c_int, C.c_int, C.c_int]; lib.sp2_create.restype = C.c_int
     lib.sp2_destroy.argtypes = [vp]; lib.sp2_destroy.restype = C.c_int
     lib.sp2_workspace_bytes.argtypes = [C.c_int, C.c_int, C.c_int]; lib.sp2_workspace_bytes.restype = C.c_size_t
+    lib.sp2_workspace_bytes_lazy.argtypes = [C.c_int]; lib.sp2_workspace_bytes_lazy.restype = C.c_size_t
     lib.sp2_density_matrix.argtypes = [vp, vp, C.c_int, C.c_int, C.c_double, C.POINTER(Opts), vp, C.c_int,
                                        C.POINTER(LayerStat), ip, dp, vp]
     lib.sp2_density_matrix.restype = C.c_int
@@ -81,10 +84,13 @@ def load() -> C.CDLL:
     lib.sp2_generalized_wb.argtypes = [vp, vp, C.c_int, C.c_int, ip, dp, dp, C.c_int, C.c_double, C.c_double,
                                        C.POINTER(Opts), vp, C.c_int, C.POINTER(LayerStat), vp]
     lib.sp2_generalized_wb.restype = C.c_int
-    lib.sp2_density_matrix_batched.argtypes = [vp, vp, C.c_int, C.c_int, dp, C.c_int, C.POINTER(Opts), vp,
+    lib.sp2_density_matrix_batched.argtypes = [vp, vp, C.c_int, C.c_int, dp, C.c_int, dp, C.POINTER(Opts), vp,
                                                C.POINTER(LayerStat), ip, ip, vp]
     lib.sp2_density_matrix_batched.restype = C.c_int
-    lib.sp2_refine_energy.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int, vp, C.c_int, vp, C.c_int,
+    lib.sp2_generalized_batched.argtypes = [vp, vp, C.c_int, C.c_int, dp, C.c_int, C.c_double, C.c_double,
+                                            C.POINTER(Opts), vp, C.POINTER(LayerStat), ip, vp]
+    lib.sp2_generalized_batched.restype = C.c_int
+    lib.sp2_refine_energy.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int, vp, C.c_int, C.POINTER(Opts), vp, C.c_int,
                                       C.POINTER(RefineResult), vp]
     lib.sp2_refine_energy.restype = C.c_int
     lib.sp2_split_fp16.argtypes = [vp, C.c_int, C.c_int, vp, vp, C.c_int, C.c_int, vp]
@@ -93,6 +99,7 @@ def load() -> C.CDLL:
     lib.sp2_status_string.argtypes = [C.c_int]; lib.sp2_status_string.restype = C.c_char_p
     lib.sp2_last_cuda_error.argtypes = []; lib.sp2_last_cuda_error.restype = C.c_char_p
     lib.sp2_last_launch_count.argtypes = [vp]; lib.sp2_last_launch_count.restype = C.c_int
+    lib.sp2_last_round_sync_broken.argtypes = [vp]; lib.sp2_last_round_sync_broken.restype = C.c_int
     lib.sp2_version.argtypes = []; lib.sp2_version.restype = C.c_char_p
     _lib = lib
     return lib
@@ -119,7 +126,7 @@ def _stats_to_dict(stats, n):
 
 
 def make_opts(bounds=None, tol=0.0, max_layers=120, eps_alt=0.0, fp16_scale_log2=-1, control=0, tile_config=0,
-              exact_diag=1, homo_lumo=None) -> Opts:
+              exact_diag=1, homo_lumo=None, noise_kappa=-1.0, enh_kc=0, trunc_tau=0.0, accelerated=None) -> Opts:
     o = Opts()
     load().sp2_default_opts(C.byref(o))
     if bounds is not None:
@@ -127,8 +134,11 @@ def make_opts(bounds=None, tol=0.0, max_layers=120, eps_alt=0.0, fp16_scale_log2
     o.tol, o.max_layers, o.eps_alt = float(tol), int(max_layers), float(eps_alt)
     o.fp16_scale_log2, o.control, o.tile_config = int(fp16_scale_log2), int(control), int(tile_config)
     o.exact_diag = int(exact_diag)
+    o.noise_kappa, o.enh_kc, o.trunc_tau = float(noise_kappa), int(enh_kc), float(trunc_tau)
     if homo_lumo is not None:        # accelerated Deep-NN SP2 (section V.A)
         o.accelerated, o.homo, o.lumo = 1, float(homo_lumo[0]), float(homo_lumo[1])
+    if accelerated is not None:      # batched call: the estimates travel as a per-matrix array
+        o.accelerated = int(accelerated)
     return o
 
 
@@ -271,7 +281,7 @@ class Handle:
         return X, info
 
     # -- final refinement + energy (Eq. 16)
-    def refine_energy(self, S, last_sigma: int, H, out=None, stream=None):
+    def refine_energy(self, S, last_sigma: int, H, out=None, stream=None, opts: Optional[Opts] = None):
         """D' = f_final(S) in enhanced precision and the observables of S and D' against H."""
         import torch
 
@@ -281,13 +291,15 @@ class Handle:
         D = torch.empty((N, N), dtype=torch.float32, device=S.device) if out is None else _dev_f32(out, "out")
         res = RefineResult()
         st = self.lib.sp2_refine_energy(self._h, S.data_ptr(), N, S.stride(0), int(last_sigma), H.data_ptr(),
-                                        H.stride(0), D.data_ptr(), D.stride(0), C.byref(res), _stream_ptr(stream))
+                                        H.stride(0), C.byref(opts) if opts is not None else None, D.data_ptr(),
+                                        D.stride(0), C.byref(res), _stream_ptr(stream))
         if st < 0:
             raise SP2Error(st, "sp2_refine_energy")
         return D, {k: getattr(res, k) for k, _ in RefineResult._fields_}
 
     # -- batched small-N
-    def density_matrix_batched(self, H, N_occ, opts: Optional[Opts] = None, out=None, stream=None):
+    def density_matrix_batched(self, H, N_occ, opts: Optional[Opts] = None, out=None, stream=None, homo_lumo=None):
+        """homo_lumo: None, or a [B, 2] array of per-matrix HOMO / LUMO estimates (accelerated weights, section V.A)."""
         import torch
 
         H = _dev_f32(H, "H")
@@ -298,17 +310,46 @@ class Handle:
         D = torch.empty_like(H) if out is None else out
         scalar = np.isscalar(N_occ)
         nocc = np.ascontiguousarray([N_occ] if scalar else N_occ, dtype=np.float64)
+        hl = None
+        if homo_lumo is not None:
+            hl = np.ascontiguousarray(homo_lumo, dtype=np.float64)
+            if hl.shape != (B, 2):
+                raise ValueError("homo_lumo must have shape [B, 2]")
+            opts.accelerated = 1
         stats = (LayerStat * (B * opts.max_layers))()
         nl = (C.c_int * B)()
         status = (C.c_int * B)()
         st = self.lib.sp2_density_matrix_batched(self._h, H.data_ptr(), N, B, nocc.ctypes.data_as(C.POINTER(C.c_double)),
-                                                 1 if scalar else 0, C.byref(opts), D.data_ptr(), stats, nl, status,
-                                                 _stream_ptr(stream))
+                                                 1 if scalar else 0,
+                                                 None if hl is None else hl.ctypes.data_as(C.POINTER(C.c_double)),
+                                                 C.byref(opts), D.data_ptr(), stats, nl, status, _stream_ptr(stream))
         if st < 0:
             raise SP2Error(st, "sp2_density_matrix_batched")
         n_layers = np.frombuffer(nl, dtype=np.int32).copy()
         return D, {"status": st, "n_layers": n_layers, "per_status": np.frombuffer(status, dtype=np.int32).copy(),
                    "stats": stats, "max_layers": opts.max_layers}
+
+    def generalized_batched(self, H, theta: np.ndarray, bounds=None, opts: Optional[Opts] = None, out=None, stream=None):
+        """The same L generalized layers (theta [L][3]) applied to each matrix of H [B, N, N], N <= 256."""
+        import torch
+
+        H = _dev_f32(H, "H")
+        if H.dim() != 3 or not H.is_contiguous():
+            raise TypeError("H must be a contiguous [B, N, N] CUDA float32 tensor")
+        B, N = H.shape[0], H.shape[1]
+        theta = np.ascontiguousarray(theta, dtype=np.float64)
+        L = theta.shape[0]
+        X = torch.empty_like(H) if out is None else out
+        stats = (LayerStat * (B * L))()
+        status = (C.c_int * B)()
+        e0, e1 = (0.0, 0.0) if bounds is None else (float(bounds[0]), float(bounds[1]))
+        st = self.lib.sp2_generalized_batched(self._h, H.data_ptr(), N, B, theta.ctypes.data_as(C.POINTER(C.c_double)),
+                                              L, e0, e1, C.byref(opts) if opts is not None else None, X.data_ptr(),
+                                              stats, status, _stream_ptr(stream))
+        if st < 0:
+            raise SP2Error(st, "sp2_generalized_batched")
+        return X, {"status": st, "per_status": np.frombuffer(status, dtype=np.int32).copy(), "stats": stats,
+                   "max_layers": L, "n_layers": np.full(B, L, dtype=np.int32)}
 
     def gershgorin(self, H, stream=None):
         H = _dev_f32(H, "H")

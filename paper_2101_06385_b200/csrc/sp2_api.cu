@@ -44,7 +44,7 @@ struct sp2_handle_s {
     // single-matrix workspace
     float* S = nullptr;
     __half* hl[2][2] = {{nullptr, nullptr}, {nullptr, nullptr}};   // [ping-pong][hi, lo]
-    double* R = nullptr;
+    float* gpart = nullptr;         // Gershgorin: per-tile row / column sums (gershgorin_part_floats)
     double* diag = nullptr;
     unsigned long long* rowsq[2] = {nullptr, nullptr};   // fixed-point row sums of squares of S (ping-pong)
     Ctrl* ctrl = nullptr;
@@ -58,6 +58,7 @@ struct sp2_handle_s {
     int* bstatus_dev = nullptr;
     double* bbounds_dev = nullptr;
     double* bnocc_dev = nullptr;
+    double* bhl_dev = nullptr;      // [batch][2] HOMO / LUMO estimates of the accelerated batched solve
     // pinned host mirrors
     Ctrl* ctrl_host = nullptr;
     sp2_layer_stat_t* stats_host = nullptr;
@@ -68,7 +69,8 @@ struct sp2_handle_s {
     float* stage_D = nullptr;
     size_t stage_elems = 0;
     PFN_encodeTiled encode = nullptr;
-    std::map<std::tuple<int, int, int, int, int>, LoopGraph> graphs;   // (N, Np, cfg, scale_log2, exact_diag | mix << 1)
+    // (N, Np, cfg, scale_log2, exact_diag | mix << 1 | enh_kc << 2): everything a captured launch bakes in
+    std::map<std::tuple<int, int, int, int, int>, LoopGraph> graphs;
     int items_key_np[2] = {-1, -1}, items_key_cfg[2] = {-1, -1}, items_key_split[2] = {-1, -1};
     int n_items[2] = {0, 0}, n_slots[2] = {0, 0};
     float* mix = nullptr;           // output mix M = sum_i c_i S_i (Eq. 18), allocated on first use
@@ -76,9 +78,8 @@ struct sp2_handle_s {
     double* obs_host = nullptr;
     int tail_split = 1;
     int last_launches = 0;
-    double noise_kappa = 0.125;
     int round_sync = 1;
-    int enh_kc = 2;
+    unsigned int round_spins = 1u << 16;
     cudaStream_t cap_stream = nullptr;
 };
 
@@ -117,18 +118,34 @@ extern "C" void sp2_default_opts(sp2_opts_t* o) {
     o->accelerated = 0;
     o->homo = 0.0;
     o->lumo = 0.0;
+    o->noise_kappa = -1.0;
+    o->enh_kc = 0;
+    o->trunc_tau = 0.0;
 }
+
+static double opt_kappa(const sp2_opts_t& o) { return o.noise_kappa < 0.0 ? 0.125 : o.noise_kappa; }
+static int opt_enh_kc(const sp2_opts_t* o) { return (o && o->enh_kc > 0) ? o->enh_kc : 2; }
 
 extern "C" size_t sp2_workspace_bytes(int N_max, int batch_max, int max_layers) {
     if (N_max < 1 || max_layers < 1) return 0;
     const size_t Np = (size_t)round_up(N_max, 256);
     size_t b = Np * (size_t)ws_ld_f32((int)Np) * 4 + 4 * Np * (size_t)ws_ld_f16((int)Np) * 2;   // S + two hi/lo pairs
-    b += 4 * Np * sizeof(double);                             // Gershgorin radii, diagonal, two row-sum vectors
+    b += gershgorin_part_floats((int)Np) * 4;                 // Gershgorin per-tile sums
+    b += 3 * Np * sizeof(double);                             // diagonal, two row-sum vectors
     b += sizeof(Ctrl) + (size_t)max_layers * (sizeof(sp2_layer_stat_t) + kThetaStride * sizeof(double));
     b += 2 * ((Np / 128) * (Np / 128 + 1) / 2 + 1024) * sizeof(WorkItem);
     b += (size_t)(batch_max > 0 ? batch_max : 1) *
-         ((size_t)max_layers * sizeof(sp2_layer_stat_t) + 2 * sizeof(int) + 3 * sizeof(double));
+         ((size_t)max_layers * sizeof(sp2_layer_stat_t) + 2 * sizeof(int) + 5 * sizeof(double));
     return b;
+}
+
+// Allocations made on first use (see the header): the output-mix matrix, the two staging matrices of the host entry
+// point at N = N_max, the block norms of the blocked-sparse variant.
+extern "C" size_t sp2_workspace_bytes_lazy(int N_max) {
+    if (N_max < 1) return 0;
+    const size_t Np = (size_t)round_up(N_max, 256);
+    const size_t nb = Np / 128;
+    return Np * (size_t)ws_ld_f32((int)Np) * 4 + 2 * (size_t)N_max * (size_t)N_max * 4 + 2 * nb * nb * sizeof(double);
 }
 
 extern "C" sp2_status_t sp2_destroy(sp2_handle_t h) {
@@ -142,9 +159,9 @@ extern "C" sp2_status_t sp2_destroy(sp2_handle_t h) {
     for (int a = 0; a < 2; ++a)
         for (int b = 0; b < 2; ++b) cudaFree(h->hl[a][b]);
     cudaFree(h->rowsq[0]); cudaFree(h->rowsq[1]);
-    cudaFree(h->R); cudaFree(h->diag); cudaFree(h->ctrl); cudaFree(h->stats_dev); cudaFree(h->thetas_dev);
+    cudaFree(h->gpart); cudaFree(h->diag); cudaFree(h->ctrl); cudaFree(h->stats_dev); cudaFree(h->thetas_dev);
     cudaFree(h->items_dev[0]); cudaFree(h->items_dev[1]); cudaFree(h->obs_dev); cudaFree(h->mix); cudaFreeHost(h->obs_host); cudaFree(h->bstats_dev); cudaFree(h->bnl_dev); cudaFree(h->bstatus_dev);
-    cudaFree(h->bbounds_dev); cudaFree(h->bnocc_dev);
+    cudaFree(h->bbounds_dev); cudaFree(h->bnocc_dev); cudaFree(h->bhl_dev);
     cudaFreeHost(h->ctrl_host); cudaFreeHost(h->stats_host); cudaFreeHost(h->thetas_host);
     cudaFreeHost(h->bounds_host); cudaFree(h->stage_H); cudaFree(h->stage_D);
     delete h;
@@ -164,10 +181,10 @@ extern "C" sp2_status_t sp2_create(sp2_handle_t* out, int N_max, int batch_max, 
     }
     sp2_handle_s* h = new sp2_handle_s();
     h->N_max = N_max; h->batch_max = batch_max; h->max_layers = max_layers;
-    if (const char* e = getenv("SP2_NOISE_KAPPA")) h->noise_kappa = atof(e);   // tuning hook (C25)
-    if (const char* e = getenv("SP2_TAIL_SPLIT")) h->tail_split = atoi(e);     // tuning hook
-    if (const char* e = getenv("SP2_ENH_KC")) { h->enh_kc = atoi(e); if (h->enh_kc < 1) h->enh_kc = 1; }   // tuning hook
-    if (const char* e = getenv("SP2_ROUND_SYNC")) h->round_sync = atoi(e);     // tuning hook
+    // performance toggles only (results are bit-identical for any setting)
+    if (const char* e = getenv("SP2_TAIL_SPLIT")) h->tail_split = atoi(e);
+    if (const char* e = getenv("SP2_ROUND_SYNC")) h->round_sync = atoi(e);
+    if (const char* e = getenv("SP2_ROUND_SYNC_SPINS")) { const long v = atol(e); h->round_spins = v < 1 ? 1u : (unsigned int)v; }
     h->Np_max = round_up(N_max, 256);
     h->num_sms = prop.multiProcessorCount; h->device = dev;
     const size_t Np = (size_t)h->Np_max;
@@ -180,7 +197,7 @@ extern "C" sp2_status_t sp2_create(sp2_handle_t* out, int N_max, int batch_max, 
     A((void**)&h->S, Np * (size_t)ws_ld_f32(h->Np_max) * 4);
     for (int a = 0; a < 2; ++a)
         for (int b = 0; b < 2; ++b) A((void**)&h->hl[a][b], Np * (size_t)ws_ld_f16(h->Np_max) * 2);
-    A((void**)&h->R, Np * sizeof(double));
+    A((void**)&h->gpart, gershgorin_part_floats(h->Np_max) * sizeof(float));
     A((void**)&h->diag, Np * sizeof(double));
     A((void**)&h->rowsq[0], Np * sizeof(unsigned long long));
     A((void**)&h->rowsq[1], Np * sizeof(unsigned long long));
@@ -198,6 +215,7 @@ extern "C" sp2_status_t sp2_create(sp2_handle_t* out, int N_max, int batch_max, 
         A((void**)&h->bstatus_dev, bm * sizeof(int));
         A((void**)&h->bbounds_dev, bm * 2 * sizeof(double));
         A((void**)&h->bnocc_dev, bm * sizeof(double));
+        A((void**)&h->bhl_dev, bm * 2 * sizeof(double));
     }
     auto AH = [&](void** p, size_t bytes) {
         if (st != SP2_OK) return;
@@ -303,7 +321,7 @@ static int choose_tile_config(int N, int requested, int num_sms) {
 }
 
 struct Problem {
-    int N, Np, cfg, scale_log2, n_items, n_slots, exact_diag, list, mix;
+    int N, Np, cfg, scale_log2, n_items, n_slots, exact_diag, list, mix, enh_kc;
     float scale, inv_scale2;
 };
 
@@ -322,6 +340,7 @@ static sp2_status_t prepare_problem(sp2_handle_s* h, int N, const sp2_opts_t* o,
     if (k > 14) return SP2_ERR_INVALID_ARG;
     pb->scale_log2 = k;
     pb->exact_diag = (o && o->exact_diag == 0) ? 0 : 1;
+    pb->enh_kc = opt_enh_kc(o);
     pb->scale = ldexpf(1.0f, k);
     pb->inv_scale2 = ldexpf(1.0f, -2 * k);
     const int nt = pb->Np / edge;
@@ -353,7 +372,7 @@ static LayerParams layer_params(sp2_handle_s* h, const Problem& pb, int parity, 
     p.rowsq_next = pb.exact_diag ? h->rowsq[parity ^ 1] : nullptr;
     p.items = h->items_dev[pb.list]; p.ld = ws_ld_f32(pb.Np); p.ldf = ws_ld_f16(pb.Np); p.N = pb.N; p.Np = pb.Np;
     p.n_items = pb.n_items; p.n_slots = pb.n_slots;
-    p.scale = pb.scale; p.inv_scale2 = pb.inv_scale2; p.cond_handle = cond; p.round_sync = h->round_sync; p.enh_kc = h->enh_kc;
+    p.scale = pb.scale; p.inv_scale2 = pb.inv_scale2; p.cond_handle = cond; p.round_sync = h->round_sync; p.round_spins = h->round_spins; p.enh_kc = pb.enh_kc;
     return p;
 }
 
@@ -372,9 +391,16 @@ static sp2_status_t launch_one_layer(sp2_handle_s* h, const Problem& pb, int par
 // WHILE(ctrl->running) { layer(ping -> pong); layer(pong -> ping); } as a CUDA graph with a conditional node; the
 // condition is set on the device by the last CTA of each layer kernel (cudaGraphSetConditional).
 static sp2_status_t get_loop_graph(sp2_handle_s* h, const Problem& pb, LoopGraph** out) {
-    auto key = std::make_tuple(pb.N, pb.Np, pb.cfg, pb.scale_log2, pb.exact_diag | (pb.mix << 1));
+    auto key = std::make_tuple(pb.N, pb.Np, pb.cfg, pb.scale_log2, pb.exact_diag | (pb.mix << 1) | (pb.enh_kc << 2));
     auto it = h->graphs.find(key);
     if (it != h->graphs.end()) { *out = &it->second; return SP2_OK; }
+    if (h->graphs.size() >= 16) {            // bounded cache: start over rather than grow without limit
+        for (auto& kv : h->graphs) {
+            if (kv.second.exec) cudaGraphExecDestroy(kv.second.exec);
+            if (kv.second.graph) cudaGraphDestroy(kv.second.graph);
+        }
+        h->graphs.clear();
+    }
     LoopGraph lg;
     CK(cudaGraphCreate(&lg.graph, 0));
     cudaGraphConditionalHandle handle;
@@ -401,10 +427,21 @@ static sp2_status_t get_loop_graph(sp2_handle_s* h, const Problem& pb, LoopGraph
     return SP2_OK;
 }
 
+// A handle belongs to the device that was current at sp2_create (its workspace and graphs live there).
+static sp2_status_t check_device(sp2_handle_s* h) {
+    int dev = -1;
+    CK(cudaGetDevice(&dev));
+    if (dev != h->device) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "handle was created on device %d, current device is %d", h->device, dev);
+        return SP2_ERR_INVALID_ARG;
+    }
+    return SP2_OK;
+}
+
 static sp2_status_t check_common(sp2_handle_s* h, const void* in, int N, int ldin, const void* outp, int ldout) {
     if (!h || !in || !outp || N < 1 || ldin < N || ldout < N) return SP2_ERR_INVALID_ARG;
     if (N > h->N_max) return SP2_ERR_WORKSPACE;
-    return SP2_OK;
+    return check_device(h);
 }
 
 // Shared body of the single-matrix solves.  mode = MODE_STANDARD or MODE_GENERALIZED (thetas already in
@@ -417,7 +454,8 @@ static sp2_status_t solve_single(sp2_handle_s* h, const float* H_dev, int N, int
     sp2_status_t s = prepare_problem(h, N, o, &pb, st);
     if (s != SP2_OK) return s;
     if (mix) {
-        if (pb.cfg == TILE_128x256) return SP2_ERR_INVALID_ARG;      // the mix epilogue exists for configs 1 and 3
+        // the mix epilogue exists for tile configurations 1 and 3 only
+        if (pb.cfg == TILE_128x256 || pb.cfg == TILE_128x128_ENH) return SP2_ERR_INVALID_ARG;
         if (!h->mix) CK(cudaMalloc((void**)&h->mix, (size_t)h->Np_max * (size_t)ws_ld_f32(h->Np_max) * 4));
         pb.mix = 1;
     }
@@ -428,7 +466,7 @@ static sp2_status_t solve_single(sp2_handle_s* h, const float* H_dev, int N, int
     c->N_occ = N_occ; c->eps_alt = o->eps_alt; c->tol = o->tol;
     c->eps_min = o->eps_min; c->eps_max = o->eps_max;
     c->N = N; c->mode = mode; c->max_layers = max_layers; c->auto_bounds = o->auto_bounds;
-    c->noise_kappa = h->noise_kappa;
+    c->noise_kappa = opt_kappa(*o);
     c->accelerated = (mode == MODE_STANDARD && o->accelerated) ? 1 : 0;
     c->homo = o->homo; c->lumo = o->lumo;
     CK(cudaMemcpyAsync(h->ctrl, c, ctrl_header_bytes(), cudaMemcpyHostToDevice, st));
@@ -445,7 +483,7 @@ static sp2_status_t solve_single(sp2_handle_s* h, const float* H_dev, int N, int
         CK(cudaMemsetAsync(h->hl[0][1], 0, (size_t)pb.Np * ldF * 2, st));
     }
     // ---- a1: bounds, a2: initial affine layer + first split + first control step
-    if (o->auto_bounds) CK(launch_gershgorin(H_dev, N, ldh, h->R, h->diag, h->ctrl, nullptr, h->num_sms, st));
+    if (o->auto_bounds) CK(launch_gershgorin(H_dev, N, ldh, h->gpart, h->diag, h->ctrl, h->num_sms, st));
     if (pb.exact_diag) {
         CK(cudaMemsetAsync(h->rowsq[0], 0, (size_t)pb.Np * sizeof(unsigned long long), st));
         CK(cudaMemsetAsync(h->rowsq[1], 0, (size_t)pb.Np * sizeof(unsigned long long), st));
@@ -496,7 +534,8 @@ static sp2_status_t solve_single(sp2_handle_s* h, const float* H_dev, int N, int
 
 static sp2_status_t resident_solve(sp2_handle_s* h, const float* H_dev, int N, int B, const double* N_occ,
                                    int nocc_is_scalar, const sp2_opts_t& o, float* D_dev, sp2_layer_stat_t* stats_host,
-                                   int* n_layers, int* status_out, double* bounds_out, cudaStream_t st);
+                                   int* n_layers, int* status_out, double* bounds_out, cudaStream_t st, int mode,
+                                   const double* homo_lumo);
 
 extern "C" sp2_status_t sp2_density_matrix(sp2_handle_t h, const float* H_dev, int N, int ldh, double N_occ,
                                            const sp2_opts_t* opts, float* D_dev, int ldd,
@@ -521,7 +560,7 @@ extern "C" sp2_status_t sp2_density_matrix(sp2_handle_t h, const float* H_dev, i
         // one kernel per layer.  (exact_diag does not apply there: the diagonal comes from the tensor core.)
         int nl = 0;
         sp2_status_t s2 = resident_solve(h, H_dev, N, 1, &N_occ, 1, o, D_dev, stats_host, &nl, nullptr, bounds_out,
-                                         (cudaStream_t)stream);
+                                         (cudaStream_t)stream, MODE_STANDARD, nullptr);
         if (n_layers) *n_layers = nl;
         return s2;
     }
@@ -556,7 +595,7 @@ extern "C" sp2_status_t sp2_density_matrix_host(sp2_handle_t h, const float* H_h
 
 // NEXT-1: final refinement f_final (Eq. 16) as two layers with enhanced accumulation, plus Tr[D H].
 extern "C" sp2_status_t sp2_refine_energy(sp2_handle_t h, const float* S_dev, int N, int lds, int last_sigma,
-                                          const float* H_dev, int ldh, float* D_dev, int ldd,
+                                          const float* H_dev, int ldh, const sp2_opts_t* opts, float* D_dev, int ldd,
                                           sp2_refine_result_t* result, void* stream) {
     sp2_status_t s = check_common(h, S_dev, N, lds, D_dev, ldd);
     if (s != SP2_OK) return s;
@@ -564,7 +603,10 @@ extern "C" sp2_status_t sp2_refine_energy(sp2_handle_t h, const float* S_dev, in
     if (h->max_layers < 2) return SP2_ERR_WORKSPACE;
     cudaStream_t st = (cudaStream_t)stream;
     Problem pb;
-    s = prepare_problem(h, N, nullptr, &pb, st, TILE_128x128_ENH);
+    sp2_opts_t ro;
+    sp2_default_opts(&ro);
+    if (opts) { ro.fp16_scale_log2 = opts->fp16_scale_log2; ro.enh_kc = opts->enh_kc; }
+    s = prepare_problem(h, N, &ro, &pb, st, TILE_128x128_ENH);
     if (s != SP2_OK) return s;
     pb.exact_diag = 1;                               // diag(X) from row sums of squares (reading C24), as in the solve
     // Reading C15: continue the alternation from the last applied sign.
@@ -685,21 +727,31 @@ extern "C" sp2_status_t sp2_generalized_wb(sp2_handle_t h, const float* H_dev, i
     return sp2_generalized(h, H_dev, N, ldh, th.data(), L, eps_min, eps_max, opts, X_L_dev, ldx, stats_host, stream);
 }
 
-// Shared body of the batched call and of small single matrices: B contiguous N x N problems, one resident-kernel launch.
+// Shared body of the batched calls and of small single matrices: B contiguous N x N problems, one resident-kernel
+// launch.  mode = MODE_STANDARD (Alg. 1, optionally with the accelerated weights and per-matrix estimates
+// homo_lumo[B][2]) or MODE_GENERALIZED (L = o.max_layers layers with the thetas already in h->thetas_host).
 static sp2_status_t resident_solve(sp2_handle_s* h, const float* H_dev, int N, int B, const double* N_occ,
                                    int nocc_is_scalar, const sp2_opts_t& o, float* D_dev, sp2_layer_stat_t* stats_host,
                                    int* n_layers, int* status_out, double* bounds_out /*[B][2] or NULL*/,
-                                   cudaStream_t st) {
+                                   cudaStream_t st, int mode, const double* homo_lumo) {
     int k = o.fp16_scale_log2;
     if (k < 0) k = 13;
     if (k > 14) return SP2_ERR_INVALID_ARG;
-    CK(cudaMemcpyAsync(h->bnocc_dev, N_occ, (size_t)(nocc_is_scalar ? 1 : B) * sizeof(double), cudaMemcpyHostToDevice, st));
+    if (N_occ)
+        CK(cudaMemcpyAsync(h->bnocc_dev, N_occ, (size_t)(nocc_is_scalar ? 1 : B) * sizeof(double), cudaMemcpyHostToDevice, st));
+    if (homo_lumo) CK(cudaMemcpyAsync(h->bhl_dev, homo_lumo, (size_t)B * 2 * sizeof(double), cudaMemcpyHostToDevice, st));
+    if (mode == MODE_GENERALIZED)
+        CK(cudaMemcpyAsync(h->thetas_dev, h->thetas_host, (size_t)o.max_layers * kThetaStride * sizeof(double),
+                           cudaMemcpyHostToDevice, st));
     CK(cudaMemsetAsync(h->bstats_dev, 0, (size_t)B * o.max_layers * sizeof(sp2_layer_stat_t), st));
     ResidentParams p;
     memset(&p, 0, sizeof(p));
     p.H = H_dev; p.D = D_dev; p.N_occ = h->bnocc_dev; p.nocc_is_scalar = nocc_is_scalar; p.N = N; p.B = B;
     p.auto_bounds = o.auto_bounds; p.eps_min = o.eps_min; p.eps_max = o.eps_max; p.tol = o.tol; p.eps_alt = o.eps_alt;
-    p.max_layers = o.max_layers; p.mode = MODE_STANDARD; p.thetas = nullptr; p.noise_kappa = h->noise_kappa;
+    p.max_layers = o.max_layers; p.mode = mode; p.thetas = (mode == MODE_GENERALIZED) ? h->thetas_dev : nullptr;
+    p.noise_kappa = opt_kappa(o);
+    p.accelerated = (mode == MODE_STANDARD && homo_lumo) ? 1 : 0;
+    p.homo_lumo = h->bhl_dev;
     p.scale = ldexpf(1.0f, k); p.inv_scale2 = ldexpf(1.0f, -2 * k);
     p.stats = h->bstats_dev; p.n_layers = h->bnl_dev; p.status = h->bstatus_dev; p.bounds = h->bbounds_dev;
     CK(launch_resident(p, h->num_sms, st));
@@ -725,21 +777,62 @@ static sp2_status_t resident_solve(sp2_handle_s* h, const float* H_dev, int N, i
 }
 
 extern "C" sp2_status_t sp2_density_matrix_batched(sp2_handle_t h, const float* H_dev, int N, int B,
-                                                   const double* N_occ, int nocc_is_scalar, const sp2_opts_t* opts,
-                                                   float* D_dev, sp2_layer_stat_t* stats_host, int* n_layers,
-                                                   int* status_out, void* stream) {
+                                                   const double* N_occ, int nocc_is_scalar, const double* homo_lumo,
+                                                   const sp2_opts_t* opts, float* D_dev, sp2_layer_stat_t* stats_host,
+                                                   int* n_layers, int* status_out, void* stream) {
     if (!h || !H_dev || !D_dev || !N_occ || N < 1 || B < 1) return SP2_ERR_INVALID_ARG;
     if (N > 256) return SP2_ERR_UNSUPPORTED_N;
     if (B > h->batch_max) return SP2_ERR_WORKSPACE;
+    sp2_status_t sd = check_device(h);
+    if (sd != SP2_OK) return sd;
     sp2_opts_t o;
     if (opts) o = *opts; else sp2_default_opts(&o);
     if (o.max_layers < 1 || o.max_layers > h->max_layers) return SP2_ERR_INVALID_ARG;
-    if (!o.auto_bounds && !(o.eps_max > o.eps_min)) return SP2_ERR_BOUNDS_DEGENERATE;
-    if (o.accelerated) return SP2_ERR_INVALID_ARG;       // per-matrix HOMO/LUMO estimates: single-matrix call only
+    if (!o.auto_bounds) {
+        if (!isfinite(o.eps_min) || !isfinite(o.eps_max)) return SP2_ERR_INVALID_ARG;
+        if (!(o.eps_max > o.eps_min)) return SP2_ERR_BOUNDS_DEGENERATE;
+    }
+    // accelerated weights (section V.A): per-matrix estimates through homo_lumo[B][2]; opts->homo / lumo are not read
+    if ((o.accelerated != 0) != (homo_lumo != nullptr)) return SP2_ERR_INVALID_ARG;
+    if (homo_lumo)
+        for (int i = 0; i < B; ++i) {
+            const double ho = homo_lumo[2 * i], lu = homo_lumo[2 * i + 1];
+            if (!isfinite(ho) || !isfinite(lu) || !(lu > ho)) return SP2_ERR_INVALID_ARG;
+            if (!o.auto_bounds && !(o.eps_min <= ho && lu <= o.eps_max)) return SP2_ERR_INVALID_ARG;
+        }
     for (int i = 0; i < (nocc_is_scalar ? 1 : B); ++i)
         if (!(N_occ[i] >= 0.0 && N_occ[i] <= (double)N)) return SP2_ERR_INVALID_ARG;
     return resident_solve(h, H_dev, N, B, N_occ, nocc_is_scalar, o, D_dev, stats_host, n_layers, status_out, nullptr,
-                          (cudaStream_t)stream);
+                          (cudaStream_t)stream, MODE_STANDARD, homo_lumo);
+}
+
+// The generalized network (Eq. 17) on a batch: the same L layers (shared weights) applied to B inputs.
+extern "C" sp2_status_t sp2_generalized_batched(sp2_handle_t h, const float* H_dev, int N, int B,
+                                                const double* theta_host, int L, double eps_min, double eps_max,
+                                                const sp2_opts_t* opts, float* X_L_dev, sp2_layer_stat_t* stats_host,
+                                                int* status_out, void* stream) {
+    if (!h || !H_dev || !X_L_dev || !theta_host || N < 1 || B < 1 || L < 1) return SP2_ERR_INVALID_ARG;
+    if (N > 256) return SP2_ERR_UNSUPPORTED_N;
+    if (B > h->batch_max) return SP2_ERR_WORKSPACE;
+    if (L > h->max_layers) return SP2_ERR_INVALID_ARG;
+    sp2_status_t sd = check_device(h);
+    if (sd != SP2_OK) return sd;
+    sp2_opts_t o;
+    if (opts) o = *opts; else sp2_default_opts(&o);
+    o.max_layers = L; o.tol = 0.0; o.eps_alt = 0.0;
+    o.auto_bounds = !(eps_max > eps_min);
+    o.eps_min = eps_min; o.eps_max = eps_max;
+    if (!o.auto_bounds && (!isfinite(eps_min) || !isfinite(eps_max))) return SP2_ERR_INVALID_ARG;
+    for (int n = 0; n < L; ++n) {
+        for (int k = 0; k < 3; ++k) {
+            if (!isfinite(theta_host[3 * n + k])) return SP2_ERR_INVALID_ARG;
+            h->thetas_host[kThetaStride * n + k] = theta_host[3 * n + k];
+        }
+        h->thetas_host[kThetaStride * n + 3] = 0.0;
+    }
+    std::vector<int> nl((size_t)B);
+    return resident_solve(h, H_dev, N, B, nullptr, 1, o, X_L_dev, stats_host, nl.data(), status_out, nullptr,
+                          (cudaStream_t)stream, MODE_GENERALIZED, nullptr);
 }
 
 extern "C" sp2_status_t sp2_split_fp16(const float* X_dev, int N, int ldx, unsigned short* hi_dev,
@@ -758,8 +851,11 @@ extern "C" sp2_status_t sp2_gershgorin(sp2_handle_t h, const float* H_dev, int N
                                        void* stream) {
     if (!h || !H_dev || !bounds_host || N < 1 || ldh < N) return SP2_ERR_INVALID_ARG;
     if (N > h->N_max) return SP2_ERR_WORKSPACE;
+    sp2_status_t sd = check_device(h);
+    if (sd != SP2_OK) return sd;
     cudaStream_t st = (cudaStream_t)stream;
-    CK(launch_gershgorin(H_dev, N, ldh, h->R, h->diag, h->ctrl, nullptr, h->num_sms, st));
+    CK(cudaMemsetAsync(&h->ctrl->done_counter, 0, sizeof(unsigned int), st));
+    CK(launch_gershgorin(H_dev, N, ldh, h->gpart, h->diag, h->ctrl, h->num_sms, st));
     CK(cudaMemcpyAsync(h->bounds_host, &h->ctrl->eps_min, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
     bounds_host[0] = h->bounds_host[0];
@@ -768,3 +864,4 @@ extern "C" sp2_status_t sp2_gershgorin(sp2_handle_t h, const float* H_dev, int N
 }
 
 extern "C" int sp2_last_launch_count(sp2_handle_t h) { return h ? h->last_launches : 0; }
+extern "C" int sp2_last_round_sync_broken(sp2_handle_t h) { return (h && h->ctrl_host) ? (int)h->ctrl_host->round_sync_broken : 0; }

@@ -1,6 +1,6 @@
 // Device-side branch and convergence control of Alg. 1 (stop rule P:186-190, Thm 1).
 // One Ctrl block per problem lives in device memory; the last CTA of each layer kernel calls
-// control_after_layer(), so no scalar crosses to the host between layers.
+// control_finish_layer(), so no scalar crosses to the host between layers.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -41,7 +41,8 @@ struct CtrlCore {
     double noise_kappa;              // reading C25: stop when IdErr_n <= kappa |Tr X_n(tc) - N_X|; 0 disables
     float  theta[4];                 // th1, th2, th3, c of the NEXT layer (FP32: the epilogue's arithmetic type)
     unsigned int done_counter;       // CTAs finished in the current kernel
-    unsigned int round_counter;      // CTAs that reached a round boundary of the current layer kernel (round sync)
+    unsigned int round_counter;      // round-boundary check-ins of all layer kernels of this solve (round sync);
+                                     // monotonic: layer n+1's targets start at n (n_rounds - 1) gridDim.x
     unsigned int round_sync_broken;  // a round wait timed out once (CTAs not co-resident): stop waiting in this solve
     unsigned int pad_rs_;
 };
@@ -56,6 +57,10 @@ __device__ inline void control_plan_next(CtrlCore* c, sp2_layer_stat_t* stats, c
     const int m = c->n + 1;                      // layer about to run
     if (c->mode == MODE_GENERALIZED) {
         if (c->n >= c->max_layers) { c->running = 0; c->stop_reason = SP2_STOP_MAX_LAYERS; return; }
+        if (!(isfinite(c->N_S) && isfinite(c->fro2))) {      // a NaN/Inf in H or an overflowing network
+            c->running = 0; c->stop_reason = SP2_STOP_NONFINITE; c->error = SP2_ERR_NONFINITE;
+            return;
+        }
         c->theta[0] = (float)thetas[kThetaStride * c->n + 0];
         c->theta[1] = (float)thetas[kThetaStride * c->n + 1];
         c->theta[2] = (float)thetas[kThetaStride * c->n + 2];
@@ -158,7 +163,7 @@ __device__ inline void control_finish_layer(CtrlCore* c, sp2_layer_stat_t* stats
         stats[c->n - 1].t_end_ns = t;
     }
     c->done_counter = 0;
-    c->round_counter = 0;
+    // (round_counter is never reset inside a solve: the layer kernel's round targets count from c->n)
     // Reading C25: "IdErr_n <= 0" at the resolution of the arithmetic.  iderr_prev = IdErr_n of the layer just
     // applied; |trX - nx_inflight| = measured error of the tensor-core trace of X_n.
     if (c->mode == MODE_STANDARD && c->pending_stop == SP2_STOP_NONE && c->n > 2 &&
@@ -172,17 +177,6 @@ __device__ inline void control_finish_layer(CtrlCore* c, sp2_layer_stat_t* stats
         return;
     }
     control_plan_next(c, stats, thetas);
-}
-
-// Called by ONE thread once every CTA of the layer kernel has published its partial sums.
-__device__ inline void control_after_layer(Ctrl* c, sp2_layer_stat_t* stats, const double* thetas, int n_partials) {
-    double trS = 0.0, fro2 = 0.0, trX = 0.0;
-    for (int i = 0; i < n_partials; ++i) {       // fixed order: deterministic for a static tile schedule
-        trS += c->partial[i][0];
-        fro2 += c->partial[i][1];
-        trX += c->partial[i][2];
-    }
-    control_finish_layer(c, stats, thetas, trS, fro2, trX);
 }
 
 }  // namespace sp2

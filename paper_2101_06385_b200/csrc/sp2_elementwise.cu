@@ -49,9 +49,13 @@ __device__ __forceinline__ float row16_sum(float v) {
 
 // ------------------------------------------------------------------------------------------------ a1
 // Gershgorin radii of the lower-triangle-symmetrised H: R_i = sum_{j<i} |H_ij| + sum_{j>i} |H_ji|: element (i,j),
-// i > j, adds |H_ij| to R_i (row sum) and to R_j (column sum).  FP32 sums inside a tile, FP64 atomics across tiles.
+// i > j, adds |H_ij| to R_i (row sum) and to R_j (column sum).  FP32 sums inside a 64 x 64 tile in a fixed order;
+// every tile writes its 64 row sums and 64 column sums to slots of their own (no atomics), and the finalize kernel
+// adds the slots of a row in index order in FP64: the bounds are bit-reproducible run to run.
+//   part[J][i]       = row sums of tile (I = i / 64, J), J <= I
+//   part[nt + I][j]  = column sums of tile (I, J = j / 64), I >= J
 __global__ void __launch_bounds__(256) k_gershgorin_rows(const float* __restrict__ H, int N, long long ldh,
-                                                         double* __restrict__ R, double* __restrict__ diag) {
+                                                         float* __restrict__ part, double* __restrict__ diag) {
     __shared__ float colacc[16][ET];
     const int nt = (N + ET - 1) / ET;
     const long long ntiles = (long long)nt * (nt + 1) / 2;
@@ -82,7 +86,7 @@ __global__ void __launch_bounds__(256) k_gershgorin_rows(const float* __restrict
             a.x = fabsf(a.x); a.y = fabsf(a.y); a.z = fabsf(a.z); a.w = fabsf(a.w);
             cs0 += a.x; cs1 += a.y; cs2 += a.z; cs3 += a.w;
             const float rs = row16_sum((a.x + a.y) + (a.z + a.w));
-            if ((threadIdx.x & 15) == 0 && i < N && rs != 0.f) atomicAdd(R + i, (double)rs);
+            if ((threadIdx.x & 15) == 0 && i < N) part[(long long)J * N + i] = rs;
         }
         *reinterpret_cast<float4*>(&colacc[r0][c4]) = make_float4(cs0, cs1, cs2, cs3);
         __syncthreads();
@@ -91,33 +95,65 @@ __global__ void __launch_bounds__(256) k_gershgorin_rows(const float* __restrict
 #pragma unroll
             for (int g = 0; g < 16; ++g) c += colacc[g][threadIdx.x];
             const int jj = J * ET + threadIdx.x;
-            if (jj < N && c != 0.f) atomicAdd(R + jj, (double)c);
+            if (jj < N) part[(long long)(nt + I) * N + jj] = c;
         }
         __syncthreads();
     }
 }
 
-// eps_min = min_i (H_ii - R_i), eps_max = max_i (H_ii + R_i) -> ctrl (one block).
-__global__ void __launch_bounds__(1024) k_gershgorin_finalize(const double* __restrict__ R,
-                                                              const double* __restrict__ diag, int N, Ctrl* ctrl,
-                                                              double* bounds_out) {
-    __shared__ double smin[32], smax[32];
+// R_i from the per-tile slots (fixed order, FP64), then eps_min = min_i (H_ii - R_i), eps_max = max_i (H_ii + R_i)
+// -> ctrl.  One row per thread; per-block extrema -> ctrl->partial; the last block takes the extrema over the blocks
+// (min / max are exact, so their order does not matter).
+__global__ void __launch_bounds__(256) k_gershgorin_finalize(const float* __restrict__ part,
+                                                             const double* __restrict__ diag, int N, Ctrl* ctrl) {
+    __shared__ double smin[8], smax[8];
+    const int nt = (N + ET - 1) / ET;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
     double lo = INFINITY, hi = -INFINITY;
-    for (int i = threadIdx.x; i < N; i += blockDim.x) {
-        lo = fmin(lo, diag[i] - R[i]);
-        hi = fmax(hi, diag[i] + R[i]);
+    if (i < N) {
+        const int Ib = i / ET;
+        double R = 0.0;
+        for (int J = 0; J <= Ib; ++J) R += (double)__ldg(part + (long long)J * N + i);
+        for (int I = Ib; I < nt; ++I) R += (double)__ldg(part + (long long)(nt + I) * N + i);
+        lo = diag[i] - R;
+        hi = diag[i] + R;
+        // fmin / fmax drop NaNs: a non-finite row must poison the bounds (-> SP2_ERR_BOUNDS_DEGENERATE / NONFINITE)
+        if (!isfinite(lo) || !isfinite(hi)) { lo = NAN; hi = NAN; }
     }
+    bool bad = isnan(lo);
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
         lo = fmin(lo, __shfl_xor_sync(0xffffffffu, lo, o));
         hi = fmax(hi, __shfl_xor_sync(0xffffffffu, hi, o));
     }
-    if ((threadIdx.x & 31) == 0) { smin[threadIdx.x >> 5] = lo; smax[threadIdx.x >> 5] = hi; }
+    bad = __any_sync(0xffffffffu, bad);
+    if ((threadIdx.x & 31) == 0) { smin[threadIdx.x >> 5] = bad ? NAN : lo; smax[threadIdx.x >> 5] = bad ? NAN : hi; }
     __syncthreads();
     if (threadIdx.x == 0) {
-        for (int w = 1; w < (int)(blockDim.x >> 5); ++w) { lo = fmin(lo, smin[w]); hi = fmax(hi, smax[w]); }
-        if (ctrl) { ctrl->eps_min = lo; ctrl->eps_max = hi; ctrl->launches += 2; }
-        if (bounds_out) { bounds_out[0] = lo; bounds_out[1] = hi; }
+        bool nan = false;
+        lo = INFINITY; hi = -INFINITY;
+        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) {
+            nan = nan || isnan(smin[w]);
+            lo = fmin(lo, smin[w]); hi = fmax(hi, smax[w]);
+        }
+        ctrl->partial[blockIdx.x][0] = nan ? NAN : lo;
+        ctrl->partial[blockIdx.x][1] = nan ? NAN : hi;
+        __threadfence();
+        const unsigned int done = atomicAdd(&ctrl->done_counter, 1u);
+        if (done == gridDim.x - 1) {
+            __threadfence();
+            nan = false;
+            lo = INFINITY; hi = -INFINITY;
+            for (unsigned int b = 0; b < gridDim.x; ++b) {
+                const double l = ((volatile double*)ctrl->partial[b])[0], h = ((volatile double*)ctrl->partial[b])[1];
+                nan = nan || isnan(l);
+                lo = fmin(lo, l); hi = fmax(hi, h);
+            }
+            ctrl->eps_min = nan ? NAN : lo;
+            ctrl->eps_max = nan ? NAN : hi;
+            ctrl->launches += 2;
+            ctrl->done_counter = 0;
+        }
     }
 }
 
@@ -162,7 +198,8 @@ __global__ void __launch_bounds__(256, 4) k_affine_split(const float* __restrict
     const double e0 = ctrl->eps_min, e1 = ctrl->eps_max;
     if (!(e1 > e0) || !isfinite(e0) || !isfinite(e1)) {
         if (blockIdx.x == 0 && threadIdx.x == 0) {
-            ctrl->error = SP2_ERR_BOUNDS_DEGENERATE;
+            // caller-given bounds were checked on the host: non-finite ones here are Gershgorin's of a non-finite H
+            ctrl->error = (isfinite(e0) && isfinite(e1)) ? SP2_ERR_BOUNDS_DEGENERATE : SP2_ERR_NONFINITE;
             ctrl->running = 0;
         }
         return;
@@ -264,7 +301,6 @@ __global__ void __launch_bounds__(256, 4) k_affine_split(const float* __restrict
             ctrl->fro2 = s1;
             ctrl->n = 0;
             ctrl->done_counter = 0;
-            ctrl->round_counter = 0;
             ctrl->launches += 1;
             control_plan_next(ctrl, stats, thetas);
         }
@@ -395,7 +431,6 @@ __global__ void __launch_bounds__(256) k_energy_traces(const float* __restrict__
                 ctrl->N_S = s1;
                 ctrl->fro2 = s2;
                 ctrl->n = 0;
-                ctrl->round_counter = 0;
                 control_plan_next(ctrl, stats, thetas);
             }
         }
@@ -467,15 +502,14 @@ __global__ void __launch_bounds__(256) k_one_minus(const float* __restrict__ M, 
 }
 
 // ------------------------------------------------------------------------------------------------ launchers
-cudaError_t launch_gershgorin(const float* H, int N, long long ldh, double* R, double* diag, Ctrl* ctrl,
-                              double* bounds_out, int num_sms, cudaStream_t st) {
-    cudaError_t e = cudaMemsetAsync(R, 0, sizeof(double) * (size_t)N, st);
-    if (e != cudaSuccess) return e;
+cudaError_t launch_gershgorin(const float* H, int N, long long ldh, float* part, double* diag, Ctrl* ctrl,
+                              int num_sms, cudaStream_t st) {
     const int nt = (N + ET - 1) / ET;
     const long long ntiles = (long long)nt * (nt + 1) / 2;
     const int grid = (int)(ntiles < (long long)num_sms * 16 ? ntiles : (long long)num_sms * 16);
-    k_gershgorin_rows<<<grid, 256, 0, st>>>(H, N, ldh, R, diag);
-    k_gershgorin_finalize<<<1, 1024, 0, st>>>(R, diag, N, ctrl, bounds_out);
+    if ((N + 255) / 256 > kMaxPartials) return cudaErrorInvalidValue;
+    k_gershgorin_rows<<<grid, 256, 0, st>>>(H, N, ldh, part, diag);
+    k_gershgorin_finalize<<<(N + 255) / 256, 256, 0, st>>>(part, diag, N, ctrl);
     return cudaGetLastError();
 }
 

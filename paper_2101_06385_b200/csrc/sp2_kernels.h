@@ -10,8 +10,10 @@
 namespace sp2 {
 
 // ---- HBM-bound kernels (sp2_elementwise.cu)
-cudaError_t launch_gershgorin(const float* H, int N, long long ldh, double* R, double* diag, Ctrl* ctrl,
-                              double* bounds_out, int num_sms, cudaStream_t st);
+// part: scratch of gershgorin_part_floats(N) floats (per-tile row / column sums, see k_gershgorin_rows)
+cudaError_t launch_gershgorin(const float* H, int N, long long ldh, float* part, double* diag, Ctrl* ctrl,
+                              int num_sms, cudaStream_t st);
+inline size_t gershgorin_part_floats(int N) { return 2 * (size_t)((N + 63) / 64) * (size_t)N; }
 cudaError_t launch_affine_split(const float* H, int N, long long ldh, float* S, __half* hi, __half* lo, long long ld,
                                 long long ldf, float scale, Ctrl* ctrl, sp2_layer_stat_t* stats, const double* thetas,
                                 unsigned long long* rowsq, float* mix, float c0, int num_sms, cudaStream_t st);
@@ -73,6 +75,7 @@ struct LayerParams {
     float inv_scale2;              // 1 / c^2
     int enh_kc;                    // enhanced accumulation: K-blocks (of 64) per tensor-core accumulation chunk
     int round_sync;                // 1: producers of all CTAs meet at every round boundary (keeps the wave in lockstep)
+    unsigned int round_spins;      // bound of that wait in 64 ns sleeps (a CTA that is not co-resident must not hang it)
     unsigned long long cond_handle;  // cudaGraphConditionalHandle (0 = none)
 };
 
@@ -98,7 +101,9 @@ struct ResidentParams {
     double eps_min, eps_max, tol, eps_alt, noise_kappa;
     int max_layers;
     int mode;                      // MODE_STANDARD / MODE_GENERALIZED
-    const double* thetas;          // generalized: [L][3]
+    const double* thetas;          // generalized: [L][kThetaStride] on the device
+    int accelerated;               // standard mode with the accelerated weights (section V.A, reading C27)
+    const double* homo_lumo;       // accelerated: [B][2] HOMO / LUMO estimates in energy units (device)
     float scale, inv_scale2;
     sp2_layer_stat_t* stats;       // [B][max_layers] (device)
     int* n_layers;                 // [B]

@@ -45,13 +45,16 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
         : "memory");
     return ok != 0;
 }
-// Bounded wait: a protocol bug traps (the launch fails loudly) instead of hanging the GPU.
+// Bounded wait: a protocol bug traps (the launch fails with a sticky error, the call returns SP2_ERR_CUDA) instead
+// of hanging the GPU; documented in include/sp2_b200.h.  The device-side message exists in -DSP2_DEBUG builds only.
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
     uint32_t spins = 0;
     while (!mbar_try_wait(bar, parity)) {
         if (++spins > (1u << 26)) {
+#ifdef SP2_DEBUG
             printf("sp2: mbarrier wait timed out (block %d thread %d bar %u parity %u)\n", blockIdx.x, threadIdx.x,
                    smem_u32(bar), parity);
+#endif
             __trap();
         }
     }

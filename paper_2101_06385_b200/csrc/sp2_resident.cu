@@ -233,13 +233,15 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
         const bool bounds_ok = (e1 > e0) && isfinite(e0) && isfinite(e1);
         if (threadIdx.x == 0) {
             CtrlCore* c = &sh->ctrl;
-            c->N_occ = p.nocc_is_scalar ? p.N_occ[0] : p.N_occ[m];
+            c->N_occ = (p.mode == MODE_GENERALIZED) ? 0.0 : (p.nocc_is_scalar ? p.N_occ[0] : p.N_occ[m]);
             c->eps_alt = p.eps_alt; c->tol = p.tol; c->eps_min = e0; c->eps_max = e1;
             c->N = N; c->mode = p.mode; c->max_layers = p.max_layers; c->auto_bounds = p.auto_bounds;
             c->n = 0; c->running = 0; c->stop_reason = 0; c->pending_stop = 0; c->sigma_prev = 0; c->sigma_prev2 = 0;
             c->error = bounds_ok ? 0 : SP2_ERR_BOUNDS_DEGENERATE; c->launches = 0;
             c->N_S = 0; c->fro2 = 0; c->iderr_prev = 0; c->iderr_prev2 = 0; c->nx_inflight = 0; c->noise_kappa = p.noise_kappa;
-            c->accelerated = 0; c->acc_h = 1.0; c->acc_l = 0.0; c->homo = 0.0; c->lumo = 0.0;
+            c->accelerated = p.accelerated; c->acc_h = 1.0; c->acc_l = 0.0;
+            c->homo = p.accelerated ? p.homo_lumo[2 * m] : 0.0;
+            c->lumo = p.accelerated ? p.homo_lumo[2 * m + 1] : 0.0;
         }
         if (!bounds_ok) {           // uniform over the cluster (same e0, e1 everywhere)
             if (rank == 0 && threadIdx.x == 0) {

@@ -5,7 +5,7 @@
 //                                                                              transpose term is lo[I,:] . hi[J,:])
 //   S_n      = th1 acc / c^2 + th2 S_{n-1} + th3 I                              (Alg. 1's W_n, B_n; Eq. 17)
 //   epilogue: Tr S_n, ||S_n||_F^2 (= next layer's N_X), Tr X_n in FP64; next layer's hi/lo (Eqs. 12-13);
-//   last CTA: sigma_{n+1}, IdErr_{n+1}, stop tests (control_after_layer).
+//   last CTA: sigma_{n+1}, IdErr_{n+1}, stop tests (control_finish_layer).
 // Only lower-triangle tiles (I >= J) are computed; every hi/lo value is also stored at its mirrored position, so the
 // operands stay exactly symmetric and the next layer can read full row panels as K-major operands.  Of the FP32
 // master only the mirrored (upper-triangle) copy is kept current outside the diagonal chunks: that is the copy the
@@ -108,20 +108,24 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
             // Round sync: the CTAs of a round share row panels through L2 only while they walk K together.  Nothing
             // else keeps them together (each runs its tiles back to back), so every producer checks in at each round
             // boundary and starts the next tile's loads when all have (bounded spin: never a hang, at worst no sync).
+            // The counter is monotonic over a solve (every CTA checks in exactly n_rounds - 1 times per layer), so the
+            // targets of layer n + 1 start at n (n_rounds - 1) gridDim.x and a late check-in of the previous layer
+            // can never be lost to a reset.
             const int n_rounds = (n_work + nslots - 1) / nslots;
+            const unsigned int base = (unsigned int)(*((volatile int*)&ctrl->n)) * (unsigned int)(n_rounds - 1);
             int round = 0;
             for (int w = slot; ; w += nslots, ++round) {
                 if (p.round_sync && round > 0 && round < n_rounds) {
                     __threadfence();
                     atomicAdd(&ctrl->round_counter, 1u);
                     if (w < n_work && *((volatile unsigned int*)&ctrl->round_sync_broken) == 0u) {
-                        const unsigned int target = (unsigned int)round * gridDim.x;
+                        const unsigned int target = (base + (unsigned int)round) * gridDim.x;
                         unsigned int spins = 0;
-                        while (*((volatile unsigned int*)&ctrl->round_counter) < target && ++spins < (1u << 16))
+                        while (*((volatile unsigned int*)&ctrl->round_counter) < target && ++spins < p.round_spins)
                             __nanosleep(64);
                         // timed out: the grid is not co-resident (shared GPU); the sync is only an optimisation, so
                         // give it up for the rest of this solve instead of paying the timeout at every boundary
-                        if (spins >= (1u << 16)) ctrl->round_sync_broken = 1u;
+                        if (spins >= p.round_spins) ctrl->round_sync_broken = 1u;
                     }
                 }
                 if (w >= n_work) break;
@@ -164,6 +168,7 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                 }
             }
         }
+        __syncwarp();     // reconverge before the .aligned cluster barrier of the teardown
     } else if (warp == 1) {
         // =============================== MMA issuer (leader CTA only, one elected lane)
         if (rank == 0) {
@@ -211,6 +216,7 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                 }
             }
         }
+        __syncwarp();     // reconverge before the .aligned barrier / tcgen05.dealloc of the teardown
     } else {
         // =============================== epilogue warps (TMEM lane quarter = warp % 4)
         const int q = warp & 3;

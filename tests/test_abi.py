@@ -54,10 +54,11 @@ def test_struct_layouts_match_header():
 #include <stddef.h>
 #include "sp2_b200.h"
 int main(void) {
-  printf("%zu %zu %zu %zu %zu %zu %zu %zu %zu %zu\n", sizeof(sp2_layer_stat_t), offsetof(sp2_layer_stat_t, trace_X_diag),
+  printf("%zu %zu %zu %zu %zu %zu %zu %zu %zu %zu %zu %zu %zu\n", sizeof(sp2_layer_stat_t), offsetof(sp2_layer_stat_t, trace_X_diag),
          offsetof(sp2_layer_stat_t, sigma), offsetof(sp2_layer_stat_t, t_end_ns), sizeof(sp2_opts_t),
          offsetof(sp2_opts_t, tol), offsetof(sp2_opts_t, eps_alt), offsetof(sp2_opts_t, tile_config),
-         offsetof(sp2_opts_t, accelerated), offsetof(sp2_opts_t, lumo));
+         offsetof(sp2_opts_t, accelerated), offsetof(sp2_opts_t, lumo), offsetof(sp2_opts_t, noise_kappa),
+         offsetof(sp2_opts_t, enh_kc), offsetof(sp2_opts_t, trunc_tau));
   return 0; }'''
     import tempfile
 
@@ -69,7 +70,8 @@ int main(void) {
         got = [int(x) for x in subprocess.run([exe], capture_output=True, text=True, check=True).stdout.split()]
     L, Op = api.LayerStat, api.Opts
     want = [C.sizeof(L), L.trace_X_diag.offset, L.sigma.offset, L.t_end_ns.offset, C.sizeof(Op), Op.tol.offset,
-            Op.eps_alt.offset, Op.tile_config.offset, Op.accelerated.offset, Op.lumo.offset]
+            Op.eps_alt.offset, Op.tile_config.offset, Op.accelerated.offset, Op.lumo.offset, Op.noise_kappa.offset,
+            Op.enh_kc.offset, Op.trunc_tau.offset]
     assert got == want
 
 
@@ -81,6 +83,8 @@ def test_host_only_calls_do_not_need_a_gpu(lib):
     o = api.Opts()
     lib.sp2_default_opts(C.byref(o))
     assert o.auto_bounds == 1 and o.max_layers == 120 and o.tol == 0.0
+    assert o.noise_kappa < 0 and o.enh_kc == 0 and o.trunc_tau == 0.0
+    assert lib.sp2_workspace_bytes_lazy(16384) >= 3 * 16384 * 16384 * 4      # mix matrix + two staging matrices
     assert lib.sp2_workspace_bytes(16384, 0, 120) >= 3 * 16384 * 16384 * 4
     assert lib.sp2_workspace_bytes(0, 0, 120) == 0
 

@@ -4,6 +4,7 @@ import json
 import os
 
 import numpy as np
+import pytest
 
 from oracle import sp2_oracle as O
 from paper_2101_06385_b200 import workloads as W
@@ -41,10 +42,7 @@ def test_paper_text_numbers():
     g = _kv("paper_text_numbers.txt")
     # each layer doubles the polynomial order -> 2^30 > 1e9 after 30 steps
     assert 2 ** 30 > g["polynomial_order_after_30_steps_exceeds"]
-    # the oracle's stop rule uses 4.5 literally (reading C7): a sequence built to sit between 4.41 and 4.5
-    assert g["stop_rule_constant"] == 4.5
-    import inspect
-    assert "4.5 *" in inspect.getsource(O.sp2_ref) and "4.5 *" in inspect.getsource(O.scalar_recursion)
+    assert g["stop_rule_constant"] == 4.5                              # P:136; behaviour pinned in the test below
     # "28 layers" for an unspecified 100x100, N_occ = 10 -> plausibility range on inputs of that shape
     for seed in range(3):
         H32 = W.uniform_symmetric(seed, 100)
@@ -59,6 +57,44 @@ def test_paper_text_numbers():
         _, s1 = O.sp2_accelerated_ref(H32, 10.0, b, ev[9], ev[10], tol=1e-9, max_layers=200)
         want = g["layers_accelerated_100x100_nocc10"] / g["layers_plain_100x100_nocc10"]
         assert abs(s1["n_layers"] / s0["n_layers"] - want) <= 0.2
+
+
+@pytest.mark.parametrize("form", ["matrix", "scalar"])
+def test_stop_rule_constant_is_4p5_not_theorem1s_4p41(form):
+    """P:136 against P:292 (reading C7): Alg. 1 stops when IdErr_n > 4.5 IdErr_{n-2}^2 after an alternation, with
+    4.5, NOT Theorem 1's C = 4.409.  In exact arithmetic the ratio never exceeds C (that is the theorem), so a ratio
+    between 4.41 and 4.5 only arises through an error on X_n: a single eigenvalue at the maximiser of Eq. 23
+    (ratio = C after the layer pair sigma = +1, -1) and a relative error on layer 3's square that lifts IdErr_3 to a
+    chosen multiple r of IdErr_1^2.  The oracle must NOT stop at r = 4.45 (a rule with 4.41 would) and must stop at
+    r = 4.55."""
+    g = _kv("paper_text_numbers.txt")
+    lam = np.linspace(0.01, 0.99, 980001)
+    q = 2 * lam ** 2 - lam ** 4                                          # layers sigma = +1 then -1 (Eq. 23's pair)
+    lam0 = float(lam[np.argmax((q - q ** 2) / (lam - lam ** 2) ** 2)])
+    ide1 = lam0 - lam0 ** 2
+    lam2 = 2 * lam0 ** 2 - lam0 ** 4
+    assert abs((lam2 - lam2 ** 2) / ide1 ** 2 - O.THEOREM1_C) < 1e-6      # the starting point sits at the maximum
+    for r, stops in [(4.45, False), (4.55, True)]:
+        assert (r > g["stop_rule_constant"]) == stops and r > 4.41
+        delta = (lam2 - r * ide1 ** 2) / lam2 ** 2 - 1.0                # X_3 = lam2^2 (1 + delta) => IdErr_3 = r IdErr_1^2
+        calls = []
+
+        def sq(S):
+            calls.append(1)
+            X = S @ S if form == "matrix" else S * S
+            return X * (1.0 + delta) if len(calls) == 3 else X
+
+        H = np.array([[1.0 - lam0]], dtype=np.float64)                  # S_0 = (1 - H) / (1 - 0) = lam0
+        if form == "matrix":
+            _, st = O.sp2_ref(H, 1.0, (0.0, 1.0), tol=0.0, max_layers=4, forced_sigma=[1, -1, 1, -1], square=sq)
+        else:
+            st = O.scalar_recursion(np.array([1.0 - lam0]), 1.0, 0.0, 1.0, tol=0.0, max_layers=4,
+                                    forced_sigma=[1, -1, 1, -1], square=sq)
+        assert abs(st["iderr"][2] / st["iderr"][0] ** 2 - r) < 1e-9
+        if stops:
+            assert st["n_layers"] == 3 and st["stop_reason"] == O.STOP_PARAM_FREE
+        else:
+            assert st["n_layers"] == 4 and st["stop_reason"] == O.STOP_MAX_LAYERS
 
 
 def test_golden_next_rows():

@@ -54,11 +54,26 @@ def test_config3_full_size(big, auto):
     assert idem <= P.TOL_IDEM
     assert comm <= 1e-3
     assert torch.equal(D, D.T)
+    del Hd, Hs
+    # EVERY element against the closed form D* = Q_occ Q_occ^T (Eq. 6): one FP64 product on the device in the
+    # harness (the samples above are the fast pre-check; a defect confined to one tail strip cannot hide from this)
+    Qo = torch.from_numpy(np.ascontiguousarray(w.Q[:, : int(w.N_occ)])).cuda()
+    Dstar = Qo @ Qo.T
+    del Qo
+    diff = (Dc - Dstar).abs_()
+    full_err = float(diff.max())
+    worst = int(diff.argmax())
+    print(f"config3 N={N} auto={auto}: FULL elementwise max|D - D*| = {full_err:.3e} at ({worst // N}, {worst % N}); "
+          f"rms = {float(diff.pow(2).mean().sqrt()):.3e}")
+    del diff, Dstar
+    assert full_err <= P.TOL_D
     # branch sequence / traces per reading C6: scalar recursion on the known eigenvalues
     st = O.scalar_recursion(w.eps, w.N_occ, used[0], used[1], tol=w.tol, max_layers=w.max_layers)
     P.branch_prefix_check(info, st, w.N_occ)
     P.replay_check(info, None, w.N_occ, used, eigs=w.eps)
-    assert info["n_layers"] <= st["n_layers"] + 2 and info["n_layers"] >= st["n_layers"] - 6
+    # the GPU stops 3-4 layers before the FP64 recursion (27 / 46 layers with these bounds against 23 / 43): its
+    # noise-floor reading of "IdErr <= 0" (C25) fires where FP64 still resolves IdErr.  Measured: -4, -3.
+    assert st["n_layers"] - 4 <= info["n_layers"] <= st["n_layers"] + 2
 
 
 def test_config3_literal_tensor_core_diagonal_explicit_bounds(big):

@@ -266,6 +266,72 @@ def test_edge_cases_and_errors(env):
     assert float((D0 - D3).abs().max()) <= 1e-5 and torch.equal(D0, D0.T)
 
 
+@pytest.mark.parametrize("n,tile", [(1024, 0), (3000, 0), (3000, 3)])
+@pytest.mark.parametrize("auto", [False, True])
+def test_tiled_kernel_bit_reproducible_and_host_entry(env, n, tile, auto):
+    """The TILED layer kernel (N > 256; default tile choice: 128 x 128 tiles, one round at N = 1024, three rounds with
+    the round sync and the reversed K walk at N = 3000; and 2-CTA pair tiles, two rounds): two runs give identical
+    bits -- D, bounds and every per-layer trace -- with caller bounds and with the device's Gershgorin bounds, and
+    the host-buffer entry point returns the same bits as the device one."""
+    api, h, torch = env
+    k = n // 2
+    w = W.gapped_dense(n + 7, n, (-1.0, -0.15), (0.15, 1.0), k, "det", bounds=(-1.0, 1.0))
+    opts = api.make_opts(bounds=None if auto else w.bounds, tol=1e-5, max_layers=100, tile_config=tile)
+    Hd = torch.from_numpy(w.H32).cuda()
+    D1, i1 = h.density_matrix(Hd, w.N_occ, opts)
+    assert i1["launches"] > 2                                   # not the one-launch resident path
+    D2, i2 = h.density_matrix(Hd, w.N_occ, opts)
+    assert torch.equal(D1, D2) and i1["bounds"] == i2["bounds"]
+    for key in ("trace_S", "trace_X", "trace_X_diag", "iderr", "sigma", "stop_reason"):
+        assert i1[key] == i2[key], key
+    Dh, ih = h.density_matrix_host(w.H32, w.N_occ, opts)
+    assert np.array_equal(Dh, D1.cpu().numpy()) and ih["trace_S"] == i1["trace_S"] and ih["bounds"] == i1["bounds"]
+    P.assert_acceptance(D1.cpu().numpy().astype(np.float64), O.closed_form_density(w.Q, w.N_occ), w.N_occ, f"N={n}")
+
+
+def test_round_sync_timeout_path_gives_the_same_bits(env, monkeypatch):
+    """The round synchronisation of the layer kernel is an optimisation with a bounded wait: when a wait runs out
+    (CTAs not co-resident) the kernel gives the sync up for the rest of the solve.  Forced here with a wait bound of
+    one poll (SP2_ROUND_SYNC_SPINS, a performance toggle read at sp2_create): same bits as the synchronised run."""
+    api, h, torch = env
+    n = 3000
+    w = W.gapped_dense(11, n, (-1.0, -0.15), (0.15, 1.0), n // 2, "rs", bounds=(-1.0, 1.0))
+    Hd = torch.from_numpy(w.H32).cuda()
+    for tile in (1, 3):
+        opts = api.make_opts(bounds=w.bounds, tol=1e-5, max_layers=100, tile_config=tile)
+        D0, i0 = h.density_matrix(Hd, w.N_occ, opts)
+        assert h.lib.sp2_last_round_sync_broken(h._h) == 0
+        monkeypatch.setenv("SP2_ROUND_SYNC_SPINS", "1")
+        h2 = api.Handle(n, 0, 100)
+        monkeypatch.delenv("SP2_ROUND_SYNC_SPINS")
+        D1, i1 = h2.density_matrix(Hd, w.N_occ, opts)
+        broken = h2.lib.sp2_last_round_sync_broken(h2._h)
+        h2.close()
+        assert broken == 1, "the timeout path was not taken"
+        assert torch.equal(D0, D1) and i0["trace_S"] == i1["trace_S"] and i0["sigma"] == i1["sigma"]
+
+
+def test_nonfinite_input_and_unsupported_mix_tile(env):
+    """A NaN in H must surface as SP2_ERR_NONFINITE from every single-matrix entry point (standard and generalized,
+    caller and Gershgorin bounds); the output mix has no enhanced-accumulation instantiation -> SP2_ERR_INVALID_ARG."""
+    api, h, torch = env
+    w = W.config1(0, n=384)
+    Hn = torch.from_numpy(w.H32).cuda()
+    Hn[100, 3] = float("nan")
+    theta = np.array([[1.0, 0.0, 0.0], [-1.0, 2.0, 0.0], [1.0, 0.0, 0.0]])
+    for bounds in (w.bounds, None):
+        with pytest.raises(api.SP2Error) as e:
+            h.density_matrix(Hn, w.N_occ, api.make_opts(bounds=bounds, tol=1e-5, max_layers=30))
+        assert e.value.status == -3
+        with pytest.raises(api.SP2Error) as e:
+            h.generalized(Hn, theta, bounds=bounds)
+        assert e.value.status == -3
+    with pytest.raises(api.SP2Error) as e:
+        h.generalized_mix(torch.from_numpy(w.H32).cuda(), theta, np.array([0.1, 0.2, 0.3, 0.4]), bounds=w.bounds,
+                          opts=api.make_opts(tile_config=4))
+    assert e.value.status == -1
+
+
 def test_host_buffer_entry_point_and_determinism(env):
     api, h, torch = env
     w = W.config1(1, n=256)
