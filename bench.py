@@ -165,6 +165,92 @@ def cpu_oracle_sample(w, budget_s: float = 20.0):
             "ms_per_layer": dt / st["n_layers"] * 1e3, "n": n}
 
 
+def other_configs(api, W, torch, dev, stream, _time):
+    """detail.configs: BASELINE.json configs[0], [1], [3], [4] (the headline is configs[2]) through the same C ABI:
+    ms per call (CUDA events, median of 5 after a warm-up call), layers, and the parity triple of BASELINE north_star
+    -- max |X - X*|, |Tr - N_occ|, ||X^2 - X||_F / sqrt(N) -- against the CLOSED FORM each input is built for
+    (Eq. 6: D* = Q_occ Q_occ^T; config 2: the LAPACK eigenprojector, FP64 on the device; config 4:
+    X* = Q diag(p(eps)) Q^T with p the scalar polynomial of Eq. 17), all evaluated here in FP64 with torch / numpy."""
+    out = {}
+
+    def triple(X, Xstar, nocc):
+        Xd = X.double()
+        return {"max_abs_err": float((Xd - Xstar).abs().max()),
+                "trace_err": (float(torch.trace(Xd)) - nocc) if nocc is not None else None,
+                "idempotency": (float(torch.linalg.norm(Xd @ Xd - Xd)) / np.sqrt(X.shape[-1])) if nocc is not None else None,
+                "symmetric": bool(torch.equal(X, X.transpose(-1, -2)))}
+
+    # ---- config 1: N = 128, explicit (-1, 1) and Gershgorin bounds (one launch of the resident kernel)
+    w = W.config1(0)
+    Hd = torch.from_numpy(w.H32).to(dev)
+    Qo = torch.from_numpy(w.Q[:, : int(w.N_occ)]).to(dev)
+    Dstar = Qo @ Qo.T
+    h1 = api.Handle(128, 0, 120)
+    for name, bnd in (("explicit", w.bounds), ("gershgorin", None)):
+        o = api.make_opts(bounds=bnd, tol=w.tol, max_layers=w.max_layers)
+        ms = _time(lambda: h1.density_matrix(Hd, w.N_occ, o, stream=stream))
+        D, info = h1.density_matrix(Hd, w.N_occ, o, stream=stream)
+        out[f"config1_N128_{name}"] = dict(ms_per_D=ms, layers=info["n_layers"], launches=info["launches"],
+                                           **triple(D, Dstar, w.N_occ))
+    h1.close()
+    # ---- config 2: N = 2048 tight-binding-like, Gershgorin bounds
+    w = W.config2(0)
+    Hd = torch.from_numpy(w.H32).to(dev)
+    E, V = torch.linalg.eigh(torch.tril(Hd.double()) + torch.tril(Hd.double(), -1).T)
+    k = int(w.N_occ)
+    Dstar = V[:, :k] @ V[:, :k].T
+    h2 = api.Handle(4096, 0, 120)
+    o = api.make_opts(bounds=None, tol=w.tol, max_layers=w.max_layers)
+    ms = _time(lambda: h2.density_matrix(Hd, w.N_occ, o, stream=stream))
+    D, info = h2.density_matrix(Hd, w.N_occ, o, stream=stream)
+    t = np.diff(np.array(info["t_end_ns"], dtype=np.float64)) * 1e-3
+    out["config2_N2048_tight_binding"] = dict(ms_per_D=ms, layers=info["n_layers"], us_per_layer=float(np.median(t)),
+                                              executed_tflops_3N3=3.0 * 2048 ** 3 / (float(np.median(t)) * 1e-6) / 1e12,
+                                              homo_lumo_gap=float(E[k] - E[k - 1]), **triple(D, Dstar, w.N_occ))
+    # ---- config 4: N = 4096 generalized network, 30 layers (sigma alternating +1, -1; w_n, b_n from the seed)
+    w = W.config4(0, device=dev)
+    L = w.extra["layers"]
+    sig = np.array([1, -1] * (L // 2 + 1))[:L]
+    wt, bs = w.extra["weights"], w.extra["biases"]
+    lam = (w.bounds[1] - w.eps) / (w.bounds[1] - w.bounds[0])          # eigenvalues of S_0 (Alg. 1, P:136)
+    for n in range(L):                                                 # Eq. 17 on each eigenvalue (reading C19)
+        lam = wt[n] * (sig[n] * lam * lam + (1 - sig[n]) * lam) + bs[n]
+    Hd = torch.from_numpy(w.H32).to(dev)
+    Qd = torch.from_numpy(w.Q).to(dev)
+    Xstar = (Qd * torch.from_numpy(lam).to(dev)[None, :]) @ Qd.T
+    ms = _time(lambda: h2.generalized_wb(Hd, sig, wt, bs, bounds=w.bounds, stream=stream))
+    X, info = h2.generalized_wb(Hd, sig, wt, bs, bounds=w.bounds, stream=stream)
+    tr = triple(X, Xstar, None)
+    tr["trace_err"] = float(torch.trace(X.double())) - float(lam.sum())
+    out["config4_N4096_generalized_30_layers"] = dict(ms_per_call=ms, layers=L, us_per_layer=ms / L * 1e3,
+                                                      executed_tflops_3N3=3.0 * 4096 ** 3 * L / (ms * 1e-3) / 1e12, **tr)
+    h2.close()
+    del Qd, Xstar, X, Hd
+    # ---- config 5: 1024 matrices of N = 256, one launch
+    w = W.config5(0)
+    Hd = torch.from_numpy(w.H32).to(dev)
+    Qo = torch.from_numpy(np.ascontiguousarray(w.Q[:, :, : int(w.N_occ)])).to(dev)
+    Dstar = Qo @ Qo.transpose(1, 2)
+    h5 = api.Handle(256, 1024, 60)
+    Db = torch.empty_like(Hd)
+    for name, bnd in (("explicit", w.bounds), ("gershgorin", None)):
+        o = api.make_opts(bounds=bnd, tol=w.tol, max_layers=w.max_layers)
+        ms = _time(lambda: h5.density_matrix_batched(Hd, w.N_occ, o, out=Db, stream=stream))
+        _, info = h5.density_matrix_batched(Hd, w.N_occ, o, out=Db, stream=stream)
+        Dd = Db.double()
+        idem = torch.linalg.norm((Dd @ Dd - Dd).reshape(1024, -1), dim=1) / 16.0
+        trs = torch.diagonal(Dd, dim1=1, dim2=2).sum(1) - w.N_occ
+        layers = float(info["n_layers"].mean())
+        out[f"config5_1024xN256_{name}"] = dict(
+            ms_per_batch=ms, matrices_per_s=1024 / (ms * 1e-3), layers_mean=layers,
+            executed_tflops_3N3=3.0 * 256 ** 3 * float(info["n_layers"].sum()) / (ms * 1e-3) / 1e12,
+            max_abs_err=float((Dd - Dstar).abs().max()), trace_err=float(trs.abs().max()),
+            idempotency=float(idem.max()), symmetric=bool(torch.equal(Db, Db.transpose(1, 2))),
+            worst_status=int(info["status"]))
+    h5.close()
+    return out
+
+
 def run_reference(args):
     """--impl reference: the oracle timed on the host cores (rank 0 only)."""
     rank = int(os.environ.get("RANK", "0"))
@@ -216,6 +302,7 @@ def main():
     ap.add_argument("--exact-diag", type=int, default=1)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-configs", action="store_true", help="skip detail.configs (BASELINE configs 1, 2, 4, 5)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -284,29 +371,29 @@ def main():
     del Dc
     info_timed = info
 
-    # ---- dominant kernel (fused layer) duration: CUDA events, (T(all layers) - T(1 layer)) / (layers - 1)
-    opts1 = api.make_opts(bounds=bounds, tol=w.tol, max_layers=1, tile_config=args.tile, control=args.control,
-                          exact_diag=args.exact_diag)
-    e1 = []
-    for i in range(4):
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record(stream)
-        h.density_matrix(H, w.N_occ, opts1, out=D, stream=stream, check=False)
-        b.record(stream)
-        torch.cuda.synchronize()
-        if i:
-            e1.append(a.elapsed_time(b))
-    t_one = float(np.median(e1))
-    t_layer_ms = (float(np.median(ms_steps)) - t_one) / max(1.0, n_layers - 1)
-    t_layer_dev_ms = float(np.median(layer_ms)) if layer_ms else None
+    # ---- dominant kernel (fused layer) duration.  The layer launches sit inside the device-side WHILE graph, so CUDA
+    # events cannot bracket one of them; two measurements of the same timed region instead:
+    #   launch_ms              = event-timed step / layers of the step: a purely event-based UPPER bound on the average
+    #                            launch (it still holds the ~0.3 % of setup kernels), used for `achieved`;
+    #   launch_ms_device_timer = mean interval between consecutive layer completions (%globaltimer stamps written by
+    #                            each layer's last CTA), the kernel-to-kernel period itself.
+    # (Differences of separately timed solves are not used: under the 1 kW cap the clock state depends on what ran
+    # just before, which biased them in both directions.)
+    t_layer_ms = float(np.median(ms_steps)) / max(1.0, n_layers)
+    t_layer_dev_ms = float(np.mean(layer_ms)) if layer_ms else None
+    t_setup_ms = max(0.0, float(np.median(ms_steps)) - n_layers * t_layer_dev_ms) if layer_ms else None
     exec_tflops = 3.0 * N ** 3 / (t_layer_ms * 1e-3) / 1e12
     peak = float(peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]))
     roofline = {"bound": "tensor", "kernel": "k_sp2_layer (fused symmetric square + epilogue)",
                 "achieved": exec_tflops, "peak": peak, "unit": "TFLOP/s", "frac": exec_tflops / peak,
                 "peak_source": peak_src + ": cuBLAS bf16 sustained (fp16 and bf16 share the tensor rate)",
                 "algorithmic_flops_per_launch": 3.0 * N ** 3, "launch_ms": t_layer_ms,
+                "launch_ms_how": "CUDA events on the launching stream: median step time / layers of the step (upper "
+                                 "bound: includes the setup kernels' ~0.3 %)",
                 "launch_ms_device_timer": t_layer_dev_ms, "traffic": None}
-    prof = os.path.join(ROOT, "profiles", "r01_layer_traffic.json")
+    prof = os.path.join(ROOT, "profiles", "r02_layer_traffic.json")
+    if not os.path.exists(prof):
+        prof = os.path.join(ROOT, "profiles", "r01_layer_traffic.json")
     if os.path.exists(prof):
         try:
             with open(prof) as f:
@@ -328,16 +415,20 @@ def main():
     hbm_peak = float(peaks["hbm_gbs"])
     t_g = _time(lambda: h.gershgorin(H, stream=stream))
     t_s = _time(lambda: api.split_fp16(H, 13, stream=stream))
+    tri_bytes = 2.0 * N * (N + 1)              # lower triangle incl. diagonal, 4 B each
     hbm_kernels = {
-        "gershgorin": {"ms": t_g, "algorithmic_GBps": 4.0 * N * N / (t_g * 1e-3) / 1e9,
-                       "read_GBps_lower_triangle_only": 2.0 * N * N / (t_g * 1e-3) / 1e9,
-                       "frac_of_measured_hbm": 4.0 * N * N / (t_g * 1e-3) / 1e9 / hbm_peak,
-                       "note": "SURVEY 8(d): 4 B/element; the kernel reads only H's lower triangle (2 B/element), "
-                               "time includes the call's final sync + 16-byte D2H"},
-        "split_fp16": {"ms": t_s, "algorithmic_GBps": 8.0 * N * N / (t_s * 1e-3) / 1e9,
+        "gershgorin": {"ms": t_g, "bytes_moved": tri_bytes + 8.0 * N * ((N + 63) // 64) * 2,
+                       "moved_GBps": (tri_bytes + 16.0 * N * ((N + 63) // 64)) / (t_g * 1e-3) / 1e9,
+                       "frac_of_measured_hbm": (tri_bytes + 16.0 * N * ((N + 63) // 64)) / (t_g * 1e-3) / 1e9 / hbm_peak,
+                       "algorithmic_GBps_4B_per_element": 4.0 * N * N / (t_g * 1e-3) / 1e9,
+                       "note": "reads H's lower triangle only (2 B/element) + writes/reads the per-tile row and column "
+                               "sums; SURVEY 8(d) counts 4 B/element (algorithmic rate, not a utilisation); the time "
+                               "includes the call's final sync + 16-byte D2H"},
+        "split_fp16": {"ms": t_s, "bytes_moved": 8.0 * N * N, "moved_GBps": 8.0 * N * N / (t_s * 1e-3) / 1e9,
                        "frac_of_measured_hbm": 8.0 * N * N / (t_s * 1e-3) / 1e9 / hbm_peak,
                        "note": "4 B read + 4 B written per element; time includes two torch.empty allocations"},
-        "setup_ms_bounds_affine_split_copyout": t_one - t_layer_ms,
+        "setup_ms_bounds_affine_split_copyout": t_setup_ms,
+        "setup_how": "event-timed step - layers x mean device-timer layer interval of the same steps (clamped at 0)",
     }
     yard = None
     if rank == 0:
@@ -393,17 +484,32 @@ def main():
         _barrier(world)
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         k2, lay2 = max(1, min(args.steps, 3)), 0
+        ph = []
         a.record(stream)
         for _ in range(k2):
             _, i2 = h.density_matrix_host(Hh, w.N_occ, opts, out=Dh, stream=stream)
             lay2 += i2["n_layers"]
+            ph.append((i2["h2d_ms"], i2["solve_ms"], i2["d2h_ms"]))
         b.record(stream)
         torch.cuda.synchronize()
         t2 = _max_over_ranks(a.elapsed_time(b) * 1e-3, world)
+        ph = np.median(np.array(ph), axis=0)
+        nb = int(N) * int(N) * 4
         e2e = {"value": world * 6.0 * N ** 3 * lay2 / t2 / 1e12, "unit": UNIT, "ms_per_step": t2 / k2 * 1e3,
-               "h2d_bytes_per_step": int(N) * int(N) * 4, "d2h_bytes_per_step": int(N) * int(N) * 4,
+               "h2d_bytes_per_step": nb, "d2h_bytes_per_step": nb,
+               "h2d_ms": float(ph[0]), "solve_ms": float(ph[1]), "d2h_ms": float(ph[2]),
+               "h2d_GBps": nb / (ph[0] * 1e-3) / 1e9, "d2h_GBps": nb / (ph[2] * 1e-3) / 1e9,
+               "phases_how": "CUDA events recorded by the library around each phase of the same calls (median)",
                "api": "sp2_density_matrix_host (pinned host buffers)"}
         del Hh, Dh
+
+    configs = None
+    if rank == 0 and not args.no_configs:
+        h.close()
+        del H, D
+        torch.cuda.empty_cache()
+        configs = other_configs(api, W, torch, dev, stream, _time)
+        h = None
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -433,13 +539,15 @@ def main():
                        "D_exactly_symmetric": symmetric,
                        "frac_of_same_run_cublas_fp16": (exec_tflops / yard["tflops"]) if yard else None,
                        "cublas_fp16_yardstick": yard, "hbm_kernels": hbm_kernels, "refinement_next1": refine, "accelerated_next3": accel,
+                       "configs": configs,
                        "paper_context": "paper: ~120 TFLOP/s on A100 (P:204), other hardware, count unstated",
                        "wall_s_timed_region": t_wall},
             "clocks": clocks, "roofline": roofline, "e2e": e2e, "cpu_baseline": cpu,
             "gpu_launches": int(launches),
         }
         print(json.dumps(line))
-    h.close()
+    if h is not None:
+        h.close()
     if world > 1:
         import torch.distributed as dist
 

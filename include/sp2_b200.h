@@ -227,6 +227,9 @@ const char* sp2_last_cuda_error(void);
 /* Number of kernels the last solve call on this handle launched (graph nodes executed are counted by the
  * device-side layer counter: setup kernels + layers + copy-out). */
 int         sp2_last_launch_count(sp2_handle_t h);
+/* Device-side durations (CUDA events on `stream`) of the three phases of the last sp2_density_matrix_host call on
+ * this handle, in ms: {host -> device copy of H, the solve, device -> host copy of D}. */
+void        sp2_last_host_timing(sp2_handle_t h, double ms[3]);
 /* Diagnostic: 1 if, during the last single-matrix solve on this handle, a round-synchronisation wait of the layer
  * kernel ran out and the kernel gave the synchronisation up (performance only: results are unaffected). */
 int         sp2_last_round_sync_broken(sp2_handle_t h);

@@ -21,7 +21,7 @@ EXPORTS = ["sp2_default_opts", "sp2_create", "sp2_destroy", "sp2_workspace_bytes
            "sp2_density_matrix", "sp2_density_matrix_host", "sp2_generalized", "sp2_generalized_mix", "sp2_generalized_wb",
            "sp2_density_matrix_batched", "sp2_generalized_batched", "sp2_refine_energy", "sp2_split_fp16",
            "sp2_gershgorin", "sp2_status_string", "sp2_last_cuda_error", "sp2_last_launch_count",
-           "sp2_last_round_sync_broken", "sp2_version"]
+           "sp2_last_host_timing", "sp2_last_round_sync_broken", "sp2_version"]
 
 
 class LayerStat(C.Structure):
@@ -100,6 +100,7 @@ def load() -> C.CDLL:
     lib.sp2_last_cuda_error.argtypes = []; lib.sp2_last_cuda_error.restype = C.c_char_p
     lib.sp2_last_launch_count.argtypes = [vp]; lib.sp2_last_launch_count.restype = C.c_int
     lib.sp2_last_round_sync_broken.argtypes = [vp]; lib.sp2_last_round_sync_broken.restype = C.c_int
+    lib.sp2_last_host_timing.argtypes = [vp, dp]; lib.sp2_last_host_timing.restype = None
     lib.sp2_version.argtypes = []; lib.sp2_version.restype = C.c_char_p
     _lib = lib
     return lib
@@ -205,7 +206,10 @@ class Handle:
         if st < 0:
             raise SP2Error(st, "sp2_density_matrix_host")
         info = _stats_to_dict(stats, nl.value)
-        info.update(status=st, n_layers=nl.value, bounds=(bounds[0], bounds[1]))
+        ms = (C.c_double * 3)()
+        self.lib.sp2_last_host_timing(self._h, ms)
+        info.update(status=st, n_layers=nl.value, bounds=(bounds[0], bounds[1]),
+                    h2d_ms=ms[0], solve_ms=ms[1], d2h_ms=ms[2])
         return D, info
 
     # -- generalized network

@@ -49,7 +49,7 @@ struct sp2_handle_s {
     unsigned long long* rowsq[2] = {nullptr, nullptr};   // fixed-point row sums of squares of S (ping-pong)
     Ctrl* ctrl = nullptr;
     sp2_layer_stat_t* stats_dev = nullptr;
-    double* thetas_dev = nullptr;
+    float* thetas_dev = nullptr;
     WorkItem* items_dev[2] = {nullptr, nullptr};   // [0] solves, [1] refinement layers (different tile config)
     int items_cap = 0;
     // batched workspace
@@ -57,17 +57,25 @@ struct sp2_handle_s {
     int* bnl_dev = nullptr;
     int* bstatus_dev = nullptr;
     double* bbounds_dev = nullptr;
-    double* bnocc_dev = nullptr;
+    long long* bnocc_dev = nullptr;        // per-matrix N_occ, 2^40 fixed point
+    long long* bnocc_host = nullptr;
     double* bhl_dev = nullptr;      // [batch][2] HOMO / LUMO estimates of the accelerated batched solve
+    // pinned host mirrors of the batched outputs (a device -> pageable copy is staged and slow: 2.9 MB of statistics
+    // for 1024 matrices cost ~1 ms, a fifth of the whole batched solve)
+    sp2_layer_stat_t* bstats_host = nullptr;
+    int* bnl_host = nullptr;        // [batch] layers, then [batch] status
+    double* bbounds_host = nullptr;
     // pinned host mirrors
     Ctrl* ctrl_host = nullptr;
     sp2_layer_stat_t* stats_host = nullptr;
-    double* thetas_host = nullptr;
+    float* thetas_host = nullptr;          // pinned; what is uploaded (FP32, the epilogue's type)
     double* bounds_host = nullptr;
     // host staging for the *_host entry point
     float* stage_H = nullptr;
     float* stage_D = nullptr;
     size_t stage_elems = 0;
+    cudaEvent_t host_ev[4] = {nullptr, nullptr, nullptr, nullptr};   // H2D start, solve start, D2H start, end
+    float host_ms[3] = {0.f, 0.f, 0.f};
     PFN_encodeTiled encode = nullptr;
     // (N, Np, cfg, scale_log2, exact_diag | mix << 1 | enh_kc << 2): everything a captured launch bakes in
     std::map<std::tuple<int, int, int, int, int>, LoopGraph> graphs;
@@ -124,6 +132,29 @@ extern "C" void sp2_default_opts(sp2_opts_t* o) {
 }
 
 static double opt_kappa(const sp2_opts_t& o) { return o.noise_kappa < 0.0 ? 0.125 : o.noise_kappa; }
+// kappa as a 16.16 fixed-point factor for the integer control step (sp2_control.cuh); 0 disables the test
+static int opt_kappa_q16(const sp2_opts_t& o) {
+    const double k = opt_kappa(o);
+    if (!(k > 0.0)) return 0;
+    const double q = k * 65536.0 + 0.5;
+    return q >= 2147483647.0 ? 2147483647 : (q < 1.0 ? 1 : (int)q);
+}
+// fixed-point image of a host double, saturated well inside the 64-bit range
+static fx_t to_fx(double x) {
+    if (!(x == x)) return 0;
+    if (x > 4.0e6) x = 4.0e6;
+    if (x < -4.0e6) x = -4.0e6;
+    return fx_from_double_host(x);
+}
+static void stats_to_double(sp2_layer_stat_t* st, int n) {       // the device writes raw fixed-point integers
+    for (int i = 0; i < n; ++i) {
+        fx_t v[4];
+        memcpy(&v[0], &st[i].trace_S, 8); memcpy(&v[1], &st[i].trace_X, 8);
+        memcpy(&v[2], &st[i].trace_X_diag, 8); memcpy(&v[3], &st[i].iderr, 8);
+        st[i].trace_S = fx_to_double(v[0]); st[i].trace_X = fx_to_double(v[1]);
+        st[i].trace_X_diag = fx_to_double(v[2]); st[i].iderr = fx_to_double(v[3]);
+    }
+}
 static int opt_enh_kc(const sp2_opts_t* o) { return (o && o->enh_kc > 0) ? o->enh_kc : 2; }
 
 extern "C" size_t sp2_workspace_bytes(int N_max, int batch_max, int max_layers) {
@@ -155,6 +186,7 @@ extern "C" sp2_status_t sp2_destroy(sp2_handle_t h) {
         if (kv.second.graph) cudaGraphDestroy(kv.second.graph);
     }
     if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
+    for (int i = 0; i < 4; ++i) if (h->host_ev[i]) cudaEventDestroy(h->host_ev[i]);
     cudaFree(h->S);
     for (int a = 0; a < 2; ++a)
         for (int b = 0; b < 2; ++b) cudaFree(h->hl[a][b]);
@@ -164,6 +196,7 @@ extern "C" sp2_status_t sp2_destroy(sp2_handle_t h) {
     cudaFree(h->bbounds_dev); cudaFree(h->bnocc_dev); cudaFree(h->bhl_dev);
     cudaFreeHost(h->ctrl_host); cudaFreeHost(h->stats_host); cudaFreeHost(h->thetas_host);
     cudaFreeHost(h->bounds_host); cudaFree(h->stage_H); cudaFree(h->stage_D);
+    cudaFreeHost(h->bstats_host); cudaFreeHost(h->bnl_host); cudaFreeHost(h->bbounds_host); cudaFreeHost(h->bnocc_host);
     delete h;
     return SP2_OK;
 }
@@ -203,7 +236,7 @@ extern "C" sp2_status_t sp2_create(sp2_handle_t* out, int N_max, int batch_max, 
     A((void**)&h->rowsq[1], Np * sizeof(unsigned long long));
     A((void**)&h->ctrl, sizeof(Ctrl));
     A((void**)&h->stats_dev, (size_t)max_layers * sizeof(sp2_layer_stat_t));
-    A((void**)&h->thetas_dev, (size_t)max_layers * kThetaStride * sizeof(double));
+    A((void**)&h->thetas_dev, (size_t)max_layers * kThetaStride * sizeof(float));
     h->items_cap = (int)((Np / 128) * (Np / 128 + 1) / 2) + 1024;
     A((void**)&h->items_dev[0], (size_t)h->items_cap * sizeof(WorkItem));
     A((void**)&h->items_dev[1], (size_t)h->items_cap * sizeof(WorkItem));
@@ -214,7 +247,7 @@ extern "C" sp2_status_t sp2_create(sp2_handle_t* out, int N_max, int batch_max, 
         A((void**)&h->bnl_dev, bm * sizeof(int));
         A((void**)&h->bstatus_dev, bm * sizeof(int));
         A((void**)&h->bbounds_dev, bm * 2 * sizeof(double));
-        A((void**)&h->bnocc_dev, bm * sizeof(double));
+        A((void**)&h->bnocc_dev, bm * sizeof(long long));
         A((void**)&h->bhl_dev, bm * 2 * sizeof(double));
     }
     auto AH = [&](void** p, size_t bytes) {
@@ -224,9 +257,16 @@ extern "C" sp2_status_t sp2_create(sp2_handle_t* out, int N_max, int batch_max, 
     };
     AH((void**)&h->ctrl_host, sizeof(Ctrl));
     AH((void**)&h->stats_host, (size_t)max_layers * sizeof(sp2_layer_stat_t));
-    AH((void**)&h->thetas_host, (size_t)max_layers * kThetaStride * sizeof(double));
+    AH((void**)&h->thetas_host, (size_t)max_layers * kThetaStride * sizeof(float));
     AH((void**)&h->bounds_host, 2 * sizeof(double));
     AH((void**)&h->obs_host, 8 * sizeof(double));
+    {
+        const size_t bm = (size_t)(batch_max > 0 ? batch_max : 1);
+        AH((void**)&h->bstats_host, bm * max_layers * sizeof(sp2_layer_stat_t));
+        AH((void**)&h->bnl_host, bm * 2 * sizeof(int));
+        AH((void**)&h->bbounds_host, bm * 2 * sizeof(double));
+        AH((void**)&h->bnocc_host, bm * sizeof(long long));
+    }
     if (st == SP2_OK) {
         cudaError_t e = cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking);
         if (e != cudaSuccess) st = cuda_fail(e, "cudaStreamCreate");
@@ -463,15 +503,15 @@ static sp2_status_t solve_single(sp2_handle_s* h, const float* H_dev, int N, int
     // ---- control block
     Ctrl* c = h->ctrl_host;
     memset(c, 0, ctrl_header_bytes());
-    c->N_occ = N_occ; c->eps_alt = o->eps_alt; c->tol = o->tol;
+    c->N_occ = to_fx(N_occ); c->eps_alt = to_fx(o->eps_alt); c->tol = (o->tol > 0.0) ? (to_fx(o->tol) > 0 ? to_fx(o->tol) : 1) : 0;
     c->eps_min = o->eps_min; c->eps_max = o->eps_max;
     c->N = N; c->mode = mode; c->max_layers = max_layers; c->auto_bounds = o->auto_bounds;
-    c->noise_kappa = opt_kappa(*o);
+    c->kappa_q16 = opt_kappa_q16(*o);
     c->accelerated = (mode == MODE_STANDARD && o->accelerated) ? 1 : 0;
     c->homo = o->homo; c->lumo = o->lumo;
     CK(cudaMemcpyAsync(h->ctrl, c, ctrl_header_bytes(), cudaMemcpyHostToDevice, st));
     if (mode == MODE_GENERALIZED)
-        CK(cudaMemcpyAsync(h->thetas_dev, h->thetas_host, (size_t)max_layers * kThetaStride * sizeof(double),
+        CK(cudaMemcpyAsync(h->thetas_dev, h->thetas_host, (size_t)max_layers * kThetaStride * sizeof(float),
                            cudaMemcpyHostToDevice, st));
     CK(cudaMemsetAsync(h->stats_dev, 0, (size_t)max_layers * sizeof(sp2_layer_stat_t), st));
     // ---- padding rows/columns of S_0 are zero (inert: eigenvalue 0 is a fixed point of both branches)
@@ -525,7 +565,11 @@ static sp2_status_t solve_single(sp2_handle_s* h, const float* H_dev, int N, int
     h->last_launches = c->launches + 1;      // + the copy-out kernel (k_copy_sym / k_one_minus)
     if (bounds_out) { bounds_out[0] = c->eps_min; bounds_out[1] = c->eps_max; }
     if (n_layers_out) *n_layers_out = c->n;
-    if (stats_out) memcpy(stats_out, h->stats_host, (size_t)(c->n < max_layers ? c->n : max_layers) * sizeof(sp2_layer_stat_t));
+    if (stats_out) {
+        const int ns = c->n < max_layers ? c->n : max_layers;
+        memcpy(stats_out, h->stats_host, (size_t)ns * sizeof(sp2_layer_stat_t));
+        stats_to_double(stats_out, ns);
+    }
     if (c->error < 0) return (sp2_status_t)c->error;
     if (c->running) return SP2_ERR_CUDA;     // loop ended while the device still wanted layers: should not happen
     if (mode == MODE_STANDARD && c->stop_reason == SP2_STOP_MAX_LAYERS) return SP2_NOT_CONVERGED;
@@ -583,13 +627,20 @@ extern "C" sp2_status_t sp2_density_matrix_host(sp2_handle_t h, const float* H_h
         CK(cudaMalloc((void**)&h->stage_D, elems * 4));
         h->stage_elems = elems;
     }
+    for (int i = 0; i < 4; ++i)
+        if (!h->host_ev[i]) CK(cudaEventCreate(&h->host_ev[i]));
+    CK(cudaEventRecord(h->host_ev[0], st));
     CK(cudaMemcpy2DAsync(h->stage_H, (size_t)N * 4, H_host, (size_t)ldh * 4, (size_t)N * 4, (size_t)N,
                          cudaMemcpyHostToDevice, st));
+    CK(cudaEventRecord(h->host_ev[1], st));
     s = sp2_density_matrix(h, h->stage_H, N, N, N_occ, opts, h->stage_D, N, stats_host, n_layers, bounds_out, stream);
     if (s < 0) return s;
+    CK(cudaEventRecord(h->host_ev[2], st));
     CK(cudaMemcpy2DAsync(D_host, (size_t)ldd * 4, h->stage_D, (size_t)N * 4, (size_t)N * 4, (size_t)N,
                          cudaMemcpyDeviceToHost, st));
+    CK(cudaEventRecord(h->host_ev[3], st));
     CK(cudaStreamSynchronize(st));
+    for (int i = 0; i < 3; ++i) CK(cudaEventElapsedTime(&h->host_ms[i], h->host_ev[i], h->host_ev[i + 1]));
     return s;
 }
 
@@ -611,15 +662,15 @@ extern "C" sp2_status_t sp2_refine_energy(sp2_handle_t h, const float* S_dev, in
     pb.exact_diag = 1;                               // diag(X) from row sums of squares (reading C24), as in the solve
     // Reading C15: continue the alternation from the last applied sign.
     //   last sigma = -1: X = S^2, then 2X - X^2  ->  2 S^2 - S^4 ;   last sigma = +1: T = 2S - S^2, then T^2.
-    double* th = h->thetas_host;
-    memset(th, 0, 2 * kThetaStride * sizeof(double));
+    float* th = h->thetas_host;
+    memset(th, 0, 2 * kThetaStride * sizeof(float));
     if (last_sigma < 0) { th[0] = 1; th[kThetaStride] = -1; th[kThetaStride + 1] = 2; }
     else                { th[0] = -1; th[1] = 2; th[kThetaStride] = 1; }
     Ctrl* c = h->ctrl_host;
     memset(c, 0, ctrl_header_bytes());
     c->N = N; c->mode = MODE_GENERALIZED; c->max_layers = 2;
     CK(cudaMemcpyAsync(h->ctrl, c, ctrl_header_bytes(), cudaMemcpyHostToDevice, st));
-    CK(cudaMemcpyAsync(h->thetas_dev, th, 2 * kThetaStride * sizeof(double), cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(h->thetas_dev, th, 2 * kThetaStride * sizeof(float), cudaMemcpyHostToDevice, st));
     CK(cudaMemsetAsync(h->stats_dev, 0, 2 * sizeof(sp2_layer_stat_t), st));
     const size_t ldS = (size_t)ws_ld_f32(pb.Np), ldF = (size_t)ws_ld_f16(pb.Np);
     if (pb.Np != N) CK(cudaMemsetAsync(h->S, 0, (size_t)pb.Np * ldS * 4, st));
@@ -669,11 +720,11 @@ static sp2_status_t generalized_impl(sp2_handle_t h, const float* H_dev, int N, 
     for (int n = 0; n < L; ++n) {
         for (int k = 0; k < 3; ++k) {
             if (!isfinite(theta_host[3 * n + k])) return SP2_ERR_INVALID_ARG;
-            h->thetas_host[kThetaStride * n + k] = theta_host[3 * n + k];
+            h->thetas_host[kThetaStride * n + k] = (float)theta_host[3 * n + k];
         }
         const double cn = c_host ? c_host[n + 1] : 0.0;      // weight of the output of layer n+1
         if (!isfinite(cn)) return SP2_ERR_INVALID_ARG;
-        h->thetas_host[kThetaStride * n + 3] = cn;
+        h->thetas_host[kThetaStride * n + 3] = (float)cn;
     }
     double c0 = 0.0, diag_const = 1.0;
     if (c_host) {
@@ -683,9 +734,9 @@ static sp2_status_t generalized_impl(sp2_handle_t h, const float* H_dev, int N, 
         //   eps_1 = th1 S_0^2 - (2 th1 + th2) S_0 + (th1 + th2 + th3) I
         //   F~ = I - sum c_i eps_i = (1 - c_0) I - [ (-c_0) S_0 + sum_{i>=1} c_i eps_i ]
         const double t1 = theta_host[0], t2 = theta_host[1], t3 = theta_host[2];
-        h->thetas_host[0] = t1;
-        h->thetas_host[1] = -(2.0 * t1 + t2);
-        h->thetas_host[2] = t1 + t2 + t3;
+        h->thetas_host[0] = (float)t1;
+        h->thetas_host[1] = (float)(-(2.0 * t1 + t2));
+        h->thetas_host[2] = (float)(t1 + t2 + t3);
         c0 = -c_host[0];
         diag_const = 1.0 - c_host[0];
     }
@@ -737,34 +788,49 @@ static sp2_status_t resident_solve(sp2_handle_s* h, const float* H_dev, int N, i
     int k = o.fp16_scale_log2;
     if (k < 0) k = 13;
     if (k > 14) return SP2_ERR_INVALID_ARG;
-    if (N_occ)
-        CK(cudaMemcpyAsync(h->bnocc_dev, N_occ, (size_t)(nocc_is_scalar ? 1 : B) * sizeof(double), cudaMemcpyHostToDevice, st));
+    if (N_occ) {
+        const int nn = nocc_is_scalar ? 1 : B;
+        for (int i = 0; i < nn; ++i) h->bnocc_host[i] = to_fx(N_occ[i]);
+        CK(cudaMemcpyAsync(h->bnocc_dev, h->bnocc_host, (size_t)nn * sizeof(long long), cudaMemcpyHostToDevice, st));
+    }
     if (homo_lumo) CK(cudaMemcpyAsync(h->bhl_dev, homo_lumo, (size_t)B * 2 * sizeof(double), cudaMemcpyHostToDevice, st));
     if (mode == MODE_GENERALIZED)
-        CK(cudaMemcpyAsync(h->thetas_dev, h->thetas_host, (size_t)o.max_layers * kThetaStride * sizeof(double),
+        CK(cudaMemcpyAsync(h->thetas_dev, h->thetas_host, (size_t)o.max_layers * kThetaStride * sizeof(float),
                            cudaMemcpyHostToDevice, st));
     CK(cudaMemsetAsync(h->bstats_dev, 0, (size_t)B * o.max_layers * sizeof(sp2_layer_stat_t), st));
     ResidentParams p;
     memset(&p, 0, sizeof(p));
     p.H = H_dev; p.D = D_dev; p.N_occ = h->bnocc_dev; p.nocc_is_scalar = nocc_is_scalar; p.N = N; p.B = B;
-    p.auto_bounds = o.auto_bounds; p.eps_min = o.eps_min; p.eps_max = o.eps_max; p.tol = o.tol; p.eps_alt = o.eps_alt;
+    p.auto_bounds = o.auto_bounds; p.eps_min = o.eps_min; p.eps_max = o.eps_max;
+    p.tol = (o.tol > 0.0) ? (to_fx(o.tol) > 0 ? to_fx(o.tol) : 1) : 0; p.eps_alt = to_fx(o.eps_alt);
     p.max_layers = o.max_layers; p.mode = mode; p.thetas = (mode == MODE_GENERALIZED) ? h->thetas_dev : nullptr;
-    p.noise_kappa = opt_kappa(o);
+    p.kappa_q16 = opt_kappa_q16(o);
     p.accelerated = (mode == MODE_STANDARD && homo_lumo) ? 1 : 0;
     p.homo_lumo = h->bhl_dev;
     p.scale = ldexpf(1.0f, k); p.inv_scale2 = ldexpf(1.0f, -2 * k);
     p.stats = h->bstats_dev; p.n_layers = h->bnl_dev; p.status = h->bstatus_dev; p.bounds = h->bbounds_dev;
     CK(launch_resident(p, h->num_sms, st));
-    std::vector<int> nl((size_t)B), stt((size_t)B);
-    CK(cudaMemcpyAsync(nl.data(), h->bnl_dev, (size_t)B * sizeof(int), cudaMemcpyDeviceToHost, st));
-    CK(cudaMemcpyAsync(stt.data(), h->bstatus_dev, (size_t)B * sizeof(int), cudaMemcpyDeviceToHost, st));
+    int* nl = h->bnl_host;
+    int* stt = h->bnl_host + B;
+    CK(cudaMemcpyAsync(nl, h->bnl_dev, (size_t)B * sizeof(int), cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(stt, h->bstatus_dev, (size_t)B * sizeof(int), cudaMemcpyDeviceToHost, st));
     if (stats_host)
-        CK(cudaMemcpyAsync(stats_host, h->bstats_dev, (size_t)B * o.max_layers * sizeof(sp2_layer_stat_t),
+        CK(cudaMemcpyAsync(h->bstats_host, h->bstats_dev, (size_t)B * o.max_layers * sizeof(sp2_layer_stat_t),
                            cudaMemcpyDeviceToHost, st));
     if (bounds_out)
-        CK(cudaMemcpyAsync(bounds_out, h->bbounds_dev, (size_t)B * 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+        CK(cudaMemcpyAsync(h->bbounds_host, h->bbounds_dev, (size_t)B * 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
     CK(cudaGetLastError());
+    if (bounds_out) memcpy(bounds_out, h->bbounds_host, (size_t)B * 2 * sizeof(double));
+    if (stats_host)          // only the layers that ran (the caller's buffer beyond them is left untouched)
+        for (int i = 0; i < B; ++i) {
+            const int n = nl[i] < o.max_layers ? nl[i] : o.max_layers;
+            if (n > 0) {
+                memcpy(stats_host + (size_t)i * o.max_layers, h->bstats_host + (size_t)i * o.max_layers,
+                       (size_t)n * sizeof(sp2_layer_stat_t));
+                stats_to_double(stats_host + (size_t)i * o.max_layers, n);
+            }
+        }
     h->last_launches = 1;
     int worst = SP2_OK;
     for (int i = 0; i < B; ++i) {
@@ -826,9 +892,9 @@ extern "C" sp2_status_t sp2_generalized_batched(sp2_handle_t h, const float* H_d
     for (int n = 0; n < L; ++n) {
         for (int k = 0; k < 3; ++k) {
             if (!isfinite(theta_host[3 * n + k])) return SP2_ERR_INVALID_ARG;
-            h->thetas_host[kThetaStride * n + k] = theta_host[3 * n + k];
+            h->thetas_host[kThetaStride * n + k] = (float)theta_host[3 * n + k];
         }
-        h->thetas_host[kThetaStride * n + 3] = 0.0;
+        h->thetas_host[kThetaStride * n + 3] = 0.0f;
     }
     std::vector<int> nl((size_t)B);
     return resident_solve(h, H_dev, N, B, nullptr, 1, o, X_L_dev, stats_host, nl.data(), status_out, nullptr,
@@ -864,4 +930,8 @@ extern "C" sp2_status_t sp2_gershgorin(sp2_handle_t h, const float* H_dev, int N
 }
 
 extern "C" int sp2_last_launch_count(sp2_handle_t h) { return h ? h->last_launches : 0; }
+extern "C" void sp2_last_host_timing(sp2_handle_t h, double ms[3]) {
+    if (!h || !ms) return;
+    for (int i = 0; i < 3; ++i) ms[i] = (double)h->host_ms[i];
+}
 extern "C" int sp2_last_round_sync_broken(sp2_handle_t h) { return (h && h->ctrl_host) ? (int)h->ctrl_host->round_sync_broken : 0; }

@@ -101,41 +101,50 @@ __global__ void __launch_bounds__(256) k_gershgorin_rows(const float* __restrict
     }
 }
 
-// R_i from the per-tile slots (fixed order, FP64), then eps_min = min_i (H_ii - R_i), eps_max = max_i (H_ii + R_i)
-// -> ctrl.  One row per thread; per-block extrema -> ctrl->partial; the last block takes the extrema over the blocks
-// (min / max are exact, so their order does not matter).
+// R_i from the per-tile slots, then eps_min = min_i (H_ii - R_i), eps_max = max_i (H_ii + R_i) -> ctrl.  One block per
+// 64 rows; thread (r, g) adds the slots s = g, g + 4, g + 8, ... of row r in increasing order in FP64 and the four
+// partial sums are combined as (p0 + p1) + (p2 + p3): a fixed order, so the bounds are bit-reproducible.  Per-block
+// extrema -> ctrl->partial; the last block takes the extrema over the blocks (min / max are exact).
 __global__ void __launch_bounds__(256) k_gershgorin_finalize(const float* __restrict__ part,
                                                              const double* __restrict__ diag, int N, Ctrl* ctrl) {
-    __shared__ double smin[8], smax[8];
+    __shared__ double ps[4][ET];
+    __shared__ double smin[2], smax[2];
     const int nt = (N + ET - 1) / ET;
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int Ib = blockIdx.x;
+    const int r = threadIdx.x & (ET - 1), g = threadIdx.x >> 6;
+    const int i = Ib * ET + r;
+    // slots of a row of block Ib: row sums part[J], J = 0..Ib, then column sums part[nt + I], I = Ib..nt-1
+    const int nslots = (Ib + 1) + (nt - Ib);
+    double acc = 0.0;
+    if (i < N)
+        for (int sidx = g; sidx < nslots; sidx += 4) {
+            const int slot = (sidx <= Ib) ? sidx : (nt + Ib + (sidx - Ib - 1));
+            acc += (double)__ldg(part + (long long)slot * N + i);
+        }
+    ps[g][r] = acc;
+    __syncthreads();
     double lo = INFINITY, hi = -INFINITY;
-    if (i < N) {
-        const int Ib = i / ET;
-        double R = 0.0;
-        for (int J = 0; J <= Ib; ++J) R += (double)__ldg(part + (long long)J * N + i);
-        for (int I = Ib; I < nt; ++I) R += (double)__ldg(part + (long long)(nt + I) * N + i);
-        lo = diag[i] - R;
-        hi = diag[i] + R;
-        // fmin / fmax drop NaNs: a non-finite row must poison the bounds (-> SP2_ERR_BOUNDS_DEGENERATE / NONFINITE)
-        if (!isfinite(lo) || !isfinite(hi)) { lo = NAN; hi = NAN; }
-    }
-    bool bad = isnan(lo);
+    bool bad = false;
+    if (threadIdx.x < ET) {
+        if (i < N) {
+            const double R = (ps[0][r] + ps[1][r]) + (ps[2][r] + ps[3][r]);
+            lo = diag[i] - R;
+            hi = diag[i] + R;
+            // fmin / fmax drop NaNs: a non-finite row must poison the bounds (-> SP2_ERR_NONFINITE)
+            bad = !isfinite(lo) || !isfinite(hi);
+        }
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        lo = fmin(lo, __shfl_xor_sync(0xffffffffu, lo, o));
-        hi = fmax(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+        for (int o = 16; o > 0; o >>= 1) {
+            lo = fmin(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+            hi = fmax(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+        }
+        bad = __any_sync(0xffffffffu, bad);
+        if ((threadIdx.x & 31) == 0) { smin[threadIdx.x >> 5] = bad ? NAN : lo; smax[threadIdx.x >> 5] = bad ? NAN : hi; }
     }
-    bad = __any_sync(0xffffffffu, bad);
-    if ((threadIdx.x & 31) == 0) { smin[threadIdx.x >> 5] = bad ? NAN : lo; smax[threadIdx.x >> 5] = bad ? NAN : hi; }
     __syncthreads();
     if (threadIdx.x == 0) {
-        bool nan = false;
-        lo = INFINITY; hi = -INFINITY;
-        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) {
-            nan = nan || isnan(smin[w]);
-            lo = fmin(lo, smin[w]); hi = fmax(hi, smax[w]);
-        }
+        bool nan = isnan(smin[0]) || isnan(smin[1]);
+        lo = fmin(smin[0], smin[1]); hi = fmax(smax[0], smax[1]);
         ctrl->partial[blockIdx.x][0] = nan ? NAN : lo;
         ctrl->partial[blockIdx.x][1] = nan ? NAN : hi;
         __threadfence();
@@ -190,7 +199,7 @@ __global__ void __launch_bounds__(256, 4) k_affine_split(const float* __restrict
                                                          float* __restrict__ S, __half* __restrict__ hi,
                                                          __half* __restrict__ lo, long long ld, long long ldf,
                                                          float scale, Ctrl* ctrl, sp2_layer_stat_t* stats,
-                                                         const double* thetas, unsigned long long* __restrict__ rowsq,
+                                                         const float* thetas, unsigned long long* __restrict__ rowsq,
                                                          float* __restrict__ mix, float c0) {
     __shared__ float ts[ET][ET + 1];
     __shared__ float colacc[16][ET];
@@ -249,7 +258,7 @@ __global__ void __launch_bounds__(256, 4) k_affine_split(const float* __restrict
             store_s4(S, hi, lo, ld, ldf, i, j, sv, scale, all4, ok, mix, c0);
             if (rowsq) {
                 rsq = row16_sum(rsq);
-                if ((threadIdx.x & 15) == 0 && i < N) atomicAdd(rowsq + i, rowsq_fix((double)rsq));
+                if ((threadIdx.x & 15) == 0 && i < N) atomicAdd(rowsq + i, rowsq_fix(rsq));
             }
         }
         off2 += (double)offsq;
@@ -260,7 +269,7 @@ __global__ void __launch_bounds__(256, 4) k_affine_split(const float* __restrict
 #pragma unroll
             for (int g = 0; g < 16; ++g) c += colacc[g][threadIdx.x];
             const int jj = J * ET + threadIdx.x;
-            if (jj < N && c != 0.f) atomicAdd(rowsq + jj, rowsq_fix((double)c));
+            if (jj < N && c != 0.f) atomicAdd(rowsq + jj, rowsq_fix(c));
         }
         // mirrored part: row jj = J*64 + lr, columns ii = I*64 + c4 .. +3, value s(ii, jj) for ii > jj
 #pragma unroll
@@ -297,8 +306,11 @@ __global__ void __launch_bounds__(256, 4) k_affine_split(const float* __restrict
                 s0 += ((volatile double*)ctrl->partial[i])[0];
                 s1 += ((volatile double*)ctrl->partial[i])[1];
             }
-            ctrl->N_S = s0;          // N_S = Tr[S_0]
-            ctrl->fro2 = s1;
+            // N_S = Tr[S_0]; the control works in 2^40 fixed point (sp2_control.cuh)
+            const bool fin = isfinite(s0) && isfinite(s1) && fabs(s0) < 4.0e6 && s1 < 4.0e6;
+            ctrl->N_S = fin ? __double2ll_rn(s0 * kFxScale) : 0;
+            ctrl->fro2 = fin ? __double2ll_rn(s1 * kFxScale) : 0;
+            ctrl->nonfinite = fin ? 0 : 1;
             ctrl->n = 0;
             ctrl->done_counter = 0;
             ctrl->launches += 1;
@@ -351,7 +363,7 @@ __global__ void __launch_bounds__(256) k_split_scalar(const float* __restrict__ 
 __global__ void __launch_bounds__(256) k_energy_traces(const float* __restrict__ X, long long ldx,
                                                        const float* __restrict__ H, long long ldh, int N, Ctrl* ctrl,
                                                        double* __restrict__ out, int plan, sp2_layer_stat_t* stats,
-                                                       const double* thetas, unsigned long long* __restrict__ rowsq) {
+                                                       const float* thetas, unsigned long long* __restrict__ rowsq) {
     __shared__ double red[8][3];
     __shared__ float colacc[16][ET];
     const int nt = (N + ET - 1) / ET;
@@ -387,7 +399,7 @@ __global__ void __launch_bounds__(256) k_energy_traces(const float* __restrict__
             }
             if (rowsq) {
                 rsq = row16_sum(rsq);
-                if ((threadIdx.x & 15) == 0 && i < N) atomicAdd(rowsq + i, rowsq_fix((double)rsq));
+                if ((threadIdx.x & 15) == 0 && i < N) atomicAdd(rowsq + i, rowsq_fix(rsq));
             }
         }
         if (rowsq) {                                // uniform over the block
@@ -398,7 +410,7 @@ __global__ void __launch_bounds__(256) k_energy_traces(const float* __restrict__
 #pragma unroll
                 for (int g = 0; g < 16; ++g) c += colacc[g][threadIdx.x];
                 const int jc = J * ET + threadIdx.x;
-                if (jc < N && c != 0.f) atomicAdd(rowsq + jc, rowsq_fix((double)c));
+                if (jc < N && c != 0.f) atomicAdd(rowsq + jc, rowsq_fix(c));
             }
             __syncthreads();
         }
@@ -428,8 +440,10 @@ __global__ void __launch_bounds__(256) k_energy_traces(const float* __restrict__
             ctrl->done_counter = 0;
             ctrl->launches += 1;
             if (plan) {
-                ctrl->N_S = s1;
-                ctrl->fro2 = s2;
+                const bool fin = isfinite(s1) && isfinite(s2) && fabs(s1) < 4.0e6 && s2 < 4.0e6;
+                ctrl->N_S = fin ? __double2ll_rn(s1 * kFxScale) : 0;
+                ctrl->fro2 = fin ? __double2ll_rn(s2 * kFxScale) : 0;
+                ctrl->nonfinite = fin ? 0 : 1;
                 ctrl->n = 0;
                 control_plan_next(ctrl, stats, thetas);
             }
@@ -507,14 +521,14 @@ cudaError_t launch_gershgorin(const float* H, int N, long long ldh, float* part,
     const int nt = (N + ET - 1) / ET;
     const long long ntiles = (long long)nt * (nt + 1) / 2;
     const int grid = (int)(ntiles < (long long)num_sms * 16 ? ntiles : (long long)num_sms * 16);
-    if ((N + 255) / 256 > kMaxPartials) return cudaErrorInvalidValue;
+    if (nt > kMaxPartials) return cudaErrorInvalidValue;
     k_gershgorin_rows<<<grid, 256, 0, st>>>(H, N, ldh, part, diag);
-    k_gershgorin_finalize<<<(N + 255) / 256, 256, 0, st>>>(part, diag, N, ctrl);
+    k_gershgorin_finalize<<<nt, 256, 0, st>>>(part, diag, N, ctrl);
     return cudaGetLastError();
 }
 
 cudaError_t launch_affine_split(const float* H, int N, long long ldh, float* S, __half* hi, __half* lo, long long ld,
-                                long long ldf, float scale, Ctrl* ctrl, sp2_layer_stat_t* stats, const double* thetas,
+                                long long ldf, float scale, Ctrl* ctrl, sp2_layer_stat_t* stats, const float* thetas,
                                 unsigned long long* rowsq, float* mix, float c0, int num_sms, cudaStream_t st) {
     const int nt = (N + ET - 1) / ET;
     const long long ntiles = (long long)nt * (nt + 1) / 2;
@@ -557,7 +571,7 @@ cudaError_t launch_one_minus(const float* M, long long ldm, float* F, long long 
     return cudaGetLastError();
 }
 cudaError_t launch_energy_traces(const float* X, long long ldx, const float* H, long long ldh, int N, Ctrl* ctrl,
-                                 double* out, int plan, sp2_layer_stat_t* stats, const double* thetas,
+                                 double* out, int plan, sp2_layer_stat_t* stats, const float* thetas,
                                  unsigned long long* rowsq, int num_sms, cudaStream_t st) {
     const int nt = (N + ET - 1) / ET;
     const long long ntiles = (long long)nt * (nt + 1) / 2;

@@ -15,21 +15,23 @@ cudaError_t launch_gershgorin(const float* H, int N, long long ldh, float* part,
                               int num_sms, cudaStream_t st);
 inline size_t gershgorin_part_floats(int N) { return 2 * (size_t)((N + 63) / 64) * (size_t)N; }
 cudaError_t launch_affine_split(const float* H, int N, long long ldh, float* S, __half* hi, __half* lo, long long ld,
-                                long long ldf, float scale, Ctrl* ctrl, sp2_layer_stat_t* stats, const double* thetas,
+                                long long ldf, float scale, Ctrl* ctrl, sp2_layer_stat_t* stats, const float* thetas,
                                 unsigned long long* rowsq, float* mix, float c0, int num_sms, cudaStream_t st);
 cudaError_t launch_copy_sym(const float* S, long long ld, float* D, long long ldd, int N, int num_sms, cudaStream_t st);
 cudaError_t launch_one_minus(const float* M, long long ldm, float* F, long long ldo, int N, float d, int num_sms,
                              cudaStream_t st);
 
 // Row sums of squares r_i = sum_j S_ij^2 (= diag(S^2)_i for symmetric S) are kept in 2^44 fixed point so that the
-// atomic accumulation is order-independent (bit-reproducible results).
-constexpr double kRowSqScale = 17592186044416.0;           // 2^44
-constexpr double kRowSqInv = 1.0 / 17592186044416.0;
-__device__ __forceinline__ unsigned long long rowsq_fix(double x) {
-    return (unsigned long long)__double2ll_rn(x * kRowSqScale);
+// atomic accumulation is order-independent (bit-reproducible results).  FP32 values convert exactly (power-of-two
+// scale), without touching the FP64 datapath (see sp2_control.cuh).
+constexpr int kRowSqBits = 44;
+constexpr float kRowSqScaleF = 17592186044416.0f;          // 2^44
+constexpr float kRowSqInvF = 1.0f / 17592186044416.0f;
+__device__ __forceinline__ unsigned long long rowsq_fix(float x) {
+    return (unsigned long long)__float2ll_rn(x * kRowSqScaleF);
 }
 cudaError_t launch_energy_traces(const float* X, long long ldx, const float* H, long long ldh, int N, Ctrl* ctrl,
-                                 double* out, int plan, sp2_layer_stat_t* stats, const double* thetas,
+                                 double* out, int plan, sp2_layer_stat_t* stats, const float* thetas,
                                  unsigned long long* rowsq, int num_sms, cudaStream_t st);
 cudaError_t launch_split(const float* X, int N, long long ldx, __half* hi, __half* lo, long long ldo, float scale,
                          int num_sms, cudaStream_t st);
@@ -57,7 +59,7 @@ struct WorkItem {
 struct LayerParams {
     Ctrl* ctrl;
     sp2_layer_stat_t* stats;
-    const double* thetas;          // generalized mode: [L][3] on the device
+    const float* thetas;           // generalized mode: [L][kThetaStride] on the device
     float* S;                      // FP32 master, Np x Np, updated in place; below the diagonal chunks only the UPPER
                                    // triangle is kept current (it is what the epilogue reads back): see k_copy_sym
     float* mix;                    // output mix M = sum_i c_i S_i (Eq. 18), same layout as S; nullptr = none
@@ -94,14 +96,16 @@ cudaError_t layer_kernel_setup(int cfg);   // cudaFuncSetAttribute(max dynamic s
 struct ResidentParams {
     const float* H;                // [B][N][N]
     float* D;                      // [B][N][N]
-    const double* N_occ;           // [B] or [1]
+    const long long* N_occ;        // [B] or [1], 2^40 fixed point
     int nocc_is_scalar;
     int N, B;
     int auto_bounds;
-    double eps_min, eps_max, tol, eps_alt, noise_kappa;
+    double eps_min, eps_max;
+    long long tol, eps_alt;        // 2^40 fixed point
+    int kappa_q16;                 // noise-floor kappa * 2^16
     int max_layers;
     int mode;                      // MODE_STANDARD / MODE_GENERALIZED
-    const double* thetas;          // generalized: [L][kThetaStride] on the device
+    const float* thetas;           // generalized: [L][kThetaStride] on the device
     int accelerated;               // standard mode with the accelerated weights (section V.A, reading C27)
     const double* homo_lumo;       // accelerated: [B][2] HOMO / LUMO estimates in energy units (device)
     float scale, inv_scale2;

@@ -5,10 +5,20 @@
 // Residency: each CTA owns 128 rows.  Its FP16 hi/lo row panels live in shared memory in the UMMA K-major
 // 128B-swizzled layout and are at the same time the A operand (its M rows) and its half of the B operand of a
 // cta_group::2 MMA (M = 256, N = 256), so no operand ever moves.  The FP32 master S lives in the upper half of
-// TMEM (columns NP..2NP-1, lane = row), the accumulator in the lower half.  Only the lower triangle (j <= i) is
-// finalised; each value is written to (i,j) and mirrored to (j,i) in the panels (through distributed shared
-// memory when row j belongs to the peer CTA), which keeps S exactly symmetric (an antisymmetric rounding
-// residue would be amplified by the 2S - S^2 branch).
+// TMEM (columns NP..2NP-1, lane = row), the accumulator in the lower half.
+//
+// Work split of the epilogue.  The matrix is cut into 32 x 32 blocks; the 32 rows of a block row ("row group" g,
+// one TMEM lane quarter of one CTA) belong to two warps, each taking 16 of a block's 32 columns.  The MMA computes
+// the full square, so an off-diagonal block pair {g, c} can be finalised from either of its two accumulator copies:
+// it is given to the row group g with (c - g) mod NG in 1 .. NG/2 - 1 (the pairs at distance NG/2 go to the outer
+// groups).  Every group then owns its diagonal block plus NG/2 - 1 or NG/2 off-diagonal ones, so the triangular work
+// is even across the warps and the two CTAs.  Each value is written to (i,j) and mirrored to (j,i) in the panels
+// (through distributed shared memory when row j belongs to the peer CTA), which keeps S exactly symmetric (an
+// antisymmetric rounding residue would be amplified by the 2S - S^2 branch).
+//
+// Per layer: MMA (one elected thread) -> epilogue (8 warps) -> cluster barrier -> the control step (one thread,
+// Alg. 1) runs WHILE the next layer's MMAs are already issued (their operands do not depend on sigma; a layer is
+// wasted only when the stop comes from the noise-floor test, which needs the layer's own trace) -> block barrier.
 #include "sp2_kernels.h"
 #include "sp2_ptx.cuh"
 
@@ -20,21 +30,22 @@ struct ResCfg {
     static constexpr int KBLK = NP / 64;
     static constexpr int PANEL_BYTES = KBLK * 16384;      // 128 rows x NP fp16
     static constexpr int TMEM_COLS = 2 * NP;
-    // warps 0-7: rows / epilogue (warp w owns TMEM lanes 32 (w % 4) .. +31 and every second 32-column chunk of them:
-    // two warps per scheduler hide each other's latencies and halve the longest chunk list), warp 8: MMA + TMEM alloc
+    static constexpr int NG = NP / 32;                    // row groups = column chunks of 32
+    // warps 0-7: epilogue (warp w owns TMEM lanes 32 (w % 4) .. +31 and columns 16 (w / 4) .. +15 of every block of
+    // its row group), warp 8: MMA issue + TMEM alloc
     static constexpr int THREADS = 288;
     static constexpr int MMA_WARP = 8;
-    static constexpr int STAGE_FLOATS = 8 * 32 * 33;
+    static constexpr int STAGE_FLOATS = 8 * 32 * 17;
 };
 
 struct ResShared {
     uint64_t mma_bar;
     uint32_t tmem_slot;
     uint32_t pad0;
-    double part[2][8][4];        // [iteration parity][warp][trS, fro2, trX, -]
-    float rrow[2][128];          // Gershgorin: per chunk-half row sums of the strictly-lower entries
+    long long part[2][8][4];     // [iteration parity][warp][trS, fro2, trX (2^40 fixed point), non-finite flag]
+    float rrow[2][128];          // Gershgorin: per column-half row sums of the off-diagonal entries
     float dii[128];              // Gershgorin: diagonal entries
-    float rcol[4][256];          // Gershgorin: per-warp column sums of the strictly-lower triangle (this CTA's rows)
+    float rcol[4][256];          // Gershgorin: column sums of the blocks finalised by row group q of this CTA
     float mm[4][2];              // per-warp min(d - R), max(d + R)
     CtrlCore ctrl;
 };
@@ -46,6 +57,9 @@ __device__ __forceinline__ uint32_t mapa_u32(uint32_t addr, uint32_t cta) {
 }
 __device__ __forceinline__ void st_cluster_u16(uint32_t addr, unsigned short v) {
     asm volatile("st.shared::cluster.u16 [%0], %1;\n" ::"r"(addr), "h"(v) : "memory");
+}
+__device__ __forceinline__ void st_shared_u16(uint32_t addr, unsigned short v) {
+    asm volatile("st.shared.u16 [%0], %1;\n" ::"r"(addr), "h"(v) : "memory");
 }
 __device__ __forceinline__ float ld_cluster_f32(uint32_t addr) {
     float v;
@@ -63,19 +77,23 @@ __device__ __forceinline__ uint32_t panel_off(int t, int j) {
                       (j & 7) * 2);
 }
 
-// Which 32-column chunks does the warp owning rows [row0, row0 + 31] finalise?  Every unordered pair {i, j} exactly
-// once.  Plain rule: the lower triangle (c0 <= row0).  With two CTAs that leaves CTA 1 (rows 128-255) 26 chunk tasks
-// and CTA 0 ten, so the block rows 192-255 x columns 0-127 is handed to CTA 0, which finalises it from its own
-// accumulator's transposed copy (rows 0-127, columns 192-255: the MMA computes the full square): 18 tasks each,
-// at most 3 per warp instead of 4.  Returns -1 not handled, 0 all 32 x 32 entries (off-diagonal), 1 diagonal chunk.
-template <int CG>
-__device__ __forceinline__ int chunk_kind(int row0, int c0) {
-    if (CG == 2) {
-        if (row0 < 128 && c0 >= 192) return 0;
-        if (row0 >= 192 && c0 < 128) return -1;
-    }
-    if (c0 > row0) return -1;
-    return c0 == row0 ? 1 : 0;
+// Does row group g finalise the block in column chunk c?  Every unordered pair {g, c} exactly once (see the header).
+template <int NG>
+__device__ __forceinline__ bool owns_block(int g, int c) {
+    const int d = (c - g) & (NG - 1);
+    if (d < NG / 2) return true;                          // the diagonal block and the next NG/2 - 1 chunks
+    if (d > NG / 2) return false;
+    return NG == 8 ? (g < 2 || g >= 6) : (g == 0 || g == NG - 1);
+}
+
+// The trace sums are 2^40 fixed-point integers and the control step is integer-only (sp2_control.cuh): with FP64
+// shuffle reductions and an FP64 control step a pass spent more time waking the FP64 datapath than on its MMAs.
+__device__ __forceinline__ long long to_fix(float x) { return fx_from_float(x); }
+__device__ __forceinline__ long long sq_fix(float x) { return fx_square(x); }
+__device__ __forceinline__ long long ld_cluster_s64(uint32_t addr) {
+    long long v;
+    asm volatile("ld.shared::cluster.s64 %0, [%1];\n" : "=l"(v) : "r"(addr) : "memory");
+    return v;
 }
 
 template <int CG>
@@ -83,26 +101,9 @@ __device__ __forceinline__ void group_sync() {
     if (CG == 2) cluster_sync_all(); else __syncthreads();
 }
 
-// Load the 32 x 32 block H[row0 + r][c0 + l] (lower-triangle entries only, zero elsewhere / outside N) coalesced,
-// transpose it through `stg` so that lane `l` ends up with its own row's 32 values.
-__device__ __forceinline__ void load_block_rows(const float* __restrict__ Hm, int N, int row0, int c0, float* stg,
-                                                int lane, float (&vals)[32]) {
-    __syncwarp();
-#pragma unroll 8
-    for (int r = 0; r < 32; ++r) {
-        const int i = row0 + r, j = c0 + lane;
-        float v = 0.f;
-        if (i < N && j <= i) v = __ldg(Hm + (size_t)i * N + j);
-        stg[r * 33 + lane] = v;
-    }
-    __syncwarp();
-#pragma unroll
-    for (int c = 0; c < 32; ++c) vals[c] = stg[lane * 33 + c];
-}
-
 template <class C>
 __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentParams p) {
-    constexpr int NP = C::NP, CG = C::CG;
+    constexpr int NP = C::NP, CG = C::CG, NG = C::NG;
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     uint8_t* hiP = smem;
@@ -129,15 +130,15 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
     tc_fence_after();
     const uint32_t tmem_base = *((volatile uint32_t*)&sh->tmem_slot);
     const uint32_t hi_addr = smem_u32(hiP), lo_addr = smem_u32(loP);
-    uint32_t mma_phase = 0;
+    uint32_t mma_uses = 0;                        // MMA batches issued so far (uniform over the cluster)
 
     const int q = warp & 3;
-    const int hf = (warp >> 2) & 1;               // which half of the 32-column chunks this warp takes
+    const int hf = (warp >> 2) & 1;               // which 16 of a block's 32 columns this warp takes
     const int tl = q * 32 + lane;                  // row inside this CTA's panel (TMEM lane)
     const int gi = (int)rank * 128 + tl;           // global row
-    const int row0 = (int)rank * 128 + q * 32;     // first row of this warp
-    float* stg = stage + (warp & 7) * (32 * 33);
-    const uint32_t t_acc = tmem_base + ((uint32_t)(q * 32) << 16);
+    const int g = (int)rank * 4 + q;               // row group
+    float* stg = stage + (warp & 7) * (32 * 17);
+    const uint32_t t_acc = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(16 * hf);
     const uint32_t t_S = t_acc + NP;
     const float cs = p.scale, inv2 = p.inv_scale2;
     // mirror-store address pieces that depend on this thread's column gi only (panel_off(row, gi) split by row bits)
@@ -151,56 +152,67 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
         float* __restrict__ Dm = p.D + (size_t)m * N * N;
         sp2_layer_stat_t* stats_m = (rank == 0) ? p.stats + (size_t)m * p.max_layers : nullptr;
 
-        // ------------------------------------------------------------------ a1: Gershgorin bounds (Alg. 1)
-        double e0 = p.eps_min, e1 = p.eps_max;
+        // ------------------------------------------------------------------ load H (lower triangle, reading C22) into
+        // the master region of TMEM; a1: Gershgorin bounds on the way (Alg. 1)
         if (p.auto_bounds) {
             for (int i = threadIdx.x; i < 1024; i += blockDim.x) (&sh->rcol[0][0])[i] = 0.f;
             __syncthreads();
+        }
+        if (warp < 8) {
             float Rrow = 0.f;
-            if (warp < 8) {
-                for (int c0 = 0; c0 < NP; c0 += 32) {
-                    const int kind = chunk_kind<CG>(row0, c0);
-                    if (kind < 0 || ((c0 >> 5) & 1) != hf) continue;
+#pragma unroll 1
+            for (int c = 0; c < NG; ++c) {
+                if (!owns_block<NG>(g, c)) continue;
+                const int j0 = 32 * c + 16 * hf;              // first matrix column of this warp's half block
+                float hv[16];
+                if (c > g) {
+                    // block above the diagonal: entry (gi, j) is read as H(j, gi); lane = row already
+#pragma unroll
+                    for (int e = 0; e < 16; ++e)
+                        hv[e] = (gi < N && j0 + e < N) ? __ldg(Hm + (size_t)(j0 + e) * N + gi) : 0.f;
+                } else {
+                    // coalesced row segments (two rows of 16 per load), transposed through the staging tile
                     __syncwarp();
-                    float colp = 0.f;
-                    if (c0 > row0) {
-                        // transposed block: entry (gi, c0 + c) is read as H(c0 + c, gi) (lower triangle, reading C22);
-                        // lane = row already, the column sums go through the staging tile
-#pragma unroll 8
-                        for (int c = 0; c < 32; ++c) {
-                            const int j = c0 + c;
-                            float v = 0.f;
-                            if (gi < N && j < N) v = fabsf(__ldg(Hm + (size_t)j * N + gi));
-                            Rrow += v;
-                            stg[lane * 33 + c] = v;
-                        }
-                        __syncwarp();
-#pragma unroll 8
-                        for (int r = 0; r < 32; ++r) colp += stg[r * 33 + lane];
-                        sh->rcol[q][c0 + lane] = colp;
-                        continue;
-                    }
-                    // column partial sums in the load layout (lane = column), row sums after the transpose
-#pragma unroll 8
-                    for (int r = 0; r < 32; ++r) {
-                        const int i = row0 + r, j = c0 + lane;
+#pragma unroll 4
+                    for (int r2 = 0; r2 < 32; r2 += 2) {
+                        const int r = r2 + (lane >> 4), i = g * 32 + r, j = j0 + (lane & 15);
                         float v = 0.f;
                         if (i < N && j <= i) v = __ldg(Hm + (size_t)i * N + j);
-                        if (j < i) colp += fabsf(v);
-                        stg[r * 33 + lane] = v;
+                        stg[r * 17 + (lane & 15)] = v;
                     }
                     __syncwarp();
-                    sh->rcol[q][c0 + lane] = colp;      // each (warp, column) slot is written once: deterministic
 #pragma unroll
-                    for (int c = 0; c < 32; ++c) {
-                        const float v = stg[lane * 33 + c];
-                        const int j = c0 + c;
-                        if (j < gi) Rrow += fabsf(v);
-                        if (j == gi) sh->dii[tl] = v;
+                    for (int e = 0; e < 16; ++e) hv[e] = stg[lane * 17 + e];
+                }
+                uint32_t hu[16];
+#pragma unroll
+                for (int e = 0; e < 16; ++e) hu[e] = __float_as_uint(hv[e]);
+                tmem_st_32x32_x16(t_S + (uint32_t)(32 * c), hu);
+                if (p.auto_bounds) {
+                    // |entry| adds to the radius of its row (this thread) and of its column (sum over the 32 rows)
+                    __syncwarp();
+#pragma unroll
+                    for (int e = 0; e < 16; ++e) {
+                        const int j = j0 + e;
+                        const float a = (c == g && j >= gi) ? 0.f : fabsf(hv[e]);   // diagonal block: j < i only
+                        if (c == g && j == gi) sh->dii[tl] = hv[e];
+                        Rrow += a;
+                        stg[lane * 17 + e] = a;
+                    }
+                    __syncwarp();
+                    if (lane < 16) {
+                        float colp = 0.f;
+#pragma unroll 8
+                        for (int r = 0; r < 32; ++r) colp += stg[r * 17 + lane];
+                        sh->rcol[q][j0 + lane] = colp;      // each (row group, column) slot is written once
                     }
                 }
-                sh->rrow[hf][tl] = Rrow;
             }
+            tmem_st_wait();
+            if (p.auto_bounds) sh->rrow[hf][tl] = Rrow;
+        }
+        double e0 = p.eps_min, e1 = p.eps_max;
+        if (p.auto_bounds) {
             group_sync<CG>();
             float lo = INFINITY, hi = -INFINITY;
             if (warp < 4) {
@@ -233,137 +245,150 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
         const bool bounds_ok = (e1 > e0) && isfinite(e0) && isfinite(e1);
         if (threadIdx.x == 0) {
             CtrlCore* c = &sh->ctrl;
-            c->N_occ = (p.mode == MODE_GENERALIZED) ? 0.0 : (p.nocc_is_scalar ? p.N_occ[0] : p.N_occ[m]);
+            c->N_occ = (p.mode == MODE_GENERALIZED) ? 0 : (p.nocc_is_scalar ? p.N_occ[0] : p.N_occ[m]);
             c->eps_alt = p.eps_alt; c->tol = p.tol; c->eps_min = e0; c->eps_max = e1;
             c->N = N; c->mode = p.mode; c->max_layers = p.max_layers; c->auto_bounds = p.auto_bounds;
             c->n = 0; c->running = 0; c->stop_reason = 0; c->pending_stop = 0; c->sigma_prev = 0; c->sigma_prev2 = 0;
             c->error = bounds_ok ? 0 : SP2_ERR_BOUNDS_DEGENERATE; c->launches = 0;
-            c->N_S = 0; c->fro2 = 0; c->iderr_prev = 0; c->iderr_prev2 = 0; c->nx_inflight = 0; c->noise_kappa = p.noise_kappa;
-            c->accelerated = p.accelerated; c->acc_h = 1.0; c->acc_l = 0.0;
+            c->N_S = 0; c->fro2 = 0; c->iderr_prev = 0; c->iderr_prev2 = 0; c->nx_inflight = 0; c->kappa_q16 = p.kappa_q16;
+            c->nonfinite = 0;
+            c->accelerated = p.accelerated; c->acc_h = 1.0f; c->acc_l = 0.0f;
             c->homo = p.accelerated ? p.homo_lumo[2 * m] : 0.0;
             c->lumo = p.accelerated ? p.homo_lumo[2 * m + 1] : 0.0;
         }
         if (!bounds_ok) {           // uniform over the cluster (same e0, e1 everywhere)
             if (rank == 0 && threadIdx.x == 0) {
-                p.status[m] = SP2_ERR_BOUNDS_DEGENERATE; p.n_layers[m] = 0;
+                p.status[m] = (isnan(e0) || isnan(e1)) ? SP2_ERR_NONFINITE : SP2_ERR_BOUNDS_DEGENERATE;
+                p.n_layers[m] = 0;
                 p.bounds[2 * m] = e0; p.bounds[2 * m + 1] = e1;
             }
+            tc_fence_before();
             group_sync<CG>();
+            tc_fence_after();
             continue;
         }
+        __syncthreads();            // ctrl initialised before anyone reads it
 
-        // ------------------------------------------------------------------ a2: S_0, first split, Tr S_0, ||S_0||_F^2
-        const float w0 = (float)(-1.0 / (e1 - e0)), b0 = (float)(e1 / (e1 - e0));
-        double trS = 0.0, fro2 = 0.0, trX = 0.0;
-        float th1s = 0.f, th2 = 0.f, th3 = 0.f;
+        // ------------------------------------------------------------------ the layers.  Pass 0 is a2: S_0 = W_0 H + B_0
+        // (Alg. 1) = the generic update with th1 = 0, th2 = W_0, th3 = B_0 applied to the master (= H);
+        // pass n >= 1 is S_n = th1 X_n / c^2 + th2 S_{n-1} + th3 I from layer n's accumulator.
+        float th1s = 0.f, th2 = (float)(-1.0 / (e1 - e0)), th3 = (float)(e1 / (e1 - e0));
+        bool use_acc = false;
         int iter = 0;
-        bool first = true;
         while (true) {
+            // Will the MMAs of the NEXT layer be issued right after this pass's barrier?  Decided from the control state
+            // as the previous pass left it (the same for every thread of the cluster): not if this layer's own stop test
+            // has already fired, nor when a fixed-depth network ends here.
+            const bool issue_next = (sh->ctrl.pending_stop == SP2_STOP_NONE) &&
+                                    !(p.mode == MODE_GENERALIZED && iter >= p.max_layers);
             if (warp < 8) {
-                // ---- finalise the lower-triangle part of this thread's row: chunk by chunk
-                for (int c0 = 0; c0 < NP; c0 += 32) {
-                    const int kind = chunk_kind<CG>(row0, c0);
-                    if (kind < 0 || ((c0 >> 5) & 1) != hf) continue;
-                    const bool upper = (c0 > row0);             // transposed block (columns beyond the rows)
-                    float sn[32];
-                    if (first) {
-                        float hv[32];
-                        if (upper) {
-#pragma unroll 8
-                            for (int c = 0; c < 32; ++c)
-                                hv[c] = (gi < N && c0 + c < N) ? __ldg(Hm + (size_t)(c0 + c) * N + gi) : 0.f;
-                        } else {
-                            load_block_rows(Hm, N, row0, c0, stg, lane, hv);
-                        }
+                if (use_acc) {
+                    mbar_wait(&sh->mma_bar, (mma_uses - 1u) & 1u);
+                    tc_fence_after();
+                }
+                const bool use_S = (th2 != 0.f);
+                long long trS = 0, fro2 = 0, trX = 0;       // 2^40 fixed point
+                bool bad = false;                           // a non-finite (or absurdly large) value was seen
+#pragma unroll 1
+                for (int c = 0; c < NG; ++c) {
+                    if (!owns_block<NG>(g, c)) continue;
+                    const uint32_t tc = (uint32_t)(32 * c);
+                    const int j0 = 32 * c + 16 * hf;
+                    uint32_t va[16], vs[16];
+                    if (use_acc) tmem_ld_32x32_x16(t_acc + tc, va);
+                    if (use_S) tmem_ld_32x32_x16(t_S + tc, vs);
+                    tmem_ld_wait();
+                    float sn[16];
 #pragma unroll
-                        for (int c = 0; c < 32; ++c) {
-                            const int j = c0 + c;
-                            float s = 0.f;
-                            if (gi < N && (upper ? j < N : j <= gi)) { s = w0 * hv[c]; if (j == gi) s += b0; }
-                            sn[c] = s;
-                        }
-                    } else {
-                        uint32_t va[32], vs[32];
-                        tmem_ld_32x32(t_acc + (uint32_t)c0, va);
-                        tmem_ld_32x32(t_S + (uint32_t)c0, vs);
-                        tmem_ld_wait();
-#pragma unroll
-                        for (int c = 0; c < 32; ++c) {
-                            const int j = c0 + c;
-                            const float x = __uint_as_float(va[c]);
-                            float val = fmaf(th1s, x, th2 * __uint_as_float(vs[c]));
-                            if (j == gi) {
-                                if (gi < N) val += th3;
-                                trX += (double)(x * inv2);
-                            }
-                            sn[c] = val;
-                        }
+                    for (int e = 0; e < 16; ++e) {
+                        float v = 0.f;
+                        if (use_S) v = th2 * __uint_as_float(vs[e]);
+                        if (use_acc) v = fmaf(th1s, __uint_as_float(va[e]), v);
+                        sn[e] = v;
                     }
-                    uint32_t so[32];
-                    uint32_t hp[16], lp[16];
-                    // squares of the strictly-lower entries: FP32 over one chunk (4 partial sums), FP64 across chunks;
-                    // FP64 per element only on the diagonal (the FP64 pipe is narrow)
-                    float q0 = 0.f, q1 = 0.f, q2 = 0.f, q3 = 0.f;
+                    uint32_t hp[8], lp[8];
+                    const uint32_t jr = (uint32_t)(j0 >> 7);                     // CTA that owns rows j0 .. j0 + 15
+                    // mirror (j, i): row j = j0 + e of CTA jr, column gi.  Byte offset inside the 128-row panel
+                    // = mir_base + ((j0 & 127) / 8 + (e >> 3)) * 1024 + mir_x[e & 7]  (see panel_off)
+                    const uint32_t mb = mir_base + (uint32_t)(((j0 & 127) >> 3) * 1024);
+                    if (c != g) {
+                        // ---- off-diagonal block: every entry is finalised here, no per-element predicate
 #pragma unroll
-                    for (int c = 0; c < 32; ++c) {
-                        const int j = c0 + c;
-                        so[c] = __float_as_uint(sn[c]);
-                        if ((c & 1) == 0) split_hi_lo2(sn[c], sn[c + 1], cs, hp[c >> 1], lp[c >> 1]);
-                        const float sq = (upper || j < gi) ? sn[c] * sn[c] : 0.f;
-                        if ((c & 3) == 0) q0 += sq; else if ((c & 3) == 1) q1 += sq;
-                        else if ((c & 3) == 2) q2 += sq; else q3 += sq;
-                        if (j == gi) {
-                            const double vd = (double)sn[c];
-                            trS += vd; fro2 += vd * vd;
-                        }
-                    }
-                    fro2 += 2.0 * (double)((q0 + q1) + (q2 + q3));
-                    tmem_st_32x32(t_S + (uint32_t)c0, so);      // FP32 master (entries j > i are never read)
-                    const bool below = (kind == 0);             // every entry of the chunk is off-diagonal and handled here
-                    const uint32_t jr = (uint32_t)(c0 >> 7);    // CTA that owns rows c0..c0+31
-                    if (below) {
+                        for (int e = 0; e < 16; e += 2) split_hi_lo2(sn[e], sn[e + 1], cs, hp[e >> 1], lp[e >> 1]);
+                        float q0 = 0.f, q1 = 0.f, q2 = 0.f, q3 = 0.f;
 #pragma unroll
-                        for (int g = 0; g < 4; ++g) {           // own row: four 16-byte pieces per matrix
-                            const uint32_t off = panel_off(tl, c0 + 8 * g);
-                            *reinterpret_cast<uint4*>(hiP + off) = make_uint4(hp[4 * g], hp[4 * g + 1], hp[4 * g + 2], hp[4 * g + 3]);
-                            *reinterpret_cast<uint4*>(loP + off) = make_uint4(lp[4 * g], lp[4 * g + 1], lp[4 * g + 2], lp[4 * g + 3]);
+                        for (int e = 0; e < 16; e += 4) {
+                            q0 = fmaf(sn[e], sn[e], q0); q1 = fmaf(sn[e + 1], sn[e + 1], q1);
+                            q2 = fmaf(sn[e + 2], sn[e + 2], q2); q3 = fmaf(sn[e + 3], sn[e + 3], q3);
                         }
-                    }
-                    // mirror (j, i): row j = c0 + c of CTA jr, column gi.  Byte offset inside the 128-row panel
-                    // = mir_base + (c >> 3) * 1024 + mir_x[c & 7]  (see panel_off): one add per element
-                    const uint32_t mb = mir_base + (uint32_t)(((c0 & 127) >> 3) * 1024);
-                    if (below) {                                // every j < gi: straight-line stores
+                        const float qsum = (q0 + q1) + (q2 + q3);        // FP32 over 16 entries, fixed point across blocks
+                        bad = bad || !(qsum <= 1.0e6f);
+                        fro2 += 2 * to_fix(qsum);
+                        uint32_t so[16];
+#pragma unroll
+                        for (int e = 0; e < 16; ++e) so[e] = __float_as_uint(sn[e]);
+                        tmem_st_32x32_x16(t_S + tc, so);                // FP32 master
+#pragma unroll
+                        for (int h8 = 0; h8 < 2; ++h8) {                // own row: two 16-byte pieces per matrix
+                            const uint32_t off = panel_off(tl, j0 + 8 * h8);
+                            *reinterpret_cast<uint4*>(hiP + off) = make_uint4(hp[4 * h8], hp[4 * h8 + 1], hp[4 * h8 + 2], hp[4 * h8 + 3]);
+                            *reinterpret_cast<uint4*>(loP + off) = make_uint4(lp[4 * h8], lp[4 * h8 + 1], lp[4 * h8 + 2], lp[4 * h8 + 3]);
+                        }
                         if (CG == 2 && jr != rank) {
                             const uint32_t rh = mapa_u32(hi_addr, jr) + mb, rl = mapa_u32(lo_addr, jr) + mb;
 #pragma unroll
-                            for (int c = 0; c < 32; ++c) {
-                                const uint32_t off = (uint32_t)((c >> 3) * 1024) + mir_x[c & 7];
-                                st_cluster_u16(rh + off, (unsigned short)(hp[c >> 1] >> (16 * (c & 1))));
-                                st_cluster_u16(rl + off, (unsigned short)(lp[c >> 1] >> (16 * (c & 1))));
+                            for (int e = 0; e < 16; ++e) {
+                                const uint32_t off = (uint32_t)((e >> 3) * 1024) + mir_x[e & 7];
+                                st_cluster_u16(rh + off, (unsigned short)(hp[e >> 1] >> (16 * (e & 1))));
+                                st_cluster_u16(rl + off, (unsigned short)(lp[e >> 1] >> (16 * (e & 1))));
                             }
                         } else {
+                            const uint32_t rh = hi_addr + mb, rl = lo_addr + mb;
 #pragma unroll
-                            for (int c = 0; c < 32; ++c) {
-                                const uint32_t off = mb + (uint32_t)((c >> 3) * 1024) + mir_x[c & 7];
-                                *reinterpret_cast<unsigned short*>(hiP + off) = (unsigned short)(hp[c >> 1] >> (16 * (c & 1)));
-                                *reinterpret_cast<unsigned short*>(loP + off) = (unsigned short)(lp[c >> 1] >> (16 * (c & 1)));
+                            for (int e = 0; e < 16; ++e) {
+                                const uint32_t off = (uint32_t)((e >> 3) * 1024) + mir_x[e & 7];
+                                st_shared_u16(rh + off, (unsigned short)(hp[e >> 1] >> (16 * (e & 1))));
+                                st_shared_u16(rl + off, (unsigned short)(lp[e >> 1] >> (16 * (e & 1))));
                             }
                         }
-                    } else {                                    // diagonal chunk (rows and columns of this CTA)
+                    } else {
+                        // ---- diagonal block: entries j <= i are authoritative; bias and traces on j == i
+                        float qs = 0.f;
 #pragma unroll
-                        for (int c = 0; c < 32; ++c) {
-                            const int j = c0 + c;
-                            const unsigned short hb = (unsigned short)(hp[c >> 1] >> (16 * (c & 1)));
-                            const unsigned short lb = (unsigned short)(lp[c >> 1] >> (16 * (c & 1)));
+                        for (int e = 0; e < 16; ++e) {
+                            const int j = j0 + e;
+                            if (j == gi) {
+                                if (gi < N) sn[e] += th3;
+                                if (use_acc) trX += to_fix(__uint_as_float(va[e]) * inv2);
+                                bad = bad || !(fabsf(sn[e]) <= 1.0e3f);
+                                trS += to_fix(sn[e]); fro2 += sq_fix(sn[e]);
+                            } else if (j < gi) {
+                                qs = fmaf(sn[e], sn[e], qs);
+                            }
+                        }
+                        bad = bad || !(qs <= 1.0e6f);
+                        fro2 += 2 * to_fix(qs);
+#pragma unroll
+                        for (int e = 0; e < 16; e += 2) split_hi_lo2(sn[e], sn[e + 1], cs, hp[e >> 1], lp[e >> 1]);
+                        uint32_t so[16];
+#pragma unroll
+                        for (int e = 0; e < 16; ++e) so[e] = __float_as_uint(sn[e]);
+                        tmem_st_32x32_x16(t_S + tc, so);                // entries j > i are never read back
+                        const uint32_t rh = hi_addr + mb, rl = lo_addr + mb;
+#pragma unroll
+                        for (int e = 0; e < 16; ++e) {
+                            const int j = j0 + e;
+                            const unsigned short hb = (unsigned short)(hp[e >> 1] >> (16 * (e & 1)));
+                            const unsigned short lb = (unsigned short)(lp[e >> 1] >> (16 * (e & 1)));
                             if (j <= gi) {                      // own entries one by one
                                 const uint32_t off = panel_off(tl, j);
-                                *reinterpret_cast<unsigned short*>(hiP + off) = hb;
-                                *reinterpret_cast<unsigned short*>(loP + off) = lb;
+                                st_shared_u16(hi_addr + off, hb);
+                                st_shared_u16(lo_addr + off, lb);
                             }
                             if (j < gi) {
-                                const uint32_t off = mb + (uint32_t)((c >> 3) * 1024) + mir_x[c & 7];
-                                *reinterpret_cast<unsigned short*>(hiP + off) = hb;
-                                *reinterpret_cast<unsigned short*>(loP + off) = lb;
+                                const uint32_t off = (uint32_t)((e >> 3) * 1024) + mir_x[e & 7];
+                                st_shared_u16(rh + off, hb);
+                                st_shared_u16(rl + off, lb);
                             }
                         }
                     }
@@ -376,10 +401,12 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
                     fro2 += __shfl_xor_sync(0xffffffffu, fro2, o);
                     trX += __shfl_xor_sync(0xffffffffu, trX, o);
                 }
+                bad = __any_sync(0xffffffffu, bad);
                 if (lane == 0) {
                     sh->part[iter & 1][warp][0] = trS;
                     sh->part[iter & 1][warp][1] = fro2;
                     sh->part[iter & 1][warp][2] = trX;
+                    sh->part[iter & 1][warp][3] = bad ? 1 : 0;
                 }
             }
             // panels (generic-proxy writes, local and remote) -> visible to the tensor core (async proxy)
@@ -387,79 +414,88 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
             tc_fence_before();
             group_sync<CG>();
             tc_fence_after();
+            // ---- a4 of the NEXT layer, X = S^2 (Eq. 15): 3 MMAs per 16 columns of K, operands = the resident panels;
+            // issued before the control step below has decided anything (it runs meanwhile)
+            if (issue_next) {
+                if (warp == C::MMA_WARP && rank == 0 && lane == 0) {
+                    constexpr uint32_t idesc = umma_idesc_f16(128 * CG, NP);
+#pragma unroll 1
+                    for (int kb = 0; kb < C::KBLK; ++kb) {
+#pragma unroll
+                        for (int k = 0; k < 4; ++k) {
+                            const uint64_t dh = umma_desc_sw128(hi_addr + kb * 16384 + k * 32);
+                            const uint64_t dl = umma_desc_sw128(lo_addr + kb * 16384 + k * 32);
+                            umma_f16<CG>(tmem_base, dh, dh, idesc, (kb | k) != 0);
+                            umma_f16<CG>(tmem_base, dh, dl, idesc, 1u);
+                            umma_f16<CG>(tmem_base, dl, dh, idesc, 1u);
+                        }
+                    }
+                    if (CG == 1) umma_commit(&sh->mma_bar); else umma_commit_pair(&sh->mma_bar, 0x3);
+                }
+                ++mma_uses;
+            }
             // ---- a8: control (Alg. 1), evaluated redundantly by both CTAs from identical sums
             // Lane l < 8 CG of warp 0 fetches the partial sums of epilogue warp (l & 7) of CTA (l >> 3) (own shared
             // memory or the peer's through DSMEM: all remote loads in flight at once), then a fixed xor-shuffle tree:
             // the same order in both CTAs, so both take identical decisions.
             if (warp == 0) {
-                double a = 0.0, b = 0.0, cX = 0.0;
+                long long a = 0, b = 0, cX = 0, nf = 0;
                 if (lane < 8 * CG) {
                     const uint32_t r = (uint32_t)lane >> 3;
                     const int w = lane & 7;
                     if (r == rank) {
                         a = sh->part[iter & 1][w][0]; b = sh->part[iter & 1][w][1]; cX = sh->part[iter & 1][w][2];
+                        nf = sh->part[iter & 1][w][3];
                     } else {
                         const uint32_t base = mapa_u32(smem_u32(&sh->part[iter & 1][w][0]), r);
-                        a = ld_cluster_f64(base); b = ld_cluster_f64(base + 8); cX = ld_cluster_f64(base + 16);
+                        a = ld_cluster_s64(base); b = ld_cluster_s64(base + 8); cX = ld_cluster_s64(base + 16);
+                        nf = ld_cluster_s64(base + 24);
                     }
                 }
 #pragma unroll
-                for (int o = 8; o > 0; o >>= 1) {
+                for (int o = 8; o > 0; o >>= 1) {           // integer adds: exact, so both CTAs get identical sums
                     a += __shfl_xor_sync(0xffffffffu, a, o);
                     b += __shfl_xor_sync(0xffffffffu, b, o);
                     cX += __shfl_xor_sync(0xffffffffu, cX, o);
+                    nf += __shfl_xor_sync(0xffffffffu, nf, o);
                 }
                 if (lane == 0) {
                     CtrlCore* c = &sh->ctrl;
-                    if (first) {
-                        c->N_S = a; c->fro2 = b;         // N_S = Tr[S_0]
+                    if (iter == 0) {
+                        c->N_S = a; c->fro2 = b; c->nonfinite = nf ? 1 : 0;       // N_S = Tr[S_0]
                         control_plan_next(c, stats_m, p.thetas);
                     } else {
-                        control_finish_layer(c, stats_m, p.thetas, a, b, cX);
+                        control_finish_layer(c, stats_m, p.thetas, a, b, cX, nf != 0);
                     }
                 }
             }
             __syncthreads();
-            first = false;
             ++iter;
-            if (!sh->ctrl.running) break;
-            th1s = sh->ctrl.theta[0] * inv2; th2 = sh->ctrl.theta[1]; th3 = sh->ctrl.theta[2];
-            trS = fro2 = trX = 0.0;
-            // ---- a4: X = S^2 (Eq. 15): 3 MMAs per 16 columns of K, operands = the resident panels
-            if (warp == C::MMA_WARP && rank == 0 && lane == 0) {
-                constexpr uint32_t idesc = umma_idesc_f16(128 * CG, NP);
-#pragma unroll 1
-                for (int kb = 0; kb < C::KBLK; ++kb) {
-#pragma unroll
-                    for (int k = 0; k < 4; ++k) {
-                        const uint64_t dh = umma_desc_sw128(hi_addr + kb * 16384 + k * 32);
-                        const uint64_t dl = umma_desc_sw128(lo_addr + kb * 16384 + k * 32);
-                        umma_f16<CG>(tmem_base, dh, dh, idesc, (kb | k) != 0);
-                        umma_f16<CG>(tmem_base, dh, dl, idesc, 1u);
-                        umma_f16<CG>(tmem_base, dl, dh, idesc, 1u);
-                    }
+            if (!sh->ctrl.running) {
+                if (issue_next) {                        // drain the speculative MMAs before anything is reused
+                    mbar_wait(&sh->mma_bar, (mma_uses - 1u) & 1u);
+                    tc_fence_after();
                 }
-                if (CG == 1) umma_commit(&sh->mma_bar); else umma_commit_pair(&sh->mma_bar, 0x3);
+                break;
             }
-            __syncwarp();
-            mbar_wait(&sh->mma_bar, mma_phase);
-            mma_phase ^= 1u;
-            tc_fence_after();
+            th1s = sh->ctrl.theta[0] * inv2; th2 = sh->ctrl.theta[1]; th3 = sh->ctrl.theta[2];
+            use_acc = true;
         }
 
         // ------------------------------------------------------------------ output: D = S_n, both triangles
         if (warp < 8) {
-            for (int c0 = 0; c0 < NP; c0 += 32) {
-                const int kind = chunk_kind<CG>(row0, c0);
-                if (kind < 0 || ((c0 >> 5) & 1) != hf) continue;
-                uint32_t vs[32];
-                tmem_ld_32x32(t_S + (uint32_t)c0, vs);
+#pragma unroll 1
+            for (int c = 0; c < NG; ++c) {
+                if (!owns_block<NG>(g, c)) continue;
+                const int j0 = 32 * c + 16 * hf;
+                uint32_t vs[16];
+                tmem_ld_32x32_x16(t_S + (uint32_t)(32 * c), vs);
                 tmem_ld_wait();
 #pragma unroll
-                for (int c = 0; c < 32; ++c) {
-                    const int j = c0 + c;
-                    if (gi < N && (c0 > row0 ? j < N : j <= gi)) {
-                        const float v = __uint_as_float(vs[c]);
+                for (int e = 0; e < 16; ++e) {
+                    const int j = j0 + e;
+                    if (gi < N && j < N && (c != g || j <= gi)) {
+                        const float v = __uint_as_float(vs[e]);
                         Dm[(size_t)j * N + gi] = v;      // mirrored position: coalesced across the warp
                         Dm[(size_t)gi * N + j] = v;
                     }

@@ -64,7 +64,7 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
     uint64_t* tfull_bar = bars + 2 * STAGES;         // [2]
     uint64_t* tempty_bar = bars + 2 * STAGES + 2;    // [2]
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * STAGES + 4);
-    __shared__ double red[4][3];
+    __shared__ fx_t red[4][4];
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
@@ -235,11 +235,13 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
         __half* __restrict__ LO = p.lo_out;
         unsigned long long* __restrict__ Rcur = p.rowsq_cur;
         unsigned long long* __restrict__ Rnext = p.rowsq_next;
-        // FP64 is kept off the per-element path (the FP64 pipe of sm_100 is narrow: per-element DMUL/DFMA made the
-        // epilogue as long as the mainloop).  Off-diagonal squares are summed in FP32 over one 32-element chunk
-        // (4 independent partial sums, |error| <= ~2^-22 of a sum of ~1e-3) and promoted to FP64 once per chunk;
-        // the diagonal chunk (one per 128 rows of a diagonal supertile) keeps per-element FP64.
-        double trS = 0.0, off2 = 0.0, dg2 = 0.0, trX = 0.0;   // ||S_n||_F^2 = 2 off2 + dg2
+        // No FP64 anywhere in the kernel (an isolated FP64 instruction pays ~170 cycles to wake the datapath, see
+        // sp2_control.cuh): the traces are 2^40 fixed-point integers.  Off-diagonal squares are summed in FP32 over one
+        // 32-element chunk (4 independent partial sums, |error| <= ~2^-22 of a sum of ~1e-3) and converted once per
+        // chunk (exact); the diagonal chunk (one per 128 rows of a diagonal supertile) converts per element, squares
+        // as exact FP32 pairs.
+        fx_t trS = 0, off2 = 0, dg2 = 0, trX = 0;           // ||S_n||_F^2 = 2 off2 + dg2
+        bool bad = false;                                   // a non-finite (or out-of-range) value went into a trace
         int it = 0;                                         // accumulator uses so far (same count as the MMA warp)
         const int nch = C::ENH ? (KB + p.enh_kc - 1) / p.enh_kc : 1;
         const uint32_t lane_off = (uint32_t)(q * 32) << 16;
@@ -250,7 +252,7 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
             const int ncols = wi.ncols;
             const int gi = m0 + rl;
             const int gi_wmin = m0 + q * 32, gi_wmax = gi_wmin + 31;
-            double rowacc = 0.0;                            // sum_j S_n(gi, j)^2 over the own entries (j <= gi) of this tile
+            fx_t rowacc = 0;                                // sum_j S_n(gi, j)^2 over the own entries (j <= gi) of this tile
             if (C::ENH) {
                 // all chunks but the last: fold the chunk sum into the running FP32 pair (two-sum, error-free)
                 const uint32_t t_rh = tmem_base + (uint32_t)(2 * BN) + lane_off, t_rl = t_rh + (uint32_t)BN;
@@ -324,13 +326,25 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                     }
                 }
                 const bool below = (gj0 + 31 <= gi_wmin);   // whole 32x32 chunk strictly in the lower triangle
-                // S_{n-1}: read at the mirrored position (S is exactly symmetric) -> coalesced across the warp
-#pragma unroll
-                for (int c = 0; c < 32; ++c) so[c] = __ldcs(S + (long long)(gj0 + c) * ld + gi);
+                // S_{n-1}: read at the mirrored position (S is exactly symmetric) -> coalesced across the warp.  In a
+                // diagonal chunk only the entries gj <= gi are used; the others (which a neighbouring lane rewrites
+                // further down) are not even loaded.
                 float mo[C::MIX ? 32 : 1];
-                if (C::MIX) {
+                if (below) {
 #pragma unroll
-                    for (int c = 0; c < 32; ++c) mo[C::MIX ? c : 0] = __ldcs(M + (long long)(gj0 + c) * ld + gi);
+                    for (int c = 0; c < 32; ++c) so[c] = __ldcs(S + (long long)(gj0 + c) * ld + gi);
+                    if (C::MIX) {
+#pragma unroll
+                        for (int c = 0; c < 32; ++c) mo[C::MIX ? c : 0] = __ldcs(M + (long long)(gj0 + c) * ld + gi);
+                    }
+                } else {
+#pragma unroll
+                    for (int c = 0; c < 32; ++c) so[c] = (gj0 + c <= gi) ? __ldcs(S + (long long)(gj0 + c) * ld + gi) : 0.f;
+                    if (C::MIX) {
+#pragma unroll
+                        for (int c = 0; c < 32; ++c)
+                            mo[C::MIX ? c : 0] = (gj0 + c <= gi) ? __ldcs(M + (long long)(gj0 + c) * ld + gi) : 0.f;
+                    }
                 }
                 if (below) {
                     tmem_ld_wait();
@@ -380,7 +394,9 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                         __stcs(reinterpret_cast<uint4*>(rowH) + g, make_uint4(hp[0], hp[1], hp[2], hp[3]));
                         __stcs(reinterpret_cast<uint4*>(rowL) + g, make_uint4(lp[0], lp[1], lp[2], lp[3]));
                     }
-                    const double sd = (double)((a0 + a1) + (a2 + a3));
+                    const float sdf = (a0 + a1) + (a2 + a3);
+                    bad = bad || !(sdf <= 1.0e6f);
+                    const fx_t sd = fx_from_float(sdf);
                     off2 += sd;
                     rowacc += sd;
                 } else {
@@ -388,11 +404,11 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                     // of X_n: diag(S_{n-1}^2)_i = sum_j S_{n-1}(i,j)^2, accumulated while S_{n-1} was written
                     float xdiag = 0.f;
                     if (Rcur != nullptr) {
-                        xdiag = (float)((double)(long long)Rcur[gi] * kRowSqInv);
+                        xdiag = (float)(long long)Rcur[gi] * kRowSqInvF;       // one rounding, as through FP64
                         Rcur[gi] = 0ull;                    // this buffer is the accumulator of the layer after next
                     }
                     tmem_ld_wait();
-                    double sq_own = 0.0;
+                    fx_t sq_own = 0;
 #pragma unroll
                     for (int c = 0; c < 32; ++c) {
                         const int gj = gj0 + c;
@@ -406,9 +422,13 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                         __half h, l;
                         split_hi_lo(val, cs, h, l);
                         const unsigned short hb = __half_as_ushort(h), lb = __half_as_ushort(l);
-                        const double vd = (double)val;
-                        if (gj < gi) { sq_own += vd * vd; off2 += vd * vd; }
-                        if (on_diag) { sq_own += vd * vd; dg2 += vd * vd; trS += vd; trX += (double)(x * inv2); }
+                        if (gj <= gi) {
+                            bad = bad || !(fabsf(val) <= 1.0e3f);
+                            const fx_t v2 = fx_square(val);
+                            sq_own += v2;
+                            if (on_diag) { dg2 += v2; trS += fx_from_float(val); trX += fx_from_float(x * inv2); }
+                            else off2 += v2;
+                        }
                         so[c] = (gj < gi) ? val * val : 0.f;
                         if (gj <= gi) {
                             const long long o = (long long)gj * ldf + gi, o2 = (long long)gi * ldf + gj;
@@ -436,10 +456,10 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                             so[i] = keep + __shfl_xor_sync(0xffffffffu, send, sft);
                         }
                     }
-                    if (so[0] != 0.f) atomicAdd(Rnext + gj0 + lane, rowsq_fix((double)so[0]));
+                    if (so[0] != 0.f) atomicAdd(Rnext + gj0 + lane, rowsq_fix(so[0]));
                 }
             }
-            if (Rnext != nullptr && rowacc != 0.0) atomicAdd(Rnext + gi, rowsq_fix(rowacc));
+            if (Rnext != nullptr && rowacc != 0) atomicAdd(Rnext + gi, (unsigned long long)(rowacc << (kRowSqBits - kFxBits)));
             // all tcgen05.ld of this accumulator have completed (tmem_ld_wait above): hand it back to the MMA warp
             tc_fence_before();
             __syncwarp();
@@ -447,44 +467,47 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                 if (CG == 1) mbar_arrive(&tempty_bar[buf]); else mbar_arrive_cluster(&tempty_bar[buf], 0);
             }
         }
-        // ---- block partials -> ctrl -> last CTA runs the control step
-        double fro2 = 2.0 * off2 + dg2;
+        // ---- block partials -> ctrl -> last CTA runs the control step (integer adds: exact, any order)
+        fx_t fro2 = 2 * off2 + dg2;
         for (int o = 16; o > 0; o >>= 1) {
             trS += __shfl_xor_sync(0xffffffffu, trS, o);
             fro2 += __shfl_xor_sync(0xffffffffu, fro2, o);
             trX += __shfl_xor_sync(0xffffffffu, trX, o);
         }
-        if (lane == 0) { red[q][0] = trS; red[q][1] = fro2; red[q][2] = trX; }
+        bad = __any_sync(0xffffffffu, bad);
+        if (lane == 0) { red[q][0] = trS; red[q][1] = fro2; red[q][2] = trX; red[q][3] = bad ? 1 : 0; }
         asm volatile("bar.sync 1, 128;\n" ::: "memory");     // the four epilogue warps only
         if (warp == 2) {
             unsigned int done = 0;
             if (lane == 0) {
-                double a = 0.0, b = 0.0, c = 0.0;
-                for (int i = 0; i < 4; ++i) { a += red[i][0]; b += red[i][1]; c += red[i][2]; }
-                ctrl->partial[blockIdx.x][0] = a;
-                ctrl->partial[blockIdx.x][1] = b;
-                ctrl->partial[blockIdx.x][2] = c;
+                fx_t a = 0, b = 0, c = 0, f = 0;
+                for (int i = 0; i < 4; ++i) { a += red[i][0]; b += red[i][1]; c += red[i][2]; f += red[i][3]; }
+                ctrl->ipartial[blockIdx.x][0] = a;
+                ctrl->ipartial[blockIdx.x][1] = b;
+                ctrl->ipartial[blockIdx.x][2] = c;
+                ctrl->ipartial[blockIdx.x][3] = f;
                 __threadfence();
                 done = atomicAdd(&ctrl->done_counter, 1u);
             }
             done = __shfl_sync(0xffffffffu, done, 0);
             if (done == gridDim.x - 1) {
-                // last CTA: sum the per-CTA partials (each lane a strided subset in index order, then a fixed shuffle
-                // tree: deterministic for a given grid) and run the control step of Alg. 1
+                // last CTA: sum the per-CTA partials and run the control step of Alg. 1
                 __threadfence();
-                double a = 0.0, b = 0.0, c = 0.0;
+                fx_t a = 0, b = 0, c = 0, f = 0;
                 for (unsigned int i = lane; i < gridDim.x; i += 32) {
-                    a += ((volatile double*)ctrl->partial[i])[0];
-                    b += ((volatile double*)ctrl->partial[i])[1];
-                    c += ((volatile double*)ctrl->partial[i])[2];
+                    a += ((volatile fx_t*)ctrl->ipartial[i])[0];
+                    b += ((volatile fx_t*)ctrl->ipartial[i])[1];
+                    c += ((volatile fx_t*)ctrl->ipartial[i])[2];
+                    f += ((volatile fx_t*)ctrl->ipartial[i])[3];
                 }
                 for (int o = 16; o > 0; o >>= 1) {
                     a += __shfl_xor_sync(0xffffffffu, a, o);
                     b += __shfl_xor_sync(0xffffffffu, b, o);
                     c += __shfl_xor_sync(0xffffffffu, c, o);
+                    f += __shfl_xor_sync(0xffffffffu, f, o);
                 }
                 if (lane == 0) {
-                    control_finish_layer(ctrl, p.stats, p.thetas, a, b, c);
+                    control_finish_layer(ctrl, p.stats, p.thetas, a, b, c, f != 0);
                     __threadfence();
                     if (p.cond_handle != 0) cudaGraphSetConditional(p.cond_handle, ctrl->running ? 1u : 0u);
                 }
