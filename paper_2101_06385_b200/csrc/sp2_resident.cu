@@ -24,26 +24,29 @@
 
 namespace sp2 {
 
-template <int NP_, int CG_>
+template <int NP_, int CG_, int CW_>
 struct ResCfg {
     static constexpr int NP = NP_, CG = CG_;
+    static constexpr int CW = CW_;                        // columns of a 32 x 32 block per warp (16 or 8)
+    static constexpr int WPG = 32 / CW;                   // warps per row group
     static constexpr int KBLK = NP / 64;
     static constexpr int PANEL_BYTES = KBLK * 16384;      // 128 rows x NP fp16
     static constexpr int TMEM_COLS = 2 * NP;
     static constexpr int NG = NP / 32;                    // row groups = column chunks of 32
-    // warps 0-7: epilogue (warp w owns TMEM lanes 32 (w % 4) .. +31 and columns 16 (w / 4) .. +15 of every block of
-    // its row group), warp 8: MMA issue + TMEM alloc
-    static constexpr int THREADS = 288;
-    static constexpr int MMA_WARP = 8;
-    static constexpr int STAGE_FLOATS = 8 * 32 * 17;
+    // warps 0 .. 4 WPG - 1: epilogue (warp w owns TMEM lanes 32 (w % 4) .. +31 and columns CW (w / 4) .. + CW - 1 of
+    // every block of its row group), the last warp: MMA issue + TMEM alloc
+    static constexpr int EPI_WARPS = 4 * WPG;
+    static constexpr int THREADS = (EPI_WARPS + 1) * 32;
+    static constexpr int MMA_WARP = EPI_WARPS;
+    static constexpr int STAGE_FLOATS = EPI_WARPS * 32 * (CW + 1);
 };
 
 struct ResShared {
     uint64_t mma_bar;
     uint32_t tmem_slot;
     uint32_t pad0;
-    long long part[2][8][4];     // [iteration parity][warp][trS, fro2, trX (2^40 fixed point), non-finite flag]
-    float rrow[2][128];          // Gershgorin: per column-half row sums of the off-diagonal entries
+    long long part[2][16][4];    // [iteration parity][warp][trS, fro2, trX (2^40 fixed point), non-finite flag]
+    float rrow[4][128];          // Gershgorin: per column-part row sums of the off-diagonal entries
     float dii[128];              // Gershgorin: diagonal entries
     float rcol[4][256];          // Gershgorin: column sums of the blocks finalised by row group q of this CTA
     float mm[4][2];              // per-warp min(d - R), max(d + R)
@@ -96,14 +99,77 @@ __device__ __forceinline__ long long ld_cluster_s64(uint32_t addr) {
     return v;
 }
 
+// Stores with a compile-time byte offset folded into the instruction (REMOTE: the address is a shared::cluster one).
+template <bool REMOTE, int IMM>
+__device__ __forceinline__ void st_u16_imm(uint32_t addr, uint32_t v) {
+    if (REMOTE) asm volatile("st.shared::cluster.u16 [%0+%2], %1;\n" ::"r"(addr), "h"((unsigned short)v), "n"(IMM) : "memory");
+    else asm volatile("st.shared.u16 [%0+%2], %1;\n" ::"r"(addr), "h"((unsigned short)v), "n"(IMM) : "memory");
+}
+__device__ __forceinline__ void st_shared_v4(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};\n" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
+}
+// hi/lo split of two already-scaled values (the master is kept as c S, see the layer loop): Eqs. 12-13
+__device__ __forceinline__ void split_scaled2(float a0, float a1, uint32_t& hi2, uint32_t& lo2) {
+    const __half2 h = __floats2half2_rn(a0, a1);
+    const float2 hf = __half22float2(h);
+    const __half2 l = __floats2half2_rn(a0 - hf.x, a1 - hf.y);
+    hi2 = *reinterpret_cast<const uint32_t*>(&h);
+    lo2 = *reinterpret_cast<const uint32_t*>(&l);
+}
+template <int CW> __device__ __forceinline__ void tmem_ld_cw(uint32_t taddr, uint32_t (&v)[CW]);
+template <> __device__ __forceinline__ void tmem_ld_cw<16>(uint32_t taddr, uint32_t (&v)[16]) { tmem_ld_32x32_x16(taddr, v); }
+template <> __device__ __forceinline__ void tmem_ld_cw<8>(uint32_t taddr, uint32_t (&v)[8]) { tmem_ld_32x32_x8(taddr, v); }
+template <int CW> __device__ __forceinline__ void tmem_st_cw(uint32_t taddr, const uint32_t (&v)[CW]);
+template <> __device__ __forceinline__ void tmem_st_cw<16>(uint32_t taddr, const uint32_t (&v)[16]) { tmem_st_32x32_x16(taddr, v); }
+template <> __device__ __forceinline__ void tmem_st_cw<8>(uint32_t taddr, const uint32_t (&v)[8]) { tmem_st_32x32_x8(taddr, v); }
+
+// Mirror stores of a CW-column part of a block: element e goes to panel row (j0 + e), column gi.  bh / bl = the hi /
+// lo panel address of row (j0 + (e & 7)) at column gi; rows 8 further down are 1024 bytes on.  PRED: only e < lim.
+#ifndef SP2_RES_EXP
+#define SP2_RES_EXP 0        // timing experiments only (results are wrong when non-zero): 1 no remote mirror, 2 no mirror
+#endif                       // at all, 4 no master traffic, 8 no own-row stores
+template <int E, bool REMOTE, bool PRED, int CW>
+__device__ __forceinline__ void mirror_cw(const uint32_t (&bh)[8], const uint32_t (&bl)[8], const uint32_t (&hp)[CW / 2],
+                                          const uint32_t (&lp)[CW / 2], int lim) {
+    if ((SP2_RES_EXP & 2) || ((SP2_RES_EXP & 1) && REMOTE)) return;
+    if constexpr (E < CW) {
+        constexpr int IMM = (E >> 3) * 1024;
+        const uint32_t h = (E & 1) ? (hp[E >> 1] >> 16) : hp[E >> 1];
+        const uint32_t l = (E & 1) ? (lp[E >> 1] >> 16) : lp[E >> 1];
+        if (!PRED || E < lim) {
+            st_u16_imm<REMOTE, IMM>(bh[E & 7], h);
+            st_u16_imm<REMOTE, IMM>(bl[E & 7], l);
+        }
+        mirror_cw<E + 1, REMOTE, PRED, CW>(bh, bl, hp, lp, lim);
+    }
+}
+
 template <int CG>
 __device__ __forceinline__ void group_sync() {
     if (CG == 2) cluster_sync_all(); else __syncthreads();
 }
 
+#ifdef SP2_RES_TIMING
+// experiment builds only: cycles per phase, summed over passes, for (CTA 0, warp 1): [0] MMA wait, [1] block loop,
+// [2] reduce + publish, [3] cluster barrier, [4] MMA issue + control + block barrier, [5] passes, [6] load H + bounds,
+// [7] output + end-of-matrix barrier
+__device__ unsigned long long g_res_timing[8];
+__device__ unsigned long long g_res_span[3 * 160];      // per CTA: cycles start -> end, globaltimer start, end
+#define RT_MARK(i) do { if (rt_on) { const long long t_ = clock64(); rt_acc[i] += t_ - rt_t; rt_t = t_; } } while (0)
+#else
+#define RT_MARK(i) do { } while (0)
+#endif
+
 template <class C>
 __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentParams p) {
-    constexpr int NP = C::NP, CG = C::CG, NG = C::NG;
+#ifdef SP2_RES_TIMING
+    const bool rt_on = (blockIdx.x == 0 && threadIdx.x == 32);
+    long long rt_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0}, rt_t = clock64();
+    const long long rt_c0 = clock64();
+    unsigned long long rt_g0;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(rt_g0));
+#endif
+    constexpr int NP = C::NP, CG = C::CG, NG = C::NG, CW = C::CW, WPG = C::WPG, EW = C::EPI_WARPS;
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     uint8_t* hiP = smem;
@@ -133,14 +199,16 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
     uint32_t mma_uses = 0;                        // MMA batches issued so far (uniform over the cluster)
 
     const int q = warp & 3;
-    const int hf = (warp >> 2) & 1;               // which 16 of a block's 32 columns this warp takes
+    const int hf = (warp >> 2) & (WPG - 1);       // which CW of a block's 32 columns this warp takes
     const int tl = q * 32 + lane;                  // row inside this CTA's panel (TMEM lane)
     const int gi = (int)rank * 128 + tl;           // global row
     const int g = (int)rank * 4 + q;               // row group
-    float* stg = stage + (warp & 7) * (32 * 17);
-    const uint32_t t_acc = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(16 * hf);
+    float* stg = stage + (warp & (EW - 1)) * (32 * (CW + 1));
+    const uint32_t t_acc = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(CW * hf);
     const uint32_t t_S = t_acc + NP;
     const float cs = p.scale, inv2 = p.inv_scale2;
+    const float inv_c = 1.0f / cs;                // exact: c is a power of two
+    const uint32_t own_row = (uint32_t)((tl >> 3) * 1024 + (tl & 7) * 128);    // panel_off(tl, .) without the column part
     // mirror-store address pieces that depend on this thread's column gi only (panel_off(row, gi) split by row bits)
     const uint32_t mir_base = (uint32_t)((gi >> 6) * 16384 + (gi & 7) * 2);
     uint32_t mir_x[8];
@@ -152,58 +220,59 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
         float* __restrict__ Dm = p.D + (size_t)m * N * N;
         sp2_layer_stat_t* stats_m = (rank == 0) ? p.stats + (size_t)m * p.max_layers : nullptr;
 
+        RT_MARK(5);
         // ------------------------------------------------------------------ load H (lower triangle, reading C22) into
         // the master region of TMEM; a1: Gershgorin bounds on the way (Alg. 1)
         if (p.auto_bounds) {
             for (int i = threadIdx.x; i < 1024; i += blockDim.x) (&sh->rcol[0][0])[i] = 0.f;
             __syncthreads();
         }
-        if (warp < 8) {
+        if (warp < EW) {
             float Rrow = 0.f;
 #pragma unroll 1
             for (int c = 0; c < NG; ++c) {
                 if (!owns_block<NG>(g, c)) continue;
-                const int j0 = 32 * c + 16 * hf;              // first matrix column of this warp's half block
-                float hv[16];
+                const int j0 = 32 * c + CW * hf;              // first matrix column of this warp's part of the block
+                float hv[CW];
                 if (c > g) {
                     // block above the diagonal: entry (gi, j) is read as H(j, gi); lane = row already
 #pragma unroll
-                    for (int e = 0; e < 16; ++e)
+                    for (int e = 0; e < CW; ++e)
                         hv[e] = (gi < N && j0 + e < N) ? __ldg(Hm + (size_t)(j0 + e) * N + gi) : 0.f;
                 } else {
-                    // coalesced row segments (two rows of 16 per load), transposed through the staging tile
+                    // coalesced row segments (32 / CW rows of CW per load), transposed through the staging tile
                     __syncwarp();
 #pragma unroll 4
-                    for (int r2 = 0; r2 < 32; r2 += 2) {
-                        const int r = r2 + (lane >> 4), i = g * 32 + r, j = j0 + (lane & 15);
+                    for (int r2 = 0; r2 < 32; r2 += 32 / CW) {
+                        const int r = r2 + lane / CW, i = g * 32 + r, j = j0 + (lane & (CW - 1));
                         float v = 0.f;
                         if (i < N && j <= i) v = __ldg(Hm + (size_t)i * N + j);
-                        stg[r * 17 + (lane & 15)] = v;
+                        stg[r * (CW + 1) + (lane & (CW - 1))] = v;
                     }
                     __syncwarp();
 #pragma unroll
-                    for (int e = 0; e < 16; ++e) hv[e] = stg[lane * 17 + e];
+                    for (int e = 0; e < CW; ++e) hv[e] = stg[lane * (CW + 1) + e];
                 }
-                uint32_t hu[16];
+                uint32_t hu[CW];
 #pragma unroll
-                for (int e = 0; e < 16; ++e) hu[e] = __float_as_uint(hv[e]);
-                tmem_st_32x32_x16(t_S + (uint32_t)(32 * c), hu);
+                for (int e = 0; e < CW; ++e) hu[e] = __float_as_uint(hv[e]);
+                tmem_st_cw<CW>(t_S + (uint32_t)(32 * c), hu);
                 if (p.auto_bounds) {
                     // |entry| adds to the radius of its row (this thread) and of its column (sum over the 32 rows)
                     __syncwarp();
 #pragma unroll
-                    for (int e = 0; e < 16; ++e) {
+                    for (int e = 0; e < CW; ++e) {
                         const int j = j0 + e;
                         const float a = (c == g && j >= gi) ? 0.f : fabsf(hv[e]);   // diagonal block: j < i only
                         if (c == g && j == gi) sh->dii[tl] = hv[e];
                         Rrow += a;
-                        stg[lane * 17 + e] = a;
+                        stg[lane * (CW + 1) + e] = a;
                     }
                     __syncwarp();
-                    if (lane < 16) {
+                    if (lane < CW) {
                         float colp = 0.f;
 #pragma unroll 8
-                        for (int r = 0; r < 32; ++r) colp += stg[r * 17 + lane];
+                        for (int r = 0; r < 32; ++r) colp += stg[r * (CW + 1) + lane];
                         sh->rcol[q][j0 + lane] = colp;      // each (row group, column) slot is written once
                     }
                 }
@@ -216,7 +285,8 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
             group_sync<CG>();
             float lo = INFINITY, hi = -INFINITY;
             if (warp < 4) {
-                float R = sh->rrow[0][tl] + sh->rrow[1][tl];
+                float R = 0.f;
+                for (int w = 0; w < WPG; ++w) R += sh->rrow[w][tl];
                 const float dii = (gi < N) ? sh->dii[tl] : 0.f;
                 for (uint32_t r = 0; r < (uint32_t)CG; ++r)
                     for (int w = 0; w < 4; ++w)
@@ -268,11 +338,15 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
             continue;
         }
         __syncthreads();            // ctrl initialised before anyone reads it
+        RT_MARK(6);
 
         // ------------------------------------------------------------------ the layers.  Pass 0 is a2: S_0 = W_0 H + B_0
         // (Alg. 1) = the generic update with th1 = 0, th2 = W_0, th3 = B_0 applied to the master (= H);
         // pass n >= 1 is S_n = th1 X_n / c^2 + th2 S_{n-1} + th3 I from layer n's accumulator.
-        float th1s = 0.f, th2 = (float)(-1.0 / (e1 - e0)), th3 = (float)(e1 / (e1 - e0));
+        // The master in TMEM holds c S (c = 2^k of the split, reading C10: an exact rescale), so a layer reads
+        //   c S_n = (th1 / c) (c^2 X_n) + th2 (c S_{n-1}) + c th3 I
+        // and the split needs no multiply.  Traces are taken of S itself (the power-of-two factors come off exactly).
+        float th1s = 0.f, th2 = (float)(-1.0 / (e1 - e0)) * cs, th3 = (float)(e1 / (e1 - e0)) * cs;
         bool use_acc = false;
         int iter = 0;
         while (true) {
@@ -281,11 +355,13 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
             // has already fired, nor when a fixed-depth network ends here.
             const bool issue_next = (sh->ctrl.pending_stop == SP2_STOP_NONE) &&
                                     !(p.mode == MODE_GENERALIZED && iter >= p.max_layers);
-            if (warp < 8) {
+            RT_MARK(5);
+            if (warp < EW) {
                 if (use_acc) {
                     mbar_wait(&sh->mma_bar, (mma_uses - 1u) & 1u);
                     tc_fence_after();
                 }
+                RT_MARK(0);
                 const bool use_S = (th2 != 0.f);
                 long long trS = 0, fro2 = 0, trX = 0;       // 2^40 fixed point
                 bool bad = false;                           // a non-finite (or absurdly large) value was seen
@@ -293,107 +369,105 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
                 for (int c = 0; c < NG; ++c) {
                     if (!owns_block<NG>(g, c)) continue;
                     const uint32_t tc = (uint32_t)(32 * c);
-                    const int j0 = 32 * c + 16 * hf;
-                    uint32_t va[16], vs[16];
-                    if (use_acc) tmem_ld_32x32_x16(t_acc + tc, va);
-                    if (use_S) tmem_ld_32x32_x16(t_S + tc, vs);
+                    const int j0 = 32 * c + CW * hf;
+                    uint32_t va[CW], vs[CW];
+                    float sn[CW];
+                    if (use_acc) tmem_ld_cw<CW>(t_acc + tc, va);
+                    if (use_S && !(SP2_RES_EXP & 4)) tmem_ld_cw<CW>(t_S + tc, vs);
                     tmem_ld_wait();
-                    float sn[16];
+                    if (use_acc && use_S) {
 #pragma unroll
-                    for (int e = 0; e < 16; ++e) {
-                        float v = 0.f;
-                        if (use_S) v = th2 * __uint_as_float(vs[e]);
-                        if (use_acc) v = fmaf(th1s, __uint_as_float(va[e]), v);
-                        sn[e] = v;
+                        for (int e = 0; e < CW; ++e) sn[e] = fmaf(th1s, __uint_as_float(va[e]), th2 * __uint_as_float(vs[e]));
+                    } else if (use_acc) {
+#pragma unroll
+                        for (int e = 0; e < CW; ++e) sn[e] = th1s * __uint_as_float(va[e]);
+                    } else {
+#pragma unroll
+                        for (int e = 0; e < CW; ++e) sn[e] = th2 * __uint_as_float(vs[e]);
                     }
-                    uint32_t hp[8], lp[8];
-                    const uint32_t jr = (uint32_t)(j0 >> 7);                     // CTA that owns rows j0 .. j0 + 15
+                    uint32_t hp[CW / 2], lp[CW / 2];
+                    const uint32_t jr = (uint32_t)(j0 >> 7);                     // CTA that owns rows j0 .. j0 + CW - 1
+                    // own row: columns j0 .. j0 + CW - 1 = CW / 8 16-byte pieces per matrix (swizzled chunk index ^ (tl & 7))
+                    const uint32_t own0 = (uint32_t)((j0 >> 6) * 16384) + own_row + ((uint32_t)((((j0 & 63) >> 3)) ^ (tl & 7)) << 4);
+                    const uint32_t own1 = (uint32_t)((j0 >> 6) * 16384) + own_row + ((uint32_t)((((j0 & 63) >> 3) + 1) ^ (tl & 7)) << 4);
                     // mirror (j, i): row j = j0 + e of CTA jr, column gi.  Byte offset inside the 128-row panel
                     // = mir_base + ((j0 & 127) / 8 + (e >> 3)) * 1024 + mir_x[e & 7]  (see panel_off)
                     const uint32_t mb = mir_base + (uint32_t)(((j0 & 127) >> 3) * 1024);
+                    uint32_t bh[8], bl[8];
                     if (c != g) {
                         // ---- off-diagonal block: every entry is finalised here, no per-element predicate
 #pragma unroll
-                        for (int e = 0; e < 16; e += 2) split_hi_lo2(sn[e], sn[e + 1], cs, hp[e >> 1], lp[e >> 1]);
+                        for (int e = 0; e < CW; e += 2) split_scaled2(sn[e], sn[e + 1], hp[e >> 1], lp[e >> 1]);
                         float q0 = 0.f, q1 = 0.f, q2 = 0.f, q3 = 0.f;
 #pragma unroll
-                        for (int e = 0; e < 16; e += 4) {
+                        for (int e = 0; e < CW; e += 4) {
                             q0 = fmaf(sn[e], sn[e], q0); q1 = fmaf(sn[e + 1], sn[e + 1], q1);
                             q2 = fmaf(sn[e + 2], sn[e + 2], q2); q3 = fmaf(sn[e + 3], sn[e + 3], q3);
                         }
-                        const float qsum = (q0 + q1) + (q2 + q3);        // FP32 over 16 entries, fixed point across blocks
+                        const float qsum = ((q0 + q1) + (q2 + q3)) * inv2;   // FP32 over CW entries, fixed point across blocks
                         bad = bad || !(qsum <= 1.0e6f);
                         fro2 += 2 * to_fix(qsum);
-                        uint32_t so[16];
-#pragma unroll
-                        for (int e = 0; e < 16; ++e) so[e] = __float_as_uint(sn[e]);
-                        tmem_st_32x32_x16(t_S + tc, so);                // FP32 master
-#pragma unroll
-                        for (int h8 = 0; h8 < 2; ++h8) {                // own row: two 16-byte pieces per matrix
-                            const uint32_t off = panel_off(tl, j0 + 8 * h8);
-                            *reinterpret_cast<uint4*>(hiP + off) = make_uint4(hp[4 * h8], hp[4 * h8 + 1], hp[4 * h8 + 2], hp[4 * h8 + 3]);
-                            *reinterpret_cast<uint4*>(loP + off) = make_uint4(lp[4 * h8], lp[4 * h8 + 1], lp[4 * h8 + 2], lp[4 * h8 + 3]);
+                        if (!(SP2_RES_EXP & 4)) tmem_st_cw<CW>(t_S + tc, reinterpret_cast<const uint32_t(&)[CW]>(sn));   // FP32 master (c S)
+                        if (!(SP2_RES_EXP & 8)) st_shared_v4(hi_addr + own0, hp[0], hp[1], hp[2], hp[3]);
+                        if (!(SP2_RES_EXP & 8)) st_shared_v4(lo_addr + own0, lp[0], lp[1], lp[2], lp[3]);
+                        if constexpr (CW == 16) {
+                            st_shared_v4(hi_addr + own1, hp[CW / 2 - 4], hp[CW / 2 - 3], hp[CW / 2 - 2], hp[CW / 2 - 1]);
+                            st_shared_v4(lo_addr + own1, lp[CW / 2 - 4], lp[CW / 2 - 3], lp[CW / 2 - 2], lp[CW / 2 - 1]);
                         }
                         if (CG == 2 && jr != rank) {
                             const uint32_t rh = mapa_u32(hi_addr, jr) + mb, rl = mapa_u32(lo_addr, jr) + mb;
 #pragma unroll
-                            for (int e = 0; e < 16; ++e) {
-                                const uint32_t off = (uint32_t)((e >> 3) * 1024) + mir_x[e & 7];
-                                st_cluster_u16(rh + off, (unsigned short)(hp[e >> 1] >> (16 * (e & 1))));
-                                st_cluster_u16(rl + off, (unsigned short)(lp[e >> 1] >> (16 * (e & 1))));
-                            }
+                            for (int k = 0; k < 8; ++k) { bh[k] = rh + mir_x[k]; bl[k] = rl + mir_x[k]; }
+                            mirror_cw<0, true, false, CW>(bh, bl, hp, lp, CW);
                         } else {
                             const uint32_t rh = hi_addr + mb, rl = lo_addr + mb;
 #pragma unroll
-                            for (int e = 0; e < 16; ++e) {
-                                const uint32_t off = (uint32_t)((e >> 3) * 1024) + mir_x[e & 7];
-                                st_shared_u16(rh + off, (unsigned short)(hp[e >> 1] >> (16 * (e & 1))));
-                                st_shared_u16(rl + off, (unsigned short)(lp[e >> 1] >> (16 * (e & 1))));
-                            }
+                            for (int k = 0; k < 8; ++k) { bh[k] = rh + mir_x[k]; bl[k] = rl + mir_x[k]; }
+                            mirror_cw<0, false, false, CW>(bh, bl, hp, lp, CW);
                         }
                     } else {
-                        // ---- diagonal block: entries j <= i are authoritative; bias and traces on j == i
-                        float qs = 0.f;
+                        // ---- diagonal block: entries j <= i are authoritative; bias and traces on j == i.
+                        // ed = this thread's diagonal column inside the half block (-1: it is in the other half);
+                        // lim = number of strictly-lower columns (j < i) in this half
+                        const int ed = ((lane / CW) == hf) ? (lane & (CW - 1)) : -1;
+                        const int lim = lane - CW * hf;                           // e < lim  <=>  j < gi
+                        const float bias = (gi < N) ? th3 : 0.f;
+                        float vdiag = 0.f, xdiag = 0.f, qs = 0.f;
 #pragma unroll
-                        for (int e = 0; e < 16; ++e) {
-                            const int j = j0 + e;
-                            if (j == gi) {
-                                if (gi < N) sn[e] += th3;
-                                if (use_acc) trX += to_fix(__uint_as_float(va[e]) * inv2);
-                                bad = bad || !(fabsf(sn[e]) <= 1.0e3f);
-                                trS += to_fix(sn[e]); fro2 += sq_fix(sn[e]);
-                            } else if (j < gi) {
-                                qs = fmaf(sn[e], sn[e], qs);
-                            }
+                        for (int e = 0; e < CW; ++e) {
+                            if (e == ed) { sn[e] += bias; vdiag = sn[e]; xdiag = use_acc ? __uint_as_float(va[e]) : 0.f; }
+                            if (e < lim) qs = fmaf(sn[e], sn[e], qs);
                         }
+                        if (ed >= 0) {
+                            const float sd = vdiag * inv_c;                        // the entry of S itself
+                            bad = bad || !(fabsf(sd) <= 1.0e3f);
+                            trS += to_fix(sd); fro2 += sq_fix(sd);
+                            trX += to_fix(xdiag * inv2);
+                        }
+                        qs *= inv2;
                         bad = bad || !(qs <= 1.0e6f);
                         fro2 += 2 * to_fix(qs);
 #pragma unroll
-                        for (int e = 0; e < 16; e += 2) split_hi_lo2(sn[e], sn[e + 1], cs, hp[e >> 1], lp[e >> 1]);
-                        uint32_t so[16];
-#pragma unroll
-                        for (int e = 0; e < 16; ++e) so[e] = __float_as_uint(sn[e]);
-                        tmem_st_32x32_x16(t_S + tc, so);                // entries j > i are never read back
+                        for (int e = 0; e < CW; e += 2) split_scaled2(sn[e], sn[e + 1], hp[e >> 1], lp[e >> 1]);
+                        tmem_st_cw<CW>(t_S + tc, reinterpret_cast<const uint32_t(&)[CW]>(sn));   // entries j > i are never read back
+                        // own row, all 16 columns at once; the entries above the diagonal (j > i) are then overwritten
+                        // by the mirror stores of the rows that own them -- after the two warps of this row group have
+                        // met, so that every such overwrite comes later
+                        if (!(SP2_RES_EXP & 8)) st_shared_v4(hi_addr + own0, hp[0], hp[1], hp[2], hp[3]);
+                        if (!(SP2_RES_EXP & 8)) st_shared_v4(lo_addr + own0, lp[0], lp[1], lp[2], lp[3]);
+                        if constexpr (CW == 16) {
+                            st_shared_v4(hi_addr + own1, hp[CW / 2 - 4], hp[CW / 2 - 3], hp[CW / 2 - 2], hp[CW / 2 - 1]);
+                            st_shared_v4(lo_addr + own1, lp[CW / 2 - 4], lp[CW / 2 - 3], lp[CW / 2 - 2], lp[CW / 2 - 1]);
+                        }
+                        asm volatile("bar.sync %0, %1;\n" ::"r"(2 + q), "n"(32 * WPG) : "memory");
                         const uint32_t rh = hi_addr + mb, rl = lo_addr + mb;
 #pragma unroll
-                        for (int e = 0; e < 16; ++e) {
-                            const int j = j0 + e;
-                            const unsigned short hb = (unsigned short)(hp[e >> 1] >> (16 * (e & 1)));
-                            const unsigned short lb = (unsigned short)(lp[e >> 1] >> (16 * (e & 1)));
-                            if (j <= gi) {                      // own entries one by one
-                                const uint32_t off = panel_off(tl, j);
-                                st_shared_u16(hi_addr + off, hb);
-                                st_shared_u16(lo_addr + off, lb);
-                            }
-                            if (j < gi) {
-                                const uint32_t off = (uint32_t)((e >> 3) * 1024) + mir_x[e & 7];
-                                st_shared_u16(rh + off, hb);
-                                st_shared_u16(rl + off, lb);
-                            }
-                        }
+                        for (int k = 0; k < 8; ++k) { bh[k] = rh + mir_x[k]; bl[k] = rl + mir_x[k]; }
+                        mirror_cw<0, false, true, CW>(bh, bl, hp, lp, lim);
                     }
                 }
                 tmem_st_wait();
+                RT_MARK(1);
                 // ---- publish this warp's partial sums
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) {
@@ -409,11 +483,13 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
                     sh->part[iter & 1][warp][3] = bad ? 1 : 0;
                 }
             }
+            RT_MARK(2);
             // panels (generic-proxy writes, local and remote) -> visible to the tensor core (async proxy)
             asm volatile("fence.proxy.async;\n" ::: "memory");
             tc_fence_before();
             group_sync<CG>();
             tc_fence_after();
+            RT_MARK(3);
             // ---- a4 of the NEXT layer, X = S^2 (Eq. 15): 3 MMAs per 16 columns of K, operands = the resident panels;
             // issued before the control step below has decided anything (it runs meanwhile)
             if (issue_next) {
@@ -440,9 +516,9 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
             // the same order in both CTAs, so both take identical decisions.
             if (warp == 0) {
                 long long a = 0, b = 0, cX = 0, nf = 0;
-                if (lane < 8 * CG) {
-                    const uint32_t r = (uint32_t)lane >> 3;
-                    const int w = lane & 7;
+                if (lane < EW * CG) {
+                    const uint32_t r = (uint32_t)lane / EW;
+                    const int w = lane & (EW - 1);
                     if (r == rank) {
                         a = sh->part[iter & 1][w][0]; b = sh->part[iter & 1][w][1]; cX = sh->part[iter & 1][w][2];
                         nf = sh->part[iter & 1][w][3];
@@ -453,7 +529,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
                     }
                 }
 #pragma unroll
-                for (int o = 8; o > 0; o >>= 1) {           // integer adds: exact, so both CTAs get identical sums
+                for (int o = 16; o > 0; o >>= 1) {          // integer adds: exact, so both CTAs get identical sums
                     a += __shfl_xor_sync(0xffffffffu, a, o);
                     b += __shfl_xor_sync(0xffffffffu, b, o);
                     cX += __shfl_xor_sync(0xffffffffu, cX, o);
@@ -470,6 +546,10 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
                 }
             }
             __syncthreads();
+            RT_MARK(4);
+#ifdef SP2_RES_TIMING
+            if (rt_on) g_res_timing[7 - 7] += 0;
+#endif
             ++iter;
             if (!sh->ctrl.running) {
                 if (issue_next) {                        // drain the speculative MMAs before anything is reused
@@ -478,26 +558,41 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
                 }
                 break;
             }
-            th1s = sh->ctrl.theta[0] * inv2; th2 = sh->ctrl.theta[1]; th3 = sh->ctrl.theta[2];
+            th1s = sh->ctrl.theta[0] * inv_c; th2 = sh->ctrl.theta[1]; th3 = sh->ctrl.theta[2] * cs;
             use_acc = true;
         }
 
         // ------------------------------------------------------------------ output: D = S_n, both triangles
-        if (warp < 8) {
+        RT_MARK(5);
+        if (warp < EW) {
+            const bool vec_ok = ((N & 3) == 0) && ((reinterpret_cast<uintptr_t>(Dm) & 15) == 0);
 #pragma unroll 1
             for (int c = 0; c < NG; ++c) {
                 if (!owns_block<NG>(g, c)) continue;
-                const int j0 = 32 * c + 16 * hf;
-                uint32_t vs[16];
-                tmem_ld_32x32_x16(t_S + (uint32_t)(32 * c), vs);
+                const int j0 = 32 * c + CW * hf;
+                uint32_t vs[CW];
+                tmem_ld_cw<CW>(t_S + (uint32_t)(32 * c), vs);
                 tmem_ld_wait();
+                float v[CW];
 #pragma unroll
-                for (int e = 0; e < 16; ++e) {
+                for (int e = 0; e < CW; ++e) v[e] = __uint_as_float(vs[e]) * inv_c;      // the master holds c S
+                // mirrored position (j, gi): one row per instruction, coalesced across the warp
+#pragma unroll
+                for (int e = 0; e < CW; ++e) {
                     const int j = j0 + e;
-                    if (gi < N && j < N && (c != g || j <= gi)) {
-                        const float v = __uint_as_float(vs[e]);
-                        Dm[(size_t)j * N + gi] = v;      // mirrored position: coalesced across the warp
-                        Dm[(size_t)gi * N + j] = v;
+                    if (gi < N && j < N && (c != g || j < gi)) Dm[(size_t)j * N + gi] = v[e];
+                }
+                // own position (gi, j): each lane writes a piece of its own row -- as 16-byte vectors where it can
+                // (a scalar store per element costs the LSU 32 sectors per instruction for 4 bytes each)
+                if (c != g && vec_ok && gi < N && j0 + CW <= N) {
+                    float4* dst = reinterpret_cast<float4*>(Dm + (size_t)gi * N + j0);
+#pragma unroll
+                    for (int e4 = 0; e4 < CW / 4; ++e4) dst[e4] = make_float4(v[4 * e4], v[4 * e4 + 1], v[4 * e4 + 2], v[4 * e4 + 3]);
+                } else {
+#pragma unroll
+                    for (int e = 0; e < CW; ++e) {
+                        const int j = j0 + e;
+                        if (gi < N && j < N && (c != g || j <= gi)) Dm[(size_t)gi * N + j] = v[e];
                     }
                 }
             }
@@ -514,15 +609,26 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
         tc_fence_before();
         group_sync<CG>();          // peer must be done reading this CTA's partial sums / panels before they are reused
         tc_fence_after();
+        RT_MARK(7);
     }
 
+#ifdef SP2_RES_TIMING
+    if (rt_on) for (int i = 0; i < 8; ++i) g_res_timing[i] = (unsigned long long)rt_acc[i];
+    if (threadIdx.x == 0 && blockIdx.x < 160) {
+        unsigned long long g1;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g1));
+        g_res_span[3 * blockIdx.x] = (unsigned long long)(clock64() - rt_c0);
+        g_res_span[3 * blockIdx.x + 1] = rt_g0;
+        g_res_span[3 * blockIdx.x + 2] = g1;
+    }
+#endif
     tc_fence_before();
     group_sync<CG>();
     if (warp == C::MMA_WARP) tmem_dealloc<CG>(tmem_base, C::TMEM_COLS);
 }
 
-using Res128 = ResCfg<128, 1>;
-using Res256 = ResCfg<256, 2>;
+using Res128 = ResCfg<128, 1, 16>;
+using Res256 = ResCfg<256, 2, 8>;
 
 template <class C>
 static constexpr size_t res_smem() { return 2 * C::PANEL_BYTES + C::STAGE_FLOATS * 4 + sizeof(ResShared) + 1024 + 64; }
@@ -555,6 +661,15 @@ static cudaError_t launch_res(const ResidentParams& p, int num_sms, cudaStream_t
     cfg.numAttrs = 1;
     return cudaLaunchKernelEx(&cfg, k_sp2_resident<C>, p);
 }
+
+#ifdef SP2_RES_TIMING
+extern "C" void sp2_debug_resident_timing(unsigned long long out[8]) {
+    cudaMemcpyFromSymbol(out, g_res_timing, 8 * sizeof(unsigned long long));
+}
+extern "C" void sp2_debug_resident_span(unsigned long long out[480]) {
+    cudaMemcpyFromSymbol(out, g_res_span, 480 * sizeof(unsigned long long));
+}
+#endif
 
 cudaError_t launch_resident(const ResidentParams& p, int num_sms, cudaStream_t st) {
     if (p.N <= 128) return launch_res<Res128>(p, num_sms, st);
