@@ -33,6 +33,10 @@ can be checked against PAPER.md by eye (P:n = /root/reference/PAPER.md line n):
                            alternating signs; which of the two forms applies follows reading C15 of
                            DESIGN.md (continue the alternation from the last applied sign).
   energy_ref               alpha = Tr[D H] (the observable of Fig. 2), plain FP64.
+  truncate_blocks,         the blocked-sparse variant the paper suggests for matrices with decay ("further performance
+  sp2_blocked_ref          increases might also be gained by considering a sparse matrix implementation"): Alg. 1
+                           in which, before every square, the off-diagonal b x b blocks of S whose Frobenius norm is
+                           <= tau are set to zero (reading C28).  tau = 0 is sp2_ref exactly.
   sp2_mixed_ref            Alg. 1 with Alg. 2 as the activation, emulated: FP16 hi/lo split,
                            Eq. 15 products, FP32 rounding of X_n and S_n.  An EMULATION of the arithmetic
                            (FP64 accumulation instead of the tensor core's FP32), used only to size
@@ -401,6 +405,74 @@ def sp2_accelerated_ref(H32, N_occ, bounds, homo, lumo, tol=0.0, max_layers=120,
         elif tol > 0.0 and iderr <= tol:
             stop = STOP_TOL
         elif n >= max_layers:
+            stop = STOP_MAX_LAYERS
+    st["stop_reason"], st["n_layers"], st["bounds"] = stop, n, (eps_min, eps_max)
+    return S, st
+
+
+def truncate_blocks(S, tau, block=128):
+    """Reading C28 (P:206 names no rule): cut S into block x block blocks on a fixed grid; an OFF-DIAGONAL block whose
+    Frobenius norm is <= tau is set to zero (with its mirror image, so S stays symmetric); diagonal blocks are always
+    kept (they carry the trace).  Returns (S_truncated, kept) with kept[I, J] = 1 for blocks that survive."""
+    S = np.array(S, dtype=np.float64)
+    n = S.shape[0]
+    nb = (n + block - 1) // block
+    kept = np.ones((nb, nb), dtype=np.int8)
+    if tau <= 0.0:
+        return S, kept
+    for I in range(nb):
+        for J in range(I):
+            blk = S[I * block:(I + 1) * block, J * block:(J + 1) * block]
+            if np.sqrt(np.sum(blk * blk)) <= tau:
+                S[I * block:(I + 1) * block, J * block:(J + 1) * block] = 0.0
+                S[J * block:(J + 1) * block, I * block:(I + 1) * block] = 0.0
+                kept[I, J] = kept[J, I] = 0
+    return S, kept
+
+
+def sp2_blocked_ref(H32, N_occ, bounds=None, tau=0.0, block=128, tol=0.0, max_layers=120, eps_alt=0.0,
+                    forced_sigma=None):
+    """Alg. 1 on block-truncated iterates (reading C28).  Layer n:
+         S' = truncate_blocks(S_{n-1}, tau);  X_n = S' S';  N_X = Tr X_n;  IdErr_n = N_S - N_X with N_S = Tr S'
+         (= Tr S_{n-1}: diagonal blocks are never cut);  sigma_n by Alg. 1's rule;  S_n = sigma_n X_n + (1 - sigma_n) S'.
+    Same stop tests and outputs as sp2_ref, plus st["kept_fraction"][n-1] = surviving fraction of the b x b blocks and
+    st["work_fraction"][n-1] = fraction of the block products S'_IK S'_KJ (I >= J) whose two factors both survive --
+    the tensor-core work a blocked implementation has left."""
+    H = symmetrize_lower(H32)
+    eps_min, eps_max = gershgorin_bounds(H) if bounds is None else (float(bounds[0]), float(bounds[1]))
+    if not (eps_max > eps_min):
+        raise ValueError("degenerate spectral bounds")
+    S = initial_layer(H, eps_min, eps_max)
+    N_S = float(np.trace(S))
+    sigma_hist, iderr_hist = [0], [None]
+    st = {"trace_S": [], "trace_X": [], "iderr": [], "sigma": [], "margin": [], "kept_fraction": [],
+          "work_fraction": []}
+    n, stop = 0, STOP_NONE
+    while stop == STOP_NONE:
+        n += 1
+        Sp, kept = truncate_blocks(S, tau, block)
+        X = Sp @ Sp
+        N_X = float(np.trace(X))
+        iderr = N_S - N_X
+        sigma, d = _sign_rule(N_S, N_X, N_occ, sigma_hist[n - 1], eps_alt)
+        if forced_sigma is not None:
+            sigma = int(forced_sigma[n - 1])
+        S = sigma * X + (1 - sigma) * Sp
+        N_S = sigma * N_X + (1 - sigma) * N_S
+        sigma_hist.append(sigma); iderr_hist.append(iderr)
+        st["trace_S"].append(N_S); st["trace_X"].append(N_X); st["iderr"].append(iderr)
+        st["sigma"].append(sigma); st["margin"].append(d)
+        k = kept.astype(np.float64)
+        st["kept_fraction"].append(float(k.mean()))
+        pairs = np.tril(k @ k)                       # pairs[I, J] = number of K with both factors kept
+        st["work_fraction"].append(float(pairs.sum() / (kept.shape[0] * np.tril(np.ones_like(k)).sum())))
+        if iderr <= 0.0:
+            stop = STOP_IDERR_NONPOS
+        elif n > 2 and sigma_hist[n - 1] != sigma_hist[n - 2] and iderr > 4.5 * iderr_hist[n - 2] ** 2:
+            stop = STOP_PARAM_FREE
+        elif tol > 0.0 and iderr <= tol:
+            stop = STOP_TOL
+        elif n >= max_layers or (forced_sigma is not None and n >= len(forced_sigma)):
             stop = STOP_MAX_LAYERS
     st["stop_reason"], st["n_layers"], st["bounds"] = stop, n, (eps_min, eps_max)
     return S, st

@@ -75,8 +75,8 @@ struct CtrlCore {
     unsigned int pad_rs_;
 };
 struct Ctrl : CtrlCore {
-    double partial[kMaxPartials][4]; // HBM kernels (bounds, initial layer, observables): per-CTA FP64 partial sums
-    fx_t ipartial[kMaxPartials][4];  // layer kernel: per-CTA {Tr S, ||S||_F^2, Tr X (diag), non-finite flag}
+    alignas(32) double partial[kMaxPartials][4]; // HBM kernels (bounds, initial layer, observables): per-CTA FP64 partial sums
+    alignas(32) fx_t ipartial[kMaxPartials][4];  // layer kernel: per-CTA {Tr S, ||S||_F^2, Tr X (diag), non-finite flag}
 };
 
 // The statistics travel as raw fixed-point integers in the double-typed fields; the host converts them.

@@ -43,6 +43,15 @@ struct TileCfg {
     static constexpr int THREADS = 192;
 };
 
+#ifdef SP2_LAYER_TIMING
+// experiment builds only: per CTA {globaltimer at entry, after setup, first accumulator ready, last epilogue done, exit}
+__device__ unsigned long long g_layer_timing[160 * 8];
+extern "C" void sp2_debug_layer_timing(unsigned long long* out) { cudaMemcpyFromSymbol(out, g_layer_timing, 160 * 8 * 8); }
+#define LT_MARK(i) do { if (blockIdx.x < 160) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); g_layer_timing[blockIdx.x * 8 + (i)] = t_; } } while (0)
+#else
+#define LT_MARK(i) do { } while (0)
+#endif
+
 template <class C>
 __global__ void __launch_bounds__(C::THREADS, 1)
 k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ CUtensorMap tm_lo,
@@ -56,6 +65,7 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
         return;
     }
 
+    if (threadIdx.x == 64) LT_MARK(0);
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + STAGES * C::STAGE_BYTES);
@@ -98,6 +108,7 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
     if (CG == 2) cluster_sync_all(); else __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *((volatile uint32_t*)tmem_slot);
+    if (threadIdx.x == 64) LT_MARK(1);
 
     if (warp == 0) {
         // =============================== TMA producer (one elected lane)
@@ -300,6 +311,7 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
             const uint32_t use = (uint32_t)(it >> 1);
             mbar_wait(&tfull_bar[buf], use & 1u);
             tc_fence_after();
+            if (threadIdx.x == 64 && w == slot) LT_MARK(2);
             const uint32_t taddr = tmem_base + (uint32_t)(buf * BN) + lane_off;
             unsigned short* HOu = reinterpret_cast<unsigned short*>(HO);
             unsigned short* LOu = reinterpret_cast<unsigned short*>(LO);
@@ -467,6 +479,7 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                 if (CG == 1) mbar_arrive(&tempty_bar[buf]); else mbar_arrive_cluster(&tempty_bar[buf], 0);
             }
         }
+        if (threadIdx.x == 64) LT_MARK(3);
         // ---- block partials -> ctrl -> last CTA runs the control step (integer adds: exact, any order)
         fx_t fro2 = 2 * off2 + dg2;
         for (int o = 16; o > 0; o >>= 1) {
@@ -494,11 +507,22 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                 // last CTA: sum the per-CTA partials and run the control step of Alg. 1
                 __threadfence();
                 fx_t a = 0, b = 0, c = 0, f = 0;
-                for (unsigned int i = lane; i < gridDim.x; i += 32) {
-                    a += ((volatile fx_t*)ctrl->ipartial[i])[0];
-                    b += ((volatile fx_t*)ctrl->ipartial[i])[1];
-                    c += ((volatile fx_t*)ctrl->ipartial[i])[2];
-                    f += ((volatile fx_t*)ctrl->ipartial[i])[3];
+                // L2 loads (the partials were written by other SMs), 32-byte vectors, all of a lane's loads in flight
+                // before the first add
+                for (unsigned int i0 = lane; i0 < gridDim.x; i0 += 128) {
+                    longlong4 v[4];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const unsigned int i = i0 + 32u * u;
+                        v[u] = make_longlong4(0, 0, 0, 0);
+                        if (i < gridDim.x) {
+                            const longlong2 lo = __ldcg(reinterpret_cast<const longlong2*>(ctrl->ipartial[i]));
+                            const longlong2 hi = __ldcg(reinterpret_cast<const longlong2*>(ctrl->ipartial[i]) + 1);
+                            v[u] = make_longlong4(lo.x, lo.y, hi.x, hi.y);
+                        }
+                    }
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) { a += v[u].x; b += v[u].y; c += v[u].z; f += v[u].w; }
                 }
                 for (int o = 16; o > 0; o >>= 1) {
                     a += __shfl_xor_sync(0xffffffffu, a, o);
@@ -519,6 +543,7 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
     tc_fence_before();
     if (CG == 2) cluster_sync_all(); else __syncthreads();
     if (warp == 1) tmem_dealloc<CG>(tmem_base, C::TMEM_COLS);
+    if (threadIdx.x == 64) LT_MARK(4);
 }
 
 using Cfg128 = TileCfg<128, 1>;

@@ -176,3 +176,22 @@ def uniform_symmetric(seed: int, n: int) -> np.ndarray:
     rng = np.random.default_rng(seed)
     A = rng.uniform(-1.0, 1.0, (n, n))
     return _sym32(np.triu(A) + np.triu(A, 1).T)
+
+
+def decaying_chain(seed: int = 0, n: int = 2048, gap: float = 1.0, decay: float = 3.0, cutoff: int = 24) -> Workload:
+    """A Hamiltonian WITH DECAY, the case the paper's sparse-matrix remark is about: a one-
+    dimensional chain of n orbitals with alternating onsite energies -gap/2, +gap/2 and hoppings
+    H_ij = -0.25 exp(-|i - j| / decay) N(1, 0.1) for 0 < |i - j| <= cutoff.  The staggered onsite term keeps a gap
+    open at half filling, so the density matrix decays exponentially away from the diagonal and its far
+    off-diagonal blocks are numerically zero.  N_occ = n / 2; no spectrum is known in closed form (the tests use
+    LAPACK for the reference projector)."""
+    rng = np.random.default_rng(seed)
+    H = np.zeros((n, n))
+    idx = np.arange(n)
+    H[idx, idx] = np.where(idx % 2 == 0, -0.5 * gap, 0.5 * gap)
+    for d in range(1, cutoff + 1):
+        v = -0.25 * np.exp(-d / decay) * rng.normal(1.0, 0.1, n - d)
+        H[idx[:-d], idx[:-d] + d] = v
+        H[idx[:-d] + d, idx[:-d]] = v
+    return Workload(name=f"decaying_chain_N{n}", H32=_sym32(H), N=n, N_occ=float(n // 2), bounds=None, tol=1e-5,
+                    max_layers=120, extra={"seed": seed, "gap": gap, "decay": decay, "cutoff": cutoff})
