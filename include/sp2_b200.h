@@ -110,9 +110,11 @@ typedef struct {
                                core accumulates before the chunk sum is folded into the error-free FP32 pair
                                (DESIGN.md section 9).  <= 0: library default (2 = 128 values of K)       */
     double trunc_tau;       /* blocked-sparse variant for decaying matrices (DESIGN.md section 9 NEXT-4):
-                               > 0: before every square, 128 x 128 blocks of S with Frobenius norm <= trunc_tau are
-                               set to zero and their tensor-core work is skipped.  0 (default): dense.
-                               sp2_density_matrix with tile_config 0 or 1 only.                               */
+                               > 0: before every square, the off-diagonal 128 x 128 blocks of S with Frobenius norm
+                               <= trunc_tau count as zero (reading C28): their operand tiles are neither
+                               loaded nor multiplied, and N_X = ||S'||_F^2 leaves them out.  0 (default): dense.
+                               sp2_density_matrix / sp2_generalized(_wb) with tile_config 0 or 1, N <= 16384;
+                               exact_diag does not apply (the diagonal of X comes from the masked products).     */
 } sp2_opts_t;
 
 /* Fill *o with defaults: auto_bounds=1, tol=0, max_layers=120, eps_alt=0, fp16_scale_log2=-1, control=0,
@@ -230,6 +232,10 @@ int         sp2_last_launch_count(sp2_handle_t h);
 /* Device-side durations (CUDA events on `stream`) of the three phases of the last sp2_density_matrix_host call on
  * this handle, in ms: {host -> device copy of H, the solve, device -> host copy of D}. */
 void        sp2_last_host_timing(sp2_handle_t h, double ms[3]);
+/* Blocked-sparse variant (opts->trunc_tau > 0): out[0] = 128-wide block products the tensor cores executed during the
+ * last single-matrix solve on this handle, summed over tiles and layers; out[1] = what a dense solve of the same layers
+ * would have executed.  Both 0 after a dense solve. */
+void        sp2_last_sparse_work(sp2_handle_t h, double out[2]);
 /* Diagnostic: 1 if, during the last single-matrix solve on this handle, a round-synchronisation wait of the layer
  * kernel ran out and the kernel gave the synchronisation up (performance only: results are unaffected). */
 int         sp2_last_round_sync_broken(sp2_handle_t h);

@@ -21,7 +21,7 @@ EXPORTS = ["sp2_default_opts", "sp2_create", "sp2_destroy", "sp2_workspace_bytes
            "sp2_density_matrix", "sp2_density_matrix_host", "sp2_generalized", "sp2_generalized_mix", "sp2_generalized_wb",
            "sp2_density_matrix_batched", "sp2_generalized_batched", "sp2_refine_energy", "sp2_split_fp16",
            "sp2_gershgorin", "sp2_status_string", "sp2_last_cuda_error", "sp2_last_launch_count",
-           "sp2_last_host_timing", "sp2_last_round_sync_broken", "sp2_version"]
+           "sp2_last_host_timing", "sp2_last_round_sync_broken", "sp2_last_sparse_work", "sp2_version"]
 
 
 class LayerStat(C.Structure):
@@ -101,6 +101,7 @@ def load() -> C.CDLL:
     lib.sp2_last_launch_count.argtypes = [vp]; lib.sp2_last_launch_count.restype = C.c_int
     lib.sp2_last_round_sync_broken.argtypes = [vp]; lib.sp2_last_round_sync_broken.restype = C.c_int
     lib.sp2_last_host_timing.argtypes = [vp, dp]; lib.sp2_last_host_timing.restype = None
+    lib.sp2_last_sparse_work.argtypes = [vp, dp]; lib.sp2_last_sparse_work.restype = None
     lib.sp2_version.argtypes = []; lib.sp2_version.restype = C.c_char_p
     _lib = lib
     return lib
@@ -184,6 +185,10 @@ class Handle:
         info.update(status=st, n_layers=nl.value, bounds=(bounds[0], bounds[1]),
                     stop_reason=(info["stop_reason"][-1] if nl.value else 0),
                     launches=self.lib.sp2_last_launch_count(self._h))
+        if opts.trunc_tau > 0.0:
+            wk = (C.c_double * 2)()
+            self.lib.sp2_last_sparse_work(self._h, wk)
+            info["work_fraction"] = (wk[0] / wk[1]) if wk[1] > 0 else 1.0
         return D, info
 
     def density_matrix_host(self, H_host: np.ndarray, N_occ, opts: Optional[Opts] = None, out=None, stream=None):

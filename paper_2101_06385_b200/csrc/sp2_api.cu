@@ -77,11 +77,13 @@ struct sp2_handle_s {
     cudaEvent_t host_ev[4] = {nullptr, nullptr, nullptr, nullptr};   // H2D start, solve start, D2H start, end
     float host_ms[3] = {0.f, 0.f, 0.f};
     PFN_encodeTiled encode = nullptr;
-    // (N, Np, cfg, scale_log2, exact_diag | mix << 1 | enh_kc << 2): everything a captured launch bakes in
+    // (N, Np, cfg, scale_log2, exact_diag | mix << 1 | sparse << 2 | enh_kc << 3): everything a captured launch bakes in
     std::map<std::tuple<int, int, int, int, int>, LoopGraph> graphs;
     int items_key_np[2] = {-1, -1}, items_key_cfg[2] = {-1, -1}, items_key_split[2] = {-1, -1};
     int n_items[2] = {0, 0}, n_slots[2] = {0, 0};
     float* mix = nullptr;           // output mix M = sum_i c_i S_i (Eq. 18), allocated on first use
+    unsigned long long* bn[2] = {nullptr, nullptr};   // blocked-sparse variant: squared block norms (ping-pong), on first use
+    double sparse_work[2] = {0.0, 0.0};               // K-blocks multiplied / a dense solve's, last sparse solve
     double* obs_dev = nullptr;      // [6] observables of sp2_refine_energy
     double* obs_host = nullptr;
     int tail_split = 1;
@@ -192,7 +194,7 @@ extern "C" sp2_status_t sp2_destroy(sp2_handle_t h) {
         for (int b = 0; b < 2; ++b) cudaFree(h->hl[a][b]);
     cudaFree(h->rowsq[0]); cudaFree(h->rowsq[1]);
     cudaFree(h->gpart); cudaFree(h->diag); cudaFree(h->ctrl); cudaFree(h->stats_dev); cudaFree(h->thetas_dev);
-    cudaFree(h->items_dev[0]); cudaFree(h->items_dev[1]); cudaFree(h->obs_dev); cudaFree(h->mix); cudaFreeHost(h->obs_host); cudaFree(h->bstats_dev); cudaFree(h->bnl_dev); cudaFree(h->bstatus_dev);
+    cudaFree(h->items_dev[0]); cudaFree(h->items_dev[1]); cudaFree(h->obs_dev); cudaFree(h->mix); cudaFree(h->bn[0]); cudaFree(h->bn[1]); cudaFreeHost(h->obs_host); cudaFree(h->bstats_dev); cudaFree(h->bnl_dev); cudaFree(h->bstatus_dev);
     cudaFree(h->bbounds_dev); cudaFree(h->bnocc_dev); cudaFree(h->bhl_dev);
     cudaFreeHost(h->ctrl_host); cudaFreeHost(h->stats_host); cudaFreeHost(h->thetas_host);
     cudaFreeHost(h->bounds_host); cudaFree(h->stage_H); cudaFree(h->stage_D);
@@ -361,7 +363,7 @@ static int choose_tile_config(int N, int requested, int num_sms) {
 }
 
 struct Problem {
-    int N, Np, cfg, scale_log2, n_items, n_slots, exact_diag, list, mix, enh_kc;
+    int N, Np, cfg, scale_log2, n_items, n_slots, exact_diag, list, mix, enh_kc, sparse;
     float scale, inv_scale2;
 };
 
@@ -371,6 +373,11 @@ static sp2_status_t prepare_problem(sp2_handle_s* h, int N, const sp2_opts_t* o,
     pb->cfg = forced_cfg ? forced_cfg : choose_tile_config(N, o ? o->tile_config : 0, h->num_sms);
     pb->list = (pb->cfg == TILE_128x128_ENH) ? 1 : 0;   // the enhanced-accumulation layers keep their own work list
     pb->mix = 0;
+    pb->sparse = (o && o->trunc_tau > 0.0) ? 1 : 0;
+    if (pb->sparse) {                                      // 128 x 128 tiles, no strips: a block = a tile
+        if (forced_cfg || (o->tile_config != TILE_AUTO && o->tile_config != TILE_128x128)) return SP2_ERR_INVALID_ARG;
+        pb->cfg = TILE_128x128;
+    }
     const int L = pb->list;
     const int edge = tile_super_edge(pb->cfg);
     pb->Np = round_up(N, edge);
@@ -380,21 +387,23 @@ static sp2_status_t prepare_problem(sp2_handle_s* h, int N, const sp2_opts_t* o,
     if (k > 14) return SP2_ERR_INVALID_ARG;
     pb->scale_log2 = k;
     pb->exact_diag = (o && o->exact_diag == 0) ? 0 : 1;
+    if (pb->sparse) pb->exact_diag = 0;      // the diagonal of X comes from the (masked) tensor-core products
     pb->enh_kc = opt_enh_kc(o);
     pb->scale = ldexpf(1.0f, k);
     pb->inv_scale2 = ldexpf(1.0f, -2 * k);
     const int nt = pb->Np / edge;
     const int band = (pb->cfg == TILE_256x256_PAIR) ? 8 : 12;
-    if (h->items_key_np[L] != pb->Np || h->items_key_cfg[L] != pb->cfg || h->items_key_split[L] != h->tail_split) {
+    const int split = pb->sparse ? 0 : h->tail_split;
+    if (h->items_key_np[L] != pb->Np || h->items_key_cfg[L] != pb->cfg || h->items_key_split[L] != split) {
         std::vector<WorkItem> list;
         int slots = 0;
-        build_work_list(nt, band, edge, tile_subs(pb->cfg), tile_cta_group(pb->cfg), h->num_sms, h->tail_split, list,
+        build_work_list(nt, band, edge, tile_subs(pb->cfg), tile_cta_group(pb->cfg), h->num_sms, split, list,
                         &slots);
         if ((int)list.size() > h->items_cap) return SP2_ERR_WORKSPACE;
         // synchronous small copy: happens only when the problem shape changes
         CK(cudaMemcpyAsync(h->items_dev[L], list.data(), list.size() * sizeof(WorkItem), cudaMemcpyHostToDevice, st));
         CK(cudaStreamSynchronize(st));
-        h->items_key_np[L] = pb->Np; h->items_key_cfg[L] = pb->cfg; h->items_key_split[L] = h->tail_split;
+        h->items_key_np[L] = pb->Np; h->items_key_cfg[L] = pb->cfg; h->items_key_split[L] = split;
         h->n_items[L] = (int)list.size();
         h->n_slots[L] = slots;
     }
@@ -412,6 +421,8 @@ static LayerParams layer_params(sp2_handle_s* h, const Problem& pb, int parity, 
     p.rowsq_next = pb.exact_diag ? h->rowsq[parity ^ 1] : nullptr;
     p.items = h->items_dev[pb.list]; p.ld = ws_ld_f32(pb.Np); p.ldf = ws_ld_f16(pb.Np); p.N = pb.N; p.Np = pb.Np;
     p.n_items = pb.n_items; p.n_slots = pb.n_slots;
+    p.bn_cur = pb.sparse ? h->bn[parity] : nullptr; p.bn_next = pb.sparse ? h->bn[parity ^ 1] : nullptr;
+    p.nb = pb.Np / 128;
     p.scale = pb.scale; p.inv_scale2 = pb.inv_scale2; p.cond_handle = cond; p.round_sync = h->round_sync; p.round_spins = h->round_spins; p.enh_kc = pb.enh_kc;
     return p;
 }
@@ -431,7 +442,7 @@ static sp2_status_t launch_one_layer(sp2_handle_s* h, const Problem& pb, int par
 // WHILE(ctrl->running) { layer(ping -> pong); layer(pong -> ping); } as a CUDA graph with a conditional node; the
 // condition is set on the device by the last CTA of each layer kernel (cudaGraphSetConditional).
 static sp2_status_t get_loop_graph(sp2_handle_s* h, const Problem& pb, LoopGraph** out) {
-    auto key = std::make_tuple(pb.N, pb.Np, pb.cfg, pb.scale_log2, pb.exact_diag | (pb.mix << 1) | (pb.enh_kc << 2));
+    auto key = std::make_tuple(pb.N, pb.Np, pb.cfg, pb.scale_log2, pb.exact_diag | (pb.mix << 1) | (pb.sparse << 2) | (pb.enh_kc << 3));
     auto it = h->graphs.find(key);
     if (it != h->graphs.end()) { *out = &it->second; return SP2_OK; }
     if (h->graphs.size() >= 16) {            // bounded cache: start over rather than grow without limit
@@ -498,6 +509,16 @@ static sp2_status_t solve_single(sp2_handle_s* h, const float* H_dev, int N, int
         if (pb.cfg == TILE_128x256 || pb.cfg == TILE_128x128_ENH) return SP2_ERR_INVALID_ARG;
         if (!h->mix) CK(cudaMalloc((void**)&h->mix, (size_t)h->Np_max * (size_t)ws_ld_f32(h->Np_max) * 4));
         pb.mix = 1;
+        if (pb.sparse) return SP2_ERR_INVALID_ARG;
+    }
+    const int nb = pb.Np / 128;
+    if (pb.sparse) {
+        if (nb > 128 || !isfinite(o->trunc_tau)) return SP2_ERR_INVALID_ARG;      // the K-block masks hold 128 bits
+        const size_t nbm = (size_t)(h->Np_max / 128);
+        for (int a = 0; a < 2; ++a)
+            if (!h->bn[a]) CK(cudaMalloc((void**)&h->bn[a], nbm * nbm * sizeof(unsigned long long)));
+        CK(cudaMemsetAsync(h->bn[0], 0, (size_t)nb * nb * sizeof(unsigned long long), st));
+        CK(cudaMemsetAsync(h->bn[1], 0, (size_t)nb * nb * sizeof(unsigned long long), st));
     }
     const int max_layers = o->max_layers;
     // ---- control block
@@ -507,6 +528,10 @@ static sp2_status_t solve_single(sp2_handle_s* h, const float* H_dev, int N, int
     c->eps_min = o->eps_min; c->eps_max = o->eps_max;
     c->N = N; c->mode = mode; c->max_layers = max_layers; c->auto_bounds = o->auto_bounds;
     c->kappa_q16 = opt_kappa_q16(*o);
+    if (pb.sparse) {
+        const double t2 = o->trunc_tau * o->trunc_tau * 281474976710656.0;     // 2^48
+        c->tau2_fx48 = t2 >= 9.0e18 ? 9000000000000000000ull : (unsigned long long)llrint(t2);
+    }
     c->accelerated = (mode == MODE_STANDARD && o->accelerated) ? 1 : 0;
     c->homo = o->homo; c->lumo = o->lumo;
     CK(cudaMemcpyAsync(h->ctrl, c, ctrl_header_bytes(), cudaMemcpyHostToDevice, st));
@@ -530,7 +555,7 @@ static sp2_status_t solve_single(sp2_handle_s* h, const float* H_dev, int N, int
     }
     CK(launch_affine_split(H_dev, N, ldh, h->S, h->hl[0][0], h->hl[0][1], (long long)ldS, (long long)ldF, pb.scale, h->ctrl, h->stats_dev,
                            h->thetas_dev, pb.exact_diag ? h->rowsq[0] : nullptr, pb.mix ? h->mix : nullptr, (float)c0,
-                           h->num_sms, st));
+                           pb.sparse ? h->bn[0] : nullptr, nb, h->num_sms, st));
     // ---- a4-a8: the layer loop
     if (o->control == 0) {
         LoopGraph* lg = nullptr;
@@ -563,6 +588,7 @@ static sp2_status_t solve_single(sp2_handle_s* h, const float* H_dev, int N, int
     CK(cudaGetLastError());
     c = h->ctrl_host;
     h->last_launches = c->launches + 1;      // + the copy-out kernel (k_copy_sym / k_one_minus)
+    h->sparse_work[0] = (double)c->work_active; h->sparse_work[1] = (double)c->work_dense;
     if (bounds_out) { bounds_out[0] = c->eps_min; bounds_out[1] = c->eps_max; }
     if (n_layers_out) *n_layers_out = c->n;
     if (stats_out) {
@@ -933,5 +959,9 @@ extern "C" int sp2_last_launch_count(sp2_handle_t h) { return h ? h->last_launch
 extern "C" void sp2_last_host_timing(sp2_handle_t h, double ms[3]) {
     if (!h || !ms) return;
     for (int i = 0; i < 3; ++i) ms[i] = (double)h->host_ms[i];
+}
+extern "C" void sp2_last_sparse_work(sp2_handle_t h, double out[2]) {
+    if (!h || !out) return;
+    out[0] = h->sparse_work[0]; out[1] = h->sparse_work[1];
 }
 extern "C" int sp2_last_round_sync_broken(sp2_handle_t h) { return (h && h->ctrl_host) ? (int)h->ctrl_host->round_sync_broken : 0; }

@@ -73,6 +73,10 @@ struct CtrlCore {
                                      // monotonic: layer n+1's targets start at n (n_rounds - 1) gridDim.x
     unsigned int round_sync_broken;  // a round wait timed out once (CTAs not co-resident): stop waiting in this solve
     unsigned int pad_rs_;
+    // blocked-sparse variant (reading C28)
+    unsigned long long tau2_fx48;    // tau^2 in 2^48 fixed point (block norms^2 are compared with it)
+    unsigned long long work_active;  // 128-wide K-blocks the MMA warps multiplied, summed over tiles and layers
+    unsigned long long work_dense;   // ... and how many a dense layer would have
 };
 struct Ctrl : CtrlCore {
     alignas(32) double partial[kMaxPartials][4]; // HBM kernels (bounds, initial layer, observables): per-CTA FP64 partial sums

@@ -200,8 +200,10 @@ __global__ void __launch_bounds__(256, 4) k_affine_split(const float* __restrict
                                                          __half* __restrict__ lo, long long ld, long long ldf,
                                                          float scale, Ctrl* ctrl, sp2_layer_stat_t* stats,
                                                          const float* thetas, unsigned long long* __restrict__ rowsq,
-                                                         float* __restrict__ mix, float c0) {
+                                                         float* __restrict__ mix, float c0,
+                                                         unsigned long long* __restrict__ bn, int nb) {
     __shared__ float ts[ET][ET + 1];
+    __shared__ float bsum[8];
     __shared__ float colacc[16][ET];
     __shared__ double red[8][2];
     const double e0 = ctrl->eps_min, e1 = ctrl->eps_max;
@@ -263,7 +265,17 @@ __global__ void __launch_bounds__(256, 4) k_affine_split(const float* __restrict
         }
         off2 += (double)offsq;
         *reinterpret_cast<float4*>(&colacc[r0][c4]) = make_float4(cs[0], cs[1], cs[2], cs[3]);
+        if (bn) {                                   // blocked-sparse variant: squared norms of the 128 x 128 blocks of S_0
+            const float wsum = warp_sum(offsq);
+            if ((threadIdx.x & 31) == 0) bsum[threadIdx.x >> 5] = wsum;
+        }
         __syncthreads();
+        if (bn && threadIdx.x == 0 && (I >> 1) != (J >> 1)) {
+            const float tsum = ((bsum[0] + bsum[1]) + (bsum[2] + bsum[3])) + ((bsum[4] + bsum[5]) + (bsum[6] + bsum[7]));
+            const unsigned long long v = (unsigned long long)__float2ll_rn(tsum * 281474976710656.0f);   // 2^48
+            atomicAdd(bn + (size_t)(I >> 1) * nb + (J >> 1), v);
+            atomicAdd(bn + (size_t)(J >> 1) * nb + (I >> 1), v);
+        }
         if (rowsq && threadIdx.x < ET) {            // column j of the tile = row j of the mirrored part (j < i only)
             float c = 0.f;
 #pragma unroll
@@ -529,13 +541,14 @@ cudaError_t launch_gershgorin(const float* H, int N, long long ldh, float* part,
 
 cudaError_t launch_affine_split(const float* H, int N, long long ldh, float* S, __half* hi, __half* lo, long long ld,
                                 long long ldf, float scale, Ctrl* ctrl, sp2_layer_stat_t* stats, const float* thetas,
-                                unsigned long long* rowsq, float* mix, float c0, int num_sms, cudaStream_t st) {
+                                unsigned long long* rowsq, float* mix, float c0, unsigned long long* bn, int nb,
+                                int num_sms, cudaStream_t st) {
     const int nt = (N + ET - 1) / ET;
     const long long ntiles = (long long)nt * (nt + 1) / 2;
     long long cap = (long long)num_sms * 4;
     if (cap > kMaxPartials) cap = kMaxPartials;
     const int grid = (int)(ntiles < cap ? ntiles : cap);
-    k_affine_split<<<grid, 256, 0, st>>>(H, N, ldh, S, hi, lo, ld, ldf, scale, ctrl, stats, thetas, rowsq, mix, c0);
+    k_affine_split<<<grid, 256, 0, st>>>(H, N, ldh, S, hi, lo, ld, ldf, scale, ctrl, stats, thetas, rowsq, mix, c0, bn, nb);
     return cudaGetLastError();
 }
 

@@ -16,7 +16,8 @@ cudaError_t launch_gershgorin(const float* H, int N, long long ldh, float* part,
 inline size_t gershgorin_part_floats(int N) { return 2 * (size_t)((N + 63) / 64) * (size_t)N; }
 cudaError_t launch_affine_split(const float* H, int N, long long ldh, float* S, __half* hi, __half* lo, long long ld,
                                 long long ldf, float scale, Ctrl* ctrl, sp2_layer_stat_t* stats, const float* thetas,
-                                unsigned long long* rowsq, float* mix, float c0, int num_sms, cudaStream_t st);
+                                unsigned long long* rowsq, float* mix, float c0, unsigned long long* bn, int nb,
+                                int num_sms, cudaStream_t st);
 cudaError_t launch_copy_sym(const float* S, long long ld, float* D, long long ldd, int N, int num_sms, cudaStream_t st);
 cudaError_t launch_one_minus(const float* M, long long ldm, float* F, long long ldo, int N, float d, int num_sms,
                              cudaStream_t st);
@@ -79,6 +80,11 @@ struct LayerParams {
     int round_sync;                // 1: producers of all CTAs meet at every round boundary (keeps the wave in lockstep)
     unsigned int round_spins;      // bound of that wait in 64 ns sleeps (a CTA that is not co-resident must not hang it)
     unsigned long long cond_handle;  // cudaGraphConditionalHandle (0 = none)
+    // blocked-sparse variant (reading C28): squared Frobenius norms of the 128 x 128 blocks of S_{n-1} (read)
+    // and of S_n (written), nb x nb each, 2^48 fixed point; nullptr = dense.  tau^2 lives in Ctrl.
+    const unsigned long long* bn_cur;
+    unsigned long long* bn_next;
+    int nb;
 };
 
 // Supertile edge for a tile configuration (128 or 256) and CTAs launched per supertile-slot.

@@ -19,8 +19,11 @@
 
 namespace sp2 {
 
-template <int BN_, int CG_, bool ENH_ = false, bool MIX_ = false>
+template <int BN_, int CG_, bool ENH_ = false, bool MIX_ = false, bool SP_ = false>
 struct TileCfg {
+    // SP: blocked-sparse variant for matrices with decay (reading C28): 128 x 128 blocks of S_{n-1}
+    // whose Frobenius norm is <= tau count as zero -- their K-blocks are neither loaded nor multiplied.
+    static constexpr bool SP = SP_;
     // MIX: the epilogue also accumulates the output mix M += c_n S_n (Eq. 18) in one more FP32 matrix.
     static constexpr bool MIX = MIX_;
     // ENH: enhanced accumulation ("single precision with double accumulation") for the refinement layers:
@@ -42,6 +45,28 @@ struct TileCfg {
     static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*align*/ + 256 /*barriers*/;
     static constexpr int THREADS = 192;
 };
+
+// Blocked-sparse variant: which 128-wide K-blocks of tile (I, J) survive the truncation?  Bit kk says that both
+// S'_{I,kk} and S'_{J,kk} are kept (diagonal blocks always are).  bn = squared block norms of S_{n-1} in 2^48 fixed
+// point, nb x nb, symmetric.  One ballot per 32 blocks (nb <= 128).
+__device__ __forceinline__ void sparse_kmask(const unsigned long long* __restrict__ bn, int nb, int I, int J,
+                                             unsigned long long tau2, int lane, uint32_t (&m)[4]) {
+#pragma unroll
+    for (int t = 0; t < 4; ++t) {
+        const int kk = 32 * t + lane;
+        bool act = false;
+        if (kk < nb) {
+            const bool a = (kk == I) || __ldcg(bn + (size_t)I * nb + kk) > tau2;
+            const bool b = (kk == J) || __ldcg(bn + (size_t)J * nb + kk) > tau2;
+            act = a && b;
+        }
+        m[t] = __ballot_sync(0xffffffffu, act);
+    }
+}
+__device__ __forceinline__ bool sparse_bit(const uint32_t (&m)[4], int kk) {
+    const uint32_t word = (kk < 32) ? m[0] : (kk < 64) ? m[1] : (kk < 96) ? m[2] : m[3];
+    return ((word >> (kk & 31)) & 1u) != 0u;
+}
 
 #ifdef SP2_LAYER_TIMING
 // experiment builds only: per CTA {globaltimer at entry, after setup, first accumulator ready, last epilogue done, exit}
@@ -75,6 +100,7 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
     uint64_t* tempty_bar = bars + 2 * STAGES + 2;    // [2]
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * STAGES + 4);
     __shared__ fx_t red[4][4];
+    __shared__ unsigned long long red48[2][4];       // SP: per-warp sums of squares of the tile in flight (2^48 fixed point)
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
@@ -110,7 +136,38 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
     const uint32_t tmem_base = *((volatile uint32_t*)tmem_slot);
     if (threadIdx.x == 64) LT_MARK(1);
 
-    if (warp == 0) {
+    if (warp == 0 && C::SP) {
+        // =============================== TMA producer, blocked-sparse: the whole warp finds the surviving K-blocks of a
+        // tile (ballots), one lane loads them
+        int s = 0;
+        uint32_t ph = 0;
+        const uint64_t pol = l2_policy_evict_last();
+        const unsigned long long tau2 = ctrl->tau2_fx48;
+        for (int w = slot; w < n_work; w += nslots) {
+            const WorkItem wi = p.items[w];
+            uint32_t m[4];
+            sparse_kmask(p.bn_cur, p.nb, wi.I, wi.J, tau2, lane, m);
+            if (lane == 0) {
+                const int m0 = wi.I * BN, n0 = wi.J * BN;
+                for (int kk = 0; kk < p.nb; ++kk) {
+                    if (!sparse_bit(m, kk)) continue;
+#pragma unroll 1
+                    for (int half = 0; half < 2; ++half) {
+                        mbar_wait(&empty_bar[s], ph ^ 1u);
+                        uint8_t* st = smem + s * C::STAGE_BYTES;
+                        const int k0 = kk * 128 + half * BK;
+                        mbar_arrive_expect_tx(&full_bar[s], C::STAGE_BYTES);
+                        tma_load_2d_hint(st, &tm_hi, &full_bar[s], k0, m0, pol);
+                        tma_load_2d_hint(st + C::A_BYTES, &tm_lo, &full_bar[s], k0, m0, pol);
+                        tma_load_2d_hint(st + 2 * C::A_BYTES, &tm_hi, &full_bar[s], k0, n0, pol);
+                        tma_load_2d_hint(st + 2 * C::A_BYTES + C::B_BYTES, &tm_lo, &full_bar[s], k0, n0, pol);
+                        if (++s == STAGES) { s = 0; ph ^= 1u; }
+                    }
+                }
+            }
+            __syncwarp();
+        }
+    } else if (warp == 0) {
         // =============================== TMA producer (one elected lane)
         if (lane == 0) {
             int s = 0;
@@ -180,6 +237,57 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
             }
         }
         __syncwarp();     // reconverge before the .aligned cluster barrier of the teardown
+    } else if (warp == 1 && C::SP) {
+        // =============================== MMA issuer, blocked-sparse: the same K-block list as the producer
+        int s = 0;
+        uint32_t ph = 0;
+        int it = 0;
+        const unsigned long long tau2 = ctrl->tau2_fx48;
+        constexpr uint32_t idesc = umma_idesc_f16(BM, BN);
+        for (int w = slot; w < n_work; w += nslots, ++it) {
+            const WorkItem wi = p.items[w];
+            uint32_t m[4];
+            sparse_kmask(p.bn_cur, p.nb, wi.I, wi.J, tau2, lane, m);
+            const int buf = it & 1;
+            mbar_wait(&tempty_bar[buf], ((uint32_t)(it >> 1) & 1u) ^ 1u);
+            tc_fence_after();
+            const uint32_t d_tmem = tmem_base + (uint32_t)(buf * BN);
+            bool fresh = true;                                  // the tile's first MMA overwrites the accumulator
+            for (int kk = 0; kk < p.nb; ++kk) {
+                if (!sparse_bit(m, kk)) continue;
+#pragma unroll 1
+                for (int half = 0; half < 2; ++half) {
+                    mbar_wait(&full_bar[s], ph);
+                    tc_fence_after();
+                    if (lane == 0) {
+                        const uint32_t a_hi = smem_u32(smem + s * C::STAGE_BYTES);
+                        const uint32_t a_lo = a_hi + C::A_BYTES;
+                        const uint32_t b_hi = a_hi + 2 * C::A_BYTES;
+                        const uint32_t b_lo = b_hi + C::B_BYTES;
+#pragma unroll
+                        for (int k = 0; k < BK / 16; ++k) {
+                            const uint64_t dah = umma_desc_sw128(a_hi + k * 32);
+                            const uint64_t dal = umma_desc_sw128(a_lo + k * 32);
+                            const uint64_t dbh = umma_desc_sw128(b_hi + k * 32);
+                            const uint64_t dbl = umma_desc_sw128(b_lo + k * 32);
+                            umma_f16<1>(d_tmem, dah, dbh, idesc, (fresh && k == 0) ? 0u : 1u);
+                            umma_f16<1>(d_tmem, dah, dbl, idesc, 1u);
+                            umma_f16<1>(d_tmem, dal, dbh, idesc, 1u);
+                        }
+                        umma_commit(&empty_bar[s]);
+                    }
+                    __syncwarp();
+                    fresh = false;
+                    if (++s == STAGES) { s = 0; ph ^= 1u; }
+                }
+            }
+            if (lane == 0) {
+                umma_commit(&tfull_bar[buf]);                   // also when nothing was issued: arrives at once
+                atomicAdd(&ctrl->work_active, (unsigned long long)(__popc(m[0]) + __popc(m[1]) + __popc(m[2]) + __popc(m[3])));
+                atomicAdd(&ctrl->work_dense, (unsigned long long)p.nb);
+            }
+            __syncwarp();
+        }
     } else if (warp == 1) {
         // =============================== MMA issuer (leader CTA only, one elected lane)
         if (rank == 0) {
@@ -261,6 +369,17 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
             const int m0 = wi.I * BN + (wi.sub * CG + (int)rank) * BM;
             const int n0 = wi.J * BN + wi.col0;
             const int ncols = wi.ncols;
+            // blocked-sparse: is the accumulator empty (no surviving K-block), and does S_{n-1}'s own block count as zero?
+            bool sp_empty = false, sp_zero_in = false;
+            const bool sp_offdiag = C::SP && (wi.I != wi.J);
+            fx_t tile40 = 0;                                 // the tile's sum of squares, as it goes into N_X if kept
+            unsigned long long tile48 = 0;                   // the same in 2^48 fixed point, for the comparison with tau^2
+            if (C::SP) {
+                uint32_t m[4];
+                sparse_kmask(p.bn_cur, p.nb, wi.I, wi.J, ctrl->tau2_fx48, lane, m);
+                sp_empty = ((m[0] | m[1] | m[2] | m[3]) == 0u);
+                if (sp_offdiag) sp_zero_in = !(__ldcg(p.bn_cur + (size_t)wi.I * p.nb + wi.J) > ctrl->tau2_fx48);
+            }
             const int gi = m0 + rl;
             const int gi_wmin = m0 + q * 32, gi_wmax = gi_wmin + 31;
             fx_t rowacc = 0;                                // sum_j S_n(gi, j)^2 over the own entries (j <= gi) of this tile
@@ -321,7 +440,12 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                 if (gj0 > gi_wmax) break;                   // rest of the row block lies above the diagonal
                 uint32_t v[32];
                 float so[32];
-                tmem_ld_32x32(taddr + (uint32_t)c0, v);
+                if (C::SP && sp_empty) {
+#pragma unroll
+                    for (int c = 0; c < 32; ++c) v[c] = 0u;
+                } else {
+                    tmem_ld_32x32(taddr + (uint32_t)c0, v);
+                }
                 if (C::ENH && nch > 1) {
                     // last chunk: total = running pair + this chunk, rounded once to FP32
                     uint32_t rh[32], rlo[32];
@@ -342,7 +466,10 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                 // diagonal chunk only the entries gj <= gi are used; the others (which a neighbouring lane rewrites
                 // further down) are not even loaded.
                 float mo[C::MIX ? 32 : 1];
-                if (below) {
+                if (C::SP && sp_zero_in) {
+#pragma unroll
+                    for (int c = 0; c < 32; ++c) so[c] = 0.f;
+                } else if (below) {
 #pragma unroll
                     for (int c = 0; c < 32; ++c) so[c] = __ldcs(S + (long long)(gj0 + c) * ld + gi);
                     if (C::MIX) {
@@ -409,7 +536,8 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                     const float sdf = (a0 + a1) + (a2 + a3);
                     bad = bad || !(sdf <= 1.0e6f);
                     const fx_t sd = fx_from_float(sdf);
-                    off2 += sd;
+                    if (sp_offdiag) { tile40 += sd; tile48 += (unsigned long long)__float2ll_rn(sdf * 281474976710656.0f); }
+                    else off2 += sd;
                     rowacc += sd;
                 } else {
                     // diagonal chunk: only gj <= gi is authoritative (exact symmetry inside the tile).  Exact diagonal
@@ -477,6 +605,20 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
             __syncwarp();
             if (lane == 0) {
                 if (CG == 1) mbar_arrive(&tempty_bar[buf]); else mbar_arrive_cluster(&tempty_bar[buf], 0);
+            }
+            if (sp_offdiag) {
+                // the block's squared Frobenius norm decides whether the NEXT layer sees it, and -- now -- whether it
+                // counts in N_X = ||S'_n||_F^2 (the oracle squares the truncated matrix)
+                for (int o = 16; o > 0; o >>= 1) tile48 += __shfl_xor_sync(0xffffffffu, tile48, o);
+                const int par = it & 1;
+                if (lane == 0) red48[par][q] = tile48;
+                asm volatile("bar.sync 1, 128;\n" ::: "memory");
+                const unsigned long long tot = (red48[par][0] + red48[par][1]) + (red48[par][2] + red48[par][3]);
+                if (tot > ctrl->tau2_fx48) off2 += tile40;
+                if (warp == 2 && lane == 0) {
+                    p.bn_next[(size_t)wi.I * p.nb + wi.J] = tot;
+                    p.bn_next[(size_t)wi.J * p.nb + wi.I] = tot;
+                }
             }
         }
         if (threadIdx.x == 64) LT_MARK(3);
@@ -552,6 +694,7 @@ using Cfg256P = TileCfg<256, 2>;
 using Cfg128E = TileCfg<128, 1, true>;
 using Cfg128M = TileCfg<128, 1, false, true>;
 using Cfg256PM = TileCfg<256, 2, false, true>;
+using Cfg128S = TileCfg<128, 1, false, false, true>;
 
 int tile_super_edge(int cfg) { return (cfg == TILE_128x128 || cfg == TILE_128x128_ENH) ? 128 : 256; }
 int tile_subs(int cfg) { return cfg == TILE_128x256 ? Cfg256::SUB : 1; }
@@ -587,6 +730,9 @@ cudaError_t layer_kernel_setup(int cfg) {
             e = cudaFuncSetAttribute(k_sp2_layer<Cfg128M>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                      Cfg128M::SMEM_BYTES);
             if (e != cudaSuccess) return e;
+            e = cudaFuncSetAttribute(k_sp2_layer<Cfg128S>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     Cfg128S::SMEM_BYTES);
+            if (e != cudaSuccess) return e;
             return cudaFuncSetAttribute(k_sp2_layer<Cfg256PM>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                         Cfg256PM::SMEM_BYTES);
         }
@@ -616,6 +762,10 @@ static cudaError_t launch_cfg(const CUtensorMap& tm_hi, const CUtensorMap& tm_lo
 
 cudaError_t launch_layer(int cfg, const CUtensorMap& tm_hi, const CUtensorMap& tm_lo, const LayerParams& p,
                          int num_sms, cudaStream_t st) {
+    if (p.bn_cur != nullptr) {           // blocked-sparse variant: 128x128 tiles only
+        if (cfg == TILE_128x128 && p.mix == nullptr) return launch_cfg<Cfg128S>(tm_hi, tm_lo, p, num_sms, st);
+        return cudaErrorInvalidValue;
+    }
     if (p.mix != nullptr) {              // output mix: 128x128 or pair tiles only
         if (cfg == TILE_128x128) return launch_cfg<Cfg128M>(tm_hi, tm_lo, p, num_sms, st);
         if (cfg == TILE_256x256_PAIR) return launch_cfg<Cfg256PM>(tm_hi, tm_lo, p, num_sms, st);
