@@ -1,0 +1,70 @@
+"""Measurements of the two hardware facts the design leans on, as tests (they print the numbers DESIGN.md quotes):
+
+1. The tensor core's FP32 accumulation TRUNCATES: an off-diagonal entry of the mixed-precision square comes out
+   multiplied by 1 + beta, beta < 0 growing with the number of accumulations -- the noise floor of the plain layers
+   and the reason for the enhanced-accumulation layers of the refinement (NEXT-1).
+2. An isolated FP64 instruction pays a wake-up latency of the FP64 datapath (hundreds of cycles) while back-to-back
+   FP64 instructions do not -- the reason the control step and every trace are integer fixed point
+   (csrc/sp2_control.cuh)."""
+import os
+import shutil
+import subprocess
+
+import numpy as np
+import pytest
+
+from oracle import sp2_oracle as O
+from paper_2101_06385_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def test_tensor_core_accumulation_shrinks_the_off_diagonal_part(cuda_device):
+    import torch
+
+    from paper_2101_06385_b200 import api
+
+    h = api.Handle(2304, 0, 8)
+    betas = {}
+    for n in (640, 2048):
+        rng = np.random.default_rng(100 + n)
+        Q = W.haar_orthogonal(rng, n)
+        nocc = n // 2
+        s = np.concatenate([1.0 - rng.uniform(0, 2e-2, nocc), rng.uniform(0, 2e-2, n - nocc)])   # a nearly converged S
+        S64 = (Q * s) @ Q.T
+        H32 = np.ascontiguousarray((np.eye(n) - 0.5 * (S64 + S64.T)).astype(np.float32))           # S_0 = I - H with (0, 1)
+        S0 = (-H32).astype(np.float32)
+        S0[np.diag_indices(n)] = (S0[np.diag_indices(n)] + np.float32(1.0)).astype(np.float32)
+        S0 = np.tril(S0) + np.tril(S0, -1).T
+        hi, lo = O.split_fp16(S0 * np.float32(8192.0))
+        Xmix = O.mixed_square_exact(hi, lo) / 8192.0 ** 2              # Eq. 15 with exact sums: the target
+        off = ~np.eye(n, dtype=bool)
+        for tile in (1, 4):                                            # plain / enhanced accumulation
+            X, _ = h.generalized(torch.from_numpy(H32).cuda(), np.array([[1.0, 0.0, 0.0]]), bounds=(0.0, 1.0),
+                                 opts=api.make_opts(tile_config=tile))
+            d = (X.cpu().numpy().astype(np.float64) - Xmix)[off]
+            r = Xmix[off]
+            betas[(n, tile)] = float((d * r).sum() / (r * r).sum())    # least-squares factor: X_off = (1 + beta) target
+    print("off-diagonal shrink factor beta of one layer (plain | enhanced accumulation): "
+          + ", ".join(f"N={n}: {betas[(n, 1)]:+.2e} | {betas[(n, 4)]:+.2e}" for n in (640, 2048)))
+    assert -2e-5 < betas[(2048, 1)] < betas[(640, 1)] < -5e-7         # truncation: negative, growing with K
+    assert abs(betas[(2048, 4)]) < 0.1 * abs(betas[(2048, 1)])        # chunked accumulation removes it
+    h.close()
+
+
+def test_fp64_wakeup_latency(cuda_device, tmp_path):
+    nvcc = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
+    if not os.path.exists(nvcc):
+        pytest.skip("nvcc not available on this box")
+    exe = str(tmp_path / "fp64_wakeup")
+    subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-o", exe,
+                    os.path.join(HERE, "cuda", "fp64_wakeup.cu")], check=True)
+    out = subprocess.run([exe], capture_output=True, text=True, check=True).stdout
+    v = {k: float(x) for k, x in (ln.split() for ln in out.strip().splitlines())}
+    print("cycles per iteration:", v)
+    assert v["dfma_chain"] < 20.0                                      # back to back: the pipeline latency
+    sum_of_latencies = v["dfma_chain"] + 16 * v["ffma_chain"]
+    print(f"1 DFMA + 16 FFMA: {v['dfma_plus_16_ffma']:.0f} cycles against {sum_of_latencies:.0f} for the sum of the "
+          f"latencies -> wake-up {v['dfma_plus_16_ffma'] - sum_of_latencies:.0f} cycles")
+    assert v["dfma_plus_16_ffma"] > 1.5 * sum_of_latencies             # an isolated FP64 instruction is expensive
