@@ -117,9 +117,16 @@ __global__ void __launch_bounds__(256) k_gershgorin_finalize(const float* __rest
     const int nslots = (Ib + 1) + (nt - Ib);
     double acc = 0.0;
     if (i < N)
-        for (int sidx = g; sidx < nslots; sidx += 4) {
-            const int slot = (sidx <= Ib) ? sidx : (nt + Ib + (sidx - Ib - 1));
-            acc += (double)__ldg(part + (long long)slot * N + i);
+        for (int s0 = g; s0 < nslots; s0 += 32) {           // eight loads in flight, then the adds in slot order
+            float v[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const int sidx = s0 + 4 * u;
+                const int slot = (sidx <= Ib) ? sidx : (nt + Ib + (sidx - Ib - 1));
+                v[u] = (sidx < nslots) ? __ldg(part + (long long)slot * N + i) : 0.f;
+            }
+#pragma unroll
+            for (int u = 0; u < 8; ++u) acc += (double)v[u];
         }
     ps[g][r] = acc;
     __syncthreads();

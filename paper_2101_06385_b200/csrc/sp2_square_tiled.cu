@@ -19,7 +19,7 @@
 
 namespace sp2 {
 
-template <int BN_, int CG_, bool ENH_ = false, bool MIX_ = false, bool SP_ = false>
+template <int BN_, int CG_, bool ENH_ = false, bool MIX_ = false, bool SP_ = false, int EW_ = 8>
 struct TileCfg {
     // SP: blocked-sparse variant for matrices with decay (reading C28): 128 x 128 blocks of S_{n-1}
     // whose Frobenius norm is <= tau count as zero -- their K-blocks are neither loaded nor multiplied.
@@ -43,7 +43,10 @@ struct TileCfg {
     static constexpr int TMEM_COLS = ENH ? 4 * BN : 2 * BN;   // two accumulator buffers (+ running hi, lo)
     static_assert(TMEM_COLS <= 512, "TMEM has 512 columns");
     static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*align*/ + 256 /*barriers*/;
-    static constexpr int THREADS = 192;
+    // warp 0 = TMA producer, warp 1 = MMA issuer, then EPI_WARPS epilogue warps: EPI_WARPS / 4 per TMEM lane quarter,
+    // taking alternate 32-column chunks of their 32 rows
+    static constexpr int EPI_WARPS = EW_;
+    static constexpr int THREADS = 64 + 32 * EPI_WARPS;
 };
 
 // Blocked-sparse variant: which 128-wide K-blocks of tile (I, J) survive the truncation?  Bit kk says that both
@@ -99,8 +102,8 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
     uint64_t* tfull_bar = bars + 2 * STAGES;         // [2]
     uint64_t* tempty_bar = bars + 2 * STAGES + 2;    // [2]
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * STAGES + 4);
-    __shared__ fx_t red[4][4];
-    __shared__ unsigned long long red48[2][4];       // SP: per-warp sums of squares of the tile in flight (2^48 fixed point)
+    __shared__ fx_t red[8][4];
+    __shared__ unsigned long long red48[2][8];       // SP: per-warp sums of squares of the tile in flight (2^48 fixed point)
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
@@ -122,7 +125,7 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
             }
             for (int b = 0; b < 2; ++b) {
                 mbar_init(&tfull_bar[b], 1);
-                mbar_init(&tempty_bar[b], 4 * CG);
+                mbar_init(&tempty_bar[b], C::EPI_WARPS * CG);
             }
             fence_barrier_init();
         }
@@ -339,6 +342,9 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
     } else {
         // =============================== epilogue warps (TMEM lane quarter = warp % 4)
         const int q = warp & 3;
+        const int ew = warp - 2;                            // epilogue warp index
+        const int part = ew >> 2;                           // which of the alternate chunks of its rows this warp takes
+        constexpr int NPART = C::EPI_WARPS / 4;
         const int rl = q * 32 + lane;                       // accumulator row (TMEM lane) of this thread
         const float th1 = ((volatile float*)ctrl->theta)[0];
         const float th1s = th1 * p.inv_scale2;
@@ -394,6 +400,7 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
 #pragma unroll 1
                     for (int c0 = 0; c0 < ncols; c0 += 32) {
                         if (n0 + c0 > gi_wmax) break;
+                        if (NPART > 1 && ((c0 >> 5) % NPART) != part) continue;
                         uint32_t a[32], rh[32], rlo[32];
                         tmem_ld_32x32(t_acc + (uint32_t)c0, a);
                         if (ch > 0) {
@@ -438,6 +445,7 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
             for (int c0 = 0; c0 < ncols; c0 += 32) {
                 const int gj0 = n0 + c0;
                 if (gj0 > gi_wmax) break;                   // rest of the row block lies above the diagonal
+                if (NPART > 1 && ((c0 >> 5) % NPART) != part) continue;
                 uint32_t v[32];
                 float so[32];
                 if (C::SP && sp_empty) {
@@ -611,9 +619,11 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                 // counts in N_X = ||S'_n||_F^2 (the oracle squares the truncated matrix)
                 for (int o = 16; o > 0; o >>= 1) tile48 += __shfl_xor_sync(0xffffffffu, tile48, o);
                 const int par = it & 1;
-                if (lane == 0) red48[par][q] = tile48;
-                asm volatile("bar.sync 1, 128;\n" ::: "memory");
-                const unsigned long long tot = (red48[par][0] + red48[par][1]) + (red48[par][2] + red48[par][3]);
+                if (lane == 0) red48[par][ew] = tile48;
+                asm volatile("bar.sync 1, %0;\n" ::"n"(32 * C::EPI_WARPS) : "memory");
+                unsigned long long tot = 0;
+#pragma unroll
+                for (int i = 0; i < C::EPI_WARPS; ++i) tot += red48[par][i];
                 if (tot > ctrl->tau2_fx48) off2 += tile40;
                 if (warp == 2 && lane == 0) {
                     p.bn_next[(size_t)wi.I * p.nb + wi.J] = tot;
@@ -630,13 +640,13 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
             trX += __shfl_xor_sync(0xffffffffu, trX, o);
         }
         bad = __any_sync(0xffffffffu, bad);
-        if (lane == 0) { red[q][0] = trS; red[q][1] = fro2; red[q][2] = trX; red[q][3] = bad ? 1 : 0; }
-        asm volatile("bar.sync 1, 128;\n" ::: "memory");     // the four epilogue warps only
+        if (lane == 0) { red[ew][0] = trS; red[ew][1] = fro2; red[ew][2] = trX; red[ew][3] = bad ? 1 : 0; }
+        asm volatile("bar.sync 1, %0;\n" ::"n"(32 * C::EPI_WARPS) : "memory");     // the epilogue warps only
         if (warp == 2) {
             unsigned int done = 0;
             if (lane == 0) {
                 fx_t a = 0, b = 0, c = 0, f = 0;
-                for (int i = 0; i < 4; ++i) { a += red[i][0]; b += red[i][1]; c += red[i][2]; f += red[i][3]; }
+                for (int i = 0; i < C::EPI_WARPS; ++i) { a += red[i][0]; b += red[i][1]; c += red[i][2]; f += red[i][3]; }
                 ctrl->ipartial[blockIdx.x][0] = a;
                 ctrl->ipartial[blockIdx.x][1] = b;
                 ctrl->ipartial[blockIdx.x][2] = c;
