@@ -83,7 +83,11 @@ typedef struct {
                                -1 = library default (13): keeps X1 out of FP16's subnormal range            */
     int    control;         /* 0: device-side loop in a CUDA graph (WHILE node); 1: host-stepped (debug:
                                one sync per layer); 2: max_layers plain stream launches of the layer kernel, each
-                               guarded on the device (a launch after convergence returns at once), no graph  */
+                               guarded on the device (a launch after convergence returns at once), no graph;
+                               3: ONE persistent cooperative launch runs every layer, with a grid-wide barrier
+                               between layers and the operand pairs swapped inside the kernel (same tiles, same
+                               order, same bits as 0; measured no faster than 0: the barrier costs what the kernel
+                               boundary costs -- kept as the graph-free form of the device-side loop)          */
     int    tile_config;     /* 0: choose by N; 1: 128x128 1-CTA; 2: 128x256 1-CTA; 3: 256x256 2-CTA;
                                4: 128x128 1-CTA with the enhanced accumulation of sp2_refine_energy in EVERY
                                layer (accuracy option, about 2x the time of 3 at large N)  */

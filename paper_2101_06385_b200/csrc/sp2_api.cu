@@ -417,6 +417,8 @@ static LayerParams layer_params(sp2_handle_s* h, const Problem& pb, int parity, 
     p.ctrl = h->ctrl; p.stats = h->stats_dev; p.thetas = h->thetas_dev; p.S = h->S;
     p.mix = pb.mix ? h->mix : nullptr;
     p.hi_out = h->hl[parity ^ 1][0]; p.lo_out = h->hl[parity ^ 1][1];
+    p.hi_in = h->hl[parity][0]; p.lo_in = h->hl[parity][1];
+    p.persist = 0;
     p.rowsq_cur = pb.exact_diag ? h->rowsq[parity] : nullptr;
     p.rowsq_next = pb.exact_diag ? h->rowsq[parity ^ 1] : nullptr;
     p.items = h->items_dev[pb.list]; p.ld = ws_ld_f32(pb.Np); p.ldf = ws_ld_f16(pb.Np); p.N = pb.N; p.Np = pb.Np;
@@ -427,15 +429,21 @@ static LayerParams layer_params(sp2_handle_s* h, const Problem& pb, int parity, 
     return p;
 }
 
+// persist = 1: ONE launch runs every layer of the solve (grid barrier between layers, cooperative launch).
 static sp2_status_t launch_one_layer(sp2_handle_s* h, const Problem& pb, int parity, unsigned long long cond,
-                                     cudaStream_t st) {
-    CUtensorMap tm_hi, tm_lo;
+                                     cudaStream_t st, int persist = 0) {
+    CUtensorMap tm_hi, tm_lo, tm_hi1, tm_lo1;
     sp2_status_t s = make_tmap(h, &tm_hi, h->hl[parity][0], pb.Np);
     if (s != SP2_OK) return s;
     s = make_tmap(h, &tm_lo, h->hl[parity][1], pb.Np);
     if (s != SP2_OK) return s;
+    s = make_tmap(h, &tm_hi1, h->hl[parity ^ 1][0], pb.Np);
+    if (s != SP2_OK) return s;
+    s = make_tmap(h, &tm_lo1, h->hl[parity ^ 1][1], pb.Np);
+    if (s != SP2_OK) return s;
     LayerParams p = layer_params(h, pb, parity, cond);
-    CK(launch_layer(pb.cfg, tm_hi, tm_lo, p, h->num_sms, st));
+    p.persist = persist;
+    CK(launch_layer(pb.cfg, tm_hi, tm_lo, tm_hi1, tm_lo1, p, h->num_sms, st));
     return SP2_OK;
 }
 
@@ -570,6 +578,9 @@ static sp2_status_t solve_single(sp2_handle_s* h, const float* H_dev, int N, int
             s = launch_one_layer(h, pb, n & 1, 0, st);
             if (s != SP2_OK) return s;
         }
+    } else if (o->control == 3) {
+        s = launch_one_layer(h, pb, 0, 0, st, 1);       // persistent: the layer loop runs inside one cooperative launch
+        if (s != SP2_OK) return s;
     } else {
         for (int n = 0; n < max_layers; ++n) {
             s = launch_one_layer(h, pb, n & 1, 0, st);

@@ -72,7 +72,7 @@ struct CtrlCore {
     unsigned int round_counter;      // round-boundary check-ins of all layer kernels of this solve (round sync);
                                      // monotonic: layer n+1's targets start at n (n_rounds - 1) gridDim.x
     unsigned int round_sync_broken;  // a round wait timed out once (CTAs not co-resident): stop waiting in this solve
-    unsigned int pad_rs_;
+    int layer_gen;                   // persistent mode: layers applied, published with release semantics (grid barrier)
     // blocked-sparse variant (reading C28)
     unsigned long long tau2_fx48;    // tau^2 in 2^48 fixed point (block norms^2 are compared with it)
     unsigned long long work_active;  // 128-wide K-blocks the MMA warps multiplied, summed over tiles and layers

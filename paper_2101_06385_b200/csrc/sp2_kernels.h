@@ -66,6 +66,9 @@ struct LayerParams {
     float* mix;                    // output mix M = sum_i c_i S_i (Eq. 18), same layout as S; nullptr = none
     __half* hi_out;                // next layer's operands (the other ping-pong pair)
     __half* lo_out;
+    __half* hi_in;                 // this layer's operand pair (persistent mode: the output pair of odd layers)
+    __half* lo_in;
+    int persist;                   // 1: one launch runs layer after layer (grid barrier in between) until the control stops
     unsigned long long* rowsq_cur; // r_i of S_{n-1} (read at the diagonal, then zeroed); nullptr = tensor-core diagonal
     unsigned long long* rowsq_next;// r_i of S_n (accumulated by this launch)
     const WorkItem* items;         // work list in launch order: item w runs on CTA slot w % n_slots in round w / n_slots
@@ -94,8 +97,10 @@ int tile_cta_group(int cfg);
 int layer_slots(int cfg, int n_items, int num_sms);   // CTA slots a launch of n_items uses
 size_t tile_smem_bytes(int cfg);
 // Launch one layer: reads hi/lo through the tensor maps (K-major, 128B swizzle, box 64 x 128), writes S, hi_out, lo_out.
-cudaError_t launch_layer(int cfg, const CUtensorMap& tm_hi, const CUtensorMap& tm_lo, const LayerParams& p,
-                         int num_sms, cudaStream_t st);
+// tm_hi / tm_lo: the input pair of the launch's first layer; tm_hi1 / tm_lo1: the other pair (read by the odd layers of a
+// persistent launch; pass the first pair again otherwise).
+cudaError_t launch_layer(int cfg, const CUtensorMap& tm_hi, const CUtensorMap& tm_lo, const CUtensorMap& tm_hi1,
+                         const CUtensorMap& tm_lo1, const LayerParams& p, int num_sms, cudaStream_t st);
 cudaError_t layer_kernel_setup(int cfg);   // cudaFuncSetAttribute(max dynamic smem), once per process
 
 // ---- resident small-N kernel (sp2_resident.cu): whole solve in one launch, one CTA (pair) per matrix

@@ -49,6 +49,10 @@ struct TileCfg {
     static constexpr int THREADS = 64 + 32 * EPI_WARPS;
 };
 
+// Entries of the block-norm tables: low 62 bits = squared Frobenius norm in 2^48 fixed point; top 2 bits = for how many
+// consecutive layers the block has been WRITTEN as exact zeros (saturating at 3): after two such layers both ping-pong
+// operand pairs and the master hold zeros there, and a tile that would again be zero is not touched at all.
+constexpr unsigned long long kBnNormMask = (1ull << 62) - 1ull;
 // Blocked-sparse variant: which 128-wide K-blocks of tile (I, J) survive the truncation?  Bit kk says that both
 // S'_{I,kk} and S'_{J,kk} are kept (diagonal blocks always are).  bn = squared block norms of S_{n-1} in 2^48 fixed
 // point, nb x nb, symmetric.  One ballot per 32 blocks (nb <= 128).
@@ -59,8 +63,8 @@ __device__ __forceinline__ void sparse_kmask(const unsigned long long* __restric
         const int kk = 32 * t + lane;
         bool act = false;
         if (kk < nb) {
-            const bool a = (kk == I) || __ldcg(bn + (size_t)I * nb + kk) > tau2;
-            const bool b = (kk == J) || __ldcg(bn + (size_t)J * nb + kk) > tau2;
+            const bool a = (kk == I) || (__ldcg(bn + (size_t)I * nb + kk) & kBnNormMask) > tau2;
+            const bool b = (kk == J) || (__ldcg(bn + (size_t)J * nb + kk) & kBnNormMask) > tau2;
             act = a && b;
         }
         m[t] = __ballot_sync(0xffffffffu, act);
@@ -69,6 +73,30 @@ __device__ __forceinline__ void sparse_kmask(const unsigned long long* __restric
 __device__ __forceinline__ bool sparse_bit(const uint32_t (&m)[4], int kk) {
     const uint32_t word = (kk < 32) ? m[0] : (kk < 64) ? m[1] : (kk < 96) ? m[2] : m[3];
     return ((word >> (kk & 31)) & 1u) != 0u;
+}
+
+// Grid-wide layer barrier of the persistent mode: wait until `target` layers of the solve have been applied (the CTA
+// that runs the control step publishes ctrl->n with release semantics), make the other CTAs' stores visible to this
+// thread's generic and async (TMA) accesses, and tell whether another layer follows.  One lane spins; bounded (a grid
+// that is not co-resident cannot be launched in this mode -- cooperative launch -- so a time-out is a bug: trap).
+__device__ __forceinline__ bool layer_barrier_one(Ctrl* ctrl, int target) {      // called by ONE thread
+    unsigned int spins = 0;
+    int gen;
+    do {
+        asm volatile("ld.acquire.gpu.global.s32 %0, [%1];\n" : "=r"(gen) : "l"(&ctrl->layer_gen) : "memory");
+        if (gen >= target) break;
+        __nanosleep(32);
+        if (++spins > (1u << 25)) __trap();
+    } while (true);
+    __threadfence();                                      // also drops this SM's stale L1 lines
+    asm volatile("fence.proxy.async;\n" ::: "memory");
+    return *((volatile int*)&ctrl->running) != 0;
+}
+__device__ __forceinline__ bool layer_barrier(Ctrl* ctrl, int target, int lane) {  // called by a whole warp
+    int run = 0;
+    if (lane == 0) run = layer_barrier_one(ctrl, target) ? 1 : 0;
+    run = __shfl_sync(0xffffffffu, run, 0);
+    return run != 0;
 }
 
 #ifdef SP2_LAYER_TIMING
@@ -82,7 +110,8 @@ extern "C" void sp2_debug_layer_timing(unsigned long long* out) { cudaMemcpyFrom
 
 template <class C>
 __global__ void __launch_bounds__(C::THREADS, 1)
-k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ CUtensorMap tm_lo,
+k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi0, const __grid_constant__ CUtensorMap tm_lo0,
+            const __grid_constant__ CUtensorMap tm_hi1, const __grid_constant__ CUtensorMap tm_lo1,
             const LayerParams p) {
     constexpr int BN = C::BN, CG = C::CG, BM = C::BM, BK = C::BK, STAGES = C::STAGES;
     Ctrl* ctrl = p.ctrl;
@@ -114,9 +143,14 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
     const int KB = p.Np / BK;
 
     if (warp == 0 && lane == 0) {
-        tma_prefetch_desc(&tm_hi);
-        tma_prefetch_desc(&tm_lo);
+        tma_prefetch_desc(&tm_hi0);
+        tma_prefetch_desc(&tm_lo0);
+        if (p.persist) { tma_prefetch_desc(&tm_hi1); tma_prefetch_desc(&tm_lo1); }
     }
+    // Persistent mode (p.persist): this launch runs layer after layer until the control stops the solve; the CTAs meet
+    // at a grid-wide barrier after each layer (released by the CTA that ran the control step).  Layer l of the launch
+    // reads the operand pair (l & 1) and writes the other one.  n_at_entry: layers applied before this launch.
+    const int n_at_entry = *((volatile int*)&ctrl->n);
     if (warp == 1) {
         if (lane == 0) {
             for (int s = 0; s < STAGES; ++s) {
@@ -146,10 +180,14 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
         uint32_t ph = 0;
         const uint64_t pol = l2_policy_evict_last();
         const unsigned long long tau2 = ctrl->tau2_fx48;
+        for (int layer = 0;; ++layer) {
+        const CUtensorMap* tmh = (layer & 1) ? &tm_hi1 : &tm_hi0;
+        const CUtensorMap* tml = (layer & 1) ? &tm_lo1 : &tm_lo0;
+        const unsigned long long* bn_cur = (layer & 1) ? p.bn_next : p.bn_cur;
         for (int w = slot; w < n_work; w += nslots) {
             const WorkItem wi = p.items[w];
             uint32_t m[4];
-            sparse_kmask(p.bn_cur, p.nb, wi.I, wi.J, tau2, lane, m);
+            sparse_kmask(bn_cur, p.nb, wi.I, wi.J, tau2, lane, m);
             if (lane == 0) {
                 const int m0 = wi.I * BN, n0 = wi.J * BN;
                 for (int kk = 0; kk < p.nb; ++kk) {
@@ -160,15 +198,17 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                         uint8_t* st = smem + s * C::STAGE_BYTES;
                         const int k0 = kk * 128 + half * BK;
                         mbar_arrive_expect_tx(&full_bar[s], C::STAGE_BYTES);
-                        tma_load_2d_hint(st, &tm_hi, &full_bar[s], k0, m0, pol);
-                        tma_load_2d_hint(st + C::A_BYTES, &tm_lo, &full_bar[s], k0, m0, pol);
-                        tma_load_2d_hint(st + 2 * C::A_BYTES, &tm_hi, &full_bar[s], k0, n0, pol);
-                        tma_load_2d_hint(st + 2 * C::A_BYTES + C::B_BYTES, &tm_lo, &full_bar[s], k0, n0, pol);
+                        tma_load_2d_hint(st, tmh, &full_bar[s], k0, m0, pol);
+                        tma_load_2d_hint(st + C::A_BYTES, tml, &full_bar[s], k0, m0, pol);
+                        tma_load_2d_hint(st + 2 * C::A_BYTES, tmh, &full_bar[s], k0, n0, pol);
+                        tma_load_2d_hint(st + 2 * C::A_BYTES + C::B_BYTES, tml, &full_bar[s], k0, n0, pol);
                         if (++s == STAGES) { s = 0; ph ^= 1u; }
                     }
                 }
             }
             __syncwarp();
+        }
+        if (!p.persist || !layer_barrier(ctrl, n_at_entry + layer + 1, lane)) break;
         }
     } else if (warp == 0) {
         // =============================== TMA producer (one elected lane)
@@ -183,7 +223,10 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
             // targets of layer n + 1 start at n (n_rounds - 1) gridDim.x and a late check-in of the previous layer
             // can never be lost to a reset.
             const int n_rounds = (n_work + nslots - 1) / nslots;
-            const unsigned int base = (unsigned int)(*((volatile int*)&ctrl->n)) * (unsigned int)(n_rounds - 1);
+            for (int layer = 0;; ++layer) {
+            const CUtensorMap* tmh = (layer & 1) ? &tm_hi1 : &tm_hi0;
+            const CUtensorMap* tml = (layer & 1) ? &tm_lo1 : &tm_lo0;
+            const unsigned int base = (unsigned int)(n_at_entry + layer) * (unsigned int)(n_rounds - 1);
             int round = 0;
             for (int w = slot; ; w += nslots, ++round) {
                 if (p.round_sync && round > 0 && round < n_rounds) {
@@ -213,30 +256,32 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                     const int k0 = ((round & 1) ? (KB - 1 - kb) : kb) * BK;
                     if (CG == 1) {
                         mbar_arrive_expect_tx(&full_bar[s], C::STAGE_BYTES);
-                        tma_load_2d_hint(st, &tm_hi, &full_bar[s], k0, m0, pol);
-                        tma_load_2d_hint(st + C::A_BYTES, &tm_lo, &full_bar[s], k0, m0, pol);
+                        tma_load_2d_hint(st, tmh, &full_bar[s], k0, m0, pol);
+                        tma_load_2d_hint(st + C::A_BYTES, tml, &full_bar[s], k0, m0, pol);
 #pragma unroll
                         for (int h = 0; h < C::BNL / 128; ++h) {
-                            tma_load_2d_hint(st + 2 * C::A_BYTES + h * 16384, &tm_hi, &full_bar[s], k0, n0 + h * 128, pol);
-                            tma_load_2d_hint(st + 2 * C::A_BYTES + C::B_BYTES + h * 16384, &tm_lo, &full_bar[s], k0,
+                            tma_load_2d_hint(st + 2 * C::A_BYTES + h * 16384, tmh, &full_bar[s], k0, n0 + h * 128, pol);
+                            tma_load_2d_hint(st + 2 * C::A_BYTES + C::B_BYTES + h * 16384, tml, &full_bar[s], k0,
                                              n0 + h * 128, pol);
                         }
                     } else {
                         // both CTAs' loads complete_tx on the leader's barrier; only the leader arrives (a peer
                         // load landing first just leaves the transaction count negative until the expect_tx)
                         if (rank == 0) mbar_arrive_expect_tx(&full_bar[s], 2 * C::STAGE_BYTES);
-                        tma_load_2d_pair_hint(st, &tm_hi, &full_bar[s], k0, m0, pol);
-                        tma_load_2d_pair_hint(st + C::A_BYTES, &tm_lo, &full_bar[s], k0, m0, pol);
+                        tma_load_2d_pair_hint(st, tmh, &full_bar[s], k0, m0, pol);
+                        tma_load_2d_pair_hint(st + C::A_BYTES, tml, &full_bar[s], k0, m0, pol);
 #pragma unroll
                         for (int h = 0; h < C::BNL / 128; ++h) {
-                            tma_load_2d_pair_hint(st + 2 * C::A_BYTES + h * 16384, &tm_hi, &full_bar[s], k0, n0 + h * 128,
+                            tma_load_2d_pair_hint(st + 2 * C::A_BYTES + h * 16384, tmh, &full_bar[s], k0, n0 + h * 128,
                                                   pol);
-                            tma_load_2d_pair_hint(st + 2 * C::A_BYTES + C::B_BYTES + h * 16384, &tm_lo, &full_bar[s], k0,
+                            tma_load_2d_pair_hint(st + 2 * C::A_BYTES + C::B_BYTES + h * 16384, tml, &full_bar[s], k0,
                                                   n0 + h * 128, pol);
                         }
                     }
                     if (++s == STAGES) { s = 0; ph ^= 1u; }
                 }
+            }
+            if (!p.persist || !layer_barrier_one(ctrl, n_at_entry + layer + 1)) break;
             }
         }
         __syncwarp();     // reconverge before the .aligned cluster barrier of the teardown
@@ -247,10 +292,12 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
         int it = 0;
         const unsigned long long tau2 = ctrl->tau2_fx48;
         constexpr uint32_t idesc = umma_idesc_f16(BM, BN);
+        for (int layer = 0;; ++layer) {
+        const unsigned long long* bn_cur = (layer & 1) ? p.bn_next : p.bn_cur;
         for (int w = slot; w < n_work; w += nslots, ++it) {
             const WorkItem wi = p.items[w];
             uint32_t m[4];
-            sparse_kmask(p.bn_cur, p.nb, wi.I, wi.J, tau2, lane, m);
+            sparse_kmask(bn_cur, p.nb, wi.I, wi.J, tau2, lane, m);
             const int buf = it & 1;
             mbar_wait(&tempty_bar[buf], ((uint32_t)(it >> 1) & 1u) ^ 1u);
             tc_fence_after();
@@ -291,12 +338,15 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
             }
             __syncwarp();
         }
+        if (!p.persist || !layer_barrier(ctrl, n_at_entry + layer + 1, lane)) break;
+        }
     } else if (warp == 1) {
         // =============================== MMA issuer (leader CTA only, one elected lane)
         if (rank == 0) {
             int s = 0;
             uint32_t ph = 0;
             int it = 0;                                   // accumulator uses so far (one per item; per chunk if ENH)
+            for (int layer = 0;; ++layer) {
             for (int w = slot; w < n_work; w += nslots) {
                 const uint32_t idesc = umma_idesc_f16(BM * CG, p.items[w].ncols);   // N = 256, or 128 / 64 in the tail
                 const int KC = p.enh_kc;                  // K-blocks per accumulation chunk (ENH)
@@ -337,6 +387,8 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                     }
                 }
             }
+            if (!p.persist || !layer_barrier(ctrl, n_at_entry + layer + 1, lane)) break;
+            }
         }
         __syncwarp();     // reconverge before the .aligned barrier / tcgen05.dealloc of the teardown
     } else {
@@ -346,6 +398,8 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
         const int part = ew >> 2;                           // which of the alternate chunks of its rows this warp takes
         constexpr int NPART = C::EPI_WARPS / 4;
         const int rl = q * 32 + lane;                       // accumulator row (TMEM lane) of this thread
+        int it = 0;                                         // accumulator uses so far (same count as the MMA warp)
+        for (int layer = 0;; ++layer) {
         const float th1 = ((volatile float*)ctrl->theta)[0];
         const float th1s = th1 * p.inv_scale2;
         const float th2 = ((volatile float*)ctrl->theta)[1];
@@ -356,10 +410,13 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
         const float inv2 = p.inv_scale2;
         const long long ld = p.ld, ldf = p.ldf;
         float* __restrict__ S = p.S;
-        __half* __restrict__ HO = p.hi_out;
-        __half* __restrict__ LO = p.lo_out;
-        unsigned long long* __restrict__ Rcur = p.rowsq_cur;
-        unsigned long long* __restrict__ Rnext = p.rowsq_next;
+        // odd layers of a persistent launch go the other way between the two operand pairs
+        __half* __restrict__ HO = (layer & 1) ? p.hi_in : p.hi_out;
+        __half* __restrict__ LO = (layer & 1) ? p.lo_in : p.lo_out;
+        unsigned long long* __restrict__ Rcur = (layer & 1) ? p.rowsq_next : p.rowsq_cur;
+        unsigned long long* __restrict__ Rnext = (layer & 1) ? p.rowsq_cur : p.rowsq_next;
+        const unsigned long long* __restrict__ bn_cur = (layer & 1) ? p.bn_next : p.bn_cur;
+        unsigned long long* __restrict__ bn_next = (layer & 1) ? const_cast<unsigned long long*>(p.bn_cur) : p.bn_next;
         // No FP64 anywhere in the kernel (an isolated FP64 instruction pays ~170 cycles to wake the datapath, see
         // sp2_control.cuh): the traces are 2^40 fixed-point integers.  Off-diagonal squares are summed in FP32 over one
         // 32-element chunk (4 independent partial sums, |error| <= ~2^-22 of a sum of ~1e-3) and converted once per
@@ -367,7 +424,6 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
         // as exact FP32 pairs.
         fx_t trS = 0, off2 = 0, dg2 = 0, trX = 0;           // ||S_n||_F^2 = 2 off2 + dg2
         bool bad = false;                                   // a non-finite (or out-of-range) value went into a trace
-        int it = 0;                                         // accumulator uses so far (same count as the MMA warp)
         const int nch = C::ENH ? (KB + p.enh_kc - 1) / p.enh_kc : 1;
         const uint32_t lane_off = (uint32_t)(q * 32) << 16;
         for (int w = slot; w < n_work; w += nslots, ++it) {
@@ -377,15 +433,24 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
             const int ncols = wi.ncols;
             // blocked-sparse: is the accumulator empty (no surviving K-block), and does S_{n-1}'s own block count as zero?
             bool sp_empty = false, sp_zero_in = false;
+            int sp_zc = 0;
             const bool sp_offdiag = C::SP && (wi.I != wi.J);
             fx_t tile40 = 0;                                 // the tile's sum of squares, as it goes into N_X if kept
             unsigned long long tile48 = 0;                   // the same in 2^48 fixed point, for the comparison with tau^2
             if (C::SP) {
                 uint32_t m[4];
-                sparse_kmask(p.bn_cur, p.nb, wi.I, wi.J, ctrl->tau2_fx48, lane, m);
+                sparse_kmask(bn_cur, p.nb, wi.I, wi.J, ctrl->tau2_fx48, lane, m);
                 sp_empty = ((m[0] | m[1] | m[2] | m[3]) == 0u);
-                if (sp_offdiag) sp_zero_in = !(__ldcg(p.bn_cur + (size_t)wi.I * p.nb + wi.J) > ctrl->tau2_fx48);
+                if (sp_offdiag) {
+                    const unsigned long long cur = __ldcg(bn_cur + (size_t)wi.I * p.nb + wi.J);
+                    sp_zero_in = !((cur & kBnNormMask) > ctrl->tau2_fx48);
+                    sp_zc = (int)(cur >> 62);
+                }
             }
+            // the output tile is exactly zero (no surviving product, own block counts as zero; the bias touches diagonal
+            // tiles only) -- and if the last two layers already wrote zeros here, there is nothing to do
+            const bool sp_zero_out = sp_offdiag && sp_empty && sp_zero_in;
+            const bool sp_skip = sp_zero_out && sp_zc >= 2;
             const int gi = m0 + rl;
             const int gi_wmin = m0 + q * 32, gi_wmax = gi_wmin + 31;
             fx_t rowacc = 0;                                // sum_j S_n(gi, j)^2 over the own entries (j <= gi) of this tile
@@ -442,7 +507,7 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
             unsigned short* HOu = reinterpret_cast<unsigned short*>(HO);
             unsigned short* LOu = reinterpret_cast<unsigned short*>(LO);
 #pragma unroll 1
-            for (int c0 = 0; c0 < ncols; c0 += 32) {
+            for (int c0 = 0; c0 < (sp_skip ? 0 : ncols); c0 += 32) {
                 const int gj0 = n0 + c0;
                 if (gj0 > gi_wmax) break;                   // rest of the row block lies above the diagonal
                 if (NPART > 1 && ((c0 >> 5) % NPART) != part) continue;
@@ -552,7 +617,7 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                     // of X_n: diag(S_{n-1}^2)_i = sum_j S_{n-1}(i,j)^2, accumulated while S_{n-1} was written
                     float xdiag = 0.f;
                     if (Rcur != nullptr) {
-                        xdiag = (float)(long long)Rcur[gi] * kRowSqInvF;       // one rounding, as through FP64
+                        xdiag = (float)(long long)__ldcg(Rcur + gi) * kRowSqInvF;   // one rounding, as through FP64; L2 (atomics)
                         Rcur[gi] = 0ull;                    // this buffer is the accumulator of the layer after next
                     }
                     tmem_ld_wait();
@@ -614,7 +679,13 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
             if (lane == 0) {
                 if (CG == 1) mbar_arrive(&tempty_bar[buf]); else mbar_arrive_cluster(&tempty_bar[buf], 0);
             }
-            if (sp_offdiag) {
+            if (sp_zero_out) {
+                if (warp == 2 && lane == 0) {
+                    const unsigned long long v = (unsigned long long)(sp_zc < 3 ? sp_zc + 1 : 3) << 62;
+                    bn_next[(size_t)wi.I * p.nb + wi.J] = v;
+                    bn_next[(size_t)wi.J * p.nb + wi.I] = v;
+                }
+            } else if (sp_offdiag) {
                 // the block's squared Frobenius norm decides whether the NEXT layer sees it, and -- now -- whether it
                 // counts in N_X = ||S'_n||_F^2 (the oracle squares the truncated matrix)
                 for (int o = 16; o > 0; o >>= 1) tile48 += __shfl_xor_sync(0xffffffffu, tile48, o);
@@ -626,8 +697,9 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                 for (int i = 0; i < C::EPI_WARPS; ++i) tot += red48[par][i];
                 if (tot > ctrl->tau2_fx48) off2 += tile40;
                 if (warp == 2 && lane == 0) {
-                    p.bn_next[(size_t)wi.I * p.nb + wi.J] = tot;
-                    p.bn_next[(size_t)wi.J * p.nb + wi.I] = tot;
+                    const unsigned long long v = tot < kBnNormMask ? tot : kBnNormMask;
+                    bn_next[(size_t)wi.I * p.nb + wi.J] = v;
+                    bn_next[(size_t)wi.J * p.nb + wi.I] = v;
                 }
             }
         }
@@ -651,6 +723,7 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                 ctrl->ipartial[blockIdx.x][1] = b;
                 ctrl->ipartial[blockIdx.x][2] = c;
                 ctrl->ipartial[blockIdx.x][3] = f;
+                asm volatile("fence.proxy.async;\n" ::: "memory");     // persistent mode: other CTAs TMA-load what was stored
                 __threadfence();
                 done = atomicAdd(&ctrl->done_counter, 1u);
             }
@@ -686,8 +759,15 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
                     control_finish_layer(ctrl, p.stats, p.thetas, a, b, c, f != 0);
                     __threadfence();
                     if (p.cond_handle != 0) cudaGraphSetConditional(p.cond_handle, ctrl->running ? 1u : 0u);
+                    if (p.persist)       // release the grid: layer n_at_entry + layer + 1 of the solve is applied
+                        asm volatile("st.release.gpu.global.s32 [%0], %1;\n" ::"l"(&ctrl->layer_gen), "r"(ctrl->n) : "memory");
                 }
             }
+        }
+        if (!p.persist) break;
+        // this thread's stores of the layer (S, the operand pair, row sums) must be ordered before the next layer's
+        // TMA loads of other CTAs: they are released through the done counter above; here the warp just waits
+        if (!layer_barrier(ctrl, n_at_entry + layer + 1, lane)) break;
         }
     }
 
@@ -701,9 +781,11 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ C
 using Cfg128 = TileCfg<128, 1>;
 using Cfg256 = TileCfg<256, 1>;
 using Cfg256P = TileCfg<256, 2>;
-using Cfg128E = TileCfg<128, 1, true>;
-using Cfg128M = TileCfg<128, 1, false, true>;
-using Cfg256PM = TileCfg<256, 2, false, true>;
+// eight epilogue warps for the plain and the blocked-sparse layers (their epilogue is exposed at small N); four for the
+// enhanced-accumulation and output-mix instantiations, whose chunk code needs the registers (measured: no gain from eight)
+using Cfg128E = TileCfg<128, 1, true, false, false, 4>;
+using Cfg128M = TileCfg<128, 1, false, true, false, 4>;
+using Cfg256PM = TileCfg<256, 2, false, true, false, 4>;
 using Cfg128S = TileCfg<128, 1, false, false, true>;
 
 int tile_super_edge(int cfg) { return (cfg == TILE_128x128 || cfg == TILE_128x128_ENH) ? 128 : 256; }
@@ -751,8 +833,8 @@ cudaError_t layer_kernel_setup(int cfg) {
 }
 
 template <class C>
-static cudaError_t launch_cfg(const CUtensorMap& tm_hi, const CUtensorMap& tm_lo, const LayerParams& p, int num_sms,
-                              cudaStream_t st) {
+static cudaError_t launch_cfg(const CUtensorMap& tm_hi, const CUtensorMap& tm_lo, const CUtensorMap& tm_hi1,
+                              const CUtensorMap& tm_lo1, const LayerParams& p, int num_sms, cudaStream_t st) {
     (void)num_sms;
     const int slots = p.n_slots;          // chosen by the host together with the item list (layer_slots)
     cudaLaunchConfig_t cfg = {};
@@ -760,32 +842,37 @@ static cudaError_t launch_cfg(const CUtensorMap& tm_hi, const CUtensorMap& tm_lo
     cfg.blockDim = dim3(C::THREADS);
     cfg.dynamicSmemBytes = C::SMEM_BYTES;
     cfg.stream = st;
-    cudaLaunchAttribute attr[1];
+    cudaLaunchAttribute attr[2];
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = C::CG;
     attr[0].val.clusterDim.y = 1;
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, k_sp2_layer<C>, tm_hi, tm_lo, p);
+    if (p.persist) {                      // the grid barrier between layers needs every CTA resident: cooperative launch
+        attr[1].id = cudaLaunchAttributeCooperative;
+        attr[1].val.cooperative = 1;
+        cfg.numAttrs = 2;
+    }
+    return cudaLaunchKernelEx(&cfg, k_sp2_layer<C>, tm_hi, tm_lo, tm_hi1, tm_lo1, p);
 }
 
-cudaError_t launch_layer(int cfg, const CUtensorMap& tm_hi, const CUtensorMap& tm_lo, const LayerParams& p,
-                         int num_sms, cudaStream_t st) {
+cudaError_t launch_layer(int cfg, const CUtensorMap& tm_hi, const CUtensorMap& tm_lo, const CUtensorMap& tm_hi1,
+                         const CUtensorMap& tm_lo1, const LayerParams& p, int num_sms, cudaStream_t st) {
     if (p.bn_cur != nullptr) {           // blocked-sparse variant: 128x128 tiles only
-        if (cfg == TILE_128x128 && p.mix == nullptr) return launch_cfg<Cfg128S>(tm_hi, tm_lo, p, num_sms, st);
+        if (cfg == TILE_128x128 && p.mix == nullptr) return launch_cfg<Cfg128S>(tm_hi, tm_lo, tm_hi1, tm_lo1, p, num_sms, st);
         return cudaErrorInvalidValue;
     }
     if (p.mix != nullptr) {              // output mix: 128x128 or pair tiles only
-        if (cfg == TILE_128x128) return launch_cfg<Cfg128M>(tm_hi, tm_lo, p, num_sms, st);
-        if (cfg == TILE_256x256_PAIR) return launch_cfg<Cfg256PM>(tm_hi, tm_lo, p, num_sms, st);
+        if (cfg == TILE_128x128) return launch_cfg<Cfg128M>(tm_hi, tm_lo, tm_hi1, tm_lo1, p, num_sms, st);
+        if (cfg == TILE_256x256_PAIR) return launch_cfg<Cfg256PM>(tm_hi, tm_lo, tm_hi1, tm_lo1, p, num_sms, st);
         return cudaErrorInvalidValue;
     }
     switch (cfg) {
-        case TILE_128x128: return launch_cfg<Cfg128>(tm_hi, tm_lo, p, num_sms, st);
-        case TILE_128x256: return launch_cfg<Cfg256>(tm_hi, tm_lo, p, num_sms, st);
-        case TILE_256x256_PAIR: return launch_cfg<Cfg256P>(tm_hi, tm_lo, p, num_sms, st);
-        case TILE_128x128_ENH: return launch_cfg<Cfg128E>(tm_hi, tm_lo, p, num_sms, st);
+        case TILE_128x128: return launch_cfg<Cfg128>(tm_hi, tm_lo, tm_hi1, tm_lo1, p, num_sms, st);
+        case TILE_128x256: return launch_cfg<Cfg256>(tm_hi, tm_lo, tm_hi1, tm_lo1, p, num_sms, st);
+        case TILE_256x256_PAIR: return launch_cfg<Cfg256P>(tm_hi, tm_lo, tm_hi1, tm_lo1, p, num_sms, st);
+        case TILE_128x128_ENH: return launch_cfg<Cfg128E>(tm_hi, tm_lo, tm_hi1, tm_lo1, p, num_sms, st);
     }
     return cudaErrorInvalidValue;
 }

@@ -29,7 +29,7 @@ def _solve(env, w, bounds, **kw):
     return D.cpu().numpy().astype(np.float64), info
 
 
-@pytest.mark.parametrize("control", [0, 1, 2])
+@pytest.mark.parametrize("control", [0, 1, 2, 3])
 @pytest.mark.parametrize("tile", [1, 2, 3, 4])
 def test_config1_all_tiles_and_control_modes(env, tile, control):
     """BASELINE configs[0] (N=128, explicit bounds): every tile configuration and control mode gives the same
@@ -287,6 +287,30 @@ def test_tiled_kernel_bit_reproducible_and_host_entry(env, n, tile, auto):
     Dh, ih = h.density_matrix_host(w.H32, w.N_occ, opts)
     assert np.array_equal(Dh, D1.cpu().numpy()) and ih["trace_S"] == i1["trace_S"] and ih["bounds"] == i1["bounds"]
     P.assert_acceptance(D1.cpu().numpy().astype(np.float64), O.closed_form_density(w.Q, w.N_occ), w.N_occ, f"N={n}")
+
+
+@pytest.mark.parametrize("n,tile", [(1024, 0), (2048, 0), (3000, 0), (3000, 3)])
+def test_persistent_launch_gives_the_graph_loop_bits(env, n, tile):
+    """control = 3: ONE cooperative launch runs every layer (grid barrier between layers, the operand pairs swapped per
+    layer inside the kernel) -- the same tiles in the same order as the graph's WHILE loop, so the same bits, with
+    caller and with Gershgorin bounds, one to three rounds, single-CTA and pair tiles."""
+    api, h, torch = env
+    w = W.gapped_dense(n + 3, n, (-1.0, -0.15), (0.15, 1.0), n // 2, "persist", bounds=(-1.0, 1.0))
+    Hd = torch.from_numpy(w.H32).cuda()
+    for bounds in (w.bounds, None):
+        o0 = api.make_opts(bounds=bounds, tol=1e-5, max_layers=100, tile_config=tile, control=0)
+        o3 = api.make_opts(bounds=bounds, tol=1e-5, max_layers=100, tile_config=tile, control=3)
+        D0, i0 = h.density_matrix(Hd, w.N_occ, o0)
+        D3, i3 = h.density_matrix(Hd, w.N_occ, o3)
+        assert i3["n_layers"] == i0["n_layers"] and i3["sigma"] == i0["sigma"] and i3["stop_reason"] == i0["stop_reason"]
+        assert i3["trace_S"] == i0["trace_S"] and i3["iderr"] == i0["iderr"]
+        assert torch.equal(D0, D3)
+    # a solve that ends on max_layers, and the exact_diag = 0 variant
+    o3 = api.make_opts(bounds=w.bounds, tol=1e-5, max_layers=7, tile_config=tile, control=3, exact_diag=0)
+    o0 = api.make_opts(bounds=w.bounds, tol=1e-5, max_layers=7, tile_config=tile, control=0, exact_diag=0)
+    D3, i3 = h.density_matrix(Hd, w.N_occ, o3)
+    D0, i0 = h.density_matrix(Hd, w.N_occ, o0)
+    assert i3["n_layers"] == 7 and i3["status"] == api.SP2_NOT_CONVERGED and torch.equal(D0, D3)
 
 
 def test_round_sync_timeout_path_gives_the_same_bits(env, monkeypatch):
