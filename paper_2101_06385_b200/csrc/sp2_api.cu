@@ -7,6 +7,7 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <algorithm>
 #include <map>
 #include <mutex>
 #include <tuple>
@@ -90,6 +91,7 @@ struct sp2_handle_s {
     int last_launches = 0;
     int round_sync = 1;
     unsigned int round_spins = 1u << 16;
+    int ki_edge = 32, ki_mid = 32;   // K-interleave chunking (performance only; SP2_K_INTERLEAVE=edge[:mid], 0 = off)
     cudaStream_t cap_stream = nullptr;
 };
 
@@ -219,6 +221,11 @@ extern "C" sp2_status_t sp2_create(sp2_handle_t* out, int N_max, int batch_max, 
     // performance toggles only (results are bit-identical for any setting)
     if (const char* e = getenv("SP2_TAIL_SPLIT")) h->tail_split = atoi(e);
     if (const char* e = getenv("SP2_ROUND_SYNC")) h->round_sync = atoi(e);
+    if (const char* e = getenv("SP2_K_INTERLEAVE")) {
+        int a = 0, b = 0;
+        const int n = sscanf(e, "%d:%d", &a, &b);
+        if (n >= 1) { h->ki_edge = a < 0 ? 0 : a; h->ki_mid = (n >= 2 && b > 0) ? b : h->ki_edge; }
+    }
     if (const char* e = getenv("SP2_ROUND_SYNC_SPINS")) { const long v = atol(e); h->round_spins = v < 1 ? 1u : (unsigned int)v; }
     h->Np_max = round_up(N_max, 256);
     h->num_sms = prop.multiProcessorCount; h->device = dev;
@@ -311,15 +318,60 @@ static sp2_status_t make_tmap(sp2_handle_s* h, CUtensorMap* tm, void* base, int 
     return SP2_OK;
 }
 
-// Work list of a layer (launch order).  Supertiles of the lower triangle in bands of `band` supertile rows,
-// column-major inside a band, so that the CTAs of one round (n_slots consecutive items run concurrently) share few
+// Band plan of the work list: the lower triangle of the nt x nt supertile grid is cut into bands of supertile rows,
+// [b_0 = 0, b_1), [b_1, b_2), ..., and the list walks each band column by column.  The `per` consecutive items of an
+// epoch (two rounds of n_slots tiles, walked through K together: see ki_range in sp2_square_tiled.cu) then form a
+// rectangle of ~r x c supertiles that touches r + c row panels, and every panel an epoch touches is fetched from HBM
+// once.  The number of items in front of a band that starts at row a is a (a + 1) / 2 whatever the bands before it,
+// so the cost of a band (distinct panels per epoch, summed over the epochs that intersect it) depends on (a, b) only
+// and the best boundaries follow from a shortest-path recursion over b.  Bands are at most hmax rows high (the
+// panels of one round of an epoch, r + c / 2, must stay inside the L2 window).  N = 16384, pair tiles (nt = 64,
+// per = 148, hmax = 17): 336 panel loads per layer against 506 for fixed bands of 8 walked round by round.
+static std::vector<int> plan_bands(int nt, int per, int hmax) {
+    std::vector<long long> best((size_t)nt + 1, -1);
+    std::vector<int> prev((size_t)nt + 1, -1);
+    std::vector<int> seen((size_t)nt, -1);
+    best[0] = 0;
+    for (int b = 1; b <= nt; ++b)
+        for (int a = (b > hmax ? b - hmax : 0); a < b; ++a) {
+            if (best[(size_t)a] < 0) continue;
+            long long idx = (long long)a * (a + 1) / 2, cost = 0, cur = -1;
+            for (int j = 0; j < b; ++j)
+                for (int i = (j > a ? j : a); i < b; ++i, ++idx) {
+                    const long long e = idx / per;
+                    if (e != cur) { cur = e; std::fill(seen.begin(), seen.end(), -1); }
+                    if (seen[(size_t)i] < 0) { seen[(size_t)i] = 1; ++cost; }
+                    if (seen[(size_t)j] < 0) { seen[(size_t)j] = 1; ++cost; }
+                }
+            const long long c = best[(size_t)a] + cost;
+            if (best[(size_t)b] < 0 || c < best[(size_t)b]) { best[(size_t)b] = c; prev[(size_t)b] = a; }
+        }
+    std::vector<int> bounds;
+    for (int b = nt; b > 0; b = prev[(size_t)b]) bounds.push_back(b);
+    bounds.push_back(0);
+    std::reverse(bounds.begin(), bounds.end());
+    return bounds;
+}
+
+// Work list of a layer (launch order).  Supertiles of the lower triangle in bands of supertile rows (plan_bands),
+// column-major inside a band, so that the CTAs of one epoch (2 n_slots consecutive items run in K-lockstep) share few
 // row panels (L2 reuse of the operands).  If the last round is partial and short enough, its items are cut into
 // 2 or 4 column strips each (ncols = E/2, E/4 >= 64): more CTAs share the tail and it ends sooner.
 static void build_work_list(int nt, int band, int edge, int subs, int cta_group, int num_sms, int tail_split,
                             std::vector<WorkItem>& out, int* n_slots) {
     out.clear();
-    for (int i0 = 0; i0 < nt; i0 += band) {
-        const int i1 = (i0 + band < nt) ? i0 + band : nt;
+    std::vector<int> bounds;
+    if (band > 0) {
+        for (int i0 = 0; i0 < nt; i0 += band) bounds.push_back(i0);
+        bounds.push_back(nt);
+    } else {
+        int sl = num_sms / cta_group;
+        if (sl * cta_group > kMaxPartials) sl = kMaxPartials / cta_group;
+        const int per_tiles = (2 * sl) / subs > 0 ? (2 * sl) / subs : 1;
+        bounds = plan_bands(nt, per_tiles, 17);      // measured at N = 16384: 12: 9.65, 14: 9.63, 17: 9.61 ms per layer
+    }
+    for (size_t bi = 0; bi + 1 < bounds.size(); ++bi) {
+        const int i0 = bounds[bi], i1 = bounds[bi + 1];
         for (int j = 0; j < i1; ++j)
             for (int i = (j > i0 ? j : i0); i < i1; ++i)
                 for (int sub = 0; sub < subs; ++sub) {
@@ -392,7 +444,8 @@ static sp2_status_t prepare_problem(sp2_handle_s* h, int N, const sp2_opts_t* o,
     pb->scale = ldexpf(1.0f, k);
     pb->inv_scale2 = ldexpf(1.0f, -2 * k);
     const int nt = pb->Np / edge;
-    const int band = (pb->cfg == TILE_256x256_PAIR) ? 8 : 12;
+    // planned bands (plan_bands) for the plain layers; the enhanced-accumulation layers (no K-interleave) keep fixed ones
+    const int band = (pb->cfg == TILE_128x128_ENH) ? 12 : 0;
     const int split = pb->sparse ? 0 : h->tail_split;
     if (h->items_key_np[L] != pb->Np || h->items_key_cfg[L] != pb->cfg || h->items_key_split[L] != split) {
         std::vector<WorkItem> list;
@@ -426,6 +479,7 @@ static LayerParams layer_params(sp2_handle_s* h, const Problem& pb, int parity, 
     p.bn_cur = pb.sparse ? h->bn[parity] : nullptr; p.bn_next = pb.sparse ? h->bn[parity ^ 1] : nullptr;
     p.nb = pb.Np / 128;
     p.scale = pb.scale; p.inv_scale2 = pb.inv_scale2; p.cond_handle = cond; p.round_sync = h->round_sync; p.round_spins = h->round_spins; p.enh_kc = pb.enh_kc;
+    p.ki_edge = h->ki_edge; p.ki_mid = h->ki_mid;
     return p;
 }
 

@@ -80,6 +80,8 @@ struct LayerParams {
     float scale;                   // c = 2^k of the split
     float inv_scale2;              // 1 / c^2
     int enh_kc;                    // enhanced accumulation: K-blocks (of 64) per tensor-core accumulation chunk
+    int ki_edge, ki_mid;           // K-interleave of the two rounds of an epoch (see ki_range): K-blocks per chunk at both
+                                   // ends of K and in between; ki_edge = 0: one tile after the other
     int round_sync;                // 1: producers of all CTAs meet at every round boundary (keeps the wave in lockstep)
     unsigned int round_spins;      // bound of that wait in 64 ns sleeps (a CTA that is not co-resident must not hang it)
     unsigned long long cond_handle;  // cudaGraphConditionalHandle (0 = none)

@@ -99,13 +99,42 @@ __device__ __forceinline__ bool layer_barrier(Ctrl* ctrl, int target, int lane) 
     return run != 0;
 }
 
+
+// K-interleave of two consecutive rounds (an EPOCH): a CTA (pair) holds two accumulators in TMEM, so it can walk K
+// for its tile of round 2e (accumulator 0) and its tile of round 2e+1 (accumulator 1) in alternating chunks of
+// K-blocks instead of one tile after the other.  All CTAs do so in lockstep (round sync at every chunk), which makes
+// the 2 x n_slots tiles of an epoch share their operand panels through L2: a panel is fetched from HBM once per
+// epoch, not once per round.  The chunks at both ends of K are longer (ki_edge K-blocks) than the ones in between
+// (ki_mid): the epilogue of the first tile runs under the second tile's last chunk, the epilogue of the second one
+// under the next epoch's first chunk.  Per tile the K order is unchanged (monotonic), so results do not depend on
+// the chunking.  Chunk c of nchunks covers K-blocks [kb0, kb1).
+__device__ __forceinline__ int ki_nchunks(int KB, int edge, int mid) {
+    if (edge <= 0 || mid <= 0 || KB <= 2 * edge) return (edge > 0 && KB > edge) ? 2 : 1;
+    return 2 + (KB - 2 * edge + mid - 1) / mid;
+}
+__device__ __forceinline__ void ki_range(int c, int nchunks, int KB, int edge, int mid, int& kb0, int& kb1) {
+    if (nchunks == 1) { kb0 = 0; kb1 = KB; return; }
+    if (nchunks == 2) { kb0 = c == 0 ? 0 : KB / 2; kb1 = c == 0 ? KB / 2 : KB; return; }
+    if (c == 0) { kb0 = 0; kb1 = edge; return; }
+    if (c == nchunks - 1) { kb0 = KB - edge; kb1 = KB; return; }
+    kb0 = edge + (c - 1) * mid;
+    kb1 = kb0 + mid;
+    if (kb1 > KB - edge) kb1 = KB - edge;
+}
+
 #ifdef SP2_LAYER_TIMING
 // experiment builds only: per CTA {globaltimer at entry, after setup, first accumulator ready, last epilogue done, exit}
 __device__ unsigned long long g_layer_timing[160 * 8];
 extern "C" void sp2_debug_layer_timing(unsigned long long* out) { cudaMemcpyFromSymbol(out, g_layer_timing, 160 * 8 * 8); }
 #define LT_MARK(i) do { if (blockIdx.x < 160) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); g_layer_timing[blockIdx.x * 8 + (i)] = t_; } } while (0)
+#define LT_ADD(i, v) do { if (blockIdx.x < 160) g_layer_timing[blockIdx.x * 8 + (i)] += (unsigned long long)(v); } while (0)
+#define LT_CLK() clock64()
+#define LT_ZERO(i) do { if (blockIdx.x < 160) g_layer_timing[blockIdx.x * 8 + (i)] = 0ull; } while (0)
 #else
 #define LT_MARK(i) do { } while (0)
+#define LT_ADD(i, v) do { } while (0)
+#define LT_CLK() 0ll
+#define LT_ZERO(i) do { } while (0)
 #endif
 
 template <class C>
@@ -122,7 +151,7 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi0, const __grid_constant__ 
         return;
     }
 
-    if (threadIdx.x == 64) LT_MARK(0);
+    if (threadIdx.x == 64) { LT_MARK(0); LT_ZERO(5); LT_ZERO(6); LT_ZERO(7); }
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + STAGES * C::STAGE_BYTES);
@@ -217,68 +246,106 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi0, const __grid_constant__ 
             uint32_t ph = 0;
             const uint64_t pol = l2_policy_evict_last();     // operand panels: reused by the other CTAs of the wave
             // Round sync: the CTAs of a round share row panels through L2 only while they walk K together.  Nothing
-            // else keeps them together (each runs its tiles back to back), so every producer checks in at each round
-            // boundary and starts the next tile's loads when all have (bounded spin: never a hang, at worst no sync).
-            // The counter is monotonic over a solve (every CTA checks in exactly n_rounds - 1 times per layer), so the
-            // targets of layer n + 1 start at n (n_rounds - 1) gridDim.x and a late check-in of the previous layer
-            // can never be lost to a reset.
+            // else keeps them together (each runs its tiles back to back), so every producer checks in at each sync
+            // point (round boundary; with the K-interleave every chunk boundary) and goes on when all have (bounded
+            // spin: never a hang, at worst no sync).  The counter is monotonic over a solve (every CTA checks in
+            // exactly n_sync times per layer), so the targets of layer n + 1 start at n n_sync gridDim.x and a late
+            // check-in of the previous layer can never be lost to a reset.
             const int n_rounds = (n_work + nslots - 1) / nslots;
+            const bool kint = !C::ENH && p.ki_edge > 0;
+            const int nchunks = kint ? ki_nchunks(KB, p.ki_edge, p.ki_mid) : 1;
+            const int n_epochs = (n_rounds + 1) >> 1;
+            const unsigned int n_sync = kint ? (unsigned int)(n_epochs * nchunks - 1) : (unsigned int)(n_rounds - 1);
+            auto sync_point = [&](unsigned int q, bool wait) {      // q = 1 .. n_sync within the layer
+                atomicAdd(&ctrl->round_counter, 1u);
+                if (wait && *((volatile unsigned int*)&ctrl->round_sync_broken) == 0u) {
+                    const unsigned int target = q * gridDim.x;
+                    unsigned int spins = 0;
+                    while (*((volatile unsigned int*)&ctrl->round_counter) < target && ++spins < p.round_spins)
+                        __nanosleep(64);
+                    // timed out: the grid is not co-resident (shared GPU); the sync is only an optimisation, so
+                    // give it up for the rest of this solve instead of paying the timeout at every boundary
+                    if (spins >= p.round_spins) ctrl->round_sync_broken = 1u;
+                }
+            };
             for (int layer = 0;; ++layer) {
             const CUtensorMap* tmh = (layer & 1) ? &tm_hi1 : &tm_hi0;
             const CUtensorMap* tml = (layer & 1) ? &tm_lo1 : &tm_lo0;
-            const unsigned int base = (unsigned int)(n_at_entry + layer) * (unsigned int)(n_rounds - 1);
-            int round = 0;
-            for (int w = slot; ; w += nslots, ++round) {
-                if (p.round_sync && round > 0 && round < n_rounds) {
-                    __threadfence();
-                    atomicAdd(&ctrl->round_counter, 1u);
-                    if (w < n_work && *((volatile unsigned int*)&ctrl->round_sync_broken) == 0u) {
-                        const unsigned int target = (base + (unsigned int)round) * gridDim.x;
-                        unsigned int spins = 0;
-                        while (*((volatile unsigned int*)&ctrl->round_counter) < target && ++spins < p.round_spins)
-                            __nanosleep(64);
-                        // timed out: the grid is not co-resident (shared GPU); the sync is only an optimisation, so
-                        // give it up for the rest of this solve instead of paying the timeout at every boundary
-                        if (spins >= p.round_spins) ctrl->round_sync_broken = 1u;
+            const unsigned int base = (unsigned int)(n_at_entry + layer) * n_sync;
+            auto load_stage = [&](int k0, int m0, int n0) {
+                mbar_wait(&empty_bar[s], ph ^ 1u);
+                uint8_t* st = smem + s * C::STAGE_BYTES;
+                if (CG == 1) {
+                    mbar_arrive_expect_tx(&full_bar[s], C::STAGE_BYTES);
+                    tma_load_2d_hint(st, tmh, &full_bar[s], k0, m0, pol);
+                    tma_load_2d_hint(st + C::A_BYTES, tml, &full_bar[s], k0, m0, pol);
+#pragma unroll
+                    for (int h = 0; h < C::BNL / 128; ++h) {
+                        tma_load_2d_hint(st + 2 * C::A_BYTES + h * 16384, tmh, &full_bar[s], k0, n0 + h * 128, pol);
+                        tma_load_2d_hint(st + 2 * C::A_BYTES + C::B_BYTES + h * 16384, tml, &full_bar[s], k0,
+                                         n0 + h * 128, pol);
+                    }
+                } else {
+                    // both CTAs' loads complete_tx on the leader's barrier; only the leader arrives (a peer
+                    // load landing first just leaves the transaction count negative until the expect_tx)
+                    if (rank == 0) mbar_arrive_expect_tx(&full_bar[s], 2 * C::STAGE_BYTES);
+                    tma_load_2d_pair_hint(st, tmh, &full_bar[s], k0, m0, pol);
+                    tma_load_2d_pair_hint(st + C::A_BYTES, tml, &full_bar[s], k0, m0, pol);
+#pragma unroll
+                    for (int h = 0; h < C::BNL / 128; ++h) {
+                        tma_load_2d_pair_hint(st + 2 * C::A_BYTES + h * 16384, tmh, &full_bar[s], k0, n0 + h * 128,
+                                              pol);
+                        tma_load_2d_pair_hint(st + 2 * C::A_BYTES + C::B_BYTES + h * 16384, tml, &full_bar[s], k0,
+                                              n0 + h * 128, pol);
                     }
                 }
-                if (w >= n_work) break;
-                const WorkItem wi = p.items[w];
-                const int m0 = wi.I * BN + (wi.sub * CG + (int)rank) * BM;                 // A rows of this CTA
-                // B rows this CTA loads: its share of the item's ncols columns (always a full 128-row box per load:
-                // for a narrow tail item the rows beyond ncols / CG are loaded but not used by the MMA)
-                const int n0 = wi.J * BN + wi.col0 + (int)rank * (wi.ncols / CG);
-                for (int kb = 0; kb < KB; ++kb) {
-                    mbar_wait(&empty_bar[s], ph ^ 1u);
-                    uint8_t* st = smem + s * C::STAGE_BYTES;
-                    // odd rounds walk K backwards: the panels a CTA shares with the previous round (same band) are
-                    // still in L2 for the K-blocks that round finished with
-                    const int k0 = ((round & 1) ? (KB - 1 - kb) : kb) * BK;
-                    if (CG == 1) {
-                        mbar_arrive_expect_tx(&full_bar[s], C::STAGE_BYTES);
-                        tma_load_2d_hint(st, tmh, &full_bar[s], k0, m0, pol);
-                        tma_load_2d_hint(st + C::A_BYTES, tml, &full_bar[s], k0, m0, pol);
+                if (++s == STAGES) { s = 0; ph ^= 1u; }
+            };
+            if (kint) {
+                for (int e = 0; e < n_epochs; ++e) {
+                    int m0[2] = {0, 0}, n0[2] = {0, 0};
+                    bool has[2];
 #pragma unroll
-                        for (int h = 0; h < C::BNL / 128; ++h) {
-                            tma_load_2d_hint(st + 2 * C::A_BYTES + h * 16384, tmh, &full_bar[s], k0, n0 + h * 128, pol);
-                            tma_load_2d_hint(st + 2 * C::A_BYTES + C::B_BYTES + h * 16384, tml, &full_bar[s], k0,
-                                             n0 + h * 128, pol);
-                        }
-                    } else {
-                        // both CTAs' loads complete_tx on the leader's barrier; only the leader arrives (a peer
-                        // load landing first just leaves the transaction count negative until the expect_tx)
-                        if (rank == 0) mbar_arrive_expect_tx(&full_bar[s], 2 * C::STAGE_BYTES);
-                        tma_load_2d_pair_hint(st, tmh, &full_bar[s], k0, m0, pol);
-                        tma_load_2d_pair_hint(st + C::A_BYTES, tml, &full_bar[s], k0, m0, pol);
-#pragma unroll
-                        for (int h = 0; h < C::BNL / 128; ++h) {
-                            tma_load_2d_pair_hint(st + 2 * C::A_BYTES + h * 16384, tmh, &full_bar[s], k0, n0 + h * 128,
-                                                  pol);
-                            tma_load_2d_pair_hint(st + 2 * C::A_BYTES + C::B_BYTES + h * 16384, tml, &full_bar[s], k0,
-                                                  n0 + h * 128, pol);
+                    for (int t = 0; t < 2; ++t) {
+                        const int w = slot + (2 * e + t) * nslots;
+                        has[t] = w < n_work;
+                        if (has[t]) {
+                            const WorkItem wi = p.items[w];
+                            m0[t] = wi.I * BN + (wi.sub * CG + (int)rank) * BM;
+                            n0[t] = wi.J * BN + wi.col0 + (int)rank * (wi.ncols / CG);
                         }
                     }
-                    if (++s == STAGES) { s = 0; ph ^= 1u; }
+                    // odd epochs walk K backwards: the panels shared with the previous epoch (same band) are still in
+                    // L2 for the K-blocks that epoch finished with
+                    const bool back = (e & 1) != 0;
+                    for (int c = 0; c < nchunks; ++c) {
+                        const int q = e * nchunks + c;
+                        if (p.round_sync && q > 0) sync_point(base + (unsigned int)q, has[0]);
+                        int kb0, kb1;
+                        ki_range(back ? nchunks - 1 - c : c, nchunks, KB, p.ki_edge, p.ki_mid, kb0, kb1);
+#pragma unroll
+                        for (int t = 0; t < 2; ++t) {
+                            if (!has[t]) continue;
+                            for (int i = 0; i < kb1 - kb0; ++i)
+                                load_stage((back ? kb1 - 1 - i : kb0 + i) * BK, m0[t], n0[t]);
+                        }
+                    }
+                }
+            } else {
+                int round = 0;
+                for (int w = slot; ; w += nslots, ++round) {
+                    if (p.round_sync && round > 0 && round < n_rounds) sync_point(base + (unsigned int)round, w < n_work);
+                    if (w >= n_work) break;
+                    const WorkItem wi = p.items[w];
+                    const int m0 = wi.I * BN + (wi.sub * CG + (int)rank) * BM;                 // A rows of this CTA
+                    // B rows this CTA loads: its share of the item's ncols columns (always a full 128-row box per load:
+                    // for a narrow tail item the rows beyond ncols / CG are loaded but not used by the MMA)
+                    const int n0 = wi.J * BN + wi.col0 + (int)rank * (wi.ncols / CG);
+                    // the K direction alternates per PAIR of rounds, as with the K-interleave (so that switching the
+                    // interleave off leaves every tile's summation order, hence every bit of the result, unchanged);
+                    // the enhanced-accumulation layers have no interleave and alternate per round
+                    const bool back = C::ENH ? ((round & 1) != 0) : (((round >> 1) & 1) != 0);
+                    for (int kb = 0; kb < KB; ++kb) load_stage((back ? (KB - 1 - kb) : kb) * BK, m0, n0);
                 }
             }
             if (!p.persist || !layer_barrier_one(ctrl, n_at_entry + layer + 1)) break;
@@ -346,44 +413,91 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi0, const __grid_constant__ 
             int s = 0;
             uint32_t ph = 0;
             int it = 0;                                   // accumulator uses so far (one per item; per chunk if ENH)
-            for (int layer = 0;; ++layer) {
-            for (int w = slot; w < n_work; w += nslots) {
-                const uint32_t idesc = umma_idesc_f16(BM * CG, p.items[w].ncols);   // N = 256, or 128 / 64 in the tail
-                const int KC = p.enh_kc;                  // K-blocks per accumulation chunk (ENH)
-                const int nch = C::ENH ? (KB + KC - 1) / KC : 1;
-                for (int ch = 0; ch < nch; ++ch, ++it) {
-                    const int buf = it & 1;
-                    const uint32_t use = (uint32_t)(it >> 1);
-                    const int kb0 = C::ENH ? ch * KC : 0;
-                    const int kb1 = C::ENH ? (kb0 + KC < KB ? kb0 + KC : KB) : KB;
-                    mbar_wait(&tempty_bar[buf], (use & 1u) ^ 1u);   // epilogue has drained this accumulator
-                    tc_fence_after();
-                    const uint32_t d_tmem = tmem_base + (uint32_t)(buf * BN);
-                    for (int kb = kb0; kb < kb1; ++kb) {
-                        mbar_wait(&full_bar[s], ph);
-                        tc_fence_after();
-                        if (lane == 0) {
-                            const uint32_t a_hi = smem_u32(smem + s * C::STAGE_BYTES);
-                            const uint32_t a_lo = a_hi + C::A_BYTES;
-                            const uint32_t b_hi = a_hi + 2 * C::A_BYTES;
-                            const uint32_t b_lo = b_hi + C::B_BYTES;
+            // one pipeline stage: wait for the operands, 3 MMAs per K = 16 into d_tmem, release the stage; `first`: the
+            // tile's (or ENH chunk's) first stage overwrites the accumulator; `last`: signal the epilogue
+            auto mma_stage = [&](uint32_t d_tmem, uint32_t idesc, bool first, bool last, int buf) {
+                const long long t0_ = LT_CLK();
+                mbar_wait(&full_bar[s], ph);
+                if (lane == 0) LT_ADD(7, LT_CLK() - t0_);
+                tc_fence_after();
+                if (lane == 0) {
+                    const uint32_t a_hi = smem_u32(smem + s * C::STAGE_BYTES);
+                    const uint32_t a_lo = a_hi + C::A_BYTES;
+                    const uint32_t b_hi = a_hi + 2 * C::A_BYTES;
+                    const uint32_t b_lo = b_hi + C::B_BYTES;
 #pragma unroll
-                            for (int k = 0; k < BK / 16; ++k) {
-                                const uint64_t dah = umma_desc_sw128(a_hi + k * 32);
-                                const uint64_t dal = umma_desc_sw128(a_lo + k * 32);
-                                const uint64_t dbh = umma_desc_sw128(b_hi + k * 32);
-                                const uint64_t dbl = umma_desc_sw128(b_lo + k * 32);
-                                umma_f16<CG>(d_tmem, dah, dbh, idesc, (kb != kb0 || k != 0) ? 1u : 0u);   // X0 X0
-                                umma_f16<CG>(d_tmem, dah, dbl, idesc, 1u);                                // X0 X1
-                                umma_f16<CG>(d_tmem, dal, dbh, idesc, 1u);                                // (X0 X1)^T
+                    for (int k = 0; k < BK / 16; ++k) {
+                        const uint64_t dah = umma_desc_sw128(a_hi + k * 32);
+                        const uint64_t dal = umma_desc_sw128(a_lo + k * 32);
+                        const uint64_t dbh = umma_desc_sw128(b_hi + k * 32);
+                        const uint64_t dbl = umma_desc_sw128(b_lo + k * 32);
+                        umma_f16<CG>(d_tmem, dah, dbh, idesc, (!first || k != 0) ? 1u : 0u);      // X0 X0
+                        umma_f16<CG>(d_tmem, dah, dbl, idesc, 1u);                                // X0 X1
+                        umma_f16<CG>(d_tmem, dal, dbh, idesc, 1u);                                // (X0 X1)^T
+                    }
+                    if (CG == 1) umma_commit(&empty_bar[s]); else umma_commit_pair(&empty_bar[s], 0x3);
+                    if (last) {
+                        if (CG == 1) umma_commit(&tfull_bar[buf]); else umma_commit_pair(&tfull_bar[buf], 0x3);
+                    }
+                }
+                __syncwarp();
+                if (++s == STAGES) { s = 0; ph ^= 1u; }
+            };
+            const bool kint = !C::ENH && p.ki_edge > 0;
+            const int n_rounds = (n_work + nslots - 1) / nslots;
+            for (int layer = 0;; ++layer) {
+            if (kint) {
+                // K-interleave: the tiles of rounds 2e and 2e + 1 advance through K in alternating chunks (see ki_range);
+                // the order of (epoch, chunk, tile, K-block) is the producer's
+                const int nchunks = ki_nchunks(KB, p.ki_edge, p.ki_mid);
+                const int n_epochs = (n_rounds + 1) >> 1;
+                for (int e = 0; e < n_epochs; ++e) {
+                    bool has[2];
+                    uint32_t idesc[2] = {0u, 0u};
+#pragma unroll
+                    for (int t = 0; t < 2; ++t) {
+                        const int w = slot + (2 * e + t) * nslots;
+                        has[t] = w < n_work;
+                        if (has[t]) idesc[t] = umma_idesc_f16(BM * CG, p.items[w].ncols);
+                    }
+                    const bool back = (e & 1) != 0;
+                    for (int c = 0; c < nchunks; ++c) {
+                        int kb0, kb1;
+                        ki_range(back ? nchunks - 1 - c : c, nchunks, KB, p.ki_edge, p.ki_mid, kb0, kb1);
+#pragma unroll
+                        for (int t = 0; t < 2; ++t) {
+                            if (!has[t]) continue;
+                            const int itt = it + t;
+                            const int buf = itt & 1;
+                            if (c == 0) {                               // epilogue has drained this accumulator
+                                const long long t0_ = LT_CLK();
+                                mbar_wait(&tempty_bar[buf], ((uint32_t)(itt >> 1) & 1u) ^ 1u);
+                                if (lane == 0) LT_ADD(6, LT_CLK() - t0_);
+                                tc_fence_after();
                             }
-                            if (CG == 1) umma_commit(&empty_bar[s]); else umma_commit_pair(&empty_bar[s], 0x3);
-                            if (kb == kb1 - 1) {
-                                if (CG == 1) umma_commit(&tfull_bar[buf]); else umma_commit_pair(&tfull_bar[buf], 0x3);
-                            }
+                            const uint32_t d_tmem = tmem_base + (uint32_t)(buf * BN);
+                            for (int i = 0; i < kb1 - kb0; ++i)
+                                mma_stage(d_tmem, idesc[t], c == 0 && i == 0, c == nchunks - 1 && i == kb1 - kb0 - 1, buf);
                         }
-                        __syncwarp();
-                        if (++s == STAGES) { s = 0; ph ^= 1u; }
+                    }
+                    it += (has[0] ? 1 : 0) + (has[1] ? 1 : 0);
+                }
+            } else {
+                for (int w = slot; w < n_work; w += nslots) {
+                    const uint32_t idesc = umma_idesc_f16(BM * CG, p.items[w].ncols);   // N = 256, or 128 / 64 in the tail
+                    const int KC = p.enh_kc;                  // K-blocks per accumulation chunk (ENH)
+                    const int nch = C::ENH ? (KB + KC - 1) / KC : 1;
+                    for (int ch = 0; ch < nch; ++ch, ++it) {
+                        const int buf = it & 1;
+                        const uint32_t use = (uint32_t)(it >> 1);
+                        const int kb0 = C::ENH ? ch * KC : 0;
+                        const int kb1 = C::ENH ? (kb0 + KC < KB ? kb0 + KC : KB) : KB;
+                        const long long t0_ = LT_CLK();
+                        mbar_wait(&tempty_bar[buf], (use & 1u) ^ 1u);   // epilogue has drained this accumulator
+                        if (lane == 0) LT_ADD(6, LT_CLK() - t0_);
+                        tc_fence_after();
+                        const uint32_t d_tmem = tmem_base + (uint32_t)(buf * BN);
+                        for (int kb = kb0; kb < kb1; ++kb) mma_stage(d_tmem, idesc, kb == kb0, kb == kb1 - 1, buf);
                     }
                 }
             }
@@ -503,6 +617,7 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi0, const __grid_constant__ 
             mbar_wait(&tfull_bar[buf], use & 1u);
             tc_fence_after();
             if (threadIdx.x == 64 && w == slot) LT_MARK(2);
+            const long long te0_ = LT_CLK();
             const uint32_t taddr = tmem_base + (uint32_t)(buf * BN) + lane_off;
             unsigned short* HOu = reinterpret_cast<unsigned short*>(HO);
             unsigned short* LOu = reinterpret_cast<unsigned short*>(LO);
@@ -679,6 +794,7 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi0, const __grid_constant__ 
             if (lane == 0) {
                 if (CG == 1) mbar_arrive(&tempty_bar[buf]); else mbar_arrive_cluster(&tempty_bar[buf], 0);
             }
+            if (threadIdx.x == 64) LT_ADD(5, LT_CLK() - te0_);
             if (sp_zero_out) {
                 if (warp == 2 && lane == 0) {
                     const unsigned long long v = (unsigned long long)(sp_zc < 3 ? sp_zc + 1 : 3) << 62;

@@ -335,6 +335,32 @@ def test_round_sync_timeout_path_gives_the_same_bits(env, monkeypatch):
         assert torch.equal(D0, D1) and i0["trace_S"] == i1["trace_S"] and i0["sigma"] == i1["sigma"]
 
 
+@pytest.mark.parametrize("n,tile", [(3000, 1), (3000, 3), (4500, 1), (5000, 3)])
+def test_k_interleave_chunking_gives_the_same_bits(env, monkeypatch, n, tile):
+    """The K-interleave of the layer kernel (the two rounds of an epoch walk K in alternating chunks so that their
+    operand panels are shared through L2; SP2_K_INTERLEAVE = edge[:mid] K-blocks per chunk, read at sp2_create) only
+    changes WHEN a tile's MMAs are issued, never their order within the tile: off (one tile after the other), the
+    default chunking and two odd chunkings (chunks that do not divide K, more chunks than K-blocks at one end) must
+    give identical bits.  Several epochs, a partial last epoch (a first tile without a second one), pair and
+    single-CTA tiles, ragged N."""
+    api, h, torch = env
+    w = W.gapped_dense(n + 5, n, (-1.0, -0.15), (0.15, 1.0), n // 2, "ki", bounds=(-1.0, 1.0))
+    Hd = torch.from_numpy(w.H32).cuda()
+    opts = api.make_opts(bounds=w.bounds, tol=1e-5, max_layers=100, tile_config=tile)
+    h0 = api.Handle(n, 0, 100)
+    D0, i0 = h0.density_matrix(Hd, w.N_occ, opts)                      # default chunking
+    h0.close()
+    for ki in ("0", "5:3", "40:7", "1000"):
+        monkeypatch.setenv("SP2_K_INTERLEAVE", ki)
+        h2 = api.Handle(n, 0, 100)
+        monkeypatch.delenv("SP2_K_INTERLEAVE")
+        D1, i1 = h2.density_matrix(Hd, w.N_occ, opts)
+        h2.close()
+        assert torch.equal(D0, D1), ki
+        assert i0["trace_S"] == i1["trace_S"] and i0["trace_X_diag"] == i1["trace_X_diag"] and i0["sigma"] == i1["sigma"], ki
+    P.assert_acceptance(D0.cpu().numpy().astype(np.float64), O.closed_form_density(w.Q, w.N_occ), w.N_occ, f"N={n}")
+
+
 def test_nonfinite_input_and_unsupported_mix_tile(env):
     """A NaN in H must surface as SP2_ERR_NONFINITE from every single-matrix entry point (standard and generalized,
     caller and Gershgorin bounds); the output mix has no enhanced-accumulation instantiation -> SP2_ERR_INVALID_ARG."""
