@@ -149,22 +149,35 @@ __global__ void __launch_bounds__(256) k_gershgorin_finalize(const float* __rest
         if ((threadIdx.x & 31) == 0) { smin[threadIdx.x >> 5] = bad ? NAN : lo; smax[threadIdx.x >> 5] = bad ? NAN : hi; }
     }
     __syncthreads();
+    __shared__ unsigned int s_last;
     if (threadIdx.x == 0) {
-        bool nan = isnan(smin[0]) || isnan(smin[1]);
+        const bool nan = isnan(smin[0]) || isnan(smin[1]);
         lo = fmin(smin[0], smin[1]); hi = fmax(smax[0], smax[1]);
         ctrl->partial[blockIdx.x][0] = nan ? NAN : lo;
         ctrl->partial[blockIdx.x][1] = nan ? NAN : hi;
         __threadfence();
-        const unsigned int done = atomicAdd(&ctrl->done_counter, 1u);
-        if (done == gridDim.x - 1) {
-            __threadfence();
-            nan = false;
-            lo = INFINITY; hi = -INFINITY;
-            for (unsigned int b = 0; b < gridDim.x; ++b) {
-                const double l = ((volatile double*)ctrl->partial[b])[0], h = ((volatile double*)ctrl->partial[b])[1];
-                nan = nan || isnan(l);
-                lo = fmin(lo, l); hi = fmax(hi, h);
-            }
+        s_last = (atomicAdd(&ctrl->done_counter, 1u) == gridDim.x - 1) ? 1u : 0u;
+    }
+    __syncthreads();
+    if (s_last != 0u && threadIdx.x < 32) {
+        // last block: extrema over the blocks by one warp (strided loads, shuffle tree; min / max are exact, so any order
+        // gives the same bits).  A serial loop of FP64 compares here cost more than the whole row pass (isolated FP64
+        // instructions pay the datapath wake-up, see sp2_control.cuh).
+        __threadfence();
+        bool nan = false;
+        lo = INFINITY; hi = -INFINITY;
+        for (unsigned int b = threadIdx.x; b < gridDim.x; b += 32) {
+            const double l = __ldcg(&ctrl->partial[b][0]), h = __ldcg(&ctrl->partial[b][1]);
+            nan = nan || isnan(l) || isnan(h);
+            lo = fmin(lo, l); hi = fmax(hi, h);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            lo = fmin(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+            hi = fmax(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+        }
+        nan = __any_sync(0xffffffffu, nan);
+        if (threadIdx.x == 0) {
             ctrl->eps_min = nan ? NAN : lo;
             ctrl->eps_max = nan ? NAN : hi;
             ctrl->launches += 2;
@@ -310,6 +323,7 @@ __global__ void __launch_bounds__(256, 4) k_affine_split(const float* __restrict
     double fro2 = warp_sum(2.0 * off2 + dg2);
     if ((threadIdx.x & 31) == 0) { red[threadIdx.x >> 5][0] = trS; red[threadIdx.x >> 5][1] = fro2; }
     __syncthreads();
+    __shared__ unsigned int s_last;
     if (threadIdx.x == 0) {
         double a = 0.0, b = 0.0;
         for (int w = 0; w < 8; ++w) { a += red[w][0]; b += red[w][1]; }
@@ -317,14 +331,20 @@ __global__ void __launch_bounds__(256, 4) k_affine_split(const float* __restrict
         ctrl->partial[blockIdx.x][1] = b;
         ctrl->partial[blockIdx.x][2] = 0.0;
         __threadfence();
-        const unsigned int done = atomicAdd(&ctrl->done_counter, 1u);
-        if (done == gridDim.x - 1) {
-            __threadfence();
-            double s0 = 0.0, s1 = 0.0;
-            for (unsigned int i = 0; i < gridDim.x; ++i) {
-                s0 += ((volatile double*)ctrl->partial[i])[0];
-                s1 += ((volatile double*)ctrl->partial[i])[1];
-            }
+        s_last = (atomicAdd(&ctrl->done_counter, 1u) == gridDim.x - 1) ? 1u : 0u;
+    }
+    __syncthreads();
+    if (s_last != 0u && threadIdx.x < 32) {
+        // last block: one warp sums the per-block partials (lane l takes blocks l, l + 32, ... in order, then a fixed
+        // shuffle tree: bit-reproducible) -- a serial FP64 loop over ~600 blocks took ~15 % of the kernel
+        __threadfence();
+        double s0 = 0.0, s1 = 0.0;
+        for (unsigned int i = threadIdx.x; i < gridDim.x; i += 32) {
+            s0 += __ldcg(&ctrl->partial[i][0]);
+            s1 += __ldcg(&ctrl->partial[i][1]);
+        }
+        s0 = warp_sum(s0); s1 = warp_sum(s1);
+        if (threadIdx.x == 0) {
             // N_S = Tr[S_0]; the control works in 2^40 fixed point (sp2_control.cuh)
             const bool fin = isfinite(s0) && isfinite(s1) && fabs(s0) < 4.0e6 && s1 < 4.0e6;
             ctrl->N_S = fin ? __double2ll_rn(s0 * kFxScale) : 0;
@@ -397,11 +417,16 @@ __global__ void __launch_bounds__(256) k_energy_traces(const float* __restrict__
         const int j = J * ET + c4;
         float eo = 0.f, fo = 0.f;                   // off-diagonal partial sums of this tile
         float cs[4] = {0.f, 0.f, 0.f, 0.f};         // squares per column (rows of the mirrored part)
+        float4 xt[4], ht[4];                        // all eight loads of the tile in flight before the first use
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            xt[k] = ld_tile4(X, N, ldx, I * ET + r0 + 16 * k, j, vx);
+            ht[k] = ld_tile4(H, N, ldh, I * ET + r0 + 16 * k, j, vh);
+        }
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
             const int i = I * ET + r0 + 16 * k;
-            const float4 x4 = ld_tile4(X, N, ldx, i, j, vx);
-            const float4 h4 = ld_tile4(H, N, ldh, i, j, vh);
+            const float4 x4 = xt[k], h4 = ht[k];
             const float xv[4] = {x4.x, x4.y, x4.z, x4.w}, hv[4] = {h4.x, h4.y, h4.z, h4.w};
             float rsq = 0.f;                        // row i: squares of its entries j <= i held by this thread
 #pragma unroll
@@ -439,6 +464,7 @@ __global__ void __launch_bounds__(256) k_energy_traces(const float* __restrict__
     e = warp_sum(e); tr = warp_sum(tr); f2 = warp_sum(f2);
     if ((threadIdx.x & 31) == 0) { red[threadIdx.x >> 5][0] = e; red[threadIdx.x >> 5][1] = tr; red[threadIdx.x >> 5][2] = f2; }
     __syncthreads();
+    __shared__ unsigned int s_last;
     if (threadIdx.x == 0) {
         double a = 0.0, b = 0.0, c = 0.0;
         for (int w = 0; w < 8; ++w) { a += red[w][0]; b += red[w][1]; c += red[w][2]; }
@@ -446,15 +472,19 @@ __global__ void __launch_bounds__(256) k_energy_traces(const float* __restrict__
         ctrl->partial[blockIdx.x][1] = b;
         ctrl->partial[blockIdx.x][2] = c;
         __threadfence();
-        const unsigned int done = atomicAdd(&ctrl->done_counter, 1u);
-        if (done == gridDim.x - 1) {
-            __threadfence();
-            double s0 = 0.0, s1 = 0.0, s2 = 0.0;
-            for (unsigned int i = 0; i < gridDim.x; ++i) {
-                s0 += ((volatile double*)ctrl->partial[i])[0];
-                s1 += ((volatile double*)ctrl->partial[i])[1];
-                s2 += ((volatile double*)ctrl->partial[i])[2];
-            }
+        s_last = (atomicAdd(&ctrl->done_counter, 1u) == gridDim.x - 1) ? 1u : 0u;
+    }
+    __syncthreads();
+    if (s_last != 0u && threadIdx.x < 32) {             // last block: one warp, fixed order (see k_affine_split)
+        __threadfence();
+        double s0 = 0.0, s1 = 0.0, s2 = 0.0;
+        for (unsigned int i = threadIdx.x; i < gridDim.x; i += 32) {
+            s0 += __ldcg(&ctrl->partial[i][0]);
+            s1 += __ldcg(&ctrl->partial[i][1]);
+            s2 += __ldcg(&ctrl->partial[i][2]);
+        }
+        s0 = warp_sum(s0); s1 = warp_sum(s1); s2 = warp_sum(s2);
+        if (threadIdx.x == 0) {
             out[0] = s0; out[1] = s1; out[2] = s2;
             ctrl->done_counter = 0;
             ctrl->launches += 1;
@@ -535,11 +565,24 @@ __global__ void __launch_bounds__(256) k_one_minus(const float* __restrict__ M, 
 }
 
 // ------------------------------------------------------------------------------------------------ launchers
+
+// Grid of a persistent tile kernel: as many blocks as are co-resident (one wave), so that the grid-stride loops end
+// together; more blocks than that run in waves and the last wave's blocks start late (k_copy_sym: 1184 blocks on 1036
+// resident slots cost 14 %).
+template <class K>
+static int resident_grid(K kernel, int threads, long long work, long long cap, int num_sms) {
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, 0) != cudaSuccess || per_sm < 1) per_sm = 1;
+    long long g = (long long)per_sm * num_sms;
+    if (cap > 0 && g > cap) g = cap;
+    if (g > work) g = work;
+    return (int)(g < 1 ? 1 : g);
+}
 cudaError_t launch_gershgorin(const float* H, int N, long long ldh, float* part, double* diag, Ctrl* ctrl,
                               int num_sms, cudaStream_t st) {
     const int nt = (N + ET - 1) / ET;
     const long long ntiles = (long long)nt * (nt + 1) / 2;
-    const int grid = (int)(ntiles < (long long)num_sms * 16 ? ntiles : (long long)num_sms * 16);
+    const int grid = resident_grid(k_gershgorin_rows, 256, ntiles, 0, num_sms);
     if (nt > kMaxPartials) return cudaErrorInvalidValue;
     k_gershgorin_rows<<<grid, 256, 0, st>>>(H, N, ldh, part, diag);
     k_gershgorin_finalize<<<nt, 256, 0, st>>>(part, diag, N, ctrl);
@@ -552,9 +595,7 @@ cudaError_t launch_affine_split(const float* H, int N, long long ldh, float* S, 
                                 int num_sms, cudaStream_t st) {
     const int nt = (N + ET - 1) / ET;
     const long long ntiles = (long long)nt * (nt + 1) / 2;
-    long long cap = (long long)num_sms * 4;
-    if (cap > kMaxPartials) cap = kMaxPartials;
-    const int grid = (int)(ntiles < cap ? ntiles : cap);
+    const int grid = resident_grid(k_affine_split, 256, ntiles, kMaxPartials, num_sms);
     k_affine_split<<<grid, 256, 0, st>>>(H, N, ldh, S, hi, lo, ld, ldf, scale, ctrl, stats, thetas, rowsq, mix, c0, bn, nb);
     return cudaGetLastError();
 }
@@ -579,8 +620,7 @@ namespace sp2 {
 cudaError_t launch_copy_sym(const float* S, long long ld, float* D, long long ldd, int N, int num_sms, cudaStream_t st) {
     const int nt = (N + ET - 1) / ET;
     const long long ntiles = (long long)nt * (nt + 1) / 2;
-    const long long cap = (long long)num_sms * 8;
-    k_copy_sym<<<(int)(ntiles < cap ? ntiles : cap), 256, 0, st>>>(S, ld, D, ldd, N);
+    k_copy_sym<<<resident_grid(k_copy_sym, 256, ntiles, 0, num_sms), 256, 0, st>>>(S, ld, D, ldd, N);
     return cudaGetLastError();
 }
 cudaError_t launch_one_minus(const float* M, long long ldm, float* F, long long ldo, int N, float d, int num_sms,
@@ -595,9 +635,7 @@ cudaError_t launch_energy_traces(const float* X, long long ldx, const float* H, 
                                  unsigned long long* rowsq, int num_sms, cudaStream_t st) {
     const int nt = (N + ET - 1) / ET;
     const long long ntiles = (long long)nt * (nt + 1) / 2;
-    long long cap = (long long)num_sms * 6;
-    if (cap > kMaxPartials) cap = kMaxPartials;
-    const int grid = (int)(ntiles < cap ? ntiles : cap);
+    const int grid = resident_grid(k_energy_traces, 256, ntiles, kMaxPartials, num_sms);
     k_energy_traces<<<grid, 256, 0, st>>>(X, ldx, H, ldh, N, ctrl, out, plan, stats, thetas, rowsq);
     return cudaGetLastError();
 }

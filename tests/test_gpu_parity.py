@@ -316,7 +316,8 @@ def test_persistent_launch_gives_the_graph_loop_bits(env, n, tile):
 def test_round_sync_timeout_path_gives_the_same_bits(env, monkeypatch):
     """The round synchronisation of the layer kernel is an optimisation with a bounded wait: when a wait runs out
     (CTAs not co-resident) the kernel gives the sync up for the rest of the solve.  Forced here with a wait bound of
-    one poll (SP2_ROUND_SYNC_SPINS, a performance toggle read at sp2_create): same bits as the synchronised run."""
+    one poll (SP2_ROUND_SYNC_SPINS, a performance toggle read at sp2_create) and a sync point every four K-blocks
+    (SP2_K_INTERLEAVE): same bits as the synchronised run."""
     api, h, torch = env
     n = 3000
     w = W.gapped_dense(11, n, (-1.0, -0.15), (0.15, 1.0), n // 2, "rs", bounds=(-1.0, 1.0))
@@ -326,8 +327,10 @@ def test_round_sync_timeout_path_gives_the_same_bits(env, monkeypatch):
         D0, i0 = h.density_matrix(Hd, w.N_occ, opts)
         assert h.lib.sp2_last_round_sync_broken(h._h) == 0
         monkeypatch.setenv("SP2_ROUND_SYNC_SPINS", "1")
-        h2 = api.Handle(n, 0, 100)
+        monkeypatch.setenv("SP2_K_INTERLEAVE", "4:4")      # a sync point every 4 K-blocks (the default chunking has
+        h2 = api.Handle(n, 0, 100)                          # none at this K; the bits do not depend on it)
         monkeypatch.delenv("SP2_ROUND_SYNC_SPINS")
+        monkeypatch.delenv("SP2_K_INTERLEAVE")
         D1, i1 = h2.density_matrix(Hd, w.N_occ, opts)
         broken = h2.lib.sp2_last_round_sync_broken(h2._h)
         h2.close()
