@@ -405,12 +405,12 @@ static int choose_tile_config(int N, int requested, int num_sms) {
     if (requested >= TILE_128x128 && requested <= TILE_128x128_ENH) return requested;
     const int n128 = round_up(N, 128) / 128;
     const long long t128 = (long long)n128 * (n128 + 1) / 2;
-    // 256x256 pair tiles once there are at least 1.5 rounds of them (N >= ~3800 on 148 SMs; measured at N = 4096:
-    // 195 us per layer against 224 us with 128x128 tiles), else 128x128 tiles (N = 2048: 136 tiles for 148 SMs)
-    const int n256 = round_up(N, 256) / 256;
-    const long long t256 = (long long)n256 * (n256 + 1) / 2;
-    if (2 * t256 >= 3LL * (num_sms / 2)) return TILE_256x256_PAIR;
-    (void)t128;
+    // 128 x 128 single-CTA tiles while they fit one round (N <= 2048 on 148 SMs: 136 tiles), 256 x 256 pair tiles as soon
+    // as they would need a second one.  An MMA with N = 128 does not run faster than one with N = 256 (measured issue
+    // interval ~117 cycles against 128: DESIGN.md section 6), so small tiles only pay while they put more SMs to work.
+    // Measured us per layer, tile 1 / tile 3: N = 2048: 51.8 / 68.7, 2304: 74.8 / 71.0, 2816: 90.7 / 82.7,
+    // 3072: 124.9 / 109.8, 3584: 162.8 / 150.7, 4096: 242.1 / 199.1.
+    if (t128 > (long long)num_sms) return TILE_256x256_PAIR;
     return TILE_128x128;
 }
 
