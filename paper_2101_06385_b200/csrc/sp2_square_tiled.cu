@@ -40,7 +40,14 @@ struct TileCfg {
     static constexpr int STAGE_BYTES = 2 * A_BYTES + 2 * B_BYTES;   // hi and lo of both panels
     static constexpr int STAGES = (STAGE_BYTES > 65536) ? 2 : 3;
     static constexpr int SUB = (BN / BM) / CG;     // 128-row work items per supertile per CTA slot
-    static constexpr int TMEM_COLS = ENH ? 4 * BN : 2 * BN;   // two accumulator buffers (+ running hi, lo)
+    // CAT (128 x 128 single-CTA tiles): the hi and lo tiles of the B rows lie one behind the other in a stage, so ONE MMA
+    // with N = 256 over both gives [X0 X0 | X0 X1] in a 256-column accumulator; a second one with N = 128 adds
+    // (X0 X1)^T = X1 X0 to the left half, and the epilogue adds the two halves.  An MMA with N = 128 occupies the tensor
+    // pipe for 64 cycles but the measured issue interval is ~117 (N = 256: 128 cycles, no gap), so three of them per
+    // K = 16 cost ~350 cycles against ~245 for one of each.
+    static constexpr bool CAT = (BN_ == 128) && (CG_ == 1) && !ENH_;
+    static constexpr int ACC_COLS = CAT ? 2 * BN : BN;       // TMEM columns of one accumulator buffer
+    static constexpr int TMEM_COLS = ENH ? 4 * BN : 2 * ACC_COLS;   // two accumulator buffers (+ running hi, lo)
     static_assert(TMEM_COLS <= 512, "TMEM has 512 columns");
     static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*align*/ + 256 /*barriers*/;
     // warp 0 = TMA producer, warp 1 = MMA issuer, then EPI_WARPS epilogue warps: EPI_WARPS / 4 per TMEM lane quarter,
@@ -371,7 +378,7 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi0, const __grid_constant__ 
             const int buf = it & 1;
             mbar_wait(&tempty_bar[buf], ((uint32_t)(it >> 1) & 1u) ^ 1u);
             tc_fence_after();
-            const uint32_t d_tmem = tmem_base + (uint32_t)(buf * BN);
+            const uint32_t d_tmem = tmem_base + (uint32_t)(buf * C::ACC_COLS);
             bool fresh = true;                                  // the tile's first MMA overwrites the accumulator
             for (int kk = 0; kk < p.nb; ++kk) {
                 if (!sparse_bit(m, kk)) continue;
@@ -390,9 +397,11 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi0, const __grid_constant__ 
                             const uint64_t dal = umma_desc_sw128(a_lo + k * 32);
                             const uint64_t dbh = umma_desc_sw128(b_hi + k * 32);
                             const uint64_t dbl = umma_desc_sw128(b_lo + k * 32);
-                            umma_f16<1>(d_tmem, dah, dbh, idesc, (fresh && k == 0) ? 0u : 1u);
-                            umma_f16<1>(d_tmem, dah, dbl, idesc, 1u);
+                            // [X0 X0 | X0 X1] with one N = 256 MMA over the adjacent hi and lo tiles of the B rows, then
+                            // X1 X0 into the left half (TileCfg::CAT)
+                            umma_f16<1>(d_tmem, dah, dbh, umma_idesc_f16(BM, 2 * BN), (fresh && k == 0) ? 0u : 1u);
                             umma_f16<1>(d_tmem, dal, dbh, idesc, 1u);
+                            (void)dbl;
                         }
                         umma_commit(&empty_bar[s]);
                     }
@@ -434,9 +443,17 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi0, const __grid_constant__ 
                         const uint64_t dal = umma_desc_sw128(a_lo + k * 32);
                         const uint64_t dbh = umma_desc_sw128(b_hi + k * 32);
                         const uint64_t dbl = umma_desc_sw128(b_lo + k * 32);
-                        umma_f16<CG>(d_tmem, dah, dbh, idesc, (!first || k != 0) ? 1u : 0u);      // X0 X0
-                        umma_f16<CG>(d_tmem, dah, dbl, idesc, 1u);                                // X0 X1
-                        umma_f16<CG>(d_tmem, dal, dbh, idesc, 1u);                                // (X0 X1)^T
+                        if (C::CAT) {
+                            // B_hi and B_lo are adjacent 128-row tiles: [X0 X0 | X0 X1] in one N = 256 MMA (whatever the
+                            // item's ncols: a strip's unused columns are computed and ignored), then X1 X0 on the left
+                            umma_f16<CG>(d_tmem, dah, dbh, umma_idesc_f16(BM, 2 * BN), (!first || k != 0) ? 1u : 0u);
+                            umma_f16<CG>(d_tmem, dal, dbh, umma_idesc_f16(BM, BN), 1u);
+                            (void)dbl;
+                        } else {
+                            umma_f16<CG>(d_tmem, dah, dbh, idesc, (!first || k != 0) ? 1u : 0u);      // X0 X0
+                            umma_f16<CG>(d_tmem, dah, dbl, idesc, 1u);                                // X0 X1
+                            umma_f16<CG>(d_tmem, dal, dbh, idesc, 1u);                                // (X0 X1)^T
+                        }
                     }
                     if (CG == 1) umma_commit(&empty_bar[s]); else umma_commit_pair(&empty_bar[s], 0x3);
                     if (last) {
@@ -478,7 +495,7 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi0, const __grid_constant__ 
                                 if (lane == 0) LT_ADD(6, LT_CLK() - t0_);
                                 tc_fence_after();
                             }
-                            const uint32_t d_tmem = tmem_base + (uint32_t)(buf * BN);
+                            const uint32_t d_tmem = tmem_base + (uint32_t)(buf * C::ACC_COLS);
                             for (int i = 0; i < kb1 - kb0; ++i)
                                 mma_stage(d_tmem, idesc[t], c == 0 && i == 0, c == nchunks - 1 && i == kb1 - kb0 - 1, buf);
                         }
@@ -499,7 +516,7 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi0, const __grid_constant__ 
                         mbar_wait(&tempty_bar[buf], (use & 1u) ^ 1u);   // epilogue has drained this accumulator
                         if (lane == 0) LT_ADD(6, LT_CLK() - t0_);
                         tc_fence_after();
-                        const uint32_t d_tmem = tmem_base + (uint32_t)(buf * BN);
+                        const uint32_t d_tmem = tmem_base + (uint32_t)(buf * C::ACC_COLS);
                         for (int kb = kb0; kb < kb1; ++kb) mma_stage(d_tmem, idesc, kb == kb0, kb == kb1 - 1, buf);
                     }
                 }
@@ -621,7 +638,7 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi0, const __grid_constant__ 
             tc_fence_after();
             if (threadIdx.x == 64 && w == slot) LT_MARK(2);
             const long long te0_ = LT_CLK();
-            const uint32_t taddr = tmem_base + (uint32_t)(buf * BN) + lane_off;
+            const uint32_t taddr = tmem_base + (uint32_t)(buf * C::ACC_COLS) + lane_off;
             unsigned short* HOu = reinterpret_cast<unsigned short*>(HO);
             unsigned short* LOu = reinterpret_cast<unsigned short*>(LO);
 #pragma unroll 1
@@ -636,6 +653,13 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi0, const __grid_constant__ 
                     for (int c = 0; c < 32; ++c) v[c] = 0u;
                 } else {
                     tmem_ld_32x32(taddr + (uint32_t)c0, v);
+                    if (C::CAT) {                           // X0 X1 lies 128 columns to the right of X0 X0 + X1 X0
+                        uint32_t v2[32];
+                        tmem_ld_32x32(taddr + (uint32_t)(BN + c0), v2);
+                        tmem_ld_wait();
+#pragma unroll
+                        for (int c = 0; c < 32; ++c) v[c] = __float_as_uint(__uint_as_float(v[c]) + __uint_as_float(v2[c]));
+                    }
                 }
                 if (C::ENH && nch > 1) {
                     // last chunk: total = running pair + this chunk, rounded once to FP32

@@ -49,7 +49,9 @@ def test_tensor_core_accumulation_shrinks_the_off_diagonal_part(cuda_device):
     print("off-diagonal shrink factor beta of one layer (plain | enhanced accumulation): "
           + ", ".join(f"N={n}: {betas[(n, 1)]:+.2e} | {betas[(n, 4)]:+.2e}" for n in (640, 2048)))
     assert -2e-5 < betas[(2048, 1)] < betas[(640, 1)] < -5e-7         # truncation: negative, growing with K
-    assert abs(betas[(2048, 4)]) < 0.1 * abs(betas[(2048, 1)])        # chunked accumulation removes it
+    # chunked accumulation removes it (measured -4.4e-7 against -4.1e-6; -6.2e-6 before the 128 x 128 tiles kept X0 X1 in
+    # an accumulator of its own, which shortens the chain of truncating adds behind the dominant term by a third)
+    assert abs(betas[(2048, 4)]) < 0.15 * abs(betas[(2048, 1)])
     h.close()
 
 
