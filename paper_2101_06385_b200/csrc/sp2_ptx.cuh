@@ -60,6 +60,16 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
     }
 }
 
+// One thread of a (converged) warp: elect.sync inside warp-uniform control flow.  Unlike `if (lane == 0)` -- a divergent
+// branch to the compiler, which then wraps every instruction that takes uniform-register operands (tcgen05.mma,
+// cp.async.bulk.tensor) in a loop of R2UR.BROADCASTs: measured 105 cycles per MMA of 64 (tests/cuda/mma_rate.cu) -- the
+// elected thread's operands are moved to uniform registers directly.
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred = 0;
+    asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}\n" : "=r"(pred));
+    return pred != 0;
+}
+
 // ---------------------------------------------------------------- TMA
 __device__ __forceinline__ void tma_prefetch_desc(const void* tmap) {
     asm volatile("prefetch.tensormap [%0];\n" ::"l"(tmap) : "memory");

@@ -250,8 +250,9 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi0, const __grid_constant__ 
         if (!p.persist || !layer_barrier(ctrl, n_at_entry + layer + 1, lane)) break;
         }
     } else if (warp == 0) {
-        // =============================== TMA producer (one elected lane)
-        if (lane == 0) {
+        // =============================== TMA producer: the whole warp walks the loops (warp-uniform control flow), one
+        // elected lane issues (elect_one: no R2UR loops around the TMA instructions)
+        {
             int s = 0;
             uint32_t ph = 0;
             const uint64_t pol = l2_policy_evict_last();     // operand panels: reused by the other CTAs of the wave
@@ -267,16 +268,19 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi0, const __grid_constant__ 
             const int n_epochs = (n_rounds + 1) >> 1;
             const unsigned int n_sync = kint ? (unsigned int)(n_epochs * nchunks - 1) : (unsigned int)(n_rounds - 1);
             auto sync_point = [&](unsigned int q, bool wait) {      // q = 1 .. n_sync within the layer
-                atomicAdd(&ctrl->round_counter, 1u);
-                if (wait && *((volatile unsigned int*)&ctrl->round_sync_broken) == 0u) {
-                    const unsigned int target = q * gridDim.x;
-                    unsigned int spins = 0;
-                    while (*((volatile unsigned int*)&ctrl->round_counter) < target && ++spins < p.round_spins)
-                        __nanosleep(64);
-                    // timed out: the grid is not co-resident (shared GPU); the sync is only an optimisation, so
-                    // give it up for the rest of this solve instead of paying the timeout at every boundary
-                    if (spins >= p.round_spins) ctrl->round_sync_broken = 1u;
+                if (lane == 0) {
+                    atomicAdd(&ctrl->round_counter, 1u);
+                    if (wait && *((volatile unsigned int*)&ctrl->round_sync_broken) == 0u) {
+                        const unsigned int target = q * gridDim.x;
+                        unsigned int spins = 0;
+                        while (*((volatile unsigned int*)&ctrl->round_counter) < target && ++spins < p.round_spins)
+                            __nanosleep(64);
+                        // timed out: the grid is not co-resident (shared GPU); the sync is only an optimisation, so
+                        // give it up for the rest of this solve instead of paying the timeout at every boundary
+                        if (spins >= p.round_spins) ctrl->round_sync_broken = 1u;
+                    }
                 }
+                __syncwarp();
             };
             for (int layer = 0;; ++layer) {
             const CUtensorMap* tmh = (layer & 1) ? &tm_hi1 : &tm_hi0;
@@ -285,7 +289,8 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi0, const __grid_constant__ 
             auto load_stage = [&](int k0, int m0, int n0) {
                 mbar_wait(&empty_bar[s], ph ^ 1u);
                 uint8_t* st = smem + s * C::STAGE_BYTES;
-                if (CG == 1) {
+                if (!elect_one()) {
+                } else if (CG == 1) {
                     mbar_arrive_expect_tx(&full_bar[s], C::STAGE_BYTES);
                     tma_load_2d_hint(st, tmh, &full_bar[s], k0, m0, pol);
                     tma_load_2d_hint(st + C::A_BYTES, tml, &full_bar[s], k0, m0, pol);
@@ -309,6 +314,7 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi0, const __grid_constant__ 
                                               n0 + h * 128, pol);
                     }
                 }
+                __syncwarp();
                 if (++s == STAGES) { s = 0; ph ^= 1u; }
             };
             if (kint) {
@@ -358,7 +364,7 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi0, const __grid_constant__ 
                     for (int kb = 0; kb < KB; ++kb) load_stage((back ? (KB - 1 - kb) : kb) * BK, m0, n0);
                 }
             }
-            if (!p.persist || !layer_barrier_one(ctrl, n_at_entry + layer + 1)) break;
+            if (!p.persist || !layer_barrier(ctrl, n_at_entry + layer + 1, lane)) break;
             }
         }
         __syncwarp();     // reconverge before the .aligned cluster barrier of the teardown
@@ -420,29 +426,29 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi0, const __grid_constant__ 
         if (!p.persist || !layer_barrier(ctrl, n_at_entry + layer + 1, lane)) break;
         }
     } else if (warp == 1) {
-        // =============================== MMA issuer (leader CTA only, one elected lane)
-        if (rank == 0) {
+        // =============================== MMA issuer: ONE elected thread of the leader CTA runs the whole loop.  What it
+        // executes between the last MMA of a stage and the first of the next one is not hidden by the tensor pipe (the
+        // pipe does not queue MMAs far ahead: tests/cuda/mma_rate.cu), so that stretch is kept short: no per-stage
+        // elect / warp barrier, and a descriptor is ONE add to a base descriptor (the address field of a 1024-byte
+        // aligned stage advances by bytes >> 4 without carries into the other fields).
+        if (rank == 0 && elect_one()) {
             int s = 0;
             uint32_t ph = 0;
             int it = 0;                                   // accumulator uses so far (one per item; per chunk if ENH)
+            const uint64_t desc0 = umma_desc_sw128(smem_u32(smem));
             // one pipeline stage: wait for the operands, 3 MMAs per K = 16 into d_tmem, release the stage; `first`: the
             // tile's (or ENH chunk's) first stage overwrites the accumulator; `last`: signal the epilogue
             auto mma_stage = [&](uint32_t d_tmem, uint32_t idesc, bool first, bool last, int buf) {
-                const long long t0_ = LT_CLK();
                 mbar_wait(&full_bar[s], ph);
-                if (lane == 0) LT_ADD(7, LT_CLK() - t0_);
                 tc_fence_after();
-                if (lane == 0) {
-                    const uint32_t a_hi = smem_u32(smem + s * C::STAGE_BYTES);
-                    const uint32_t a_lo = a_hi + C::A_BYTES;
-                    const uint32_t b_hi = a_hi + 2 * C::A_BYTES;
-                    const uint32_t b_lo = b_hi + C::B_BYTES;
+                {
+                    const uint64_t dst = desc0 + (uint64_t)((uint32_t)s * (uint32_t)(C::STAGE_BYTES >> 4));
 #pragma unroll
                     for (int k = 0; k < BK / 16; ++k) {
-                        const uint64_t dah = umma_desc_sw128(a_hi + k * 32);
-                        const uint64_t dal = umma_desc_sw128(a_lo + k * 32);
-                        const uint64_t dbh = umma_desc_sw128(b_hi + k * 32);
-                        const uint64_t dbl = umma_desc_sw128(b_lo + k * 32);
+                        const uint64_t dah = dst + (uint64_t)(2 * k);
+                        const uint64_t dal = dst + (uint64_t)((C::A_BYTES >> 4) + 2 * k);
+                        const uint64_t dbh = dst + (uint64_t)(((2 * C::A_BYTES) >> 4) + 2 * k);
+                        const uint64_t dbl = dst + (uint64_t)(((2 * C::A_BYTES + C::B_BYTES) >> 4) + 2 * k);
                         if (C::CAT) {
                             // B_hi and B_lo are adjacent 128-row tiles: [X0 X0 | X0 X1] in one N = 256 MMA (whatever the
                             // item's ncols: a strip's unused columns are computed and ignored), then X1 X0 on the left
@@ -460,7 +466,6 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi0, const __grid_constant__ 
                         if (CG == 1) umma_commit(&tfull_bar[buf]); else umma_commit_pair(&tfull_bar[buf], 0x3);
                     }
                 }
-                __syncwarp();
                 if (++s == STAGES) { s = 0; ph ^= 1u; }
             };
             const bool kint = !C::ENH && p.ki_edge > 0;
@@ -492,7 +497,7 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi0, const __grid_constant__ 
                             if (c == 0) {                               // epilogue has drained this accumulator
                                 const long long t0_ = LT_CLK();
                                 mbar_wait(&tempty_bar[buf], ((uint32_t)(itt >> 1) & 1u) ^ 1u);
-                                if (lane == 0) LT_ADD(6, LT_CLK() - t0_);
+                                LT_ADD(6, LT_CLK() - t0_);
                                 tc_fence_after();
                             }
                             const uint32_t d_tmem = tmem_base + (uint32_t)(buf * C::ACC_COLS);
@@ -514,14 +519,14 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi0, const __grid_constant__ 
                         const int kb1 = C::ENH ? (kb0 + KC < KB ? kb0 + KC : KB) : KB;
                         const long long t0_ = LT_CLK();
                         mbar_wait(&tempty_bar[buf], (use & 1u) ^ 1u);   // epilogue has drained this accumulator
-                        if (lane == 0) LT_ADD(6, LT_CLK() - t0_);
+                        LT_ADD(6, LT_CLK() - t0_);
                         tc_fence_after();
                         const uint32_t d_tmem = tmem_base + (uint32_t)(buf * C::ACC_COLS);
                         for (int kb = kb0; kb < kb1; ++kb) mma_stage(d_tmem, idesc, kb == kb0, kb == kb1 - 1, buf);
                     }
                 }
             }
-            if (!p.persist || !layer_barrier(ctrl, n_at_entry + layer + 1, lane)) break;
+            if (!p.persist || !layer_barrier_one(ctrl, n_at_entry + layer + 1)) break;
             }
         }
         __syncwarp();     // reconverge before the .aligned barrier / tcgen05.dealloc of the teardown
