@@ -493,7 +493,8 @@ __global__ void __launch_bounds__(C::THREADS, 1) k_sp2_resident(const ResidentPa
             // ---- a4 of the NEXT layer, X = S^2 (Eq. 15): 3 MMAs per 16 columns of K, operands = the resident panels;
             // issued before the control step below has decided anything (it runs meanwhile)
             if (issue_next) {
-                if (warp == C::MMA_WARP && rank == 0 && lane == 0) {
+                // one elected thread in warp-uniform control flow (elect_one: no R2UR loops around the MMAs)
+                if (warp == C::MMA_WARP && rank == 0 && elect_one()) {
                     constexpr uint32_t idesc = umma_idesc_f16(128 * CG, NP);
 #pragma unroll 1
                     for (int kb = 0; kb < C::KBLK; ++kb) {

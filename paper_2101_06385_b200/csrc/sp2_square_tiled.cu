@@ -227,7 +227,7 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi0, const __grid_constant__ 
             const WorkItem wi = p.items[w];
             uint32_t m[4];
             sparse_kmask(bn_cur, p.nb, wi.I, wi.J, tau2, lane, m);
-            if (lane == 0) {
+            if (elect_one()) {
                 const int m0 = wi.I * BN, n0 = wi.J * BN;
                 for (int kk = 0; kk < p.nb; ++kk) {
                     if (!sparse_bit(m, kk)) continue;
@@ -392,22 +392,17 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi0, const __grid_constant__ 
                 for (int half = 0; half < 2; ++half) {
                     mbar_wait(&full_bar[s], ph);
                     tc_fence_after();
-                    if (lane == 0) {
-                        const uint32_t a_hi = smem_u32(smem + s * C::STAGE_BYTES);
-                        const uint32_t a_lo = a_hi + C::A_BYTES;
-                        const uint32_t b_hi = a_hi + 2 * C::A_BYTES;
-                        const uint32_t b_lo = b_hi + C::B_BYTES;
+                    if (elect_one()) {
+                        const uint64_t dst = umma_desc_sw128(smem_u32(smem)) + (uint64_t)((uint32_t)s * (uint32_t)(C::STAGE_BYTES >> 4));
 #pragma unroll
                         for (int k = 0; k < BK / 16; ++k) {
-                            const uint64_t dah = umma_desc_sw128(a_hi + k * 32);
-                            const uint64_t dal = umma_desc_sw128(a_lo + k * 32);
-                            const uint64_t dbh = umma_desc_sw128(b_hi + k * 32);
-                            const uint64_t dbl = umma_desc_sw128(b_lo + k * 32);
+                            const uint64_t dah = dst + (uint64_t)(2 * k);
+                            const uint64_t dal = dst + (uint64_t)((C::A_BYTES >> 4) + 2 * k);
+                            const uint64_t dbh = dst + (uint64_t)(((2 * C::A_BYTES) >> 4) + 2 * k);
                             // [X0 X0 | X0 X1] with one N = 256 MMA over the adjacent hi and lo tiles of the B rows, then
                             // X1 X0 into the left half (TileCfg::CAT)
                             umma_f16<1>(d_tmem, dah, dbh, umma_idesc_f16(BM, 2 * BN), (fresh && k == 0) ? 0u : 1u);
                             umma_f16<1>(d_tmem, dal, dbh, idesc, 1u);
-                            (void)dbl;
                         }
                         umma_commit(&empty_bar[s]);
                     }
@@ -416,7 +411,7 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi0, const __grid_constant__ 
                     if (++s == STAGES) { s = 0; ph ^= 1u; }
                 }
             }
-            if (lane == 0) {
+            if (elect_one()) {
                 umma_commit(&tfull_bar[buf]);                   // also when nothing was issued: arrives at once
                 atomicAdd(&ctrl->work_active, (unsigned long long)(__popc(m[0]) + __popc(m[1]) + __popc(m[2]) + __popc(m[3])));
                 atomicAdd(&ctrl->work_dense, (unsigned long long)p.nb);
