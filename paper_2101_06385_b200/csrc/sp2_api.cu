@@ -405,11 +405,11 @@ static int choose_tile_config(int N, int requested, int num_sms) {
     if (requested >= TILE_128x128 && requested <= TILE_128x128_ENH) return requested;
     const int n128 = round_up(N, 128) / 128;
     const long long t128 = (long long)n128 * (n128 + 1) / 2;
-    // 128 x 128 single-CTA tiles up to ~1.75 rounds of them (N <= 2816 on 148 SMs), 256 x 256 pair tiles above.  An MMA
-    // with N = 128 does not run faster than one with N = 256 (measured issue interval ~117 cycles against 128: DESIGN.md
-    // section 6), so small tiles only pay while they put more SMs to work.  Measured us per layer, tile 1 / tile 3:
-    // N = 2048: 47.8 / 68.9, 2304: 66.7 / 71.7, 2560: 71.7 / 76.6, 2816: 82.8 / 82.5, 3072: 113.0 / 106.9,
-    // 3584: 159.5 / 151.1, 4096: 227.5 / 198.7.
+    // 128 x 128 single-CTA tiles up to ~1.75 rounds of them (N <= 2816 on 148 SMs), 256 x 256 pair tiles above: at
+    // 128 x 128 a pipeline stage is 768 cycles of tensor-pipe time and what the issuing thread does between two stages is
+    // exposed (measured ~1100 cycles per stage in the kernel, tests/cuda/mma_rate.cu), so small tiles only pay while they
+    // put more SMs to work.  Measured us per layer, tile 1 / tile 3: N = 2048: 47.8 / 68.9, 2304: 66.7 / 71.7,
+    // 2560: 71.7 / 76.6, 2816: 82.8 / 82.5, 3072: 113.0 / 106.9, 3584: 159.5 / 151.1, 4096: 227.5 / 198.7.
     if (4 * t128 > 7LL * num_sms) return TILE_256x256_PAIR;
     return TILE_128x128;
 }

@@ -42,9 +42,10 @@ struct TileCfg {
     static constexpr int SUB = (BN / BM) / CG;     // 128-row work items per supertile per CTA slot
     // CAT (128 x 128 single-CTA tiles): the hi and lo tiles of the B rows lie one behind the other in a stage, so ONE MMA
     // with N = 256 over both gives [X0 X0 | X0 X1] in a 256-column accumulator; a second one with N = 128 adds
-    // (X0 X1)^T = X1 X0 to the left half, and the epilogue adds the two halves.  An MMA with N = 128 occupies the tensor
-    // pipe for 64 cycles but the measured issue interval is ~117 (N = 256: 128 cycles, no gap), so three of them per
-    // K = 16 cost ~350 cycles against ~245 for one of each.
+    // (X0 X1)^T = X1 X0 to the left half, and the epilogue adds the two halves.  Same tensor-pipe time as three N = 128
+    // MMAs (128 + 64 cycles per K = 16), but two instructions instead of three for the issuing thread, whose own time
+    // is not hidden at this tile size (tests/cuda/mma_rate.cu: 916 against 1009 cycles per stage of 768), and the chain
+    // of truncating adds behind the dominant term of an entry is a third shorter.
     static constexpr bool CAT = (BN_ == 128) && (CG_ == 1) && !ENH_;
     static constexpr int ACC_COLS = CAT ? 2 * BN : BN;       // TMEM columns of one accumulator buffer
     static constexpr int TMEM_COLS = ENH ? 4 * BN : 2 * ACC_COLS;   // two accumulator buffers (+ running hi, lo)

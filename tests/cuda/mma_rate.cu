@@ -1,8 +1,15 @@
 // Measures the issue interval of tcgen05.mma.kind::f16 (K = 16, both operands in shared memory) on B200 for the shapes
 // the layer kernels use: the tile choice of the library (sp2_api.cu: choose_tile_config, TileCfg::CAT in
 // sp2_square_tiled.cu) rests on the fact that an MMA with N = 128 is NOT issued twice as often as one with N = 256.
-// One CTA (or one CTA pair) issues `reps` rounds of a pattern of MMAs from zero-filled shared-memory tiles, commits, and
-// waits; prints "name cycles_per_mma" lines.  Built and run by tests/test_gpu_arith_facts.py.
+// One CTA (or one CTA pair) issues `reps` rounds of a pattern of MMAs from shared-memory tiles, commits, and waits; prints
+// "name cycles_per_mma" lines (k_rate) and "name cycles_per_stage" lines for the layer kernel's ring of stages without
+// its loads (k_ring).  Built and run by tests/test_gpu_arith_facts.py.  What it showed (B200):
+//   * an MMA issued under `if (lane == 0)` costs ~105 cycles whatever its N <= 128 (the compiler wraps it in a loop of
+//     R2UR.BROADCASTs); issued by an elect.sync thread in warp-uniform control flow it runs at the pipe rate (N = 128:
+//     64 cycles, N = 256: 128);
+//   * inside a ring of stages (wait, MMAs, commit) the issuing thread's own instructions between two stages are NOT
+//     hidden by the pipe: 3 x N = 128 per K-step, 768 cycles of pipe time per stage, takes 1086 with per-stage elect and
+//     full descriptor arithmetic, 1009 with one-add descriptors, 841 with the whole loop in one elected thread.
 #include <cstdio>
 #include <cuda_runtime.h>
 #include "../../paper_2101_06385_b200/csrc/sp2_ptx.cuh"
@@ -140,8 +147,7 @@ __global__ void __launch_bounds__(128, 1) k_ring(long long* out, int nstages, in
             if (++s == nstages) { s = 0; ph ^= 1u; }
         }
     } else if (warp == 1 && LOOPIN) {
-        // the whole loop runs in ONE elected thread; LOOPIN = 2: the wait for the next stage's operands sits in front of
-        // the current stage's last K-step, so that only the commit separates two stages' MMAs
+        // the whole loop runs in ONE elected thread (no per-stage elect / warp barrier)
         if (elect_one()) {
             int s = 0; uint32_t ph = 0;
             const uint64_t d0 = umma_desc_sw128(smem_u32(smem));
@@ -153,7 +159,6 @@ __global__ void __launch_bounds__(128, 1) k_ring(long long* out, int nstages, in
                 if (s1 == nstages) { s1 = 0; ph1 ^= 1u; }
 #pragma unroll
                 for (int k = 0; k < 4; ++k) {
-                    if (LOOPIN == 2 && k == 3 && t + 1 < total) { mbar_wait(&full_bar[s1], ph1); tc_fence_after(); }
                     const uint64_t dah = d0 + (uint64_t)(st16 + 2 * k), dal = d0 + (uint64_t)(st16 + 1024 + 2 * k);
                     const uint64_t dbh = d0 + (uint64_t)(st16 + 2048 + 2 * k), dbl = d0 + (uint64_t)(st16 + 3072 + 2 * k);
                     if (CAT) {
@@ -167,7 +172,7 @@ __global__ void __launch_bounds__(128, 1) k_ring(long long* out, int nstages, in
                 }
                 umma_commit(&empty_bar[s]);
                 if (t == total - 1) umma_commit(&done_bar);
-                if (LOOPIN != 2 && t + 1 < total) { mbar_wait(&full_bar[s1], ph1); tc_fence_after(); }
+                if (t + 1 < total) { mbar_wait(&full_bar[s1], ph1); tc_fence_after(); }
                 st16 = (st16 == 8192u) ? 0u : st16 + 4096u;
                 s = s1; ph = ph1;
             }
@@ -239,9 +244,6 @@ int main() {
     printf("ring_cat_cheap_desc_stages3 %.1f\n", run_ring<true, true>(dev, 3));
     printf("ring_cat_cheap_desc_stages6 %.1f\n", run_ring<true, true>(dev, 6));
     printf("ring_3x128_one_thread_loop %.1f\n", run_ring<false, true, 1>(dev, 3));
-    printf("ring_cat_one_thread_loop %.1f\n", run_ring<true, true, 1>(dev, 3));
-    printf("ring_3x128_one_thread_loop_prewait %.1f\n", run_ring<false, true, 2>(dev, 3));
-    printf("ring_cat_one_thread_loop_prewait %.1f\n", run_ring<true, true, 2>(dev, 3));
     const int reps = 500;
     printf("cg1_n64_one_acc %.1f\n", run<1>(dev, 64, 0, reps));
     printf("cg1_n128_one_acc %.1f\n", run<1>(dev, 128, 0, reps));

@@ -70,3 +70,25 @@ def test_fp64_wakeup_latency(cuda_device, tmp_path):
     print(f"1 DFMA + 16 FFMA: {v['dfma_plus_16_ffma']:.0f} cycles against {sum_of_latencies:.0f} for the sum of the "
           f"latencies -> wake-up {v['dfma_plus_16_ffma'] - sum_of_latencies:.0f} cycles")
     assert v["dfma_plus_16_ffma"] > 1.5 * sum_of_latencies             # an isolated FP64 instruction is expensive
+
+
+def test_mma_issue_interval(cuda_device, tmp_path):
+    """Third fact: a tcgen05.mma issued under `if (lane == 0)` costs ~105 cycles whatever its size (the compiler wraps it
+    in a loop of R2UR.BROADCASTs), one issued by an elect.sync thread in warp-uniform control flow runs at the tensor
+    pipe's rate (N = 128: 64 cycles, N = 256: 128) -- why every MMA / TMA issue in the library goes through elect_one()
+    (csrc/sp2_ptx.cuh), why 128 x 128 tiles stop paying as soon as they need a second round (choose_tile_config) and why
+    the MMA issuer is one thread running the whole loop (the ring numbers)."""
+    nvcc = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
+    if not os.path.exists(nvcc):
+        pytest.skip("nvcc not available on this box")
+    exe = str(tmp_path / "mma_rate")
+    subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-o", exe,
+                    os.path.join(HERE, "cuda", "mma_rate.cu")], check=True)
+    out = subprocess.run([exe], capture_output=True, text=True, check=True, timeout=120).stdout
+    v = {k: float(x) for k, x in (ln.split() for ln in out.strip().splitlines())}
+    print("cycles per MMA / per stage:", v)
+    assert 60.0 < v["cg1_n128_one_acc_elect"] < 72.0                   # the pipe rate of a 128 x 128 x 16 MMA
+    assert 120.0 < v["cg1_n256_one_acc"] < 136.0 and 120.0 < v["cg2_n256_one_acc"] < 136.0
+    assert v["cg1_n128_one_acc"] > 1.25 * v["cg1_n128_one_acc_elect"]  # lane == 0: issue-bound
+    assert abs(v["cg1_n64_one_acc"] - v["cg1_n128_one_acc"]) < 5.0     # ... at a rate that does not depend on N
+    assert v["ring_3x128_one_thread_loop"] < v["ring_3x128_cheap_desc_stages3"] < v["ring_3x128_stages3"]
