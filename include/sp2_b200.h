@@ -20,9 +20,11 @@
  *     and belongs to the device that was current at sp2_create; a call with another current device returns
  *     SP2_ERR_INVALID_ARG.
  *   - Every parameter that can change a RESULT is in sp2_opts_t.  The environment is read once, at sp2_create, for
- *     three pure performance toggles only (results are bit-identical for any setting; defaults in brackets):
+ *     four pure performance toggles only (results are bit-identical for any setting; defaults in brackets):
  *     SP2_ROUND_SYNC [1] and SP2_ROUND_SYNC_SPINS [65536] (the round synchronisation of the layer kernel and the
- *     bound of its wait), SP2_TAIL_SPLIT [1] (column strips for the last, partial round) -- DESIGN.md section 6.
+ *     bound of its wait), SP2_TAIL_SPLIT [1] (column strips for the last, partial round), SP2_K_INTERLEAVE [32]
+ *     (K-blocks per chunk of the K-interleave of two rounds, "edge:mid" for longer end chunks, 0 = off) --
+ *     DESIGN.md section 6.
  *   - Return value: SP2_OK (0); > 0 = result written but flagged; < 0 = error, outputs undefined.
  *     No exceptions, no stdout.  There is no CPU fallback: without a CUDA device calls return SP2_ERR_CUDA.
  *   - Hang guard: every mbarrier wait inside the kernels is bounded (2^26 polls, seconds); a wait that runs out --
