@@ -765,6 +765,7 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi0, const __grid_constant__ 
                     }
                     tmem_ld_wait();
                     fx_t sq_own = 0;
+                    uint32_t hp[16], lp[16];                // FP16 pairs of the row (even column in the low half)
 #pragma unroll
                     for (int c = 0; c < 32; ++c) {
                         const int gj = gj0 + c;
@@ -777,7 +778,9 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi0, const __grid_constant__ 
                         }
                         __half h, l;
                         split_hi_lo(val, cs, h, l);
-                        const unsigned short hb = __half_as_ushort(h), lb = __half_as_ushort(l);
+                        const uint32_t hb = __half_as_ushort(h), lb = __half_as_ushort(l);
+                        if (c & 1) { hp[c >> 1] |= hb << 16; lp[c >> 1] |= lb << 16; }
+                        else { hp[c >> 1] = hb; lp[c >> 1] = lb; }
                         if (gj <= gi) {
                             bad = bad || !(fabsf(val) <= 1.0e3f);
                             const fx_t v2 = fx_square(val);
@@ -786,15 +789,44 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi0, const __grid_constant__ 
                             else off2 += v2;
                         }
                         so[c] = (gj < gi) ? val * val : 0.f;
-                        if (gj <= gi) {
-                            const long long o = (long long)gj * ldf + gi, o2 = (long long)gi * ldf + gj;
-                            S[(long long)gj * ld + gi] = val; HOu[o] = hb; LOu[o] = lb;
-                            S[(long long)gi * ld + gj] = val; HOu[o2] = hb; LOu[o2] = lb;
-                            if (C::MIX) {
-                                const float mv = fmaf(cN, val, mo[C::MIX ? c : 0]);
-                                M[(long long)gj * ld + gi] = mv;
-                                M[(long long)gi * ld + gj] = mv;
-                            }
+                        v[c] = __float_as_uint(val);
+                        if (C::MIX) mo[C::MIX ? c : 0] = fmaf(cN, val, mo[C::MIX ? c : 0]);
+                    }
+                    // own rows: the whole 32-column piece of the row as vectors (a 4-byte store per lane and row costs
+                    // the LSU 32 sectors per instruction).  The entries above the diagonal (gj > gi) written here are
+                    // this thread's own rounding of a value that belongs to row gj; after the warp barrier the mirror
+                    // stores of the rows that own them overwrite them (exact symmetry inside the tile).
+                    {
+                        float4* rowS = reinterpret_cast<float4*>(S + (long long)gi * ld + gj0);
+                        uint4* rowH = reinterpret_cast<uint4*>(HO + (long long)gi * ldf + gj0);
+                        uint4* rowL = reinterpret_cast<uint4*>(LO + (long long)gi * ldf + gj0);
+#pragma unroll
+                        for (int g = 0; g < 8; ++g)
+                            rowS[g] = make_float4(__uint_as_float(v[4 * g]), __uint_as_float(v[4 * g + 1]),
+                                                  __uint_as_float(v[4 * g + 2]), __uint_as_float(v[4 * g + 3]));
+#pragma unroll
+                        for (int g = 0; g < 4; ++g) {
+                            rowH[g] = make_uint4(hp[4 * g], hp[4 * g + 1], hp[4 * g + 2], hp[4 * g + 3]);
+                            rowL[g] = make_uint4(lp[4 * g], lp[4 * g + 1], lp[4 * g + 2], lp[4 * g + 3]);
+                        }
+                        if (C::MIX) {
+                            float4* rowM = reinterpret_cast<float4*>(M + (long long)gi * ld + gj0);
+#pragma unroll
+                            for (int g = 0; g < 8; ++g)
+                                rowM[g] = make_float4(mo[C::MIX ? 4 * g : 0], mo[C::MIX ? 4 * g + 1 : 0],
+                                                      mo[C::MIX ? 4 * g + 2 : 0], mo[C::MIX ? 4 * g + 3 : 0]);
+                        }
+                    }
+                    __syncwarp();
+#pragma unroll
+                    for (int c = 0; c < 32; ++c) {
+                        const int gj = gj0 + c;
+                        if (gj < gi) {                      // mirrored position: coalesced across the warp
+                            const long long o = (long long)gj * ldf + gi;
+                            S[(long long)gj * ld + gi] = __uint_as_float(v[c]);
+                            HOu[o] = (unsigned short)((hp[c >> 1] >> (16 * (c & 1))) & 0xffffu);
+                            LOu[o] = (unsigned short)((lp[c >> 1] >> (16 * (c & 1))) & 0xffffu);
+                            if (C::MIX) M[(long long)gj * ld + gi] = mo[C::MIX ? c : 0];
                         }
                     }
                     rowacc += sq_own;
