@@ -191,6 +191,7 @@ __global__ void __launch_bounds__(256) k_gershgorin_finalize(const float* __rest
 // (Eqs. 12-13) at (i,j) and (j,i) from H's lower triangle (the mirror goes through shared memory so that both global
 // writes are row segments); Tr S_0, ||S_0||_F^2 and the row sums of squares.  FP32 sums inside a tile (FP64 only for
 // the diagonal entries), FP64 / fixed point across tiles.
+// S == nullptr: the FP32 master is not written at this position (see k_affine_split)
 __device__ __forceinline__ void store_s4(float* __restrict__ S, __half* __restrict__ hi, __half* __restrict__ lo,
                                          long long ld, long long ldf, int i, int j, const float (&s)[4], float scale,
                                          bool all4, const bool (&ok)[4], float* __restrict__ mix, float c0) {
@@ -198,7 +199,7 @@ __device__ __forceinline__ void store_s4(float* __restrict__ S, __half* __restri
 #pragma unroll
     for (int e = 0; e < 4; ++e) split_hi_lo(s[e], scale, h[e], l[e]);
     if (all4) {
-        *reinterpret_cast<float4*>(S + (long long)i * ld + j) = make_float4(s[0], s[1], s[2], s[3]);
+        if (S) *reinterpret_cast<float4*>(S + (long long)i * ld + j) = make_float4(s[0], s[1], s[2], s[3]);
         *reinterpret_cast<uint2*>(hi + (long long)i * ldf + j) = *reinterpret_cast<uint2*>(h);
         *reinterpret_cast<uint2*>(lo + (long long)i * ldf + j) = *reinterpret_cast<uint2*>(l);
         if (mix)
@@ -208,7 +209,7 @@ __device__ __forceinline__ void store_s4(float* __restrict__ S, __half* __restri
         for (int e = 0; e < 4; ++e)
             if (ok[e]) {
                 if (mix) mix[(long long)i * ld + j + e] = c0 * s[e];
-                S[(long long)i * ld + j + e] = s[e];
+                if (S) S[(long long)i * ld + j + e] = s[e];
                 hi[(long long)i * ldf + j + e] = h[e];
                 lo[(long long)i * ldf + j + e] = l[e];
             }
@@ -277,7 +278,9 @@ __global__ void __launch_bounds__(256, 4) k_affine_split(const float* __restrict
                 ts[lr][c4 + e] = sx;
             }
             const bool all4 = !dtile && (i < N);    // off-diagonal tile: j + 3 < J*64 + 64 <= i
-            store_s4(S, hi, lo, ld, ldf, i, j, sv, scale, all4, ok, mix, c0);
+            // of the FP32 master only the UPPER triangle (and the diagonal tiles) is ever read back: by the layer
+            // epilogue at the mirrored address and by k_copy_sym -- below the diagonal tiles it is not written
+            store_s4(dtile ? S : nullptr, hi, lo, ld, ldf, i, j, sv, scale, all4, ok, mix, c0);
             if (rowsq) {
                 rsq = row16_sum(rsq);
                 if ((threadIdx.x & 15) == 0 && i < N) atomicAdd(rowsq + i, rowsq_fix(rsq));
