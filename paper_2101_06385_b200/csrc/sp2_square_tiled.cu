@@ -434,13 +434,28 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi0, const __grid_constant__ 
             const uint64_t desc0 = umma_desc_sw128(smem_u32(smem));
             // one pipeline stage: wait for the operands, 3 MMAs per K = 16 into d_tmem, release the stage; `first`: the
             // tile's (or ENH chunk's) first stage overwrites the accumulator; `last`: signal the epilogue
+            // The wait for the NEXT stage's operands sits in front of the current stage's last K-step (its latency is then
+            // covered by that K-step's MMAs instead of lying between two stages); `have`: this stage's wait is done.
+            const int my_stages = (slot < n_work ? (n_work - slot + nslots - 1) / nslots : 0) * KB;   // per layer
+            int issued = 0;
+            bool have = false;
             auto mma_stage = [&](uint32_t d_tmem, uint32_t idesc, bool first, bool last, int buf) {
-                mbar_wait(&full_bar[s], ph);
-                tc_fence_after();
+                if (!have) {
+                    mbar_wait(&full_bar[s], ph);
+                    tc_fence_after();
+                }
                 {
                     const uint64_t dst = desc0 + (uint64_t)((uint32_t)s * (uint32_t)(C::STAGE_BYTES >> 4));
 #pragma unroll
                     for (int k = 0; k < BK / 16; ++k) {
+                        if (k == BK / 16 - 1) {
+                            have = (++issued < my_stages);
+                            if (have) {
+                                const int s1 = (s + 1 == STAGES) ? 0 : s + 1;
+                                mbar_wait(&full_bar[s1], (s + 1 == STAGES) ? (ph ^ 1u) : ph);
+                                tc_fence_after();
+                            }
+                        }
                         const uint64_t dah = dst + (uint64_t)(2 * k);
                         const uint64_t dal = dst + (uint64_t)((C::A_BYTES >> 4) + 2 * k);
                         const uint64_t dbh = dst + (uint64_t)(((2 * C::A_BYTES) >> 4) + 2 * k);
@@ -467,6 +482,8 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi0, const __grid_constant__ 
             const bool kint = !C::ENH && p.ki_edge > 0;
             const int n_rounds = (n_work + nslots - 1) / nslots;
             for (int layer = 0;; ++layer) {
+            issued = 0;
+            have = false;
             if (kint) {
                 // K-interleave: the tiles of rounds 2e and 2e + 1 advance through K in alternating chunks (see ki_range);
                 // the order of (epoch, chunk, tile, K-block) is the producer's
