@@ -253,6 +253,15 @@ __device__ __forceinline__ void tmem_st_32x32(uint32_t taddr, const uint32_t (&v
 }
 __device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;\n" ::: "memory"); }
 
+// 32-byte streaming store (st.global.v8, sm_100): one full sector per lane.  The epilogue's own-row stores go to a
+// different row per lane, so a 16-byte store writes half a sector per lane and costs a sector slot all the same.
+__device__ __forceinline__ void st_cs_v8(void* p, uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t a4,
+                                         uint32_t a5, uint32_t a6, uint32_t a7) {
+    asm volatile("st.global.cs.v8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};\n" ::"l"(p), "r"(a0), "r"(a1), "r"(a2),
+                 "r"(a3), "r"(a4), "r"(a5), "r"(a6), "r"(a7)
+                 : "memory");
+}
+
 // ---------------------------------------------------------------- FP16 hi/lo split (Eqs. 12-13)
 // hi = FP16[c x] (RNE, subnormals kept), lo = FP16[c x - hi]; the subtraction is exact in FP32.
 __device__ __forceinline__ void split_hi_lo(float x, float c, __half& hi, __half& lo) {
