@@ -289,7 +289,7 @@ def test_tiled_kernel_bit_reproducible_and_host_entry(env, n, tile, auto):
     P.assert_acceptance(D1.cpu().numpy().astype(np.float64), O.closed_form_density(w.Q, w.N_occ), w.N_occ, f"N={n}")
 
 
-@pytest.mark.parametrize("n,tile", [(1024, 0), (2048, 0), (3000, 1), (3000, 0)])
+@pytest.mark.parametrize("n,tile", [(1024, 0), (2048, 0), (3000, 1), (3000, 0), (4096, 0)])
 def test_persistent_launch_gives_the_graph_loop_bits(env, n, tile):
     """control = 3: ONE cooperative launch runs every layer (grid barrier between layers, the operand pairs swapped per
     layer inside the kernel) -- the same tiles in the same order as the graph's WHILE loop, so the same bits, with
