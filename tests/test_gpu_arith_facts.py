@@ -92,3 +92,22 @@ def test_mma_issue_interval(cuda_device, tmp_path):
     assert v["cg1_n128_one_acc"] > 1.25 * v["cg1_n128_one_acc_elect"]  # lane == 0: issue-bound
     assert abs(v["cg1_n64_one_acc"] - v["cg1_n128_one_acc"]) < 5.0     # ... at a rate that does not depend on N
     assert v["ring_3x128_one_thread_loop"] < v["ring_3x128_cheap_desc_stages3"] < v["ring_3x128_stages3"]
+
+
+def test_store_patterns_of_the_epilogue(cuda_device, tmp_path):
+    """Fourth fact: the layer epilogue is bound by its stores, and how a warp packages them matters.  A lane that writes
+    64 bytes of a row of its own in 16-byte stores gets well under half of what it gets with 32-byte st.global.v8 stores
+    (why the own-row stores of sp2_square_tiled.cu are st_cs_v8); 64-byte row segments (the FP16 operands of a 32-column
+    chunk) stay below 128-byte ones however they are packaged (pairing rows in one instruction does not help)."""
+    nvcc = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
+    if not os.path.exists(nvcc):
+        pytest.skip("nvcc not available on this box")
+    exe = str(tmp_path / "store_patterns")
+    subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-o", exe,
+                    os.path.join(HERE, "cuda", "store_patterns.cu")], check=True)
+    out = subprocess.run([exe], capture_output=True, text=True, check=True, timeout=120).stdout
+    v = {k: float(x) for k, x in (ln.split() for ln in out.strip().splitlines())}
+    print("GB/s:", v)
+    assert v["own_rows_32B_per_lane"] > 1.8 * v["own_rows_16B_per_lane"]
+    assert v["mirrored_128B_per_instruction"] > 1.2 * v["mirrored_64B_per_instruction"]
+    assert v["mirrored_two_rows_of_64B_per_instruction"] < 1.15 * v["mirrored_64B_per_instruction"]
