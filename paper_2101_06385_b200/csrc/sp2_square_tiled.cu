@@ -4,7 +4,8 @@
 //   acc(I,J) = sum_k  hi[I,k] hi[J,k] + hi[I,k] lo[J,k] + lo[I,k] hi[J,k]       (Eq. 15; X symmetric so the
 //                                                                              transpose term is lo[I,:] . hi[J,:])
 //   S_n      = th1 acc / c^2 + th2 S_{n-1} + th3 I                              (Alg. 1's W_n, B_n; Eq. 17)
-//   epilogue: Tr S_n, ||S_n||_F^2 (= next layer's N_X), Tr X_n in FP64; next layer's hi/lo (Eqs. 12-13);
+//   epilogue: Tr S_n, ||S_n||_F^2 (= next layer's N_X), Tr X_n as 2^40 fixed-point integers; next layer's hi/lo
+//   (Eqs. 12-13);
 //   last CTA: sigma_{n+1}, IdErr_{n+1}, stop tests (control_finish_layer).
 // Only lower-triangle tiles (I >= J) are computed; every hi/lo value is also stored at its mirrored position, so the
 // operands stay exactly symmetric and the next layer can read full row panels as K-major operands.  Of the FP32
@@ -12,8 +13,10 @@
 // epilogue reads back (coalesced), and k_copy_sym mirrors the final result once.
 //
 // Structure: persistent CTAs (or CTA pairs), static round-robin over a host-ordered supertile list;
-// warp 0 = TMA producer, warp 1 = tcgen05.mma issuer (+ TMEM alloc), warps 2-5 = epilogue
-// (TMEM -> registers -> global).  Two TMEM accumulator buffers overlap the epilogue with the next tile's MMAs.
+// warp 0 = TMA producer, warp 1 = tcgen05.mma issuer (+ TMEM alloc), both issuing through elect.sync; warps 2.. =
+// epilogue (TMEM -> registers -> global; two warps per TMEM lane quarter in the plain instantiations).  Two TMEM
+// accumulator buffers overlap the epilogue with the next tile's MMAs and let the two rounds of an epoch walk K
+// together (K-interleave, ki_range below).
 #include "sp2_kernels.h"
 #include "sp2_ptx.cuh"
 
