@@ -794,69 +794,79 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi0, const __grid_constant__ 
                     }
                     tmem_ld_wait();
                     fx_t sq_own = 0;
-                    uint32_t hp[16], lp[16];                // FP16 pairs of the row (even column in the low half)
+                    // Off-diagonal squares (gj < gi) are summed in FP32 and converted once, as in the chunks below the
+                    // diagonal; the diagonal element is converted exactly.  Own rows leave as vectors, sixteen columns at
+                    // a time (a 4-byte store per lane and row costs the LSU 32 sectors per instruction).  The entries
+                    // above the diagonal (gj > gi) written here are this thread's own rounding of a value that belongs to
+                    // row gj; after the warp barrier the mirror stores of the rows that own them overwrite them (exact
+                    // symmetry inside the tile).
+                    float q0 = 0.f, q1 = 0.f, q2 = 0.f, q3 = 0.f;
+                    float4* rowS = reinterpret_cast<float4*>(S + (long long)gi * ld + gj0);
+                    uint4* rowH = reinterpret_cast<uint4*>(HO + (long long)gi * ldf + gj0);
+                    uint4* rowL = reinterpret_cast<uint4*>(LO + (long long)gi * ldf + gj0);
 #pragma unroll
-                    for (int c = 0; c < 32; ++c) {
-                        const int gj = gj0 + c;
-                        const float x = __uint_as_float(v[c]);
-                        const bool on_diag = (gj == gi);
-                        float val = fmaf(th1s, x, th2 * so[c]);
-                        if (on_diag) {
-                            if (Rcur != nullptr) val = fmaf(th1, xdiag, th2 * so[c]);
-                            if (gi < p.N) val += th3;
+                    for (int half = 0; half < 2; ++half) {
+                        uint32_t hp[8], lp[8];              // FP16 pairs of sixteen columns (even column in the low half)
+#pragma unroll
+                        for (int cc = 0; cc < 16; ++cc) {
+                            const int c = 16 * half + cc;
+                            const int gj = gj0 + c;
+                            const float x = __uint_as_float(v[c]);
+                            const bool on_diag = (gj == gi);
+                            float val = fmaf(th1s, x, th2 * so[c]);
+                            if (on_diag) {
+                                if (Rcur != nullptr) val = fmaf(th1, xdiag, th2 * so[c]);
+                                if (gi < p.N) val += th3;
+                                const fx_t v2 = fx_square(val);
+                                sq_own += v2;
+                                dg2 += v2; trS += fx_from_float(val); trX += fx_from_float(x * inv2);
+                            }
+                            __half h, l;
+                            split_hi_lo(val, cs, h, l);
+                            const uint32_t hb = __half_as_ushort(h), lb = __half_as_ushort(l);
+                            if (cc & 1) { hp[cc >> 1] |= hb << 16; lp[cc >> 1] |= lb << 16; }
+                            else { hp[cc >> 1] = hb; lp[cc >> 1] = lb; }
+                            if (gj <= gi) bad = bad || !(fabsf(val) <= 1.0e3f);
+                            const float sq = (gj < gi) ? val * val : 0.f;
+                            so[c] = sq;
+                            if ((cc & 3) == 0) q0 += sq; else if ((cc & 3) == 1) q1 += sq;
+                            else if ((cc & 3) == 2) q2 += sq; else q3 += sq;
+                            v[c] = __float_as_uint(val);
+                            if (C::MIX) mo[C::MIX ? c : 0] = fmaf(cN, val, mo[C::MIX ? c : 0]);
                         }
-                        __half h, l;
-                        split_hi_lo(val, cs, h, l);
-                        const uint32_t hb = __half_as_ushort(h), lb = __half_as_ushort(l);
-                        if (c & 1) { hp[c >> 1] |= hb << 16; lp[c >> 1] |= lb << 16; }
-                        else { hp[c >> 1] = hb; lp[c >> 1] = lb; }
-                        if (gj <= gi) {
-                            bad = bad || !(fabsf(val) <= 1.0e3f);
-                            const fx_t v2 = fx_square(val);
-                            sq_own += v2;
-                            if (on_diag) { dg2 += v2; trS += fx_from_float(val); trX += fx_from_float(x * inv2); }
-                            else off2 += v2;
-                        }
-                        so[c] = (gj < gi) ? val * val : 0.f;
-                        v[c] = __float_as_uint(val);
-                        if (C::MIX) mo[C::MIX ? c : 0] = fmaf(cN, val, mo[C::MIX ? c : 0]);
+                        st_cs_v8(rowS + 4 * half, v[16 * half], v[16 * half + 1], v[16 * half + 2], v[16 * half + 3],
+                                 v[16 * half + 4], v[16 * half + 5], v[16 * half + 6], v[16 * half + 7]);
+                        st_cs_v8(rowS + 4 * half + 2, v[16 * half + 8], v[16 * half + 9], v[16 * half + 10], v[16 * half + 11],
+                                 v[16 * half + 12], v[16 * half + 13], v[16 * half + 14], v[16 * half + 15]);
+                        st_cs_v8(rowH + 2 * half, hp[0], hp[1], hp[2], hp[3], hp[4], hp[5], hp[6], hp[7]);
+                        st_cs_v8(rowL + 2 * half, lp[0], lp[1], lp[2], lp[3], lp[4], lp[5], lp[6], lp[7]);
                     }
-                    // own rows: the whole 32-column piece of the row as vectors (a 4-byte store per lane and row costs
-                    // the LSU 32 sectors per instruction).  The entries above the diagonal (gj > gi) written here are
-                    // this thread's own rounding of a value that belongs to row gj; after the warp barrier the mirror
-                    // stores of the rows that own them overwrite them (exact symmetry inside the tile).
+                    if (C::MIX) {
+                        float4* rowM = reinterpret_cast<float4*>(M + (long long)gi * ld + gj0);
+#pragma unroll
+                        for (int g = 0; g < 8; ++g)
+                            rowM[g] = make_float4(mo[C::MIX ? 4 * g : 0], mo[C::MIX ? 4 * g + 1 : 0],
+                                                  mo[C::MIX ? 4 * g + 2 : 0], mo[C::MIX ? 4 * g + 3 : 0]);
+                    }
                     {
-                        float4* rowS = reinterpret_cast<float4*>(S + (long long)gi * ld + gj0);
-                        uint4* rowH = reinterpret_cast<uint4*>(HO + (long long)gi * ldf + gj0);
-                        uint4* rowL = reinterpret_cast<uint4*>(LO + (long long)gi * ldf + gj0);
-#pragma unroll
-                        for (int g = 0; g < 4; ++g)
-                            st_cs_v8(rowS + 2 * g, v[8 * g], v[8 * g + 1], v[8 * g + 2], v[8 * g + 3], v[8 * g + 4],
-                                     v[8 * g + 5], v[8 * g + 6], v[8 * g + 7]);
-#pragma unroll
-                        for (int g = 0; g < 2; ++g) {
-                            st_cs_v8(rowH + 2 * g, hp[8 * g], hp[8 * g + 1], hp[8 * g + 2], hp[8 * g + 3], hp[8 * g + 4],
-                                     hp[8 * g + 5], hp[8 * g + 6], hp[8 * g + 7]);
-                            st_cs_v8(rowL + 2 * g, lp[8 * g], lp[8 * g + 1], lp[8 * g + 2], lp[8 * g + 3], lp[8 * g + 4],
-                                     lp[8 * g + 5], lp[8 * g + 6], lp[8 * g + 7]);
-                        }
-                        if (C::MIX) {
-                            float4* rowM = reinterpret_cast<float4*>(M + (long long)gi * ld + gj0);
-#pragma unroll
-                            for (int g = 0; g < 8; ++g)
-                                rowM[g] = make_float4(mo[C::MIX ? 4 * g : 0], mo[C::MIX ? 4 * g + 1 : 0],
-                                                      mo[C::MIX ? 4 * g + 2 : 0], mo[C::MIX ? 4 * g + 3 : 0]);
-                        }
+                        const float sdf = (q0 + q1) + (q2 + q3);
+                        bad = bad || !(sdf <= 1.0e6f);
+                        const fx_t sd = fx_from_float(sdf);
+                        off2 += sd;
+                        sq_own += sd;
                     }
                     __syncwarp();
 #pragma unroll
                     for (int c = 0; c < 32; ++c) {
                         const int gj = gj0 + c;
                         if (gj < gi) {                      // mirrored position: coalesced across the warp
+                            const float val = __uint_as_float(v[c]);
+                            __half h, l;
+                            split_hi_lo(val, cs, h, l);     // the same bits as in the own row
                             const long long o = (long long)gj * ldf + gi;
-                            S[(long long)gj * ld + gi] = __uint_as_float(v[c]);
-                            HOu[o] = (unsigned short)((hp[c >> 1] >> (16 * (c & 1))) & 0xffffu);
-                            LOu[o] = (unsigned short)((lp[c >> 1] >> (16 * (c & 1))) & 0xffffu);
+                            S[(long long)gj * ld + gi] = val;
+                            HOu[o] = __half_as_ushort(h);
+                            LOu[o] = __half_as_ushort(l);
                             if (C::MIX) M[(long long)gj * ld + gi] = mo[C::MIX ? c : 0];
                         }
                     }
