@@ -230,6 +230,32 @@ sp2_status_t sp2_split_fp16(const float* X_dev, int N, int ldx, unsigned short* 
 /* Gershgorin bounds of the lower-triangle-symmetrised H; synchronises; bounds_host[2] = {eps_min, eps_max}. */
 sp2_status_t sp2_gershgorin(sp2_handle_t h, const float* H_dev, int N, int ldh, double bounds_host[2], void* stream);
 
+/* Gershgorin bounds WITHOUT any allocation, for callers that cannot call cudaMalloc and so cannot own a handle
+ * (sp2_create allocates): hosts whose own arena or caching allocator already holds all of HBM, so that a library's
+ * cudaMalloc fails although the arena has room; time-step loops that cannot take the device-wide synchronisation a
+ * cudaMalloc / cudaFree implies; plug-ins that receive only pointers and a stream.  Same kernels and same bits as
+ * sp2_gershgorin; the scratch they need (per-tile sums, diagonal, per-block extrema) is a static __device__ array inside
+ * the library: sp2_gershgorin_static_bytes() bytes (about 2.2 MB) that every GPU which loads libsp2b200.so holds until
+ * the process exits.
+ *   H_dev       in : N x N, leading dimension ldh >= N, device memory, lower triangle read, not modified
+ *   bounds_dev  out: 2 doubles in DEVICE memory, {eps_min, eps_max}; NaN, NaN if a row of H is not finite
+ *   N           1 <= N <= SP2_GERSHGORIN_STATIC_MAX_N; larger N returns SP2_ERR_UNSUPPORTED_N and enqueues nothing
+ *                   (sp2_gershgorin_static_last_error() has the sentence; use sp2_gershgorin with a handle instead)
+ * The call only enqueues on `stream` (one 4-byte memset, two kernels, one 16-byte device-to-device copy) and returns;
+ * it does not synchronise and calls no cudaMalloc, cudaFree or other allocating routine.
+ *   - First call on a device: it also asks the runtime for the array's address on that device (cudaGetSymbolAddress,
+ *     with that device current) and for the SM count, which makes the runtime load the kernels.  Make this first call
+ *     before any stream capture; later calls on that device skip the set-up.
+ *   - All calls on a device share the one array, and it keeps the previous call's contents.  The call clears the one
+ *     word that must start at zero itself; everything else it reads it has written first.  Two calls that can run on the
+ *     GPU at the same time (different streams without an event between them, or two host threads) race on the array and
+ *     return garbage: order them. */
+#define SP2_GERSHGORIN_STATIC_MAX_N 4096
+sp2_status_t sp2_gershgorin_static(const float* H_dev, int N, int ldh, double* bounds_dev, void* stream);
+int          sp2_gershgorin_static_max_n(void);       /* SP2_GERSHGORIN_STATIC_MAX_N of the loaded library */
+size_t       sp2_gershgorin_static_bytes(void);       /* size of the static scratch, per GPU               */
+const char*  sp2_gershgorin_static_last_error(void);  /* text of this thread's last failed call, "" if none */
+
 const char* sp2_status_string(sp2_status_t s);
 const char* sp2_last_cuda_error(void);
 /* Number of kernels the last solve call on this handle launched (graph nodes executed are counted by the

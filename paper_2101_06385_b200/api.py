@@ -21,7 +21,9 @@ EXPORTS = ["sp2_default_opts", "sp2_create", "sp2_destroy", "sp2_workspace_bytes
            "sp2_density_matrix", "sp2_density_matrix_host", "sp2_generalized", "sp2_generalized_mix", "sp2_generalized_wb",
            "sp2_density_matrix_batched", "sp2_generalized_batched", "sp2_refine_energy", "sp2_split_fp16",
            "sp2_gershgorin", "sp2_status_string", "sp2_last_cuda_error", "sp2_last_launch_count",
-           "sp2_last_host_timing", "sp2_last_round_sync_broken", "sp2_last_sparse_work", "sp2_version"]
+           "sp2_last_host_timing", "sp2_last_round_sync_broken", "sp2_last_sparse_work", "sp2_version",
+           "sp2_gershgorin_static", "sp2_gershgorin_static_max_n", "sp2_gershgorin_static_bytes",
+           "sp2_gershgorin_static_last_error"]
 
 
 class LayerStat(C.Structure):
@@ -103,6 +105,10 @@ def load() -> C.CDLL:
     lib.sp2_last_host_timing.argtypes = [vp, dp]; lib.sp2_last_host_timing.restype = None
     lib.sp2_last_sparse_work.argtypes = [vp, dp]; lib.sp2_last_sparse_work.restype = None
     lib.sp2_version.argtypes = []; lib.sp2_version.restype = C.c_char_p
+    lib.sp2_gershgorin_static.argtypes = [vp, C.c_int, C.c_int, vp, vp]; lib.sp2_gershgorin_static.restype = C.c_int
+    lib.sp2_gershgorin_static_max_n.argtypes = []; lib.sp2_gershgorin_static_max_n.restype = C.c_int
+    lib.sp2_gershgorin_static_bytes.argtypes = []; lib.sp2_gershgorin_static_bytes.restype = C.c_size_t
+    lib.sp2_gershgorin_static_last_error.argtypes = []; lib.sp2_gershgorin_static_last_error.restype = C.c_char_p
     _lib = lib
     return lib
 
@@ -401,3 +407,23 @@ def split_fp16(X, fp16_scale_log2: int = 0, stream=None):
     if st < 0:
         raise SP2Error(st, "sp2_split_fp16")
     return hi, lo
+
+
+def gershgorin_static(H, out, stream=None):
+    """Gershgorin bounds of H through sp2_gershgorin_static: the variant for callers that cannot allocate device memory
+    (their own arena owns HBM, or a cudaMalloc's device-wide synchronisation is not acceptable where they call from).
+    No handle: the scratch is a static device array inside the library, which limits N to sp2_gershgorin_static_max_n()
+    (4096).  `out` is the CALLER's CUDA float64 tensor of 2 elements and receives {eps_min, eps_max}; nothing is
+    allocated here either, and the call does not synchronise -- read `out` after synchronising `stream`.  Calls share
+    the one scratch array: do not let two of them overlap on the GPU."""
+    import torch
+
+    H = _dev_f32(H, "H")
+    if not (isinstance(out, torch.Tensor) and out.is_cuda and out.dtype == torch.float64 and out.numel() == 2
+            and out.is_contiguous()):
+        raise TypeError("out must be a contiguous CUDA float64 tensor of 2 elements (the caller owns the output)")
+    lib = load()
+    st = lib.sp2_gershgorin_static(H.data_ptr(), H.shape[0], H.stride(0), out.data_ptr(), _stream_ptr(stream))
+    if st < 0:
+        raise RuntimeError(f"{lib.sp2_status_string(st).decode()}: {lib.sp2_gershgorin_static_last_error().decode()}")
+    return out

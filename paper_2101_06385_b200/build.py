@@ -9,7 +9,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsp2b200.so")
-SOURCES = ["sp2_elementwise.cu", "sp2_square_tiled.cu", "sp2_resident.cu", "sp2_api.cu"]
+SOURCES = ["sp2_elementwise.cu", "sp2_square_tiled.cu", "sp2_resident.cu", "sp2_api.cu", "sp2_noalloc.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 
