@@ -120,7 +120,11 @@ typedef struct {
                                <= trunc_tau count as zero (reading C28): their operand tiles are neither
                                loaded nor multiplied, and N_X = ||S'||_F^2 leaves them out.  0 (default): dense.
                                sp2_density_matrix / sp2_generalized(_wb) with tile_config 0 or 1, N <= 16384;
-                               exact_diag does not apply (the diagonal of X comes from the masked products).     */
+                               exact_diag does not apply (the diagonal of X comes from the masked products).
+                               With trunc_tau > 0, sp2_density_matrix keeps N <= 256 on the layer kernel (the
+                               resident one-launch path has no such variant); sp2_generalized_mix, sp2_refine_energy's
+                               layers and the batched calls do not take it: _mix returns SP2_ERR_INVALID_ARG, the
+                               others ignore the field.                                                          */
 } sp2_opts_t;
 
 /* Fill *o with defaults: auto_bounds=1, tol=0, max_layers=120, eps_alt=0, fp16_scale_log2=-1, control=0,

@@ -690,7 +690,8 @@ extern "C" sp2_status_t sp2_density_matrix(sp2_handle_t h, const float* H_dev, i
         if (!isfinite(o.homo) || !isfinite(o.lumo) || !(o.lumo > o.homo)) return SP2_ERR_INVALID_ARG;
         if (!o.auto_bounds && !(o.eps_min <= o.homo && o.lumo <= o.eps_max)) return SP2_ERR_INVALID_ARG;
     }
-    if (N <= 256 && o.tile_config == TILE_AUTO && o.control == 0 && !o.accelerated && ldh == N && ldd == N) {
+    if (N <= 256 && o.tile_config == TILE_AUTO && o.control == 0 && !o.accelerated && !(o.trunc_tau > 0.0) && ldh == N &&
+        ldd == N) {
         // small N: the whole solve in ONE launch of the resident kernel (matrix on chip across all layers) instead of
         // one kernel per layer.  (exact_diag does not apply there: the diagonal comes from the tensor core.)
         int nl = 0;
@@ -923,6 +924,8 @@ static sp2_status_t resident_solve(sp2_handle_s* h, const float* H_dev, int N, i
             }
         }
     h->last_launches = 1;
+    h->sparse_work[0] = h->sparse_work[1] = 0.0;             // the diagnostics of the single-matrix layer kernel do not
+    if (h->ctrl_host) h->ctrl_host->round_sync_broken = 0;   // apply here: report "dense" / "not broken", not the last solve's
     int worst = SP2_OK;
     for (int i = 0; i < B; ++i) {
         if (n_layers) n_layers[i] = nl[i];

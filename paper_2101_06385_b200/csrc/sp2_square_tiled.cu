@@ -88,9 +88,9 @@ __device__ __forceinline__ bool sparse_bit(const uint32_t (&m)[4], int kk) {
 
 // Grid-wide layer barrier of the persistent mode: wait until `target` layers of the solve have been applied (the CTA
 // that runs the control step publishes ctrl->n with release semantics), make the other CTAs' stores visible to this
-// thread's generic and async (TMA) accesses, and tell whether another layer follows.  One lane spins; bounded (a grid
+// thread's generic and async (TMA) accesses, and tell whether another layer follows.  Bounded spin (a grid
 // that is not co-resident cannot be launched in this mode -- cooperative launch -- so a time-out is a bug: trap).
-__device__ __forceinline__ bool layer_barrier_one(Ctrl* ctrl, int target) {      // called by ONE thread
+__device__ __forceinline__ bool layer_barrier_one(Ctrl* ctrl, int target) {      // per calling thread
     unsigned int spins = 0;
     int gen;
     do {
@@ -103,11 +103,14 @@ __device__ __forceinline__ bool layer_barrier_one(Ctrl* ctrl, int target) {     
     asm volatile("fence.proxy.async;\n" ::: "memory");
     return *((volatile int*)&ctrl->running) != 0;
 }
-__device__ __forceinline__ bool layer_barrier(Ctrl* ctrl, int target, int lane) {  // called by a whole warp
-    int run = 0;
-    if (lane == 0) run = layer_barrier_one(ctrl, target) ? 1 : 0;
-    run = __shfl_sync(0xffffffffu, run, 0);
-    return run != 0;
+// Whole warp: EVERY lane does the acquire load and both fences itself.  Acquire semantics and proxy fences are
+// per-thread; a value passed on by __shfl_sync orders nothing for the receiving lanes, and the lane that issues the next
+// layer's TMA loads is whichever one elect.sync picks.  (The 32 polls of one address are one L2 request.)
+__device__ __forceinline__ bool layer_barrier(Ctrl* ctrl, int target, int lane) {
+    (void)lane;
+    int run = layer_barrier_one(ctrl, target) ? 1 : 0;
+    run = __shfl_sync(0xffffffffu, run, 0);               // warp-uniform by construction (running is published before
+    return run != 0;                                      // layer_gen); the shuffle only keeps the branch convergent
 }
 
 
@@ -726,12 +729,10 @@ k_sp2_layer(const __grid_constant__ CUtensorMap tm_hi0, const __grid_constant__ 
                     float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
                     __half* __restrict__ rowH = HO + (long long)gi * ldf + gj0;
                     __half* __restrict__ rowL = LO + (long long)gi * ldf + gj0;
-#pragma unroll
                     uint32_t hq[4], lq[4];                  // the previous group's pairs (own rows leave as 32-byte stores)
 #pragma unroll
                     for (int g = 0; g < 4; ++g) {           // 8 columns at a time: values leave registers early
                         uint32_t hp[4], lp[4];              // FP16 pairs (even column in the low half)
-#pragma unroll
                         float vals[8];
 #pragma unroll
                         for (int e = 0; e < 8; ++e) vals[e] = fmaf(th1s, __uint_as_float(v[8 * g + e]), th2 * so[8 * g + e]);
