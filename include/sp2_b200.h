@@ -59,16 +59,19 @@ typedef enum {
 enum { SP2_STOP_NONE = 0, SP2_STOP_IDERR_NONPOS = 1, SP2_STOP_PARAM_FREE = 2, SP2_STOP_TOL = 3,
        SP2_STOP_MAX_LAYERS = 4, SP2_STOP_NONFINITE = 5,
        /* Alg. 1's first test "IdErr_n <= 0" taken at the resolution of the arithmetic (reading C25):
-          after layer n, IdErr_n <= |Tr X_n(tensor core) - N_X(exact, FP64)|, i.e. the idempotency estimate has
+          after layer n, IdErr_n <= kappa |Tr X_n(tensor core) - N_X(fixed-point ||S||_F^2)|, i.e. the estimate has
           dropped below the measured error of the trace it is built from.  Reduces to test 1 in exact arithmetic. */
        SP2_STOP_NOISE_FLOOR = 6 };
 
 /* Per-layer statistics, entry n-1 describes layer n (n = 1..n_layers), Alg. 1's notation. */
 typedef struct {
-    double trace_S;       /* N_S = Tr[S_n] after the layer: FP64 sum of the FP32 diagonal of S_n            */
+    /* The three traces are accumulated on the device as 64-bit integers in 2^40 fixed point (order-independent, so
+       bit-reproducible; reading C29) and converted to double by the host. */
+    double trace_S;       /* N_S = Tr[S_n] after the layer: the FP32 diagonal of S_n, each entry converted exactly */
     double trace_X;       /* N_X = Tr[X_n] used by the control, evaluated as ||S_{n-1}||_F^2 (= Tr[S^2] for
-                             symmetric S) in FP64 while S_{n-1} was written                           */
-    double trace_X_diag;  /* cross-check: FP64 sum of the diagonal of the tensor-core X_n                    */
+                             symmetric S) while S_{n-1} was written: FP32 partial sums of <= 32 squares,
+                             added as integers (relative error <= 31 * 2^-24, measured 1e-11)               */
+    double trace_X_diag;  /* cross-check: sum of the diagonal of the tensor-core X_n, entries converted exactly */
     double iderr;         /* IdErr_n = N_S(before) - N_X = Tr[S_{n-1} - S_{n-1}^2]           */
     int    sigma;         /* +1: S_n = X_n ; -1: S_n = 2 S_{n-1} - X_n ; 0 in generalized runs               */
     int    stop_reason;   /* SP2_STOP_* : nonzero only on the last layer                                     */
@@ -93,8 +96,9 @@ typedef struct {
     int    tile_config;     /* 0: choose by N; 1: 128x128 1-CTA; 2: 128x256 1-CTA; 3: 256x256 2-CTA;
                                4: 128x128 1-CTA with the enhanced accumulation of sp2_refine_energy in EVERY
                                layer (accuracy option, about 2x the time of 3 at large N)  */
-    int    exact_diag;      /* 1 (default): diag(X_n)_i = sum_j S_ij^2 is taken from FP32/FP64 row sums of the
-                               FP32 S_{n-1} (the same identity that gives N_X = ||S||_F^2) instead of the
+    int    exact_diag;      /* 1 (default): diag(X_n)_i = sum_j S_ij^2 is taken from row sums of squares of the
+                               FP32 S_{n-1} (FP32 partial sums added as 2^44 fixed-point integers; the same
+                               identity that gives N_X = ||S||_F^2) instead of the
                                tensor-core accumulator, whose truncating FP32 accumulation biases the large
                                diagonal by ~ (3N/32) ulp, ramping along the diagonal (reading C24);
                                0: Alg. 2 literally (tensor-core diagonal). Single-matrix path only.           */
@@ -110,7 +114,7 @@ typedef struct {
                                call takes per-matrix estimates through its own arguments instead.             */
     double noise_kappa;     /* kappa of the noise-floor stop (reading C25: Alg. 1's "IdErr_n <= 0", P:136,
                                at the resolution of the arithmetic): stop after layer n > 2 when
-                               IdErr_n <= kappa |Tr X_n(tensor core) - N_X(FP64)|.  < 0: library default (0.125);
+                               IdErr_n <= kappa |Tr X_n(tensor core) - N_X|.  < 0: library default (0.125);
                                0: test disabled (Alg. 1's printed tests, tol and max_layers only)              */
     int    enh_kc;          /* enhanced accumulation (tile_config 4, sp2_refine_energy): K-blocks of 64 the tensor
                                core accumulates before the chunk sum is folded into the error-free FP32 pair

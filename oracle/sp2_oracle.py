@@ -431,13 +431,15 @@ def truncate_blocks(S, tau, block=128):
 
 
 def sp2_blocked_ref(H32, N_occ, bounds=None, tau=0.0, block=128, tol=0.0, max_layers=120, eps_alt=0.0,
-                    forced_sigma=None):
+                    forced_sigma=None, square=None):
     """Alg. 1 on block-truncated iterates (reading C28).  Layer n:
          S' = truncate_blocks(S_{n-1}, tau);  X_n = S' S';  N_X = Tr X_n;  IdErr_n = N_S - N_X with N_S = Tr S'
          (= Tr S_{n-1}: diagonal blocks are never cut);  sigma_n by Alg. 1's rule;  S_n = sigma_n X_n + (1 - sigma_n) S'.
     Same stop tests and outputs as sp2_ref, plus st["kept_fraction"][n-1] = surviving fraction of the b x b blocks and
     st["work_fraction"][n-1] = fraction of the block products S'_IK S'_KJ (I >= J) whose two factors both survive --
-    the tensor-core work a blocked implementation has left."""
+    the tensor-core work a blocked implementation has left.
+    square: test hook (default None = the plain NumPy product `Sp @ Sp`): a callable A -> A @ A in FP64 computed by another
+    library routine, for the sizes (N > 8192) where NumPy needs minutes per layer.  Nothing else changes."""
     H = symmetrize_lower(H32)
     eps_min, eps_max = gershgorin_bounds(H) if bounds is None else (float(bounds[0]), float(bounds[1]))
     if not (eps_max > eps_min):
@@ -451,7 +453,7 @@ def sp2_blocked_ref(H32, N_occ, bounds=None, tau=0.0, block=128, tol=0.0, max_la
     while stop == STOP_NONE:
         n += 1
         Sp, kept = truncate_blocks(S, tau, block)
-        X = Sp @ Sp
+        X = Sp @ Sp if square is None else square(Sp)
         N_X = float(np.trace(X))
         iderr = N_S - N_X
         sigma, d = _sign_rule(N_S, N_X, N_occ, sigma_hist[n - 1], eps_alt)

@@ -8,9 +8,12 @@
 // latencies; back-to-back DFMAs run at 9).  The ~40 FP64 instructions of an FP64 control step, interleaved with
 // integer code, cost ~6000 cycles -- as much as a whole N = 256 layer on the tensor cores -- and the FP64 shuffle
 // reductions in front of it as much again.  Fixed point is also exact where FP64 is not: integer adds do not round,
-// so sums are order-independent (bit-reproducible) and IdErr = N_S - N_X cancels without loss.  An FP32 value v
-// converts exactly as llrint(v 2^40) for |v| < 8.4e6 (resolution 9.1e-13): all traces of a spectrum in [0, 1] with
-// N <= 2^22 fit.  The host converts the per-layer statistics back to doubles.
+// so sums are order-independent (bit-reproducible) and the subtraction IdErr = N_S - N_X itself loses nothing.  An FP32
+// value v converts exactly as llrint(v 2^40) for |v| < 8.4e6 (resolution 9.1e-13): all traces of a spectrum in [0, 1]
+// with N <= 2^22 fit.  What is NOT exact is N_X = ||S||_F^2: only Tr S (and the diagonal squares) are converted element
+// by element; off-diagonal squares are first summed in FP32 over at most 32 elements and that partial sum is converted,
+// so N_X carries up to 31 * 2^-24 relative error in the worst case (measured 1e-11 relative = 5e-8 absolute at
+// N = 16384, tests/test_gpu_fullsize.py).  The host converts the per-layer statistics back to doubles.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -59,7 +62,7 @@ struct CtrlCore {
     fx_t   N_S;                      // Tr S_n (measured)
     fx_t   fro2;                     // ||S_n||_F^2 = N_X of layer n+1
     fx_t   iderr_prev, iderr_prev2;  // IdErr_n, IdErr_{n-1}
-    fx_t   nx_inflight;              // N_X of the layer in flight (exact pre-trace)
+    fx_t   nx_inflight;              // N_X of the layer in flight: ||S_{n-1}||_F^2 from the fixed-point sums (see above)
     int    nonfinite;                // a trace of the current iterate was NaN / Inf / out of range
     int    kappa_q16;                // reading C25: stop when IdErr_n <= kappa |Tr X_n(tc) - N_X|; kappa * 2^16; 0 disables
     float  acc_h, acc_l;             // accelerated scheme (section V.A): lower bound of the occupied, upper bound of

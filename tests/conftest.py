@@ -10,6 +10,7 @@ if ROOT not in sys.path:
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box)")
+    config.addinivalue_line("markers", "gpu_probe: hardware timing probes on a B200 (not parity; outside -m gpu)")
 
 
 @pytest.fixture(scope="session")

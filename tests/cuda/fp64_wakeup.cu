@@ -1,6 +1,6 @@
 // Measures what the integer-only control step of the library rests on (sp2_control.cuh): on B200 an FP64 instruction
 // that follows a stretch of non-FP64 work pays a wake-up latency far above its pipeline latency, while back-to-back
-// FP64 instructions do not.  Prints "name cycles_per_iteration" lines; built and run by tests/test_gpu_arith_facts.py.
+// FP64 instructions do not.  Prints "name cycles_per_iteration" lines; built and run by tests/test_probe_hardware.py.
 #include <cstdio>
 #include <cuda_runtime.h>
 

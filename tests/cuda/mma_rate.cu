@@ -3,7 +3,7 @@
 // sp2_square_tiled.cu) rests on the fact that an MMA with N = 128 is NOT issued twice as often as one with N = 256.
 // One CTA (or one CTA pair) issues `reps` rounds of a pattern of MMAs from shared-memory tiles, commits, and waits; prints
 // "name cycles_per_mma" lines (k_rate) and "name cycles_per_stage" lines for the layer kernel's ring of stages without
-// its loads (k_ring).  Built and run by tests/test_gpu_arith_facts.py.  What it showed (B200):
+// its loads (k_ring).  Built and run by tests/test_probe_hardware.py.  What it showed (B200):
 //   * an MMA issued under `if (lane == 0)` costs ~105 cycles whatever its N <= 128 (the compiler wraps it in a loop of
 //     R2UR.BROADCASTs); issued by an elect.sync thread in warp-uniform control flow it runs at the pipe rate (N = 128:
 //     64 cycles, N = 256: 128);

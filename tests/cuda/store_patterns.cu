@@ -1,6 +1,6 @@
 // Store patterns of the layer epilogue (sp2_square_tiled.cu) in isolation: each warp owns 32 rows of a matrix with the
 // N = 2048 operand pitch and writes 64 bytes of each row per iteration (the own-row FP16 piece of a 32 x 32 chunk), or the
-// mirrored pieces row by row.  Prints "name GB_per_s" lines; built and run by tests/test_gpu_arith_facts.py.  What it
+// mirrored pieces row by row.  Prints "name GB_per_s" lines; built and run by tests/test_probe_hardware.py.  What it
 // showed (B200, all 148 SMs): a lane that writes its own row in 16-byte stores gets 1.65 TB/s, in 32-byte st.global.v8
 // 4.3 TB/s (a sector per lane either way); 64-byte row segments reach 4.5 - 4.7 TB/s however they are packaged, 128-byte
 // ones 6.3 TB/s.

@@ -29,21 +29,42 @@ def branch_prefix_check(gpu, ref, N_occ):
     return n_star, mism
 
 
-def replay_check(gpu, H32, N_occ, bounds, eigs=None):
+# Measured trace noise of the mixed-precision path against the FP64 recursion replayed under the same branch sequence
+# (C24 / C6): it grows with the size of the traces.  TRACE_NOISE_REL * max(1, N_occ) replaces the planning value
+# 1e-3 * N_occ of rounds 1-2 (8.2 absolute at N = 16384, which pinned nothing: IdErr is below 8 on nearly every layer).
+TRACE_NOISE_REL = 1.25e-4     # 1.0 absolute at N_occ = 8192 (measured there: 0.3 - 0.4)
+TRACE_NOISE_ABS = 2e-3        # floor for small problems (FP16 hi/lo operands: ~1e-6 per entry of X)
+IDERR_REL = 0.02              # IdErr while it still decays: measured <= 0.3 % of the replayed value
+IDERR_NOISE_FRAC = 0.125      # IdErr at the floor: the errors of N_S and N_X largely cancel in N_S - N_X; measured
+                              # <= 0.055 at N_occ = 8192 (bound 0.128), <= 7e-3 at N_occ = 1750 (bound 0.027)
+
+
+def replay_check(gpu, H32, N_occ, bounds, eigs=None, verbose=True):
     """Reading C6 (ii): the GPU's per-layer traces must match the FP64 recursion replayed under the GPU's own
-    branch sequence (scalar recursion on the eigenvalues when known, else the matrix oracle)."""
+    branch sequence (scalar recursion on the eigenvalues when known, else the matrix oracle).  Traces: within the
+    measured trace noise.  IdErr: within max(2 % of the replayed value, 1/8 of the trace noise), so that both the decaying part
+    (relative) and the converged tail (absolute, at the noise floor) are pinned."""
     sig = gpu["sigma"]
     if eigs is not None:
         rep = O.scalar_recursion(eigs, N_occ, bounds[0], bounds[1], forced_sigma=sig)
     else:
         _, rep = O.sp2_ref(H32, N_occ, bounds, forced_sigma=sig)
-    tol = 1e-3 * max(1.0, N_occ)
+    noise = max(TRACE_NOISE_ABS, TRACE_NOISE_REL * max(1.0, N_occ))
     n = len(sig)
+    dev = {}
     for key in ("trace_S", "trace_X"):
         a, b = np.array(gpu[key][:n]), np.array(rep[key][:n])
-        assert np.abs(a - b).max() <= tol, f"{key}: {np.abs(a - b).max()} > {tol}"
+        dev[key] = float(np.abs(a - b).max()) if n else 0.0
     a, b = np.array(gpu["iderr"][:n]), np.array(rep["iderr"][:n])
-    assert np.abs(a - b).max() <= tol
+    allowed = np.maximum(IDERR_REL * np.abs(b), IDERR_NOISE_FRAC * noise)
+    excess = (np.abs(a - b) / allowed) if n else np.zeros(1)
+    dev["iderr"] = float(np.abs(a - b).max()) if n else 0.0
+    if verbose:
+        print(f"replay_check N_occ={N_occ:g} layers={n}: max dev trace_S {dev['trace_S']:.3e} trace_X {dev['trace_X']:.3e} "
+              f"iderr {dev['iderr']:.3e} (noise bound {noise:.3e}; worst iderr dev / allowed {float(excess.max()):.3f})")
+    for key in ("trace_S", "trace_X"):
+        assert dev[key] <= noise, f"{key}: {dev[key]} > {noise}"
+    assert float(excess.max()) <= 1.0, f"iderr: layer {int(excess.argmax()) + 1} off by {float(excess.max()):.3f} x allowed"
     return rep
 
 
