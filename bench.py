@@ -261,6 +261,108 @@ def other_configs(api, W, torch, dev, stream, _time):
     return out
 
 
+def next_rows_and_sweep(api, W, torch, dev, stream, _time, sustained_tflops):
+    """detail.blocked_sparse_next4, detail.mix_next2, detail.size_sweep (rank 0, outside the timed step):
+    the two NEXT rows that had no driver-run number, and the layer kernel's throughput against N (the paper's one
+    performance figure is TFLOP/s against system size, Fig. 3)."""
+    base_time = _time
+
+    def _time(fn, reps=5):
+        t0 = time.perf_counter()
+        while time.perf_counter() - t0 < 0.03:          # clocks back up after host-side set-up (see other_configs)
+            fn()
+        return base_time(fn, reps=reps)
+
+    h = api.Handle(16384, 0, 120)
+    # ---- NEXT-4: blocked-sparse variant on the decaying chain (P:206, reading C28), tau = 1e-6, against the dense layer
+    # kernel with the same 128 x 128 tiles and the tensor-core diagonal (what the sparse instantiation computes when
+    # nothing is cut)
+    sparse = {}
+    for n in (2048, 8192, 16384):
+        w = W.decaying_chain(n, n=n)
+        Hd = torch.from_numpy(w.H32).to(dev)
+        o_s = api.make_opts(tol=w.tol, max_layers=w.max_layers, trunc_tau=1e-6)
+        o_d = api.make_opts(tol=w.tol, max_layers=w.max_layers, tile_config=1, exact_diag=0)
+        o_0 = api.make_opts(tol=w.tol, max_layers=w.max_layers)
+        Ds = torch.empty_like(Hd)
+        ms_s = _time(lambda: h.density_matrix(Hd, w.N_occ, o_s, out=Ds, stream=stream), reps=3)
+        _, i_s = h.density_matrix(Hd, w.N_occ, o_s, out=Ds, stream=stream)
+        Dd = torch.empty_like(Hd)
+        ms_d = _time(lambda: h.density_matrix(Hd, w.N_occ, o_d, out=Dd, stream=stream), reps=3)
+        _, i_d = h.density_matrix(Hd, w.N_occ, o_d, out=Dd, stream=stream)
+        ms_0 = _time(lambda: h.density_matrix(Hd, w.N_occ, o_0, out=Dd, stream=stream), reps=3)
+        _, i_0 = h.density_matrix(Hd, w.N_occ, o_0, out=Dd, stream=stream)
+        Dc = Ds.double()
+        sparse[f"decaying_chain_N{n}"] = dict(
+            ms_sparse=ms_s, layers_sparse=i_s["n_layers"], work_fraction=i_s["work_fraction"],
+            us_per_layer_sparse=ms_s / i_s["n_layers"] * 1e3,
+            ms_dense_same_tiles=ms_d, layers_dense_same_tiles=i_d["n_layers"],
+            ms_dense_default=ms_0, layers_dense_default=i_0["n_layers"],
+            max_abs_diff_sparse_vs_dense_default=float((Ds - Dd).abs().max()),
+            trace_err=float(torch.trace(Dc)) - w.N_occ,
+            idempotency=float(torch.linalg.norm(Dc @ Dc - Dc)) / np.sqrt(n), symmetric=bool(torch.equal(Ds, Ds.T)))
+        del Hd, Ds, Dd, Dc
+    sparse["what"] = ("sp2_density_matrix, Gershgorin bounds, tol 1e-5; sparse: opts.trunc_tau = 1e-6; dense_same_tiles: "
+                      "tile_config = 1, exact_diag = 0; dense_default: library defaults")
+    # ---- NEXT-2: output mix F~ = I - sum_i c_i E_i (Eqs. 17-18), N = 4096, 11 layers, against the scalar network on the
+    # known eigenvalues through the known eigenbasis
+    rng = np.random.default_rng(42)
+    n, L = 4096, 11
+    Q = W.haar_orthogonal(rng, n, dev)
+    lam = rng.uniform(-1.0, 1.0, n)
+    Qd = torch.from_numpy(Q).to(dev)
+    Hs = (Qd * torch.from_numpy(lam).to(dev)[None, :]) @ Qd.T
+    Hd = ((Hs + Hs.T) * 0.5).float().contiguous()
+    theta = []
+    for k in range(L):                                   # alternating SP2 polynomials with seeded perturbations
+        b0 = (1.0, 0.0) if k % 2 else (-1.0, 2.0)
+        wk = 1.0 + rng.normal(0, 0.02)
+        theta.append((wk * b0[0], wk * b0[1], rng.normal(0, 0.005)))
+    theta = np.array(theta)
+    c = rng.normal(0, 0.05, L + 1)
+    c[-1] += 1.0
+    ms_m = _time(lambda: h.generalized_mix(Hd, theta, c, bounds=(-1.0, 1.0), stream=stream), reps=5)
+    F, _ = h.generalized_mix(Hd, theta, c, bounds=(-1.0, 1.0), stream=stream)
+    ms_g = _time(lambda: h.generalized(Hd, theta, bounds=(-1.0, 1.0), stream=stream), reps=5)
+    e = (lam + 1.0) / 2.0
+    acc = c[0] * e
+    for k in range(L):
+        e = theta[k, 0] * e * e + theta[k, 1] * e + theta[k, 2]
+        acc = acc + c[k + 1] * e
+    Fstar = (Qd * torch.from_numpy(1.0 - acc).to(dev)[None, :]) @ Qd.T
+    mix = dict(N=n, layers=L, ms_per_call=ms_m, us_per_layer=ms_m / L * 1e3, ms_same_network_without_mix=ms_g,
+               max_abs_err_vs_scalar_network=float((F.double() - Fstar).abs().max()),
+               symmetric=bool(torch.equal(F, F.T)),
+               what="sp2_generalized_mix, caller bounds (-1, 1), seeded theta (alternating SP2 polynomials, w = 1 + N(0, "
+                    "0.02), b = N(0, 0.005)) and c; reference Q diag(1 - sum_i c_i e_i) Q^T in FP64")
+    del Q, Qd, Hs, Hd, F, Fstar
+    # ---- layer time against N: 10 fixed layers (sigma alternating), caller bounds, default tile choice
+    sweep = []
+    L = 10
+    sig = np.array([1, -1] * (L // 2))
+    ones, zeros = np.ones(L), np.zeros(L)
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(1234)
+    for n in (1024, 2048, 3072, 4096, 6144, 8192, 12288, 16384):
+        A = torch.rand((n, n), device=dev, generator=gen) * 2.0 - 1.0
+        Hd = (torch.tril(A) + torch.tril(A, -1).T).contiguous()
+        del A
+        r = 1.3 * float(np.sqrt(n))                      # encloses the semicircle of radius 2 sqrt(n / 3)
+        ms = _time(lambda: h.generalized_wb(Hd, sig, ones, zeros, bounds=(-r, r), stream=stream), reps=5)
+        X, info = h.generalized_wb(Hd, sig, ones, zeros, bounds=(-r, r), stream=stream)
+        t = np.diff(np.array(info["t_end_ns"], dtype=np.float64)) * 1e-3       # device timer, layer to layer
+        us = float(np.median(t))
+        tf = 3.0 * n ** 3 / (us * 1e-6) / 1e12
+        sweep.append(dict(N=n, us_per_layer=us, ms_per_call_10_layers=ms, executed_tflops_3N3=tf,
+                          frac_of_sustained_peak=tf / sustained_tflops, finite=bool(torch.isfinite(X).all())))
+        del Hd, X
+    h.close()
+    return sparse, mix, {"points": sweep,
+                         "what": "sp2_generalized_wb, 10 layers (sigma = +1, -1, ...; w = 1, b = 0), H uniform in [-1, 1] "
+                                 "symmetric, caller bounds; us_per_layer = median interval of the per-layer device "
+                                 "timestamps; executed flops = 3 N^3 per layer"}
+
+
 def run_reference(args):
     """--impl reference: the oracle timed on the host cores (rank 0 only)."""
     rank = int(os.environ.get("RANK", "0"))
@@ -523,12 +625,13 @@ def main():
                "api": "sp2_density_matrix_host (pinned host buffers)"}
         del Hh, Dh
 
-    configs = None
+    configs = sparse4 = mix2 = sweep = None
     if rank == 0 and not args.no_configs:
         h.close()
         del H, D
         torch.cuda.empty_cache()
         configs = other_configs(api, W, torch, dev, stream, _time)
+        sparse4, mix2, sweep = next_rows_and_sweep(api, W, torch, dev, stream, _time, float(peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"])))
         h = None
 
     cpu = None
@@ -559,6 +662,7 @@ def main():
                        "D_exactly_symmetric": symmetric,
                        "frac_of_same_run_cublas_fp16": (exec_tflops / yard["tflops"]) if yard else None,
                        "cublas_fp16_yardstick": yard, "hbm_kernels": hbm_kernels, "refinement_next1": refine, "accelerated_next3": accel,
+                       "blocked_sparse_next4": sparse4, "mix_next2": mix2, "size_sweep": sweep,
                        "configs": configs,
                        "paper_context": "paper: ~120 TFLOP/s on A100 (P:204), other hardware, count unstated",
                        "wall_s_timed_region": t_wall},
