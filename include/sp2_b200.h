@@ -158,7 +158,10 @@ sp2_status_t sp2_density_matrix(sp2_handle_t h, const float* H_dev, int N, int l
                                 sp2_layer_stat_t* stats_host, int* n_layers, double bounds_out[2],
                                 void* stream);
 
-/* Same call with HOST buffers: copies H to the device, solves, copies D back (end-to-end path). */
+/* Same call with HOST buffers: copies H to the device, solves, copies D back (end-to-end path).  Only the lower
+ * triangle of H_host is read, so for N > 1024 only it is copied (row bands of 256 rows up to the band's last diagonal
+ * element: about half the bytes); D_host receives the full symmetric matrix.  The three phases are serial by nature: the
+ * first layer needs the bounds, which need all of H, and D exists only after the last layer. */
 sp2_status_t sp2_density_matrix_host(sp2_handle_t h, const float* H_host, int N, int ldh, double N_occ,
                                      const sp2_opts_t* opts, float* D_host, int ldd,
                                      sp2_layer_stat_t* stats_host, int* n_layers, double bounds_out[2],
@@ -272,6 +275,8 @@ int         sp2_last_launch_count(sp2_handle_t h);
 /* Device-side durations (CUDA events on `stream`) of the three phases of the last sp2_density_matrix_host call on
  * this handle, in ms: {host -> device copy of H, the solve, device -> host copy of D}. */
 void        sp2_last_host_timing(sp2_handle_t h, double ms[3]);
+/* Bytes the last sp2_density_matrix_host call on this handle copied: out[0] host -> device, out[1] device -> host. */
+void        sp2_last_host_bytes(sp2_handle_t h, double out[2]);
 /* Blocked-sparse variant (opts->trunc_tau > 0): out[0] = 128-wide block products the tensor cores executed during the
  * last single-matrix solve on this handle, summed over tiles and layers; out[1] = what a dense solve of the same layers
  * would have executed.  Both 0 after a dense solve. */

@@ -21,7 +21,7 @@ EXPORTS = ["sp2_default_opts", "sp2_create", "sp2_destroy", "sp2_workspace_bytes
            "sp2_density_matrix", "sp2_density_matrix_host", "sp2_generalized", "sp2_generalized_mix", "sp2_generalized_wb",
            "sp2_density_matrix_batched", "sp2_generalized_batched", "sp2_refine_energy", "sp2_split_fp16",
            "sp2_gershgorin", "sp2_status_string", "sp2_last_cuda_error", "sp2_last_launch_count",
-           "sp2_last_host_timing", "sp2_last_round_sync_broken", "sp2_last_sparse_work", "sp2_version",
+           "sp2_last_host_timing", "sp2_last_host_bytes", "sp2_last_round_sync_broken", "sp2_last_sparse_work", "sp2_version",
            "sp2_gershgorin_static", "sp2_gershgorin_static_max_n", "sp2_gershgorin_static_bytes",
            "sp2_gershgorin_static_last_error"]
 
@@ -104,6 +104,7 @@ def load() -> C.CDLL:
     lib.sp2_last_round_sync_broken.argtypes = [vp]; lib.sp2_last_round_sync_broken.restype = C.c_int
     lib.sp2_last_host_timing.argtypes = [vp, dp]; lib.sp2_last_host_timing.restype = None
     lib.sp2_last_sparse_work.argtypes = [vp, dp]; lib.sp2_last_sparse_work.restype = None
+    lib.sp2_last_host_bytes.argtypes = [vp, dp]; lib.sp2_last_host_bytes.restype = None
     lib.sp2_version.argtypes = []; lib.sp2_version.restype = C.c_char_p
     lib.sp2_gershgorin_static.argtypes = [vp, C.c_int, C.c_int, vp, vp]; lib.sp2_gershgorin_static.restype = C.c_int
     lib.sp2_gershgorin_static_max_n.argtypes = []; lib.sp2_gershgorin_static_max_n.restype = C.c_int
@@ -219,8 +220,10 @@ class Handle:
         info = _stats_to_dict(stats, nl.value)
         ms = (C.c_double * 3)()
         self.lib.sp2_last_host_timing(self._h, ms)
+        nbytes = (C.c_double * 2)()
+        self.lib.sp2_last_host_bytes(self._h, nbytes)
         info.update(status=st, n_layers=nl.value, bounds=(bounds[0], bounds[1]),
-                    h2d_ms=ms[0], solve_ms=ms[1], d2h_ms=ms[2])
+                    h2d_ms=ms[0], solve_ms=ms[1], d2h_ms=ms[2], h2d_bytes=int(nbytes[0]), d2h_bytes=int(nbytes[1]))
         return D, info
 
     # -- generalized network

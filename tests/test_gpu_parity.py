@@ -286,6 +286,18 @@ def test_tiled_kernel_bit_reproducible_and_host_entry(env, n, tile, auto):
         assert i1[key] == i2[key], key
     Dh, ih = h.density_matrix_host(w.H32, w.N_occ, opts)
     assert np.array_equal(Dh, D1.cpu().numpy()) and ih["trace_S"] == i1["trace_S"] and ih["bounds"] == i1["bounds"]
+    # the host entry point copies the lower triangle only (bands of 256 rows, N > 1024): a poisoned upper triangle of
+    # the host matrix changes nothing, and the reported byte counts are those of the copies
+    Hp = w.H32.copy()
+    Hp[np.triu_indices(n, 1)] = np.nan
+    Dp, ip = h.density_matrix_host(Hp, w.N_occ, opts)
+    assert np.array_equal(Dp, Dh) and ip["trace_S"] == ih["trace_S"]
+    assert ip["d2h_bytes"] == 4 * n * n
+    if n > 1024:
+        bands = [(r0, min(n, r0 + 256)) for r0 in range(0, n, 256)]
+        assert ip["h2d_bytes"] == sum(4 * r1 * (r1 - r0) for r0, r1 in bands) < 0.6 * 4 * n * n
+    else:
+        assert ip["h2d_bytes"] == 4 * n * n
     P.assert_acceptance(D1.cpu().numpy().astype(np.float64), O.closed_form_density(w.Q, w.N_occ), w.N_occ, f"N={n}")
 
 
