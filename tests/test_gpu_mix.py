@@ -95,3 +95,38 @@ def test_mix_special_weights_reduce_to_known_calls(env):
         h.generalized_mix(Hd, theta, np.zeros(L + 1), bounds=w.bounds, opts=api.make_opts(tile_config=2))
     with pytest.raises(api.SP2Error):
         h.generalized_mix(Hd, theta, np.full(L + 1, np.nan), bounds=w.bounds)
+
+
+def test_fermi_function_from_the_fitted_network(env):
+    """The thing the output mix was built for (Eqs. 17-20; Fig. 6): with the LM-fitted coefficients of
+    tests/golden/fermi_fit_beta40_L11.json (11 layers, beta = 40; written by tests/golden/make_fermi_fit.py from the
+    oracle's definitions), sp2_generalized_mix turns H into the finite-temperature density matrix F(H).  Compared
+    elementwise with the oracle's matrix network, and with the exact Q diag(F(eps)) Q^T within the fit's own residual."""
+    import json
+    import os
+
+    api, h, torch = env
+    fit = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "fermi_fit_beta40_L11.json")))
+    theta, c = np.array(fit["theta"]), np.array(fit["c"])
+    n = 1024
+    rng = np.random.default_rng(2024)
+    Q = W.haar_orthogonal(rng, n)
+    lam = rng.uniform(0.0, 1.0, n)                       # the rescaled energies of Eq. 20: bounds (0, 1)
+    lam[:64] = rng.uniform(0.45, 0.55, 64)               # ... with extra weight inside the thermal window 1/beta
+    H32 = ((Q * lam) @ Q.T).astype(np.float32)
+    H32 = np.ascontiguousarray((H32 + H32.T) / 2)
+    for tile in (1, 3):
+        F, info = h.generalized_mix(torch.from_numpy(H32).cuda(), theta, c, bounds=(0.0, 1.0),
+                                    opts=api.make_opts(tile_config=tile))
+        F = F.cpu().numpy().astype(np.float64)
+        ref = O.generalized_mix_ref(H32, theta, c, (0.0, 1.0))
+        exact = (Q * O.fermi_function(lam, fit["beta"])) @ Q.T
+        e_ref, e_exact = np.abs(F - ref).max(), np.abs(F - exact).max()
+        occ = float(np.trace(F))
+        print(f"Fermi fit (11 layers, beta = 40) N={n} tile={tile}: max|F - oracle network| = {e_ref:.2e}, "
+              f"max|F - exact Fermi matrix| = {e_exact:.2e} (fit residual {fit['max_error_fine_grid']:.2e}), "
+              f"Tr F = {occ:.4f} against sum F(eps) = {O.fermi_function(lam, fit['beta']).sum():.4f}")
+        assert e_ref <= 2e-5                              # measured 1.0e-6 / 1.6e-6
+        assert e_exact <= fit["max_error_fine_grid"] + 2e-5   # measured 2.4e-6 / 2.8e-6 (the matrix error averages the fit's)
+        assert np.array_equal(F, F.T) and info["n_layers"] == 11
+        assert abs(occ - O.fermi_function(lam, fit["beta"]).sum()) <= 1e-3 * n

@@ -90,3 +90,34 @@ def test_truncated_sp2_is_a_smooth_step_like_the_fermi_function():
     # it is closer to a Fermi function of some finite beta than to the sharp step
     best = min(np.abs(f - O.fermi_function(x - mid + 0.5, b)).max() for b in np.linspace(5, 200, 80))
     assert best < 0.5 * np.abs(f - (x < mid)).max()
+
+
+def test_stored_fermi_fit_reproduces_eq20():
+    """tests/golden/fermi_fit_beta40_L11.json (written by tests/golden/make_fermi_fit.py: LM fit of Eqs. 17-18 to Eq. 20,
+    beta = 40, 11 layers -- the workload of Fig. 6): the stored coefficients, run through this file's own scalar
+    loop and through the oracle's matrix network, give the Fermi function within the stored residual.  The paper shows
+    the error curve only as an image; its text claims the accuracy of rational Pade schemes, i.e. small against
+    the width 1/beta of the step -- asserted here as < 1e-3."""
+    import json
+    import os
+
+    fit = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "fermi_fit_beta40_L11.json")))
+    theta, c = np.array(fit["theta"]), np.array(fit["c"])
+    assert theta.shape == (11, 3) and c.shape == (12,) and fit["beta"] == 40.0
+    x = np.linspace(0.0, 1.0, 401)
+    F = 1.0 / (np.exp(40.0 * (x - 0.5)) + 1.0)                       # Eq. 20 retyped
+    got = _scalar_net(x, theta, c)
+    err = np.abs(got - F).max()
+    assert err <= fit["max_error_fine_grid"] * (1 + 1e-9) < 1e-3
+    assert np.abs(O.fermi_function(x, 40.0) - F).max() < 1e-15
+    # a monotonically decreasing step: ~1 at 0, 1/2 at 1/2, ~0 at 1
+    assert abs(got[0] - 1.0) < 1e-4 and abs(got[200] - 0.5) < 1e-4 and abs(got[-1]) < 1e-4
+    # the oracle's matrix network on a rotated H with spectrum x and bounds (0, 1)
+    rng = np.random.default_rng(5)
+    Q = W.haar_orthogonal(rng, 48)
+    lam = rng.uniform(0.0, 1.0, 48)
+    H32 = ((Q * lam) @ Q.T).astype(np.float32)
+    Fm = O.generalized_mix_ref(H32, theta, c, bounds=(0.0, 1.0))
+    lam32, V = np.linalg.eigh(O.symmetrize_lower(H32))
+    ref = (V * (1.0 / (np.exp(40.0 * (lam32 - 0.5)) + 1.0))) @ V.T
+    assert np.abs(Fm - ref).max() <= fit["max_error_fine_grid"] + 1e-9
