@@ -503,7 +503,9 @@ def main():
                 "launch_ms_how": "CUDA events on the launching stream: median step time / layers of the step (upper "
                                  "bound: includes the setup kernels' ~0.3 %)",
                 "launch_ms_device_timer": t_layer_dev_ms, "traffic": None}
-    prof = os.path.join(ROOT, "profiles", "r02_layer_traffic.json")
+    prof = os.path.join(ROOT, "profiles", "r03_layer_traffic.json")
+    if not os.path.exists(prof):
+        prof = os.path.join(ROOT, "profiles", "r02_layer_traffic.json")
     if not os.path.exists(prof):
         prof = os.path.join(ROOT, "profiles", "r01_layer_traffic.json")
     if os.path.exists(prof):

@@ -118,7 +118,8 @@ typedef struct {
                                0: test disabled (Alg. 1's printed tests, tol and max_layers only)              */
     int    enh_kc;          /* enhanced accumulation (tile_config 4, sp2_refine_energy): K-blocks of 64 the tensor
                                core accumulates before the chunk sum is folded into the error-free FP32 pair
-                               (DESIGN.md section 9).  <= 0: library default (2 = 128 values of K)       */
+                               (DESIGN.md section 9).  <= 0: library default (4 = 256 values of K; 2 is
+                               ~10 % more accurate in idempotency for ~12 % more time, 8 the reverse)            */
     double trunc_tau;       /* blocked-sparse variant for decaying matrices (DESIGN.md section 9 NEXT-4):
                                > 0: before every square, the off-diagonal 128 x 128 blocks of S with Frobenius norm
                                <= trunc_tau count as zero (reading C28): their operand tiles are neither
@@ -201,7 +202,7 @@ sp2_status_t sp2_generalized_wb(sp2_handle_t h, const float* H_dev, int N, int l
  *     last_sigma = -1:  D' = 2 S^2 - S^4          last_sigma = +1:  D' = (2 S - S^2)^2
  * (the alternation is continued from the last applied sign: DESIGN.md reading C15) in enhanced precision --
  * "single precision with double accumulation": FP16 hi/lo operands as in Eq. 15, but the tensor core
- * accumulates only opts->enh_kc K-blocks (default 2 = 128 values of K) at a time and the chunk sums are added in an
+ * accumulates only opts->enh_kc K-blocks (default 4 = 256 values of K) at a time and the chunk sums are added in an
  * error-free FP32 pair -- and the observables Tr[X H], Tr[X], IdErr = Tr[X - X^2] of X = S (in) and X = D' (out), in
  * FP64.  H: the Hamiltonian (lower triangle read).  S_dev may equal D_dev.  opts may be NULL (defaults); only
  * fp16_scale_log2 and enh_kc are read. */

@@ -160,7 +160,7 @@ static void stats_to_double(sp2_layer_stat_t* st, int n) {       // the device w
         st[i].trace_X_diag = fx_to_double(v[2]); st[i].iderr = fx_to_double(v[3]);
     }
 }
-static int opt_enh_kc(const sp2_opts_t* o) { return (o && o->enh_kc > 0) ? o->enh_kc : 2; }
+static int opt_enh_kc(const sp2_opts_t* o) { return (o && o->enh_kc > 0) ? o->enh_kc : 4; }
 
 extern "C" size_t sp2_workspace_bytes(int N_max, int batch_max, int max_layers) {
     if (N_max < 1 || max_layers < 1) return 0;

@@ -33,16 +33,21 @@ def test_tensor_core_accumulation_shrinks_the_off_diagonal_part(cuda_device):
         hi, lo = O.split_fp16(S0 * np.float32(8192.0))
         Xmix = O.mixed_square_exact(hi, lo) / 8192.0 ** 2              # Eq. 15 with exact sums: the target
         off = ~np.eye(n, dtype=bool)
-        for tile in (1, 4):                                            # plain / enhanced accumulation
+        # plain / enhanced accumulation with 2 K-blocks per tensor-core chunk / with the library default (4)
+        for tile, kc in ((1, 0), (4, 2), (4, 0)):
             X, _ = h.generalized(torch.from_numpy(H32).cuda(), np.array([[1.0, 0.0, 0.0]]), bounds=(0.0, 1.0),
-                                 opts=api.make_opts(tile_config=tile))
+                                 opts=api.make_opts(tile_config=tile, enh_kc=kc))
             d = (X.cpu().numpy().astype(np.float64) - Xmix)[off]
             r = Xmix[off]
-            betas[(n, tile)] = float((d * r).sum() / (r * r).sum())    # least-squares factor: X_off = (1 + beta) target
-    print("off-diagonal shrink factor beta of one layer (plain | enhanced accumulation): "
-          + ", ".join(f"N={n}: {betas[(n, 1)]:+.2e} | {betas[(n, 4)]:+.2e}" for n in (640, 2048)))
+            # least-squares factor: X_off = (1 + beta) target
+            betas[(n, tile) if kc == 2 or tile == 1 else (n, "default")] = float((d * r).sum() / (r * r).sum())
+    print("off-diagonal shrink factor beta of one layer (plain | enhanced, 2 K-blocks per chunk | enhanced, default 4): "
+          + ", ".join(f"N={n}: {betas[(n, 1)]:+.2e} | {betas[(n, 4)]:+.2e} | {betas[(n, 'default')]:+.2e}"
+                      for n in (640, 2048)))
     assert -2e-5 < betas[(2048, 1)] < betas[(640, 1)] < -5e-7         # truncation: negative, growing with K
     # chunked accumulation removes it (measured -4.4e-7 against -4.1e-6; -6.2e-6 before the 128 x 128 tiles kept X0 X1 in
     # an accumulator of its own, which shortens the chain of truncating adds behind the dominant term by a third)
     assert abs(betas[(2048, 4)]) < 0.15 * abs(betas[(2048, 1)])
+    # the default chunk of 4 K-blocks chains twice as many truncating adds: twice the residue (measured -8.2e-7)
+    assert abs(betas[(2048, 4)]) < abs(betas[(2048, "default")]) < 0.3 * abs(betas[(2048, 1)])
     h.close()
