@@ -93,7 +93,8 @@ typedef struct {
                                between layers and the operand pairs swapped inside the kernel (same tiles, same
                                order, same bits as 0; measured no faster than 0: the barrier costs what the kernel
                                boundary costs -- kept as the graph-free form of the device-side loop)          */
-    int    tile_config;     /* 0: choose by N; 1: 128x128 1-CTA; 2: 128x256 1-CTA; 3: 256x256 2-CTA;
+    int    tile_config;     /* 0: choose by N; 1: 128x128 1-CTA; 2: 128x256 1-CTA (never chosen by 0: kept as the
+                               comparison point of the tile-shape measurements); 3: 256x256 2-CTA;
                                4: 128x128 1-CTA with the enhanced accumulation of sp2_refine_energy in EVERY
                                layer (accuracy option, about 2x the time of 3 at large N)  */
     int    exact_diag;      /* 1 (default): diag(X_n)_i = sum_j S_ij^2 is taken from row sums of squares of the
